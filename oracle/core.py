@@ -1,0 +1,150 @@
+"""ORACLE (test infrastructure only) - numpy front-end of ``spd_oracle.c``.
+
+Builds ``oracle/libspd_oracle.so`` with gcc on first use (``build()``), loads it
+with ctypes and exposes the oracle functions on numpy arrays.  Imports nothing
+from the CUDA product.  See ``spd_oracle.c`` for the passages followed and the
+pins; ``formulas.py`` for the paper's sensitivity formulae.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "spd_oracle.c")
+_LIB = os.path.join(_HERE, "libspd_oracle.so")
+_lib: Optional[ctypes.CDLL] = None
+
+_i64 = ctypes.c_int64
+_i32 = ctypes.c_int32
+_f64 = ctypes.c_double
+_vp = ctypes.c_void_p
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle shared library (plain C, -O2, OpenMP over rows)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+def _load() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_spd_direct.restype = None
+        lib.oracle_spd_direct.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
+        lib.oracle_spd_prefix.restype = None
+        lib.oracle_spd_prefix.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _vp, _vp, _vp]
+        lib.oracle_snr_of_width.restype = None
+        lib.oracle_snr_of_width.argtypes = [_vp, _i64, _f64, _f64, _i64, _vp, _i64, _vp]
+        lib.oracle_row_stats.restype = None
+        lib.oracle_row_stats.argtypes = [_vp, _i64, _i64, _vp, _vp]
+        lib.oracle_find_candidates.restype = _i64
+        lib.oracle_find_candidates.argtypes = [_vp, _vp, _i64, _i64, ctypes.c_float, _i64, _vp, _vp, _vp, _vp]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def _plane(x) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    if x.ndim == 1:
+        x = x[None, :]
+    assert x.ndim == 2
+    return x
+
+
+def _stats(v, n_dm: int) -> np.ndarray:
+    a = np.ascontiguousarray(np.broadcast_to(np.asarray(v, dtype=np.float64), (n_dm,)))
+    return a
+
+
+def _widths(widths: Sequence[int]) -> np.ndarray:
+    w = np.ascontiguousarray(sorted(set(int(v) for v in widths)), dtype=np.int32)
+    assert w.size > 0 and w[0] >= 1
+    return w
+
+
+def spd_direct(x, mean, sigma, widths, t0: int = 0, t1: Optional[int] = None
+               ) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Oracle A: direct summation.  Returns (snr f64, width_idx i32, second f64),
+    each [n_dm, t1 - t0]; samples are row positions t0 <= n < t1."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    t1 = n_t if t1 is None else int(t1)
+    t0 = int(t0)
+    assert 0 <= t0 <= t1 <= n_t
+    w = _widths(widths)
+    mu, sg = _stats(mean, n_dm), _stats(sigma, n_dm)
+    snr = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    idx = np.empty((n_dm, t1 - t0), dtype=np.int32)
+    sec = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    _load().oracle_spd_direct(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
+                              w.ctypes.data, int(w.size), t0, t1,
+                              snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
+
+
+def spd_prefix(x, mean, sigma, widths) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Oracle B: double-precision running-sum difference on full rows."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    w = _widths(widths)
+    mu, sg = _stats(mean, n_dm), _stats(sigma, n_dm)
+    snr = np.empty((n_dm, n_t), dtype=np.float64)
+    idx = np.empty((n_dm, n_t), dtype=np.int32)
+    sec = np.empty((n_dm, n_t), dtype=np.float64)
+    _load().oracle_spd_prefix(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
+                              w.ctypes.data, int(w.size),
+                              snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
+
+
+def snr_of_width(row, mean: float, sigma: float, L: int, samples) -> np.ndarray:
+    """SNR_L[n] by direct summation at the listed samples of one row."""
+    row = np.ascontiguousarray(row, dtype=np.float32).reshape(-1)
+    s = np.ascontiguousarray(samples, dtype=np.int64)
+    out = np.empty(s.shape, dtype=np.float64)
+    _load().oracle_snr_of_width(row.ctypes.data, row.size, float(mean), float(sigma), int(L),
+                                s.ctypes.data, int(s.size), out.ctypes.data)
+    return out
+
+
+def row_stats(x) -> Tuple[np.ndarray, np.ndarray]:
+    """Per-row mean and population standard deviation (reading A6)."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    mu = np.empty(n_dm, dtype=np.float64)
+    sg = np.empty(n_dm, dtype=np.float64)
+    _load().oracle_row_stats(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data)
+    return mu, sg
+
+
+def find_candidates(snr, width_idx, threshold: float, capacity: Optional[int] = None):
+    """Reading A9 candidate rule on a float32 SNR plane.  Returns
+    (count, dm i32[], t i32[], snr f32[], width_idx i32[]) in (dm, t) order."""
+    snr = _plane(snr)
+    n_dm, n_t = snr.shape
+    wid = np.ascontiguousarray(width_idx, dtype=np.int32).reshape(n_dm, n_t)
+    cap = int(snr.size if capacity is None else capacity)
+    c_dm = np.empty(cap, dtype=np.int32)
+    c_t = np.empty(cap, dtype=np.int32)
+    c_snr = np.empty(cap, dtype=np.float32)
+    c_w = np.empty(cap, dtype=np.int32)
+    count = int(_load().oracle_find_candidates(snr.ctypes.data, wid.ctypes.data, n_dm, n_t,
+                                               ctypes.c_float(threshold), cap,
+                                               c_dm.ctypes.data, c_t.ctypes.data,
+                                               c_snr.ctypes.data, c_w.ctypes.data))
+    k = min(count, cap)
+    return count, c_dm[:k], c_t[:k], c_snr[:k], c_w[:k]

@@ -1,0 +1,189 @@
+/*
+ * ORACLE - TEST INFRASTRUCTURE ONLY.  Not part of the product.
+ *
+ * A plain, slow, double-precision CPU statement of what the single-pulse-
+ * detection (SPD) hot path computes, written from /root/reference/PAPER.md
+ * (Adamek & Armour 2020).  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code, header, table or helper with the CUDA path under
+ * paper_1910_08324_b200/csrc/.
+ *
+ * What is computed, per DM trial d and time sample n:
+ *
+ *   X_L[n]   = sum_{j=0}^{L-1} x[d, n+j]                      eq. (2)
+ *   SNR_L[n] = (X_L[n] - mu(X_L)) / sigma(X_L)                eq. (4)
+ *   mu(X_L)  = L mu_d ,  sigma(X_L) = sqrt(L) sigma_d         eq. (5)
+ *   Y[n]     = max_{L in B} SNR_L[n],  W[n] = that L's index  eq. (12)
+ *
+ * Widths are visited in ascending order and the best is replaced only by a
+ * strictly higher SNR ("If the new SNR is higher than the old SNR ...",
+ * PAPER.md:287), so the smallest width wins exact ties (reading A4).
+ * Windows that would cross the end of the row are skipped (reading A3:
+ * valid-only); if no width fits, Y = -inf and W = -1.
+ *
+ *   oracle_spd_direct  : the definition, every boxcar by direct summation
+ *                        (the "ideal SPD algorithm" route).
+ *   oracle_spd_prefix  : same quantities via a double-precision running sum
+ *                        C[n] of (x - mu) and X'_L[n] = C[n+L] - C[n]; a faster
+ *                        route used on full planes, itself pinned to
+ *                        oracle_spd_direct in tests (<= 1e-9).
+ *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
+ *   oracle_row_stats   : per-row mean and population standard deviation (reading A6).
+ *   oracle_find_candidates: threshold + 1-D local-peak rule (reading A9).
+ *
+ * Pins: tests/test_oracle_pins.py (closed form eq. 22 on single-pulse planes,
+ * numpy.convolve for single widths, constant / ramp / impulse closed forms,
+ * affine and shift invariances, white-noise statistics, brute force, the
+ * Fig. 17 worked example PAPER.md:587,605, eq. 24 on noise-free twins).
+ * oracle_find_candidates: the rule is this project's reading A9 (the paper
+ * names "peak-finding" only) - pinned by closed form on
+ * isolated pulses; otherwise "parity unpinned by the paper".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* Direct summation over samples [t0, t1) of every row.  Outputs are
+ * [n_dm][t1 - t0]; out_second (may be NULL) receives the best SNR among all
+ * widths other than the arg-max one (-inf if none). */
+void oracle_spd_direct(const float* x, int64_t n_dm, int64_t n_t,
+                       const double* mean, const double* sigma,
+                       const int32_t* widths, int32_t n_w,
+                       int64_t t0, int64_t t1,
+                       double* out_snr, int32_t* out_width, double* out_second) {
+    const int64_t span = t1 - t0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 256)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        for (int64_t n = t0; n < t1; ++n) {
+            const float* row = x + d * n_t;
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = 0; k < n_w; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;                       /* valid windows only (A3) */
+                double X = 0.0;
+                for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
+                const double snr = (X - (double)L * mean[d]) / (sqrt((double)L) * sigma[d]); /* eq. (4),(5) */
+                if (snr > best) {                              /* strict '>' (A4) */
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * span + (n - t0);
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+    }
+}
+
+/* Same quantities through a double-precision running sum of (x - mu). */
+void oracle_spd_prefix(const float* x, int64_t n_dm, int64_t n_t,
+                       const double* mean, const double* sigma,
+                       const int32_t* widths, int32_t n_w,
+                       double* out_snr, int32_t* out_width, double* out_second) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float* row = x + d * n_t;
+        double* C = (double*)malloc((size_t)(n_t + 1) * sizeof(double));
+        C[0] = 0.0;
+        for (int64_t n = 0; n < n_t; ++n) C[n + 1] = C[n] + ((double)row[n] - mean[d]);
+        for (int64_t n = 0; n < n_t; ++n) {
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = 0; k < n_w; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;
+                const double snr = (C[n + L] - C[n]) / (sqrt((double)L) * sigma[d]);
+                if (snr > best) {
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * n_t + n;
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+        free(C);
+    }
+}
+
+/* SNR_L[n] by direct summation for one row, one width, at listed samples
+ * (NaN where the window does not fit). */
+void oracle_snr_of_width(const float* row, int64_t n_t, double mean, double sigma,
+                         int64_t L, const int64_t* samples, int64_t count, double* out) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < count; ++i) {
+        const int64_t n = samples[i];
+        if (n < 0 || n + L > n_t) { out[i] = NAN; continue; }
+        double X = 0.0;
+        for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];
+        out[i] = (X - (double)L * mean) / (sqrt((double)L) * sigma);
+    }
+}
+
+/* Per-row mean and population standard deviation (ddof = 0), two passes in
+ * double (reading A6 of SURVEY.md sec. 8(c) for "computed from the plane"). */
+void oracle_row_stats(const float* x, int64_t n_dm, int64_t n_t, double* mean, double* sigma) {
+#pragma omp parallel for schedule(static)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float* row = x + d * n_t;
+        double s = 0.0;
+        for (int64_t n = 0; n < n_t; ++n) s += (double)row[n];
+        const double m = s / (double)n_t;
+        double v = 0.0;
+        for (int64_t n = 0; n < n_t; ++n) {
+            const double e = (double)row[n] - m;
+            v += e * e;
+        }
+        mean[d] = m;
+        sigma[d] = sqrt(v / (double)n_t);
+    }
+}
+
+/* Candidate rule (reading A9): (d, n) is a candidate iff Y[d,n] >= thr and
+ * Y[d,n] > Y[d,n-1] and Y[d,n] >= Y[d,n+1], row ends comparing against -inf
+ * (first sample of a plateau).  Candidates are emitted in (d, n) order; the
+ * return value counts all of them, the arrays receive the first `capacity`. */
+int64_t oracle_find_candidates(const float* snr, const int32_t* width, int64_t n_dm, int64_t n_t,
+                               float thr, int64_t capacity,
+                               int32_t* c_dm, int32_t* c_t, float* c_snr, int32_t* c_width) {
+    int64_t count = 0;
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float* y = snr + d * n_t;
+        for (int64_t n = 0; n < n_t; ++n) {
+            const float v = y[n];
+            const float left = (n > 0) ? y[n - 1] : -INFINITY;
+            const float right = (n + 1 < n_t) ? y[n + 1] : -INFINITY;
+            if (v >= thr && v > left && v >= right) {
+                if (count < capacity) {
+                    c_dm[count] = (int32_t)d;
+                    c_t[count] = (int32_t)n;
+                    c_snr[count] = v;
+                    c_width[count] = width[d * n_t + n];
+                }
+                ++count;
+            }
+        }
+    }
+    return count;
+}

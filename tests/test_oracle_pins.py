@@ -1,0 +1,300 @@
+"""Pins for the CPU oracle (oracle/spd_oracle.c): each test checks it against
+something other than itself - a closed form from the paper, a library routine
+on a special case, an invariant, or brute force written out in this file."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import formulas as F
+from workloads import get_workload, make_plane_numpy, make_pulse_only_plane_numpy
+
+
+def _single_pulse_row(n_t, t0, S, snr_t):
+    x = np.zeros(n_t, dtype=np.float32)
+    x[t0:t0 + S] = np.float32(snr_t / math.sqrt(S))
+    return x
+
+
+def _closed_form_single_pulse(n_t, t0, S, amp, widths):
+    """eq. (22): SNR_L[n] = d_s A / sqrt(L) with d_s the overlap of
+    [n, n+L) and [t0, t0+S); no summation anywhere."""
+    n = np.arange(n_t)[:, None].astype(np.int64)
+    L = np.asarray(widths, dtype=np.int64)[None, :]
+    ov = np.minimum(n + L, t0 + S) - np.maximum(n, t0)
+    ov = np.clip(ov, 0, None).astype(np.float64)
+    snr = ov * amp / np.sqrt(L.astype(np.float64))
+    snr[(n + L) > n_t] = -np.inf                      # valid windows only (A3)
+    return snr                                        # [n_t, n_w]
+
+
+# --- P6: whole-plane closed form ------------------------------------------------------
+
+@pytest.mark.parametrize("S,t0", [(1, 40), (3, 17), (7, 100), (20, 100), (45, 60), (64, 0), (33, 190)])
+@pytest.mark.parametrize("kind", ["POW2", "ALL", "IGRID1", "RANDOM"])
+def test_single_pulse_plane_matches_eq22(oracle_lib, S, t0, kind):
+    n_t = 256
+    rng = np.random.default_rng(S * 1000 + t0)
+    widths = {"POW2": F.widths_pow2(64), "ALL": F.widths_all(64), "IGRID1": F.widths_igrid(1, 64),
+              "RANDOM": sorted(set(int(v) for v in rng.integers(1, 90, size=9)))}[kind]
+    x = _single_pulse_row(n_t, t0, S, 10.0)
+    amp = float(x[t0])
+    want = _closed_form_single_pulse(n_t, t0, S, amp, widths)
+    snr, idx, sec = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    assert np.allclose(snr[0], want.max(axis=1), rtol=1e-12, atol=1e-12)
+    # arg-max: first (smallest-width) maximum of the closed form, where it is unique to 1e-9
+    srt = np.sort(want, axis=1)
+    with np.errstate(invalid="ignore"):
+        unique = (srt[:, -1] - srt[:, -2]) > 1e-9 if want.shape[1] > 1 else np.ones(n_t, bool)
+    assert np.array_equal(idx[0][unique], want.argmax(axis=1)[unique])
+    if want.shape[1] > 1:
+        assert np.allclose(sec[0][unique], srt[:, -2][unique], rtol=1e-12, atol=1e-12)
+    # outside any window touching the pulse everything is exactly zero -> smallest width wins the tie (A4)
+    far = np.arange(n_t) > t0 + S
+    far &= np.arange(n_t) + widths[0] <= n_t
+    assert np.all(snr[0][far] == 0.0) and np.all(idx[0][far] == 0)
+    # prefix-difference oracle agrees
+    snr_b, idx_b, _ = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    assert np.allclose(snr_b, snr, rtol=0, atol=1e-9)
+
+
+# --- P7: the paper's worked example (Fig. 17) ----------------------------------------
+
+def test_fig17_worked_example(oracle_lib, paper_pins):
+    p = paper_pins["fig17_example"]
+    widths = F.widths_all(64)
+    for snr_t in p["snr"]:
+        x = _single_pulse_row(512, p["pulse_start"], p["pulse_width"], float(snr_t))
+        snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+        n_best = int(np.argmax(snr[0]))
+        L_best = widths[int(idx[0][n_best])]
+        assert L_best == p["detected_width"]
+        assert n_best == p["pulse_start"]                              # start-aligned (A2) ...
+        assert n_best + L_best // 2 == p["detected_centre"]            # ... whose centre is sample 110
+        assert snr[0][n_best] == pytest.approx(float(snr_t), rel=1e-6)  # eq. (6): matched boxcar returns C
+
+
+# --- P8: special cases that reduce to a library routine ------------------------------
+
+def test_width_one_is_eq3(oracle_lib):
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((4, 300)).astype(np.float32)
+    mu = np.array([0.1, -0.2, 0.0, 1.5])
+    sg = np.array([1.0, 2.0, 0.5, 3.0])
+    snr, idx, sec = oracle_lib.spd_direct(x, mu, sg, [1])
+    assert np.allclose(snr, (x.astype(np.float64) - mu[:, None]) / sg[:, None], rtol=1e-14, atol=1e-14)
+    assert np.all(idx == 0) and np.all(np.isneginf(sec))
+
+
+@pytest.mark.parametrize("L", [2, 5, 16, 37])
+def test_single_width_is_numpy_convolve(oracle_lib, L):
+    rng = np.random.default_rng(L)
+    x = rng.standard_normal(400).astype(np.float32)
+    mu, sg = 0.25, 1.7
+    snr, idx, _ = oracle_lib.spd_direct(x, mu, sg, [L])
+    box = np.convolve(x.astype(np.float64), np.ones(L), mode="valid")     # X_L[n], n = 0..n_t-L
+    want = (box - L * mu) / (math.sqrt(L) * sg)
+    assert np.allclose(snr[0][:400 - L + 1], want, rtol=1e-12, atol=1e-12)
+    assert np.all(np.isneginf(snr[0][400 - L + 1:])) and np.all(idx[0][400 - L + 1:] == -1)   # A3
+    s2 = oracle_lib.snr_of_width(x, mu, sg, L, np.arange(400 - L + 1))
+    assert np.allclose(s2, want, rtol=1e-12, atol=1e-12)
+
+
+def test_row_stats_is_numpy_mean_std(oracle_lib):
+    rng = np.random.default_rng(11)
+    x = (rng.standard_normal((5, 1000)) * 2.0 + 3.0).astype(np.float32)
+    mu, sg = oracle_lib.row_stats(x)
+    x64 = x.astype(np.float64)
+    assert np.allclose(mu, x64.mean(axis=1), rtol=1e-13)
+    assert np.allclose(sg, x64.std(axis=1, ddof=0), rtol=1e-12)
+
+
+# --- P9: brute force written out here, tiny planes ------------------------------------
+
+def _brute(x, mu, sg, widths):
+    n_dm, n_t = x.shape
+    snr = np.full((n_dm, n_t), -np.inf)
+    idx = np.full((n_dm, n_t), -1, dtype=np.int32)
+    for d in range(n_dm):
+        for n in range(n_t):
+            for k, L in enumerate(widths):
+                if n + L > n_t:
+                    continue
+                X = 0.0
+                for j in range(L):
+                    X += float(x[d, n + j])
+                s = (X - L * mu[d]) / (math.sqrt(L) * sg[d])
+                if s > snr[d, n]:
+                    snr[d, n] = s
+                    idx[d, n] = k
+    return snr, idx
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_brute_force_tiny_planes(oracle_lib, seed):
+    rng = np.random.default_rng(seed)
+    x = rng.standard_normal((3, 50)).astype(np.float32)
+    x[1, 20:27] += 2.0
+    mu = rng.normal(0, 0.1, 3)
+    sg = rng.uniform(0.5, 2.0, 3)
+    widths = sorted(set(int(v) for v in rng.integers(1, 30, size=6)))
+    want_snr, want_idx = _brute(x, mu, sg, widths)
+    for fn in (oracle_lib.spd_direct, oracle_lib.spd_prefix):
+        snr, idx, _ = fn(x, mu, sg, widths)
+        assert np.allclose(snr, want_snr, rtol=1e-12, atol=1e-12)
+        assert np.array_equal(idx, want_idx)
+
+
+# --- P10/P11: closed forms that catch index, tail and scaling mistakes ----------------
+
+def test_constant_offset_closed_form(oracle_lib):
+    n_t, mu, sg, a = 200, 1.25, 0.5, 0.75
+    widths = [1, 2, 4, 7, 16, 50]
+    x = np.full(n_t, mu + a, dtype=np.float32)
+    snr, idx, _ = oracle_lib.spd_direct(x, mu, sg, widths)
+    for n in range(n_t):
+        fit = [k for k, L in enumerate(widths) if n + L <= n_t]
+        k = fit[-1]                                       # SNR_L = a sqrt(L)/sigma grows with L
+        assert idx[0][n] == k
+        assert snr[0][n] == pytest.approx(a * math.sqrt(widths[k]) / sg, rel=1e-12)
+    snr_neg, idx_neg, _ = oracle_lib.spd_direct(np.full(n_t, mu - a, dtype=np.float32), mu, sg, widths)
+    assert np.all(idx_neg == 0) and np.allclose(snr_neg, -a / sg)
+
+
+def test_tail_rule_without_width_one(oracle_lib):
+    x = np.ones(40, dtype=np.float32)
+    snr, idx, sec = oracle_lib.spd_direct(x, 0.0, 1.0, [4, 8])
+    assert np.all(np.isneginf(snr[0][37:])) and np.all(idx[0][37:] == -1)
+    assert np.all(idx[0][33:37] == 0) and np.all(np.isneginf(sec[0][33:37]))
+    assert np.all(idx[0][:33] == 1)
+
+
+def test_ramp_closed_form(oracle_lib):
+    n_t = 120
+    widths = [1, 3, 8, 20]
+    x = np.arange(n_t, dtype=np.float32)
+    snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    for n in range(n_t):
+        vals = [(L * n + L * (L - 1) / 2) / math.sqrt(L) if n + L <= n_t else -math.inf for L in widths]
+        assert snr[0][n] == pytest.approx(max(vals), rel=1e-13)
+        assert idx[0][n] == int(np.argmax(vals))
+
+
+def test_unit_impulse_closed_form(oracle_lib):
+    n_t, t0, A = 128, 70, 5.0
+    widths = [1, 2, 4, 8, 16, 32]
+    x = np.zeros(n_t, dtype=np.float32)
+    x[t0] = A
+    snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    for n in range(n_t):
+        if n > t0 or t0 - n + 1 > widths[-1]:
+            assert snr[0][n] == 0.0 and idx[0][n] == 0
+        else:
+            k = next(k for k, L in enumerate(widths) if L >= t0 - n + 1)
+            assert idx[0][n] == k and snr[0][n] == pytest.approx(A / math.sqrt(widths[k]))
+
+
+# --- P12: invariants ---------------------------------------------------------------------
+
+def test_affine_invariance_and_superset_monotonicity(oracle_lib):
+    rng = np.random.default_rng(5)
+    x = np.round(rng.standard_normal((2, 600)) * 1024.0) / 1024.0     # exact in float32, and so is 4x + 8
+    widths = F.widths_pow2(64)
+    snr, idx, _ = oracle_lib.spd_direct(x.astype(np.float32), 0.0, 1.0, widths)
+    alpha, beta = 4.0, 8.0                       # powers of two: exact in float32
+    snr2, idx2, _ = oracle_lib.spd_direct((alpha * x.astype(np.float32) + beta).astype(np.float32), beta, alpha, widths)
+    assert np.allclose(snr2, snr, rtol=1e-12, atol=1e-12) and np.array_equal(idx2, idx)
+    full, idx_full, _ = oracle_lib.spd_direct(x.astype(np.float32), 0.0, 1.0, F.widths_all(64))
+    assert np.all(full >= snr - 1e-12)
+    all_w = F.widths_all(64)
+    chosen = np.array(all_w)[idx_full]
+    in_set = np.isin(chosen, widths)
+    assert np.allclose(full[in_set], snr[in_set], rtol=1e-12)
+
+
+def test_time_shift_equivariance(oracle_lib):
+    rng = np.random.default_rng(6)
+    x = rng.standard_normal(700).astype(np.float32)
+    widths = [1, 3, 8, 21]
+    a, ia, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    b, ib, _ = oracle_lib.spd_direct(x[50:], 0.0, 1.0, widths)
+    assert np.array_equal(a[0][50:], b[0]) and np.array_equal(ia[0][50:], ib[0])
+    # windowed evaluation equals the slice of the full evaluation
+    c, ic, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths, t0=123, t1=456)
+    assert np.array_equal(c[0], a[0][123:456]) and np.array_equal(ic[0], ia[0][123:456])
+
+
+# --- P13: white-noise statistics (eq. 5) --------------------------------------------------
+
+def test_white_noise_per_width_statistics(oracle_lib):
+    rng = np.random.default_rng(13)
+    n_t = 1 << 18
+    x = rng.standard_normal(n_t).astype(np.float32)
+    for L in (1, 4, 32, 256):
+        s = oracle_lib.snr_of_width(x, 0.0, 1.0, L, np.arange(0, n_t - L, L))   # non-overlapping windows
+        n_ind = s.size
+        assert abs(s.mean()) < 5.0 / math.sqrt(n_ind)
+        assert abs(s.var() - 1.0) < 5.0 * math.sqrt(2.0 / n_ind)
+
+
+# --- P14: eq. (24) on the noise-free twin of a workload ----------------------------------
+
+@pytest.mark.parametrize("cfg,n_dm,n_t,n_pulses", [(1, 8, 4096, 8), (2, 8, 8192, 16)])
+def test_noise_free_twin_recovers_eq24(oracle_lib, cfg, n_dm, n_t, n_pulses):
+    w = get_workload(cfg).scaled(n_dm, n_t, n_pulses)
+    plane, pulses = make_pulse_only_plane_numpy(w)
+    widths = F.width_set(w.width_kind, w.width_param, w.max_width)
+    snr, idx, _ = oracle_lib.spd_prefix(plane, 0.0, 1.0, widths)
+    ratios = []
+    for p in pulses:
+        others = [q for q in pulses if q is not p and q.dm == p.dm
+                  and q.t0 < p.t0 + p.width + w.max_width and p.t0 < q.t0 + q.width + w.max_width]
+        if others:
+            continue                                     # overlapping neighbourhoods: not an isolated pulse
+        lo, hi = max(0, p.t0 - w.max_width), min(n_t, p.t0 + p.width)
+        r = snr[p.dm, lo:hi].max() / p.snr_t
+        assert r == pytest.approx(F.rsnr_max(p.width, widths), rel=1e-6)
+        ratios.append((p.width, r))
+    assert len(ratios) >= n_pulses // 2
+    mean_loss = 1.0 - sum(r for _, r in ratios) / len(ratios)
+    assert mean_loss == pytest.approx(F.mean_loss_over_widths([s for s, _ in ratios], widths), abs=1e-6)
+
+
+# --- A vs B on a config-1-shaped plane ----------------------------------------------------
+
+def test_direct_and_prefix_agree_on_config1_shape(oracle_lib):
+    w = get_workload(1).scaled(4, 2048, 4)
+    plane, _ = make_plane_numpy(w)
+    widths = F.width_set(w.width_kind, w.width_param, w.max_width)
+    a, ia, sa = oracle_lib.spd_direct(plane, 0.0, 1.0, widths)
+    b, ib, sb = oracle_lib.spd_prefix(plane, 0.0, 1.0, widths)
+    assert np.max(np.abs(a - b)) <= 1e-9
+    clear = (a - sa) > 1e-9
+    assert np.array_equal(ia[clear], ib[clear])
+
+
+# --- candidate rule (reading A9): closed form on an isolated pulse ----------------------
+
+def test_candidates_isolated_pulse_first_sample_of_plateau(oracle_lib):
+    n_t, t0, S, snr_t = 400, 150, 20, 10.0
+    widths = F.widths_pow2(64)
+    x = _single_pulse_row(n_t, t0, S, snr_t)
+    snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    # eq. (22): width 16 fits inside the pulse at n = t0..t0+4 -> five equal maxima of 16 A / 4
+    peak = 16 * (snr_t / math.sqrt(S)) / 4.0
+    assert np.allclose(snr[0][t0:t0 + 5], peak, rtol=1e-7) and snr[0].max() == pytest.approx(peak, rel=1e-7)
+    count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.astype(np.float32), idx, 0.9 * peak)
+    assert count == 1 and c_dm[0] == 0 and c_t[0] == t0 and widths[c_w[0]] == 16
+    assert c_snr[0] == pytest.approx(peak, rel=1e-6)
+
+
+def test_candidates_rule_edges_and_capacity(oracle_lib):
+    y = np.array([[7, 7, 3, 8, 8, 8, 2, 9],
+                  [1, 2, 3, 4, 5, 6, 7, 8]], dtype=np.float32)
+    wid = np.zeros_like(y, dtype=np.int32)
+    count, c_dm, c_t, c_snr, _ = oracle_lib.find_candidates(y, wid, 6.0)
+    # row 0: n=0 (7 > -inf, >= 7), n=3 (first of the 8-plateau), n=7 (9 > 2, right edge); row 1: n=7
+    assert count == 4
+    assert list(zip(c_dm.tolist(), c_t.tolist())) == [(0, 0), (0, 3), (0, 7), (1, 7)]
+    count2, c_dm2, *_ = oracle_lib.find_candidates(y, wid, 6.0, capacity=2)
+    assert count2 == 4 and len(c_dm2) == 2
