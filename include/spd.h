@@ -1,0 +1,188 @@
+/*
+ * spd.h - C ABI of the B200-native single-pulse-detection (SPD) hot path.
+ *
+ * Method: Adamek & Armour, "Single Pulse Detection Algorithms for Real-time
+ * Fast Radio Burst Searches using GPUs" (arXiv:1910.08324).  Citations are
+ * PAPER.md:<line> of the paper text plus the equation / section they fall in.
+ *
+ * What the library computes, for every DM trial d and time sample n of a
+ * de-dispersed plane x[n_dm][n_t] (row-major float32, time contiguous):
+ *
+ *   X_L[n]   = sum_{j=0}^{L-1} x[d, n+j]                       eq. (2)
+ *   SNR_L[n] = (X_L[n] - L mu_d) / (sqrt(L) sigma_d)           eq. (4),(5) PAPER.md:69,87-91
+ *   Y[d,n]   = max_{L in B} SNR_L[n],  W[d,n] = index of that L eq. (12)
+ *
+ * over a (possibly incomplete, "lossy") set of boxcar widths B,
+ * with long boxcars built from partial sums of shorter ones (eq. 15,
+ * PAPER.md:284 eq. 16) and never summed directly, followed by a threshold /
+ * peak-candidate stage.
+ *
+ * Conventions:
+ *   - windows are start-aligned: index n is the FIRST sample of the boxcar (eq. 2);
+ *   - valid windows only: widths with n + L > n_t are skipped; if no width fits,
+ *     Y = -inf and W = -1;
+ *   - widths are visited in ascending order with a strict '>' update
+ *     (PAPER.md:287), so the smallest width wins exact ties;
+ *   - W is the INDEX into the plan's ascending, de-duplicated width table
+ *     (spd_plan_get_widths), not the width itself.
+ *
+ * Every function is thread-safe with respect to distinct plans.  No function
+ * throws, exits or synchronises the device unless stated.  All functions
+ * returning int return SPD_OK (0) or a negative spd_status; a human-readable
+ * message for the calling thread's last error is in spd_last_error_string().
+ * There is NO CPU fallback: on a machine without an sm_100 device every
+ * compute entry point fails with SPD_ERR_UNSUPPORTED_DEVICE.
+ */
+#ifndef SPD_B200_SPD_H_
+#define SPD_B200_SPD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPD_VERSION 100
+
+typedef enum spd_status {
+    SPD_OK = 0,
+    SPD_ERR_INVALID_ARG = -1,        /* NULL pointer, bad size, bad width set */
+    SPD_ERR_UNSUPPORTED_DEVICE = -2, /* no CUDA device, or not compute capability 10.x */
+    SPD_ERR_ALLOC = -3,              /* host or device allocation failed */
+    SPD_ERR_CUDA = -4                /* a CUDA runtime call or kernel launch failed */
+} spd_status;
+
+/* Width-set kinds of spd_width_set_generate. */
+typedef enum spd_width_kind {
+    SPD_WIDTHS_ALL = 0,       /* 1..max_width: the "ideal SPD algorithm" */
+    SPD_WIDTHS_POW2 = 1,      /* {1,2,4,...} <= max_width: decimation-in-time set, Alg. 3 */
+    SPD_WIDTHS_BOXDIT = 2,    /* eq. (14) PAPER.md:216 with D = 2; param = L_max per iteration */
+    SPD_WIDTHS_IGRID = 3,     /* eq. (18) / Table 1; param = depth d */
+    SPD_WIDTHS_GEOMETRIC = 4  /* round(r^j), r = param / 1000 (> 1); this project's addition */
+} spd_width_kind;
+
+/* Plan creation flags (spd_plan_create_ex). */
+#define SPD_FLAG_FORCE_GENERIC 0x1u /* use the any-width-set kernels even where the dyadic tree applies */
+
+/* Which kernels a plan dispatches to (spd_plan_info.path). */
+#define SPD_PATH_DYADIC_TREE 1 /* streaming partial-sum tree, widths {1,2,4,...,2^(K-1)} */
+#define SPD_PATH_GENERIC 2     /* any width set: per-row running partial sums in a plan-owned workspace */
+
+typedef struct spd_plan spd_plan; /* opaque */
+
+/* One detection of the candidate stage (reading A9: the paper only names
+ * "peak-finding").  t is the start sample of the boxcar. */
+typedef struct spd_candidate {
+    int32_t dm;        /* DM-trial (row) index */
+    int32_t t;         /* time sample, start-aligned */
+    float snr;         /* Y[dm, t] */
+    int32_t width_idx; /* W[dm, t] */
+} spd_candidate;
+
+typedef struct spd_plan_info {
+    int64_t n_dm, n_t;
+    int32_t n_widths, max_width;
+    int32_t path;               /* SPD_PATH_* */
+    int32_t launches_per_run;   /* kernels one spd_run enqueues */
+    int32_t threads_per_block;  /* of the dominant kernel */
+    int32_t blocks;             /* grid size of the dominant kernel */
+    int32_t chunk;              /* time samples per streaming step (dyadic tree), else 0 */
+    int32_t segments_per_row;   /* independent streams per DM row (dyadic tree), else 0 */
+    int64_t smem_bytes;         /* dynamic shared memory per block of the dominant kernel */
+    int64_t workspace_bytes;    /* plan-owned device workspace */
+} spd_plan_info;
+
+/*
+ * spd_width_set_generate - write an ascending width set into out[0..cap).
+ *   kind/param : see spd_width_kind.  max_width >= 1 caps every member
+ *                (reading A7: max_width is L_end, an upper bound).
+ *   out        : HOST array of cap int32 (may be NULL when cap == 0 to query the size).
+ *   n_out      : HOST, receives the number of widths of the set (even if > cap).
+ * Returns SPD_ERR_INVALID_ARG for unknown kind, bad param, or cap too small
+ * (n_out is still written in the last case).
+ */
+int spd_width_set_generate(int32_t kind, int32_t param, int32_t max_width,
+                           int32_t* out, int32_t cap, int32_t* n_out);
+
+/*
+ * spd_plan_create - describe one problem: plane shape, width set B, L_end.
+ *   out        : HOST, receives the plan (caller owns; free with spd_plan_destroy).
+ *   n_dm, n_t  : plane is n_dm rows (DM trials) x n_t time samples, 1 <= n_t <= 2^31-1.
+ *   width_set  : HOST array of n_widths boxcar widths in samples (copied, sorted
+ *                ascending, de-duplicated).  Error if empty, any width < 1,
+ *                any width > max_width, or more than 32768 distinct widths.
+ *   max_width  : L_end; must satisfy max_width <= n_t.
+ * The plan owns small device tables and, for SPD_PATH_GENERIC, a workspace of
+ * n_dm*(n_t+1) doubles allocated here.  Uses the current CUDA device.
+ */
+int spd_plan_create(spd_plan** out, int64_t n_dm, int64_t n_t,
+                    const int32_t* width_set, int32_t n_widths, int32_t max_width);
+
+/* Same, with SPD_FLAG_* bits. */
+int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t,
+                       const int32_t* width_set, int32_t n_widths, int32_t max_width,
+                       uint32_t flags);
+
+/* Frees the plan and everything it owns.  NULL is allowed. */
+void spd_plan_destroy(spd_plan* plan);
+
+/* Copies the plan's ascending width table to out[0..*n) (HOST); *n receives the count.
+ * out may be NULL to query the count. */
+int spd_plan_get_widths(const spd_plan* plan, int32_t* out, int32_t* n);
+
+/* Fills *info (HOST). */
+int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info);
+
+/*
+ * spd_run - the hot path on DEVICE buffers.
+ *   plane      : DEVICE, float32 [n_dm][n_t] row-major, 16-byte aligned, read only.
+ *   mean, sigma: DEVICE, float32 [n_dm]; per-DM mu(x) and sigma(x) of eq. (5).
+ *                sigma > 0 and finite inputs are preconditions (not checked).
+ *   out_snr    : DEVICE, float32 [n_dm][n_t], fully overwritten with Y.
+ *   out_width  : DEVICE, int32 [n_dm][n_t], fully overwritten with W.
+ *   cuda_stream: a cudaStream_t (NULL = default stream).  The call only
+ *                enqueues work; it never synchronises.
+ * Buffers are owned by the caller and must not alias.  A SPD_PATH_DYADIC_TREE
+ * plan is read-only during the call (concurrent runs on different streams are
+ * allowed); a SPD_PATH_GENERIC plan uses its workspace (one run at a time).
+ */
+int spd_run(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+            float* out_snr, int32_t* out_width, void* cuda_stream);
+
+/*
+ * spd_find_candidates - threshold + 1-D peak stage (row a8; reading A9):
+ * (d, n) is reported iff Y[d,n] >= threshold and Y[d,n] > Y[d,n-1] and
+ * Y[d,n] >= Y[d,n+1] (row ends compare against -inf).
+ *   out_snr, out_width : DEVICE planes produced by spd_run.
+ *   list      : DEVICE array of `capacity` spd_candidate; order unspecified.
+ *   n_found   : DEVICE int64; receives the number of peaks found, which may
+ *               exceed capacity (overflow: only the first `capacity` appends are stored).
+ * Asynchronous on cuda_stream.
+ */
+int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+                        float threshold, spd_candidate* list, int64_t capacity,
+                        int64_t* n_found, void* cuda_stream);
+
+/*
+ * spd_run_host - the same hot path on HOST buffers (end-to-end entry point):
+ * copies row blocks of the plane to the device, runs the kernels and copies
+ * Y and W back, overlapping copies and kernels on internal streams.
+ *   plane, out_snr, out_width : HOST (pinned memory recommended), shapes as spd_run.
+ *   mean, sigma               : HOST float32 [n_dm].
+ * Blocks until the results are in out_snr / out_width.  Needs a
+ * SPD_PATH_DYADIC_TREE or SPD_PATH_GENERIC plan; device staging buffers are
+ * allocated on first use and kept in the plan (hence the non-const plan).
+ */
+int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                 float* out_snr, int32_t* out_width);
+
+/* Message describing the calling thread's most recent error ("" if none). */
+const char* spd_last_error_string(void);
+
+/* Library version (SPD_VERSION). */
+int spd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPD_B200_SPD_H_ */

@@ -1,0 +1,23 @@
+"""B200-native single-pulse detection (arXiv:1910.08324 hot path).
+
+``libspd_b200.so`` (hand-written sm_100a CUDA behind the C ABI of ``include/spd.h``)
+does all the work; this package only builds it (``build()``) and marshals
+arguments (``binding``).  There is no CPU fallback and nothing here imports the
+test oracle.
+"""
+from ._build import LIB_PATH, build
+from .binding import (  # noqa: F401
+    CANDIDATE_DTYPE, EXPORTS, Plan, SpdError,
+    SPD_FLAG_FORCE_GENERIC, SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC,
+    candidates_to_numpy, load, spd_destroy, spd_find_candidates, spd_last_error_string,
+    spd_plan_create, spd_plan_destroy, spd_plan_get_info, spd_plan_get_widths, spd_run,
+    spd_run_host, spd_version, spd_width_set_generate,
+)
+
+__all__ = [
+    "LIB_PATH", "build", "load", "Plan", "SpdError", "EXPORTS", "CANDIDATE_DTYPE",
+    "SPD_FLAG_FORCE_GENERIC", "SPD_PATH_DYADIC_TREE", "SPD_PATH_GENERIC",
+    "spd_width_set_generate", "spd_plan_create", "spd_plan_destroy", "spd_destroy",
+    "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
+    "spd_run_host", "spd_last_error_string", "spd_version", "candidates_to_numpy",
+]

@@ -1,0 +1,296 @@
+"""Thin ctypes binding of the C ABI in ``include/spd.h`` - argument marshalling only.
+
+Every function has the name and the argument order of its C counterpart; device
+buffers are ``torch`` CUDA tensors (PyTorch supplies device memory and streams,
+nothing else), host buffers are numpy arrays or CPU tensors.  All arithmetic of
+the method runs in the CUDA kernels of ``csrc/``; if the shared library is not
+built or no sm_100 device is present the calls raise - there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+from . import _build
+
+SPD_OK = 0
+SPD_ERR_INVALID_ARG = -1
+SPD_ERR_UNSUPPORTED_DEVICE = -2
+SPD_ERR_ALLOC = -3
+SPD_ERR_CUDA = -4
+
+SPD_WIDTHS_ALL, SPD_WIDTHS_POW2, SPD_WIDTHS_BOXDIT, SPD_WIDTHS_IGRID, SPD_WIDTHS_GEOMETRIC = range(5)
+WIDTH_KINDS = {"ALL": 0, "POW2": 1, "BOXDIT": 2, "IGRID": 3, "GEOMETRIC": 4}
+SPD_FLAG_FORCE_GENERIC = 0x1
+SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC = 1, 2
+
+# every symbol include/spd.h declares
+EXPORTS = (
+    "spd_width_set_generate", "spd_plan_create", "spd_plan_create_ex", "spd_plan_destroy",
+    "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
+    "spd_run_host", "spd_last_error_string", "spd_version",
+)
+
+
+class SpdError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"spd status {status}: {message}")
+        self.status = status
+
+
+class spd_candidate(ctypes.Structure):
+    _fields_ = [("dm", ctypes.c_int32), ("t", ctypes.c_int32), ("snr", ctypes.c_float),
+                ("width_idx", ctypes.c_int32)]
+
+
+CANDIDATE_DTYPE = np.dtype([("dm", "<i4"), ("t", "<i4"), ("snr", "<f4"), ("width_idx", "<i4")])
+
+
+class spd_plan_info(ctypes.Structure):
+    _fields_ = [("n_dm", ctypes.c_int64), ("n_t", ctypes.c_int64),
+                ("n_widths", ctypes.c_int32), ("max_width", ctypes.c_int32),
+                ("path", ctypes.c_int32), ("launches_per_run", ctypes.c_int32),
+                ("threads_per_block", ctypes.c_int32), ("blocks", ctypes.c_int32),
+                ("chunk", ctypes.c_int32), ("segments_per_row", ctypes.c_int32),
+                ("smem_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64)]
+
+
+_lib: Optional[ctypes.CDLL] = None
+_vp, _i32, _i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+
+
+def library_path() -> str:
+    return _build.LIB_PATH
+
+
+def load(build_if_missing: bool = True) -> ctypes.CDLL:
+    """dlopen ``libspd_b200.so`` (building it first if needed) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        _build.build()
+    if not os.path.exists(_build.LIB_PATH):
+        raise SpdError(SPD_ERR_UNSUPPORTED_DEVICE,
+                       f"{_build.LIB_PATH} is not built; run paper_1910_08324_b200.build() (no CPU fallback)")
+    lib = ctypes.CDLL(_build.LIB_PATH)
+    lib.spd_version.restype = ctypes.c_int
+    lib.spd_last_error_string.restype = ctypes.c_char_p
+    lib.spd_width_set_generate.restype = ctypes.c_int
+    lib.spd_width_set_generate.argtypes = [_i32, _i32, _i32, _vp, _i32, ctypes.POINTER(_i32)]
+    lib.spd_plan_create.restype = ctypes.c_int
+    lib.spd_plan_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _i32, _i32]
+    lib.spd_plan_create_ex.restype = ctypes.c_int
+    lib.spd_plan_create_ex.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _i32, _i32, ctypes.c_uint32]
+    lib.spd_plan_destroy.restype = None
+    lib.spd_plan_destroy.argtypes = [_vp]
+    lib.spd_plan_get_widths.restype = ctypes.c_int
+    lib.spd_plan_get_widths.argtypes = [_vp, _vp, ctypes.POINTER(_i32)]
+    lib.spd_plan_get_info.restype = ctypes.c_int
+    lib.spd_plan_get_info.argtypes = [_vp, ctypes.POINTER(spd_plan_info)]
+    lib.spd_run.restype = ctypes.c_int
+    lib.spd_run.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.spd_find_candidates.restype = ctypes.c_int
+    lib.spd_find_candidates.argtypes = [_vp, _vp, _vp, ctypes.c_float, _vp, _i64, _vp, _vp]
+    lib.spd_run_host.restype = ctypes.c_int
+    lib.spd_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+    _lib = lib
+    return lib
+
+
+def spd_last_error_string() -> str:
+    return load().spd_last_error_string().decode("utf-8", "replace")
+
+
+def _check(status: int) -> None:
+    if status != SPD_OK:
+        raise SpdError(status, spd_last_error_string())
+
+
+def spd_version() -> int:
+    return int(load().spd_version())
+
+
+def spd_width_set_generate(kind, param: int, max_width: int) -> np.ndarray:
+    """Ascending int32 width set; ``kind`` is an SPD_WIDTHS_* value or its name."""
+    lib = load()
+    k = WIDTH_KINDS[kind.upper()] if isinstance(kind, str) else int(kind)
+    n = _i32(0)
+    _check(lib.spd_width_set_generate(k, int(param), int(max_width), None, 0, ctypes.byref(n)))
+    out = np.empty(n.value, dtype=np.int32)
+    _check(lib.spd_width_set_generate(k, int(param), int(max_width), out.ctypes.data, n.value, ctypes.byref(n)))
+    return out
+
+
+def spd_plan_create(n_dm: int, n_t: int, width_set: Sequence[int], max_width: int, flags: int = 0) -> int:
+    """Returns the opaque plan handle (an integer address)."""
+    lib = load()
+    w = np.ascontiguousarray(np.asarray(width_set, dtype=np.int32).reshape(-1))
+    handle = _vp(0)
+    if flags:
+        st = lib.spd_plan_create_ex(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, int(w.size),
+                                    int(max_width), int(flags))
+    else:
+        st = lib.spd_plan_create(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, int(w.size),
+                                 int(max_width))
+    _check(st)
+    return int(handle.value)
+
+
+def spd_plan_destroy(plan: int) -> None:
+    if plan:
+        load().spd_plan_destroy(_vp(plan))
+
+
+spd_destroy = spd_plan_destroy  # north_star's short name
+
+
+def spd_plan_get_widths(plan: int) -> np.ndarray:
+    lib = load()
+    n = _i32(0)
+    _check(lib.spd_plan_get_widths(_vp(plan), None, ctypes.byref(n)))
+    out = np.empty(n.value, dtype=np.int32)
+    _check(lib.spd_plan_get_widths(_vp(plan), out.ctypes.data, ctypes.byref(n)))
+    return out
+
+
+def spd_plan_get_info(plan: int) -> dict:
+    info = spd_plan_info()
+    _check(load().spd_plan_get_info(_vp(plan), ctypes.byref(info)))
+    return {name: int(getattr(info, name)) for name, _ in spd_plan_info._fields_}
+
+
+def _dev_ptr(t, dtype, numel: Optional[int], name: str) -> int:
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> int:
+    import torch
+    if stream is None:
+        return int(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+def spd_run(plan: int, plane, mean, sigma, out_snr, out_width, stream=None) -> None:
+    """Enqueue the hot path on device tensors (asynchronous on ``stream`` / torch's current stream)."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    _check(load().spd_run(
+        _vp(plan),
+        _dev_ptr(plane, torch.float32, n, "plane"),
+        _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
+        _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
+        _dev_ptr(out_snr, torch.float32, n, "out_snr"),
+        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _vp(_stream_handle(stream))))
+
+
+def spd_find_candidates(plan: int, out_snr, out_width, threshold: float, capacity: int, stream=None):
+    """Returns (list tensor uint8 [capacity*16] on the device, n_found int64 device tensor[1])."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    lst = torch.empty(max(int(capacity), 1) * ctypes.sizeof(spd_candidate), dtype=torch.uint8,
+                      device=out_snr.device)
+    n_found = torch.zeros(1, dtype=torch.int64, device=out_snr.device)
+    _check(load().spd_find_candidates(
+        _vp(plan), _dev_ptr(out_snr, torch.float32, n, "out_snr"),
+        _dev_ptr(out_width, torch.int32, n, "out_width"), ctypes.c_float(threshold),
+        _vp(lst.data_ptr()), int(capacity), _vp(n_found.data_ptr()), _vp(_stream_handle(stream))))
+    return lst, n_found
+
+
+def candidates_to_numpy(lst, n_found, capacity: int) -> Tuple[int, np.ndarray]:
+    """Synchronising helper: (count, structured array of the stored candidates sorted by (dm, t))."""
+    count = int(n_found.item())
+    k = min(count, int(capacity))
+    raw = lst[: k * ctypes.sizeof(spd_candidate)].cpu().numpy()
+    arr = raw.view(CANDIDATE_DTYPE).copy()
+    arr.sort(order=["dm", "t"])
+    return count, arr
+
+
+def _host_ptr(a, dtype, numel: int, name: str) -> Tuple[int, object]:
+    try:
+        import torch
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or not a.is_contiguous():
+                raise TypeError(f"{name} must be a contiguous CPU tensor or numpy array")
+            if a.numel() != numel:
+                raise ValueError(f"{name} has {a.numel()} elements, expected {numel}")
+            return a.data_ptr(), a
+    except ImportError:  # pragma: no cover
+        pass
+    arr = np.asarray(a)
+    if arr.dtype != dtype or not arr.flags.c_contiguous or arr.size != numel:
+        raise TypeError(f"{name} must be C-contiguous {dtype} with {numel} elements")
+    return arr.ctypes.data, arr
+
+
+def spd_run_host(plan: int, plane, mean, sigma, out_snr, out_width) -> None:
+    """End-to-end call on HOST buffers (blocking): H2D, kernels, D2H inside the library."""
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    p0, _k0 = _host_ptr(plane, np.float32, n, "plane")
+    p1, _k1 = _host_ptr(mean, np.float32, info["n_dm"], "mean")
+    p2, _k2 = _host_ptr(sigma, np.float32, info["n_dm"], "sigma")
+    p3, _k3 = _host_ptr(out_snr, np.float32, n, "out_snr")
+    p4, _k4 = _host_ptr(out_width, np.int32, n, "out_width")
+    _check(load().spd_run_host(_vp(plan), _vp(p0), _vp(p1), _vp(p2), _vp(p3), _vp(p4)))
+
+
+class Plan:
+    """Owns one ``spd_plan``; convenience wrapper over the functions above."""
+
+    def __init__(self, n_dm: int, n_t: int, width_set: Sequence[int], max_width: Optional[int] = None,
+                 flags: int = 0):
+        w = np.asarray(width_set, dtype=np.int32)
+        self.handle = spd_plan_create(n_dm, n_t, w, int(w.max()) if max_width is None else max_width, flags)
+        self.info = spd_plan_get_info(self.handle)
+        self.widths = spd_plan_get_widths(self.handle)
+        self.n_dm, self.n_t = int(n_dm), int(n_t)
+
+    def run(self, plane, mean, sigma, out_snr=None, out_width=None, stream=None):
+        import torch
+        if out_snr is None:
+            out_snr = torch.empty((self.n_dm, self.n_t), dtype=torch.float32, device=plane.device)
+        if out_width is None:
+            out_width = torch.empty((self.n_dm, self.n_t), dtype=torch.int32, device=plane.device)
+        spd_run(self.handle, plane, mean, sigma, out_snr, out_width, stream)
+        return out_snr, out_width
+
+    def find_candidates(self, out_snr, out_width, threshold: float, capacity: int, stream=None):
+        return spd_find_candidates(self.handle, out_snr, out_width, threshold, capacity, stream)
+
+    def run_host(self, plane, mean, sigma, out_snr, out_width):
+        spd_run_host(self.handle, plane, mean, sigma, out_snr, out_width)
+
+    def close(self):
+        if getattr(self, "handle", 0):
+            spd_plan_destroy(self.handle)
+            self.handle = 0
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

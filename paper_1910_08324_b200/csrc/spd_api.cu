@@ -1,0 +1,376 @@
+// C ABI of libspd_b200.so (include/spd.h): plans, width-set generators, dispatch,
+// the host-buffer entry point and error reporting.  All compute is in the kernels of
+// spd_tree.cu / spd_generic.cu / spd_candidates.cu; there is no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "spd_internal.h"
+
+namespace spd {
+
+static thread_local char g_error[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+    set_error("CUDA error while %s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-free error state
+    return SPD_ERR_CUDA;
+}
+
+namespace {
+
+// ---- width sets ------------------------------------------------------------------------
+// ALL: PAPER.md:193.  POW2: PAPER.md:311.  BOXDIT: eq. (14), D = 2 - iteration i
+// covers (2^i - 1) L_max + 2^i m, m = 1..L_max (example L_max = 4: 1,2,3,4 then 6,8,10,12,
+// PAPER.md:201).  IGRID: eq. (18) / Table 1, PAPER.md:364-387 - octave 2^i contributes
+// 2^i + j 2^(i-depth), j = 0 .. 2^depth - 1 (16 -> 16,24 | 16,20,24,28 | 16,18,..,30).
+int generate_widths(int32_t kind, int32_t param, int32_t max_width, std::vector<int32_t>& w) {
+    w.clear();
+    if (max_width < 1) {
+        set_error("max_width must be >= 1 (got %d)", max_width);
+        return SPD_ERR_INVALID_ARG;
+    }
+    switch (kind) {
+        case SPD_WIDTHS_ALL:
+            for (int64_t L = 1; L <= max_width; ++L) w.push_back(static_cast<int32_t>(L));
+            break;
+        case SPD_WIDTHS_POW2:
+            for (int64_t L = 1; L <= max_width; L *= 2) w.push_back(static_cast<int32_t>(L));
+            break;
+        case SPD_WIDTHS_BOXDIT: {
+            if (param < 1) {
+                set_error("BOXDIT needs param = L_max >= 1 (got %d)", param);
+                return SPD_ERR_INVALID_ARG;
+            }
+            for (int i = 0; i < 31; ++i) {
+                const int64_t step = int64_t(1) << i;
+                const int64_t base = (step - 1) * param;
+                if (base >= max_width) break;
+                for (int64_t m = 1; m <= param; ++m) {
+                    const int64_t L = base + step * m;
+                    if (L > max_width) break;
+                    w.push_back(static_cast<int32_t>(L));
+                }
+            }
+            break;
+        }
+        case SPD_WIDTHS_IGRID: {
+            if (param < 0 || param > 16) {
+                set_error("IGRID needs 0 <= param = depth <= 16 (got %d)", param);
+                return SPD_ERR_INVALID_ARG;
+            }
+            for (int64_t oct = 1; oct <= max_width; oct *= 2) {
+                const int64_t step = std::max<int64_t>(1, oct >> param);
+                for (int64_t L = oct; L < 2 * oct && L <= max_width; L += step) w.push_back(static_cast<int32_t>(L));
+            }
+            break;
+        }
+        case SPD_WIDTHS_GEOMETRIC: {
+            if (param <= 1000) {
+                set_error("GEOMETRIC needs param = 1000 * ratio > 1000 (got %d)", param);
+                return SPD_ERR_INVALID_ARG;
+            }
+            const double r = param / 1000.0;
+            for (double x = 1.0; nearbyint(x) <= max_width; x *= r) w.push_back(static_cast<int32_t>(nearbyint(x)));
+            break;
+        }
+        default:
+            set_error("unknown width-set kind %d", kind);
+            return SPD_ERR_INVALID_ARG;
+    }
+    std::sort(w.begin(), w.end());
+    w.erase(std::unique(w.begin(), w.end()), w.end());
+    return SPD_OK;
+}
+
+int check_device(int* device, int* sm_count) {
+    cudaError_t e = cudaGetDevice(device);
+    if (e != cudaSuccess) {
+        set_error("no usable CUDA device: %s (this library has no CPU fallback)", cudaGetErrorString(e));
+        cudaGetLastError();
+        return SPD_ERR_UNSUPPORTED_DEVICE;
+    }
+    int major = 0;
+    if ((e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, *device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(sm_count, cudaDevAttrMultiProcessorCount, *device)) != cudaSuccess) {
+        set_error("cannot query the CUDA device: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return SPD_ERR_UNSUPPORTED_DEVICE;
+    }
+    if (major != 10) {
+        set_error("device compute capability %d.x is not supported: this library is built for sm_100a only", major);
+        return SPD_ERR_UNSUPPORTED_DEVICE;
+    }
+    return SPD_OK;
+}
+
+void release_host_staging(spd_plan* plan) {
+    HostStaging& h = plan->host;
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(h.d_plane[i]);
+        cudaFree(h.d_snr[i]);
+        cudaFree(h.d_width[i]);
+        if (h.stream[i]) cudaStreamDestroy(h.stream[i]);
+        h.d_plane[i] = nullptr;
+        h.d_snr[i] = nullptr;
+        h.d_width[i] = nullptr;
+        h.stream[i] = nullptr;
+    }
+    cudaFree(h.d_mean);
+    cudaFree(h.d_sigma);
+    h.d_mean = h.d_sigma = nullptr;
+    h.ready = false;
+}
+
+int prepare_host_staging(spd_plan* plan) {
+    HostStaging& h = plan->host;
+    if (h.ready) return SPD_OK;
+    // Row blocks of about 256 MiB of input: large enough to run the device near its
+    // streaming rate, small enough that two of them (double buffering) cost 1.5 GiB.
+    const int64_t row_bytes = plan->n_t * 4;
+    h.rows_per_block = std::max<int64_t>(1, std::min<int64_t>(plan->n_dm, (int64_t(256) << 20) / row_bytes));
+    const size_t elems = static_cast<size_t>(h.rows_per_block) * static_cast<size_t>(plan->n_t);
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        if ((e = cudaStreamCreateWithFlags(&h.stream[i], cudaStreamNonBlocking)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&h.d_plane[i], elems * 4)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&h.d_snr[i], elems * 4)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&h.d_width[i], elems * 4)) != cudaSuccess) break;
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&h.d_mean, sizeof(float) * plan->n_dm);
+    if (e == cudaSuccess) e = cudaMalloc(&h.d_sigma, sizeof(float) * plan->n_dm);
+    if (e != cudaSuccess) {
+        set_error("allocating the host-run staging buffers failed: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        release_host_staging(plan);
+        return SPD_ERR_ALLOC;
+    }
+    h.ready = true;
+    return SPD_OK;
+}
+
+int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const float* mean, const float* sigma,
+             float* out_snr, int32_t* out_width, cudaStream_t stream) {
+    if (plan->path == SPD_PATH_DYADIC_TREE)
+        return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
+    return generic_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
+}
+
+}  // namespace
+}  // namespace spd
+
+using namespace spd;
+
+extern "C" {
+
+int spd_version(void) { return SPD_VERSION; }
+
+const char* spd_last_error_string(void) { return g_error; }
+
+int spd_width_set_generate(int32_t kind, int32_t param, int32_t max_width, int32_t* out, int32_t cap,
+                           int32_t* n_out) {
+    if (!n_out || cap < 0 || (cap > 0 && !out)) {
+        set_error("spd_width_set_generate: NULL output or negative capacity");
+        return SPD_ERR_INVALID_ARG;
+    }
+    std::vector<int32_t> w;
+    const int rc = generate_widths(kind, param, max_width, w);
+    if (rc != SPD_OK) return rc;
+    *n_out = static_cast<int32_t>(w.size());
+    if (cap == 0 && !out) return SPD_OK;  // size query
+    if (static_cast<size_t>(cap) < w.size()) {
+        set_error("spd_width_set_generate: capacity %d < %zu widths", cap, w.size());
+        return SPD_ERR_INVALID_ARG;
+    }
+    memcpy(out, w.data(), w.size() * sizeof(int32_t));
+    return SPD_OK;
+}
+
+int spd_plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set, int32_t n_widths,
+                    int32_t max_width) {
+    return spd_plan_create_ex(out, n_dm, n_t, width_set, n_widths, max_width, 0u);
+}
+
+int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set, int32_t n_widths,
+                       int32_t max_width, uint32_t flags) {
+    if (!out) {
+        set_error("spd_plan_create: out is NULL");
+        return SPD_ERR_INVALID_ARG;
+    }
+    *out = nullptr;
+    if (n_dm < 1 || n_t < 1 || n_t > 0x7fffffffll || n_dm > 0x7fffffffll) {
+        set_error("spd_plan_create: bad plane shape %lld x %lld", (long long)n_dm, (long long)n_t);
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (!width_set || n_widths < 1) {
+        set_error("spd_plan_create: empty width set");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (max_width < 1 || max_width > n_t) {
+        set_error("spd_plan_create: max_width %d must be in [1, n_t = %lld]", max_width, (long long)n_t);
+        return SPD_ERR_INVALID_ARG;
+    }
+    std::vector<int32_t> w(width_set, width_set + n_widths);
+    std::sort(w.begin(), w.end());
+    w.erase(std::unique(w.begin(), w.end()), w.end());
+    if (w.front() < 1 || w.back() > max_width) {
+        set_error("spd_plan_create: widths must lie in [1, max_width = %d] (got %d .. %d)", max_width, w.front(),
+                  w.back());
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (w.size() > 32768) {
+        set_error("spd_plan_create: more than 32768 distinct widths");
+        return SPD_ERR_INVALID_ARG;
+    }
+    int device = 0, sm_count = 0;
+    int rc = check_device(&device, &sm_count);
+    if (rc != SPD_OK) return rc;
+
+    spd_plan* plan = new (std::nothrow) spd_plan();
+    if (!plan) {
+        set_error("spd_plan_create: out of host memory");
+        return SPD_ERR_ALLOC;
+    }
+    plan->n_dm = n_dm;
+    plan->n_t = n_t;
+    plan->widths = w;
+    plan->max_width = max_width;
+    plan->device = device;
+    plan->sm_count = sm_count;
+    if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
+        plan->path = SPD_PATH_DYADIC_TREE;
+        rc = tree_configure(plan);
+    } else {
+        plan->path = SPD_PATH_GENERIC;
+        rc = generic_configure(plan);
+    }
+    if (rc != SPD_OK) {
+        delete plan;
+        return rc;
+    }
+    *out = plan;
+    return SPD_OK;
+}
+
+void spd_plan_destroy(spd_plan* plan) {
+    if (!plan) return;
+    release_host_staging(plan);
+    generic_release(plan);
+    delete plan;
+}
+
+int spd_plan_get_widths(const spd_plan* plan, int32_t* out, int32_t* n) {
+    if (!plan || !n) {
+        set_error("spd_plan_get_widths: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    *n = static_cast<int32_t>(plan->widths.size());
+    if (out) memcpy(out, plan->widths.data(), plan->widths.size() * sizeof(int32_t));
+    return SPD_OK;
+}
+
+int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
+    if (!plan || !info) {
+        set_error("spd_plan_get_info: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    memset(info, 0, sizeof(*info));
+    info->n_dm = plan->n_dm;
+    info->n_t = plan->n_t;
+    info->n_widths = static_cast<int32_t>(plan->widths.size());
+    info->max_width = plan->max_width;
+    info->path = plan->path;
+    if (plan->path == SPD_PATH_DYADIC_TREE) {
+        info->launches_per_run = 1;
+        info->threads_per_block = plan->tree.T;
+        info->blocks = static_cast<int32_t>(plan->n_dm * plan->tree.segs_per_row);
+        info->chunk = plan->tree.chunk;
+        info->segments_per_row = plan->tree.segs_per_row;
+        info->smem_bytes = static_cast<int64_t>(plan->tree.smem_bytes);
+    } else {
+        info->launches_per_run = 4;
+        info->threads_per_block = 256;
+        info->blocks = static_cast<int32_t>(plan->n_dm * ((plan->n_t + 255) / 256));
+    }
+    info->workspace_bytes = plan->workspace_bytes;
+    return SPD_OK;
+}
+
+int spd_run(const spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
+            int32_t* out_width, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma || !out_snr || !out_width) {
+        set_error("spd_run: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if ((reinterpret_cast<uintptr_t>(plane) | reinterpret_cast<uintptr_t>(out_snr) |
+         reinterpret_cast<uintptr_t>(out_width)) & 15u) {
+        set_error("spd_run: plane, out_snr and out_width must be 16-byte aligned");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width, float threshold,
+                        spd_candidate* list, int64_t capacity, int64_t* n_found, void* cuda_stream) {
+    if (!plan || !out_snr || !out_width || !n_found || capacity < 0 || (capacity > 0 && !list)) {
+        set_error("spd_find_candidates: NULL argument or negative capacity");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return candidates_run(plan, out_snr, out_width, threshold, list, capacity, n_found,
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
+                 int32_t* out_width) {
+    if (!plan || !plane || !mean || !sigma || !out_snr || !out_width) {
+        set_error("spd_run_host: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    int rc = prepare_host_staging(plan);
+    if (rc != SPD_OK) return rc;
+    HostStaging& h = plan->host;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(h.d_mean, mean, sizeof(float) * plan->n_dm, cudaMemcpyHostToDevice, h.stream[0])) !=
+            cudaSuccess ||
+        (e = cudaMemcpyAsync(h.d_sigma, sigma, sizeof(float) * plan->n_dm, cudaMemcpyHostToDevice, h.stream[0])) !=
+            cudaSuccess ||
+        (e = cudaStreamSynchronize(h.stream[0])) != cudaSuccess)
+        return cuda_fail(e, "copying mean / sigma to the device");
+    // The generic path shares one workspace, so its blocks run on one stream.
+    const int n_streams = plan->path == SPD_PATH_DYADIC_TREE ? 2 : 1;
+    int64_t blk = 0;
+    for (int64_t r0 = 0; r0 < plan->n_dm; r0 += h.rows_per_block, ++blk) {
+        const int64_t rows = std::min<int64_t>(h.rows_per_block, plan->n_dm - r0);
+        const int b = static_cast<int>(blk % 2);
+        cudaStream_t st = h.stream[blk % n_streams];
+        const size_t off = static_cast<size_t>(r0) * static_cast<size_t>(plan->n_t);
+        const size_t bytes = static_cast<size_t>(rows) * static_cast<size_t>(plan->n_t) * 4;
+        if (n_streams == 1 && blk >= 2) {
+            // buffer b was last used two blocks ago on the same stream: stream order suffices
+        }
+        if ((e = cudaMemcpyAsync(h.d_plane[b], plane + off, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+            return cuda_fail(e, "copying a row block to the device");
+        rc = run_rows(plan, rows, h.d_plane[b], h.d_mean + r0, h.d_sigma + r0, h.d_snr[b], h.d_width[b], st);
+        if (rc != SPD_OK) return rc;
+        if ((e = cudaMemcpyAsync(out_snr + off, h.d_snr[b], bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(out_width + off, h.d_width[b], bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+            return cuda_fail(e, "copying results to the host");
+    }
+    for (int i = 0; i < 2; ++i)
+        if ((e = cudaStreamSynchronize(h.stream[i])) != cudaSuccess) return cuda_fail(e, "waiting for the host run");
+    return SPD_OK;
+}
+
+}  // extern "C"

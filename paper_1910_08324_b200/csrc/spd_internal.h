@@ -1,0 +1,88 @@
+// Internal declarations shared by the translation units of libspd_b200.so.
+// Nothing here is part of the public C ABI (include/spd.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/spd.h"
+
+namespace spd {
+
+// Dyadic-tree geometry: a block of T threads owns "rows" of 4*T consecutive
+// samples, R = 4 rows per streaming step ("chunk").
+constexpr int kRowsPerChunk = 4;
+constexpr int kTreeMaxLevels = 16;  // widths 1 .. 32768
+constexpr int kStages = 3;          // bulk-copy ring depth
+
+struct TreeConfig {
+    int K = 0;            // number of widths: 2^0 .. 2^(K-1)
+    int T = 0;            // threads per block
+    int chunk = 0;        // 16 * T samples
+    int warm_chunks = 0;  // look-ahead chunks an interior segment replays
+    int segs_per_row = 1;
+    int seg_chunks = 0;   // chunks per segment
+    int chunks_per_row = 0;
+    int blocks_per_sm = 0;
+    size_t smem_bytes = 0;
+};
+
+struct HostStaging {
+    bool ready = false;
+    int64_t rows_per_block = 0;
+    cudaStream_t stream[2] = {nullptr, nullptr};
+    float* d_plane[2] = {nullptr, nullptr};
+    float* d_snr[2] = {nullptr, nullptr};
+    int32_t* d_width[2] = {nullptr, nullptr};
+    float* d_mean = nullptr;
+    float* d_sigma = nullptr;
+};
+
+}  // namespace spd
+
+struct spd_plan {
+    int64_t n_dm = 0, n_t = 0;
+    std::vector<int32_t> widths;
+    int32_t max_width = 0;
+    int32_t path = 0;
+    int device = 0;
+    int sm_count = 0;
+    // dyadic tree
+    spd::TreeConfig tree;
+    // generic path
+    int32_t* d_widths = nullptr;   // [n_widths]
+    float* d_wscale = nullptr;     // [n_widths] 1/sqrt(L)
+    double* d_prefix = nullptr;    // [n_dm][n_t + 1] running sums of (x - mu)
+    double* d_blocksum = nullptr;  // [n_dm][blocks_per_row]
+    int64_t generic_blocks_per_row = 0;
+    int64_t workspace_bytes = 0;
+    // spd_run_host
+    spd::HostStaging host;
+};
+
+namespace spd {
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);
+
+// spd_tree.cu
+bool tree_applicable(const std::vector<int32_t>& widths, int64_t n_t);
+int tree_configure(spd_plan* plan);
+int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
+             const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
+
+// spd_generic.cu
+int generic_configure(spd_plan* plan);
+void generic_release(spd_plan* plan);
+int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
+                const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
+
+// spd_candidates.cu
+int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+                   float threshold, spd_candidate* list, int64_t capacity, int64_t* n_found,
+                   cudaStream_t stream);
+
+}  // namespace spd
