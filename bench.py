@@ -1,0 +1,449 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the SPD hot path (arXiv:1910.08324) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload 3]
+
+One "step" = one pass of the whole hot path over one
+synthetic plane: spd_run (stage, mean removal, partial-sum tree, SNR, max/arg-max, store)
+followed by spd_find_candidates (threshold + peak list).  The default workload is
+BASELINE.json configs[2] ("SKA-MID-like", 4096 x 1,048,576 float32, widths {2^i <= 8192}),
+the configuration north_star's target is quoted on.  Prints ONE JSON line on rank 0.
+
+Multi-GPU: the path needs no exchange; under torchrun every rank
+runs the same per-GPU workload on its own DM trials (weak scaling, no data-path collective).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload; it is a deliberately slow program, reported for context.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "dm_time_samples_per_s"
+UNIT = "samples/s"
+BYTES_PER_SAMPLE = 12  # 4 read x + 4 write SNR + 4 write int32 width index
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+PAPER_SKA_SAMPLES_PER_S = 6000 * 15625  # "SKA-like" real-time load: 6000 DM trials/s at 64 us
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config number (1-based)")
+    ap.add_argument("--n-dm", type=int, default=0, help="override the number of DM trials (debugging)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the oracle sample")
+    return ap.parse_args()
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), \
+        int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def workload_config(w, widths, extra=None):
+    cfg = {
+        "workload": f"configs[{w.index - 1}] {w.name}: {w.n_dm} DM trials x {w.n_t} samples float32 per GPU",
+        "n_dm": w.n_dm, "n_t": w.n_t,
+        "width_set": f"{w.width_kind}<= {w.max_width} ({len(widths)} widths, every sample)",
+        "max_width": w.max_width, "sampling_time_s": w.sampling_time_s,
+        "n_pulses": w.n_pulses, "seed": w.seed,
+        "l2": "inputs larger than L2 (plane and outputs are each >= 8 GiB; no flush needed)"
+        if w.n_samples * 4 > (1 << 30) else "plane fits L2: rotating buffers larger than L2",
+    }
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+# ----------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the b200 arm; the whole of --impl reference)
+# ----------------------------------------------------------------------------------------
+def oracle_sample_plan(w, widths, target_s):
+    """Pick rows x samples of the workload so that the direct-summation oracle takes about
+    target_s seconds: calibrate on a small window first."""
+    import numpy as np
+    import oracle
+    from workloads import make_plane_numpy
+    oracle.build()
+    cores = oracle.num_threads()
+    n_t = min(w.n_t, 1 << 20)
+    rows = max(1, min(w.n_dm, cores))
+    sub = w.scaled(rows, n_t, max(1, min(w.n_pulses, rows)))
+    x, _ = make_plane_numpy(sub)
+    cal = min(n_t - w.max_width, 4096 * max(1, 64 // max(1, len(widths))))
+    cal = max(256, min(cal, 1 << 16))
+    t = time.perf_counter()
+    oracle.spd_direct(x, 0.0, 1.0, widths, 0, cal)
+    dt = max(time.perf_counter() - t, 1e-4)
+    rate = rows * cal / dt
+    span = int(min(n_t, max(cal, rate * target_s / rows)))
+    return x, rows, span, cores
+
+
+def time_oracle(w, widths, target_s, steps=1, warmup=0):
+    import numpy as np
+    import oracle
+    x, rows, span, cores = oracle_sample_plan(w, widths, target_s / max(1, steps + warmup))
+    times = []
+    for i in range(warmup + steps):
+        t = time.perf_counter()
+        oracle.spd_direct(x, 0.0, 1.0, widths, 0, span)
+        dt = time.perf_counter() - t
+        if i >= warmup:
+            times.append(dt)
+    n = rows * span
+    direct = n * len(times) / sum(times)
+    t = time.perf_counter()
+    oracle.spd_prefix(x, 0.0, 1.0, widths)
+    prefix = x.size / (time.perf_counter() - t)
+    sample = (f"oracle_spd_direct (double, direct summation, OpenMP) on the first {span} samples of {rows} rows "
+              f"of the same recipe ({n} samples per step); prefix_value = oracle_spd_prefix on {rows} x {x.shape[1]}")
+    return {"value": direct, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+            "prefix_value": prefix, "ms_per_step": 1e3 * sum(times) / len(times), "samples_per_step": n}
+
+
+def oracle_widths(w):
+    from oracle import formulas
+    return formulas.width_set(w.width_kind, w.width_param, w.max_width)
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from workloads import get_workload
+    w = get_workload(args.workload)
+    widths = oracle_widths(w)
+    # bounded: the whole --steps/--warmup run is sized to about 4 * cpu_seconds
+    res = time_oracle(w, widths, 4.0 * args.cpu_seconds, steps=args.steps, warmup=args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, widths, {"sample_per_step": res["sample"]}),
+        "cpu_baseline": {"value": res["value"], "unit": UNIT, "cores": res["cores"], "kind": "oracle",
+                         "sample": res["sample"]},
+        "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+        "real_time_factor_ska_like": res["value"] / PAPER_SKA_SAMPLES_PER_S,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------------
+# clocks sampling (the profiling recipe's clocks line) during the timed region
+# ----------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows = []
+        self.proc = None
+        self.gpu_index = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        inside = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.06] or [r for (_, r) in self.rows[-3:]]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in inside:
+            f = [v.strip() for v in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except (OSError, KeyError, ValueError):
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------------
+# the B200 arm
+# ----------------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+    import paper_1910_08324_b200 as spd
+    from workloads import get_workload, make_plane_torch
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the SPD path has no CPU fallback (use --impl reference "
+                         "for the oracle timing)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    distributed = world > 1
+    if distributed:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    spd.build()
+    w = get_workload(args.workload)
+    if args.n_dm:
+        w = w.scaled(args.n_dm, w.n_t)
+    # weak scaling: every rank holds its own n_dm DM trials (different seed per rank)
+    from dataclasses import replace
+    w_rank = replace(w, seed=w.seed + 1000003 * rank)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    n = w.n_samples
+
+    plane, pulses = make_plane_torch(w_rank, dev)
+    mean = torch.zeros(w.n_dm, dtype=torch.float32, device=dev)
+    sigma = torch.ones(w.n_dm, dtype=torch.float32, device=dev)
+    if w.stats == "measured":  # reading A6, computed once outside the timed region
+        mean = plane.double().mean(dim=1).float()
+        sigma = plane.double().std(dim=1, unbiased=False).float()
+    out_snr = torch.empty((w.n_dm, w.n_t), dtype=torch.float32, device=dev)
+    out_width = torch.empty((w.n_dm, w.n_t), dtype=torch.int32, device=dev)
+    thr = w.candidate_threshold if w.candidate_threshold is not None else 6.0
+    cap = 1 << 22
+    plan = spd.Plan(w.n_dm, w.n_t, widths, w.max_width)
+    info = plan.info
+    # planes smaller than L2 would be re-read from cache: flush between steps
+    need_flush = 3 * n * 4 <= (512 << 20)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if need_flush else None
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if flush is not None:
+            flush.fill_(1)
+        if ev is not None:
+            ev[0].record(stream)
+        plan.run(plane, mean, sigma, out_snr, out_width)
+        if ev is not None:
+            ev[1].record(stream)
+        lst, n_found = plan.find_candidates(out_snr, out_width, thr, cap)
+        if ev is not None:
+            ev[2].record(stream)
+        return lst, n_found
+
+    def barrier():
+        if distributed:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+
+    uuid = None
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+    except Exception:
+        pass
+    sampler = ClockSampler(uuid if uuid else local_rank)
+    sampler.start()
+    time.sleep(0.15)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    e_beg.record(stream)
+    for i in range(args.steps):
+        lst, n_found = step(evs[i])
+    e_end.record(stream)
+    barrier()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    total_ms = e_beg.elapsed_time(e_end)
+    run_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    cand_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    flush_ms = 0.0
+    if flush is not None:  # the flush is not part of the path: take it out of the step time
+        flush_ms = total_ms - sum(run_ms) - sum(cand_ms)
+        total_ms = sum(run_ms) + sum(cand_ms)
+    if distributed:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+    n_cand = int(n_found.item())
+
+    # ---- roofline of the dominant kernel (the spd_run kernel) ---------------------------
+    peak, peak_src = measured_peak()
+    k_ms = sum(run_ms) / len(run_ms)
+    achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
+    roofline = {
+        "bound": "hbm", "kernel": "spd_tree_kernel" if info["path"] == spd.SPD_PATH_DYADIC_TREE else "generic_eval",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),
+        "algorithmic_bytes_per_launch": BYTES_PER_SAMPLE * n, "bytes_per_sample": BYTES_PER_SAMPLE,
+        "kernel_ms": k_ms, "kernel_ms_min": min(run_ms), "candidates_ms": sum(cand_ms) / len(cand_ms),
+        "kernel_share_of_step": sum(run_ms) / (sum(run_ms) + sum(cand_ms)),
+    }
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(w, widths, {
+            "parallelism": f"dm-rows x{world} (independent DM trials per GPU, no collective)",
+            "path": "dyadic_tree" if info["path"] == spd.SPD_PATH_DYADIC_TREE else "generic",
+            "blocks": info["blocks"], "threads_per_block": info["threads_per_block"],
+            "segments_per_row": info["segments_per_row"], "chunk": info["chunk"], "smem_bytes": info["smem_bytes"],
+            "candidate_threshold": thr, "candidates_found": n_cand}),
+        "roofline": roofline,
+        "clocks": clocks,
+        "gpu_launches": args.steps * (info["launches_per_run"] + 1),
+        "real_time_factor_plane": (w.n_t * w.sampling_time_s) / (ms_per_step * 1e-3),
+        "real_time_factor_ska_like": value / PAPER_SKA_SAMPLES_PER_S,
+        "n_dm_real_time": value * w.sampling_time_s,
+        "hbm_gbs_whole_step": (BYTES_PER_SAMPLE + 4) * n / (ms_per_step * 1e-3) / 1e9,
+    }
+    if flush is not None:
+        line["config"]["l2_flush_ms_per_step_excluded"] = flush_ms / args.steps
+
+    # ---- end to end through the C ABI with HOST buffers (spd_run_host) -----------------
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev)
+    else:
+        line["e2e"] = None
+
+    del plane, out_snr, out_width
+    plan.close()
+
+    # ---- CPU oracle on the same box (rank 0, N=1 only) ----------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        res = time_oracle(w, oracle_widths(w), args.cpu_seconds)
+        line["cpu_baseline"] = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample", "prefix_value")}
+    else:
+        line["cpu_baseline"] = None
+
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if distributed:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of the dominant
+# kernel from the committed `ncu --set full` capture, per workload; None until captured.
+# Source files: profiles/ (see profiles/README.md).
+NCU_TRAFFIC_BYTES = {}
+
+
+def ncu_traffic_bytes(w):
+    return NCU_TRAFFIC_BYTES.get((w.index, w.n_dm))
+
+
+def host_mem_available_bytes():
+    try:
+        with open("/proc/meminfo") as f:
+            for ln in f:
+                if ln.startswith("MemAvailable:"):
+                    return int(ln.split()[1]) * 1024
+    except OSError:
+        pass
+    return 8 << 30
+
+
+def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
+    """Same metric through spd_run_host: pinned HOST plane in, HOST SNR / width planes out,
+    every copy inside the timed region (wall clock around the blocking call, max over ranks)."""
+    import torch
+    # rows: the whole plane when host memory allows 12 B/sample of pinned buffers per rank
+    budget = host_mem_available_bytes() // (3 * max(1, world))
+    rows = int(max(1, min(w.n_dm, budget // (BYTES_PER_SAMPLE * w.n_t))))
+    n = rows * w.n_t
+    h_plane = torch.empty((rows, w.n_t), dtype=torch.float32, pin_memory=True)
+    h_plane.copy_(plane[:rows])
+    h_mean = mean[:rows].cpu()
+    h_sigma = sigma[:rows].cpu()
+    h_snr = torch.empty((rows, w.n_t), dtype=torch.float32, pin_memory=True)
+    h_width = torch.empty((rows, w.n_t), dtype=torch.int32, pin_memory=True)
+    torch.cuda.synchronize()
+    times = []
+    with spd.Plan(rows, w.n_t, widths, w.max_width) as plan:
+        for i in range(1 + max(1, args.e2e_steps)):
+            if distributed:
+                torch.distributed.barrier()
+            torch.cuda.synchronize()
+            t = time.perf_counter()
+            plan.run_host(h_plane, h_mean, h_sigma, h_snr, h_width)
+            dt = time.perf_counter() - t
+            if i > 0:
+                times.append(dt)
+    dt = sum(times) / len(times)
+    if distributed:
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        dt = float(t.item())
+    checksum = float(h_snr[0, :1024].double().sum().item())
+    return {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": 4 * n + 8 * rows,
+            "d2h_bytes_per_step": 8 * n, "ms_per_step": 1e3 * dt, "steps": len(times), "rows": rows,
+            "api": "spd_run_host (pinned host buffers; H2D, kernels and D2H of Y and W inside the call)",
+            "note": "whole plane" if rows == w.n_dm else f"first {rows} of {w.n_dm} DM trials (host memory bound)",
+            "checksum": checksum}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

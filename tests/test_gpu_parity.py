@@ -1,0 +1,313 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element,
+on the same seeded inputs.  Sizes here are ones the oracle finishes in seconds; the
+full BASELINE.json sizes are in test_gpu_full_size.py.
+"""
+import numpy as np
+import pytest
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def spd():
+    import paper_1910_08324_b200 as spd
+    spd.build()
+    spd.load()
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return spd
+
+
+def run_gpu(spd, x: np.ndarray, mu, sg, widths, max_width=None, flags=0):
+    """One spd_run through the binding; returns (snr f32, idx i32) numpy arrays and plan info."""
+    n_dm, n_t = x.shape
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(dev)
+    mean = torch.from_numpy(np.broadcast_to(np.asarray(mu, dtype=np.float32), (n_dm,)).copy()).to(dev)
+    sigma = torch.from_numpy(np.broadcast_to(np.asarray(sg, dtype=np.float32), (n_dm,)).copy()).to(dev)
+    with spd.Plan(n_dm, n_t, widths, max_width, flags) as plan:
+        snr, idx = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+        return snr.cpu().numpy(), idx.cpu().numpy(), dict(plan.info)
+
+
+def check(spd, oracle, x, mu, sg, widths, what, direct=False, flags=0, expect_path=None):
+    got_snr, got_idx, info = run_gpu(spd, x, mu, sg, widths, flags=flags)
+    if expect_path is not None:
+        assert info["path"] == expect_path, f"{what}: plan took path {info['path']}"
+    # both sides see the float32-rounded mu / sigma the C ABI takes
+    mu64 = np.broadcast_to(np.asarray(mu, dtype=np.float32), (x.shape[0],)).astype(np.float64)
+    sg64 = np.broadcast_to(np.asarray(sg, dtype=np.float32), (x.shape[0],)).astype(np.float64)
+    fn = oracle.spd_direct if direct else oracle.spd_prefix
+    ref_snr, ref_idx, ref_sec = fn(x, mu64, sg64, widths)
+    return parity.assert_parity(oracle, x, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                                what=what)
+
+
+def test_config1_tiny_lossless_full_plane(spd, oracle_lib):
+    """BASELINE.json configs[0], whole plane, against the direct-summation oracle."""
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(1)
+    x, _ = make_plane_numpy(w)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    assert list(widths) == list(range(1, 65))
+    st = check(spd, oracle_lib, x, 0.0, 1.0, widths, "config1/all-widths", direct=True,
+               expect_path=spd.SPD_PATH_GENERIC)
+    assert st.n == 64 * 16384
+
+
+def test_config1_plane_dyadic_set_direct_oracle(spd, oracle_lib):
+    from workloads import get_workload, make_plane_numpy
+    x, _ = make_plane_numpy(get_workload(1))
+    widths = spd.spd_width_set_generate("POW2", 0, 64)
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, "config1/pow2", direct=True, expect_path=spd.SPD_PATH_DYADIC_TREE)
+
+
+@pytest.mark.parametrize("K", list(range(1, 17)))
+def test_dyadic_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
+    """Every kernel instantiation (widths 1..2^(K-1)); n_t spans several chunks plus a ragged
+    tail that is not a multiple of the chunk; several segments per row so that interior
+    segments replay their look-ahead."""
+    M = 1 << (K - 1)
+    T = 128 if K <= 14 else (256 if K == 15 else 512)
+    chunk = 16 * T
+    n_t = max(5 * chunk + 4 * 37, 2 * M + chunk + 4 * 5)
+    rng = np.random.default_rng(1000 + K)
+    x = rng.standard_normal((3, n_t), dtype=np.float32)
+    x[1, n_t // 3: n_t // 3 + max(1, M // 2)] += np.float32(12.0 / np.sqrt(max(1, M // 2)))
+    x[2, n_t - M // 2 - 3:] += np.float32(0.7)  # a pulse running off the end of the row
+    monkeypatch.setenv("SPD_SEGS_PER_ROW", "3")
+    widths = [1 << k for k in range(K)]
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"tree K={K}", expect_path=spd.SPD_PATH_DYADIC_TREE)
+
+
+@pytest.mark.parametrize("segs", [1, 2, 7])
+def test_dyadic_tree_segmentation_is_invisible(spd, oracle_lib, segs, monkeypatch):
+    rng = np.random.default_rng(77)
+    n_t = 2048 * 23 + 4 * 3
+    x = rng.standard_normal((2, n_t), dtype=np.float32)
+    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(segs))
+    check(spd, oracle_lib, x, 0.0, 1.0, [1 << k for k in range(12)], f"tree segs={segs}")
+
+
+def test_small_lossy_measured_statistics(spd, oracle_lib):
+    """Config-2 recipe on a reduced plane: mu, sigma measured by the oracle's definition
+    (reading A6) on data with a large offset and scale."""
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(2).scaled(16, 65536, 8)
+    x, _ = make_plane_numpy(w)
+    x = (x * np.float32(3.7) + np.float32(41.5)).astype(np.float32)
+    mu, sg = oracle_lib.row_stats(x)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    check(spd, oracle_lib, x, mu, sg, widths, "config2-recipe/tree")
+    check(spd, oracle_lib, x, mu, sg, widths, "config2-recipe/generic", flags=spd.SPD_FLAG_FORCE_GENERIC,
+          expect_path=spd.SPD_PATH_GENERIC)
+
+
+@pytest.mark.parametrize("kind,param,max_width", [("IGRID", 1, 256), ("IGRID", 2, 512), ("BOXDIT", 8, 300),
+                                                    ("GEOMETRIC", 1800, 1000), ("ALL", 0, 37)])
+def test_generic_width_sets(spd, oracle_lib, kind, param, max_width):
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal((5, 10007), dtype=np.float32)  # n_t odd: tree not applicable anyway
+    x[2, 5000:5100] += np.float32(1.5)
+    widths = spd.spd_width_set_generate(kind, param, max_width)
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"generic {kind}({param})<= {max_width}",
+          expect_path=spd.SPD_PATH_GENERIC)
+
+
+def test_width_set_generators_agree_with_formula_module(spd):
+    from oracle import formulas
+    for kind, param, mw in [("ALL", 0, 64), ("POW2", 0, 8192), ("BOXDIT", 4, 12), ("BOXDIT", 8, 8192),
+                            ("IGRID", 1, 8192), ("IGRID", 3, 32768), ("GEOMETRIC", 1800, 8192)]:
+        assert list(spd.spd_width_set_generate(kind, param, mw)) == formulas.width_set(kind, param, mw), (kind, param)
+
+
+def test_tail_rule_without_width_one(spd, oracle_lib):
+    """Reading A3: widths that do not fit are skipped; with 1 not in the set the last samples
+    have no valid width: -inf / -1."""
+    rng = np.random.default_rng(9)
+    x = rng.standard_normal((2, 64), dtype=np.float32)
+    got_snr, got_idx, _ = run_gpu(spd, x, 0.0, 1.0, [4, 8])
+    assert np.all(np.isneginf(got_snr[:, 61:])) and np.all(got_idx[:, 61:] == -1)
+    check(spd, oracle_lib, x, 0.0, 1.0, [4, 8], "tail/no-width-1", direct=True)
+
+
+@pytest.mark.parametrize("n_t", [4, 8, 64, 2044, 2048, 2052])
+def test_tiny_and_chunk_boundary_lengths(spd, oracle_lib, n_t):
+    rng = np.random.default_rng(n_t)
+    x = rng.standard_normal((1, n_t), dtype=np.float32)
+    K = min(4, int(np.log2(n_t)) + 1)
+    check(spd, oracle_lib, x, 0.0, 1.0, [1 << k for k in range(K)], f"tree n_t={n_t}", direct=True,
+          expect_path=spd.SPD_PATH_DYADIC_TREE)
+
+
+def test_max_width_equals_row_length(spd, oracle_lib):
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((2, 4096), dtype=np.float32)
+    check(spd, oracle_lib, x, 0.0, 1.0, [1 << k for k in range(13)], "tree M == n_t", direct=True)
+
+
+def test_exact_ties_take_the_smallest_width(spd, oracle_lib):
+    """Zero background (every SNR exactly 0) and a noise-free pulse: exact ties resolve to
+    the smallest width on both paths (reading A4)."""
+    n_t = 8192
+    x = np.zeros((2, n_t), dtype=np.float32)
+    x[1, 1000:1016] = np.float32(2.0)
+    for f in (0, spd.SPD_FLAG_FORCE_GENERIC):
+        got_snr, got_idx, _ = run_gpu(spd, x, 0.0, 1.0, [1, 2, 4, 8, 16, 32, 64], flags=f)
+        assert np.all(got_snr[0] == 0.0) and np.all(got_idx[0, : n_t - 64] == 0)
+        ref_snr, ref_idx, ref_sec = oracle_lib.spd_direct(x, 0.0, 1.0, [1, 2, 4, 8, 16, 32, 64])
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, [1, 2, 4, 8, 16, 32, 64], got_snr, got_idx, ref_snr,
+                             ref_idx, ref_sec, what=f"ties flags={f}")
+        # exact comparison of the index on the noise-free plane, away from float near-ties:
+        # dyadic sums of 2.0 are exact in fp32, so the decision is exact on both sides
+        assert np.array_equal(got_idx, ref_idx)
+
+
+def test_constant_offset_closed_form(spd):
+    """x = mu + a: SNR_L = a sqrt(L) / sigma, so the largest width that fits wins (pin P10)."""
+    n_t, a, sg = 4096, 0.25, 2.0
+    x = np.full((1, n_t), 10.0 + a, dtype=np.float32)
+    widths = [1 << k for k in range(9)]
+    got_snr, got_idx, _ = run_gpu(spd, x, 10.0, sg, widths)
+    room = n_t - np.arange(n_t)
+    exp_idx = np.minimum(8, np.floor(np.log2(room)).astype(np.int64))
+    exp_snr = a * np.sqrt(2.0 ** exp_idx) / sg
+    assert np.array_equal(got_idx[0], exp_idx)
+    assert np.all(np.abs(got_snr[0] - exp_snr) <= 1e-4 * np.maximum(1, exp_snr))
+
+
+@pytest.mark.parametrize("cfg,n_dm,n_t,n_pulses", [(2, 8, 32768, 16), (3, 4, 262144, 12), (4, 2, 524288, 6)])
+def test_noise_free_twin_loss_matches_eq24(spd, cfg, n_dm, n_t, n_pulses):
+    """Pin P14 through the CUDA path: on a zero-background plane each injected rectangular
+    pulse is recovered at exactly eq. (24)'s fraction of its true SNR,
+    and the mean loss equals the formula's mean over the injected widths."""
+    from oracle import formulas
+    from workloads import get_workload, make_pulse_only_plane_numpy
+    w = get_workload(cfg).scaled(n_dm, n_t, n_pulses)
+    x, pulses = make_pulse_only_plane_numpy(w)
+    widths = list(spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width))
+    got_snr, _, _ = run_gpu(spd, x, 0.0, 1.0, widths)
+    losses, predicted = [], []
+    for p in pulses:
+        others = [q for q in pulses if q is not p and q.dm == p.dm and
+                  abs(q.t0 - p.t0) < 2 * w.max_width + p.width + q.width]
+        if others:
+            continue  # overlapping pulses do not follow the single-pulse formula
+        lo, hi = max(0, p.t0 - w.max_width), min(n_t, p.t0 + p.width + 1)
+        rec = float(got_snr[p.dm, lo:hi].max()) / p.snr_t
+        exp = formulas.rsnr_max(p.width, widths)
+        assert abs(rec - exp) <= 2e-4, (p, rec, exp)
+        losses.append(1.0 - rec)
+        predicted.append(1.0 - exp)
+    assert len(losses) >= n_pulses // 2
+    assert abs(np.mean(losses) - np.mean(predicted)) <= 1e-4
+
+
+def test_candidates_match_rule_on_cuda_plane(spd, oracle_lib):
+    """Row a8: on the SNR plane the CUDA path produced, the candidate list equals the
+    reading-A9 rule evaluated by the oracle on that same float32 plane - bit-exact."""
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(5).scaled(4, 262144, 24)
+    x, _ = make_plane_numpy(w)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean = torch.zeros(4, device=dev)
+    sigma = torch.ones(4, device=dev)
+    with spd.Plan(4, 262144, widths) as plan:
+        snr, idx = plan.run(plane, mean, sigma)
+        cap = 1 << 16
+        lst, n_found = plan.find_candidates(snr, idx, 6.0, cap)
+        count, got = spd.candidates_to_numpy(lst, n_found, cap)
+        snr_h, idx_h = snr.cpu().numpy(), idx.cpu().numpy()
+        ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr_h, idx_h, 6.0)
+        assert count == ref_count and count > 0
+        assert np.array_equal(got["dm"], c_dm) and np.array_equal(got["t"], c_t)
+        assert np.array_equal(got["snr"], c_snr) and np.array_equal(got["width_idx"], c_w)
+        # overflow: the count keeps running past a small capacity
+        lst2, n2 = plan.find_candidates(snr, idx, 6.0, 5)
+        count2, got2 = spd.candidates_to_numpy(lst2, n2, 5)
+        assert count2 == ref_count and len(got2) == 5
+
+
+def test_candidates_against_oracle_plane_tolerance_aware(spd, oracle_lib):
+    """Candidates of the CUDA planes vs candidates of the ORACLE's planes (reading A9's
+    tolerance-aware rule): every oracle candidate clear of the threshold has a CUDA candidate
+    in the same row within +-width samples and SNR tolerance, and vice versa."""
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(2).scaled(8, 65536, 16)
+    x, _ = make_plane_numpy(w)
+    widths = list(spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width))
+    thr = 6.0
+    dev = torch.device("cuda:0")
+    with spd.Plan(8, 65536, widths) as plan:
+        snr, idx = plan.run(torch.from_numpy(x).to(dev), torch.zeros(8, device=dev), torch.ones(8, device=dev))
+        lst, n_found = plan.find_candidates(snr, idx, thr, 1 << 16)
+        count, got = spd.candidates_to_numpy(lst, n_found, 1 << 16)
+    ref_snr, ref_idx, _ = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    _, o_dm, o_t, o_snr, o_w = oracle_lib.find_candidates(ref_snr.astype(np.float32), ref_idx, thr)
+    assert count > 0 and len(o_dm) > 0
+
+    def covered(a_dm, a_t, a_snr, a_w, b_dm, b_t, b_snr):
+        for d, t, s, k in zip(a_dm, a_t, a_snr, a_w):
+            tol = parity.SNR_RTOL * max(1.0, abs(float(s)))
+            if s < thr + 2 * tol:
+                continue
+            m = (b_dm == d) & (np.abs(b_t - t) <= widths[k]) & (np.abs(b_snr - s) <= 2 * tol)
+            assert m.any(), f"candidate (dm={d}, t={t}, snr={s}, width={widths[k]}) has no counterpart"
+
+    covered(o_dm, o_t, o_snr, o_w, got["dm"], got["t"], got["snr"])
+    covered(got["dm"], got["t"], got["snr"], got["width_idx"], o_dm, o_t, o_snr)
+
+
+def test_run_host_equals_device_run(spd):
+    """The end-to-end host entry point (several row blocks) returns exactly what spd_run does."""
+    rng = np.random.default_rng(11)
+    n_dm, n_t = 6, 1 << 20
+    x = rng.standard_normal((n_dm, n_t), dtype=np.float32)
+    mu = rng.standard_normal(n_dm).astype(np.float32) * 0.01
+    sg = (1.0 + 0.1 * rng.random(n_dm)).astype(np.float32)
+    widths = [1 << k for k in range(14)]
+    got_snr, got_idx, _ = run_gpu(spd, x, mu, sg, widths)
+    out_snr = np.empty((n_dm, n_t), dtype=np.float32)
+    out_idx = np.empty((n_dm, n_t), dtype=np.int32)
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        plan.run_host(x, mu, sg, out_snr, out_idx)
+    assert np.array_equal(out_snr, got_snr) and np.array_equal(out_idx, got_idx)
+
+
+def test_concurrent_streams_share_a_plan(spd):
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal((8, 65536), dtype=np.float32)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(8, device=dev), torch.ones(8, device=dev)
+    with spd.Plan(8, 65536, [1 << k for k in range(10)]) as plan:
+        a = plan.run(plane, mean, sigma)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s1):
+            b = plan.run(plane, mean, sigma, stream=s1)
+        with torch.cuda.stream(s2):
+            c = plan.run(plane, mean, sigma, stream=s2)
+        torch.cuda.synchronize()
+        assert torch.equal(a[0], b[0]) and torch.equal(a[0], c[0])
+        assert torch.equal(a[1], b[1]) and torch.equal(a[1], c[1])
+
+
+def test_invalid_arguments_fail_loudly(spd):
+    with pytest.raises(spd.SpdError):
+        spd.spd_plan_create(4, 1024, [], 8)
+    with pytest.raises(spd.SpdError):
+        spd.spd_plan_create(4, 1024, [0, 2], 8)
+    with pytest.raises(spd.SpdError):
+        spd.spd_plan_create(4, 1024, [16], 8)      # width above max_width
+    with pytest.raises(spd.SpdError):
+        spd.spd_plan_create(4, 64, [1, 2], 128)    # max_width above n_t
+    with pytest.raises(spd.SpdError):
+        spd.spd_width_set_generate(99, 0, 8)
+    assert "unknown" in spd.spd_last_error_string()
