@@ -220,9 +220,10 @@ def test_candidates_match_rule_on_cuda_plane(spd, oracle_lib):
     sigma = torch.ones(4, device=dev)
     with spd.Plan(4, 262144, widths) as plan:
         snr, idx = plan.run(plane, mean, sigma)
-        cap = 1 << 16
+        cap = 1 << 20  # the config-5 drift floods the threshold: stay below capacity
         lst, n_found = plan.find_candidates(snr, idx, 6.0, cap)
         count, got = spd.candidates_to_numpy(lst, n_found, cap)
+        assert count <= cap
         snr_h, idx_h = snr.cpu().numpy(), idx.cpu().numpy()
         ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr_h, idx_h, 6.0)
         assert count == ref_count and count > 0
