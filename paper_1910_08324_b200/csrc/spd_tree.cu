@@ -17,8 +17,9 @@
 //     line instead of re-reading a (max_width - 1)-sample halo per tile.  The halo is
 //     paid once per segment (warm-up chunks), not once per tile.
 //   * Thread t owns, in each of the chunk's 4 "rows" of 4*T samples, the 4 consecutive
-//     samples 4t..4t+3 (one float4).  Levels 2^k < 4: in the thread's own registers.
-//     Levels 4 <= 2^k <= 2T: the partner belongs to another thread - exchanged through
+//     samples 4t..4t+3 (one float4).  Widths 2, 4, 8: in the thread's own registers from
+//     three float4 of raw samples (the width-4 sums of the next float4 are recomputed
+//     rather than exchanged).  Levels 8 <= 2^k <= 2T: the partner belongs to another thread - exchanged through
 //     a ping-pong shared-memory buffer with 128-bit accesses, one __syncthreads() each.
 //     Levels 2^k >= 4T: the partner is the SAME thread's float4 1, 2, 4 or 8 rows later,
 //     i.e. a register of this chunk or a delay register kept from the previous chunks.
@@ -52,6 +53,9 @@ struct TreeParams {
     int seg_chunks;
     int segs_per_row;
     int warm_chunks;
+    // ~kCodeMask, passed at run time on purpose: as a compile-time constant the tag
+    // (v & mask) | code has two immediates and costs two LOP3 per value instead of one.
+    uint32_t tag_mask;
 };
 
 // ------------------------------------------------------------------------------------
@@ -114,12 +118,13 @@ __device__ __forceinline__ float4 scale4(float4 a, float c) {
     const float2 hi = __fmul2_rn(make_float2(a.z, a.w), cc);
     return make_float4(lo.x, lo.y, hi.x, hi.y);
 }
-// (x - mu) * (1 / sigma): two roundings, no cancellation for large mu / sigma.
-__device__ __forceinline__ float4 norm4(float4 a, float mu, float inv) {
+// x - mu (eq. 4 numerator per sample; exact-ish, no cancellation later).  The division by
+// sigma is applied once per output sample at the store, not per input sample here.
+__device__ __forceinline__ float4 norm4(float4 a, float mu) {
     const float2 m = make_float2(-mu, -mu);
     const float2 lo = __fadd2_rn(make_float2(a.x, a.y), m);
     const float2 hi = __fadd2_rn(make_float2(a.z, a.w), m);
-    return scale4(make_float4(lo.x, lo.y, hi.x, hi.y), inv);
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
 }
 
 // 2^(-k/2): SNR scale of width 2^k on unit-variance data (eq. 5).
@@ -133,18 +138,18 @@ constexpr uint32_t kCodeMask = (1u << kCodeBits) - 1u;
 
 // SNR of level k with the inverted width index in the low mantissa bits.
 template <int k>
-__device__ __forceinline__ float pack1(float v) {
-    return __uint_as_float((__float_as_uint(v) & ~kCodeMask) | (kCodeMask - static_cast<uint32_t>(k)));
+__device__ __forceinline__ float pack1(float v, uint32_t tm) {
+    return __uint_as_float((__float_as_uint(v) & tm) | (kCodeMask - static_cast<uint32_t>(k)));
 }
 template <int k>
-__device__ __forceinline__ float4 key4(float4 p) {
+__device__ __forceinline__ float4 key4(float4 p, uint32_t tm) {
     const float4 v = scale4(p, level_scale<k>());
-    return make_float4(pack1<k>(v.x), pack1<k>(v.y), pack1<k>(v.z), pack1<k>(v.w));
+    return make_float4(pack1<k>(v.x, tm), pack1<k>(v.y, tm), pack1<k>(v.z, tm), pack1<k>(v.w, tm));
 }
 // Guarded variant: element v of the float4 is valid iff 2^k <= lim - v (reading A3).
 template <int k>
-__device__ __forceinline__ float4 key4_masked(float4 p, int lim) {
-    float4 q = key4<k>(p);
+__device__ __forceinline__ float4 key4_masked(float4 p, int lim, uint32_t tm) {
+    float4 q = key4<k>(p, tm);
     const int w = 1 << k;
     const float ninf = __int_as_float(0xff800000);
     if (w > lim) q.x = ninf;
@@ -161,11 +166,11 @@ __device__ __forceinline__ float4 max4(float4 a, float4 b, float4 c) {
 }
 
 template <int k, bool FAST>
-__device__ __forceinline__ float4 keyx(float4 p, int lim) {
+__device__ __forceinline__ float4 keyx(float4 p, int lim, uint32_t tm) {
     if constexpr (FAST) {
-        return key4<k>(p);
+        return key4<k>(p, tm);
     } else {
-        return key4_masked<k>(p, lim);
+        return key4_masked<k>(p, lim, tm);
     }
 }
 
@@ -173,12 +178,12 @@ __device__ __forceinline__ float4 keyx(float4 p, int lim) {
 // Levels 0..2 are folded by the caller; above, levels are folded in pairs (j-1, j) when
 // j is even so that one FMNMX3 serves two widths; a trailing odd level is folded alone.
 template <int j, int K, bool FAST>
-__device__ __forceinline__ void fold(float4& best, float4 before, float4 now, int lim) {
+__device__ __forceinline__ void fold(float4& best, float4 before, float4 now, int lim, uint32_t tm) {
     if constexpr (j >= 3) {
         if constexpr ((j & 1) == 0) {
-            best = max4(best, keyx<j - 1, FAST>(before, lim), keyx<j, FAST>(now, lim));
+            best = max4(best, keyx<j - 1, FAST>(before, lim, tm), keyx<j, FAST>(now, lim, tm));
         } else if constexpr (j == K - 1) {
-            best = max4(best, keyx<j, FAST>(now, lim));
+            best = max4(best, keyx<j, FAST>(now, lim, tm));
         }
     }
 }
@@ -194,12 +199,13 @@ struct Delay {
     float4 d1[4]; //               previous chunk
 };
 
-// One streaming step: the chunk staged at `st4` (C + 4 floats: the chunk and the first
+// One streaming step: the chunk staged at `st4` (C + 8 floats: the chunk and the first two
 // float4 of the following chunk) -> Y, W for its C samples.
 template <int T, int K, bool FAST>
 __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float4* __restrict__ pp,
                                            float4* __restrict__ halo, int& xsel, int& hsel, Delay& dl,
-                                           const float mu, const float inv, float* __restrict__ out_snr,
+                                           const float mu, const float inv, const uint32_t tm,
+                                           float* __restrict__ out_snr,
                                            int32_t* __restrict__ out_width, const long long n0,
                                            const long long n_t, const bool do_out, const int tid) {
     constexpr int R = kRowsPerChunk;
@@ -210,7 +216,7 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
     float4 P[R], best[R];
     int lim[R];
 
-    // ---- stage -> registers, normalise, levels 0..2 in the thread's own registers ----
+    // ---- stage -> registers, remove the mean, levels 0..3 in the thread's own registers ----
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         if constexpr (FAST) {
@@ -219,36 +225,48 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
             const long long left = n_t - (n0 + 4ll * (tid + T * r));
             lim[r] = left > (1ll << 30) ? (1 << 30) : (left < 0 ? 0 : static_cast<int>(left));
         }
-        const float4 a = norm4(st4[tid + T * r], mu, inv);
+        const float4 a = norm4(st4[tid + T * r], mu);
         if constexpr (K == 1) {
             P[r] = a;
-            if (FAST || do_out) best[r] = keyx<0, FAST>(a, lim[r]);
+            if (FAST || do_out) best[r] = keyx<0, FAST>(a, lim[r], tm);
         } else {
-            const float4 b = norm4(st4[tid + T * r + 1], mu, inv);
+            const float4 b = norm4(st4[tid + T * r + 1], mu);
             const float s01 = a.x + a.y, s12 = a.y + a.z, s23 = a.z + a.w, s34 = a.w + b.x;
             const float4 p1 = make_float4(s01, s12, s23, s34);
             if constexpr (K == 2) {
                 P[r] = p1;
-                if (FAST || do_out) best[r] = max4(keyx<0, FAST>(a, lim[r]), keyx<1, FAST>(p1, lim[r]));
+                if (FAST || do_out) best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm));
             } else {
                 const float s45 = b.x + b.y, s56 = b.y + b.z;
                 const float4 p2 = make_float4(s01 + s23, s12 + s34, s23 + s45, s34 + s56);
-                P[r] = p2;
                 if (FAST || do_out)
-                    best[r] = max4(keyx<0, FAST>(a, lim[r]), keyx<1, FAST>(p1, lim[r]), keyx<2, FAST>(p2, lim[r]));
+                    best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm), keyx<2, FAST>(p2, lim[r], tm));
+                if constexpr (K == 3) {
+                    P[r] = p2;
+                } else {
+                    // Width 8 from a third float4 of raw samples: recomputing the width-4 sums of
+                    // the next float4 here costs 8 adds on an idle pipe and saves one whole
+                    // shared-memory exchange (the L1/shared data pipe is the binding unit).
+                    const float4 c = norm4(st4[tid + T * r + 2], mu);
+                    const float s67 = b.z + b.w, s78 = b.w + c.x, s89 = c.x + c.y, s9a = c.y + c.z;
+                    const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
+                                                  (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
+                    if (FAST || do_out) fold<3, K, FAST>(best[r], p2, p3, lim[r], tm);
+                    P[r] = p3;
+                }
             }
         }
     }
 
-    // ---- exchange levels: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], 4 <= 2^k <= 2T -----------
+    // ---- exchange levels: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], 8 <= 2^k <= 2T -----------
     float4* const hr = halo + hsel * T;        // written by the previous (later-in-time) chunk
     float4* const hw = halo + (hsel ^ 1) * T;  // read by the next chunk
     hsel ^= 1;
 #pragma unroll
-    for (int k = 2; k <= LT + 1; ++k) {
+    for (int k = 3; k <= LT + 1; ++k) {
         if (k + 1 <= LAST) {
             const int d4 = (1 << k) / 4;  // partner distance in float4
-            const int hoff = d4 - 1;      // sum of the halo sizes of the levels below
+            const int hoff = d4 - 2;      // sum of the halo sizes of the levels below
             float4* const buf = pp + xsel * C4;
             xsel ^= 1;
 #pragma unroll
@@ -262,15 +280,14 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
                 const float4 now = add4(P[r], *src);
                 if (FAST || do_out) {
                     switch (k) {  // k is a compile-time constant after unrolling
-                        case 2: fold<3, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 3: fold<4, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 4: fold<5, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 5: fold<6, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 6: fold<7, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 7: fold<8, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 8: fold<9, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 9: fold<10, K, FAST>(best[r], P[r], now, lim[r]); break;
-                        case 10: fold<11, K, FAST>(best[r], P[r], now, lim[r]); break;
+                        case 3: fold<4, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 4: fold<5, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 5: fold<6, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 6: fold<7, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 7: fold<8, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 8: fold<9, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 9: fold<10, K, FAST>(best[r], P[r], now, lim[r], tm); break;
+                        case 10: fold<11, K, FAST>(best[r], P[r], now, lim[r], tm); break;
                         default: break;
                     }
                 }
@@ -287,7 +304,7 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
         dl.a = P[0];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (FAST || do_out) fold<LT + 3, K, FAST>(best[r], P[r], now[r], lim[r]);
+            if (FAST || do_out) fold<LT + 3, K, FAST>(best[r], P[r], now[r], lim[r], tm);
             P[r] = now[r];
         }
     }
@@ -299,7 +316,7 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
         dl.b[1] = P[1];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (FAST || do_out) fold<LT + 4, K, FAST>(best[r], P[r], now[r], lim[r]);
+            if (FAST || do_out) fold<LT + 4, K, FAST>(best[r], P[r], now[r], lim[r], tm);
             P[r] = now[r];
         }
     }
@@ -308,7 +325,7 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], dl.c[r]);
             dl.c[r] = P[r];
-            if (FAST || do_out) fold<LT + 5, K, FAST>(best[r], P[r], now, lim[r]);
+            if (FAST || do_out) fold<LT + 5, K, FAST>(best[r], P[r], now, lim[r], tm);
             P[r] = now;
         }
     }
@@ -318,7 +335,7 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
             const float4 now = add4(P[r], dl.d0[r]);
             dl.d0[r] = dl.d1[r];
             dl.d1[r] = P[r];
-            if (FAST || do_out) fold<LT + 6, K, FAST>(best[r], P[r], now, lim[r]);
+            if (FAST || do_out) fold<LT + 6, K, FAST>(best[r], P[r], now, lim[r], tm);
             P[r] = now;
         }
     }
@@ -330,8 +347,8 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
             if (FAST || lim[r] > 0) {
                 const uint32_t kx = __float_as_uint(best[r].x), ky = __float_as_uint(best[r].y);
                 const uint32_t kz = __float_as_uint(best[r].z), kw = __float_as_uint(best[r].w);
-                const float4 y = make_float4(__uint_as_float(kx & ~kCodeMask), __uint_as_float(ky & ~kCodeMask),
-                                             __uint_as_float(kz & ~kCodeMask), __uint_as_float(kw & ~kCodeMask));
+                const float4 y = make_float4(__uint_as_float(kx & tm) * inv, __uint_as_float(ky & tm) * inv,
+                                             __uint_as_float(kz & tm) * inv, __uint_as_float(kw & tm) * inv);
                 const int4 w = make_int4(static_cast<int>(~kx & kCodeMask), static_cast<int>(~ky & kCodeMask),
                                          static_cast<int>(~kz & kCodeMask), static_cast<int>(~kw & kCodeMask));
                 const long long o = n0 + 4ll * (tid + T * r);
@@ -342,26 +359,32 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
     }
     // With no exchange level there is no barrier inside the step: add the one that
     // orders this step's stage reads before the next refill of the stage.
-    if constexpr (LAST < 3) __syncthreads();
+    if constexpr (LAST < 4) __syncthreads();
 }
 
-constexpr int tree_blocks_per_sm(int T) { return T == 128 ? 4 : (T == 256 ? 2 : 1); }
+// Resident blocks per SM for T = 128.  3 (168 registers per thread, no spills) measured 3 %
+// faster than 4 (128 registers, 11 spilled delay registers): the kernel is bound by the
+// L1/shared data pipe, not by occupancy (profiles/r01b_*).
+#ifndef SPD_TREE_BPS128
+#define SPD_TREE_BPS128 3
+#endif
+constexpr int tree_blocks_per_sm(int T) { return T == 128 ? SPD_TREE_BPS128 : (T == 256 ? 2 : 1); }
 
 template <int T>
 constexpr size_t tree_smem_bytes() {
     constexpr size_t C = 16 * T;
-    return 2 * C * 4 + kStages * (C + 4) * 4 + 2 * T * 16 + kStages * 8;
+    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8;
 }
 
 template <int T, int K>
 __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(const TreeParams p) {
     constexpr int C = 16 * T;
     constexpr int M = 1 << (K - 1);
-    constexpr int GUARD = M > 4 ? M : 4;
+    constexpr int GUARD = M > 8 ? M : 8;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* const pp = reinterpret_cast<float4*>(smem_raw);
     float* const stages = reinterpret_cast<float*>(smem_raw + 2 * C * 4);
-    float4* const halo = reinterpret_cast<float4*>(stages + kStages * (C + 4));
+    float4* const halo = reinterpret_cast<float4*>(stages + kStages * (C + 8));
     uint64_t* const bars = reinterpret_cast<uint64_t*>(halo + 2 * T);
 
     const int tid = threadIdx.x;
@@ -381,6 +404,7 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
     int32_t* __restrict__ out_width = p.out_width + static_cast<long long>(d) * n_t;
     const float mu = p.mean[d];
     const float inv = 1.0f / p.sigma[d];
+    const uint32_t tm = p.tag_mask;
 
     for (int i = tid; i < 2 * T; i += T) halo[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (tid == 0) {
@@ -402,12 +426,12 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
     // ---- guarded steps: warm-up chunks of an interior segment, then the row tail -----
     for (int c = c_top - 1; c >= first_fast; --c) {
         const long long n0 = static_cast<long long>(c) * C;
-        for (int i = tid; i < C + 4; i += T) {
+        for (int i = tid; i < C + 8; i += T) {
             const long long n = n0 + i;
             stages[i] = n < n_t ? __ldg(row + n) : mu;
         }
         __syncthreads();
-        tree_chunk<T, K, false>(reinterpret_cast<const float4*>(stages), pp, halo, xsel, hsel, dl, mu, inv,
+        tree_chunk<T, K, false>(reinterpret_cast<const float4*>(stages), pp, halo, xsel, hsel, dl, mu, inv, tm,
                                 out_snr, out_width, n0, n_t, c < c_hi, tid);
         __syncthreads();
     }
@@ -417,13 +441,13 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
     if (n_fast <= 0) return;
     fence_proxy_async();
     __syncthreads();
-    constexpr uint32_t kBytes = (C + 4) * 4;
+    constexpr uint32_t kBytes = (C + 8) * 4;
     if (tid == 0) {
 #pragma unroll
         for (int j = 0; j < kStages - 1; ++j) {
             if (j < n_fast) {
                 mbar_arrive_expect_tx(&bars[j], kBytes);
-                bulk_g2s(stages + j * (C + 4), row + static_cast<long long>(first_fast - 1 - j) * C, kBytes,
+                bulk_g2s(stages + j * (C + 8), row + static_cast<long long>(first_fast - 1 - j) * C, kBytes,
                          &bars[j]);
             }
         }
@@ -436,14 +460,14 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
             if (nx < n_fast) {
                 const int sx = stage == 0 ? kStages - 1 : stage - 1;  // (it + kStages - 1) % kStages
                 mbar_arrive_expect_tx(&bars[sx], kBytes);
-                bulk_g2s(stages + sx * (C + 4), row + static_cast<long long>(first_fast - 1 - nx) * C, kBytes,
+                bulk_g2s(stages + sx * (C + 8), row + static_cast<long long>(first_fast - 1 - nx) * C, kBytes,
                          &bars[sx]);
             }
         }
         mbar_wait(&bars[stage], phase);
         const long long n0 = static_cast<long long>(first_fast - 1 - it) * C;
-        tree_chunk<T, K, true>(reinterpret_cast<const float4*>(stages + stage * (C + 4)), pp, halo, xsel, hsel,
-                               dl, mu, inv, out_snr, out_width, n0, n_t, true, tid);
+        tree_chunk<T, K, true>(reinterpret_cast<const float4*>(stages + stage * (C + 8)), pp, halo, xsel, hsel,
+                               dl, mu, inv, tm, out_snr, out_width, n0, n_t, true, tid);
         if (++stage == kStages) {
             stage = 0;
             phase ^= 1;
@@ -461,6 +485,7 @@ cudaError_t launch_tree(const TreeConfig& cfg, const TreeParams& prm, int64_t n_
 template <int T, int K>
 cudaError_t prepare_tree(TreeConfig& cfg) {
     cfg.smem_bytes = tree_smem_bytes<T>();
+    if (const char* env = std::getenv("SPD_TREE_PAD_SMEM")) cfg.smem_bytes += static_cast<size_t>(std::atoll(env));
     cudaError_t e = cudaFuncSetAttribute(spd_tree_kernel<T, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(cfg.smem_bytes));
     if (e != cudaSuccess) return e;
@@ -556,6 +581,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     prm.seg_chunks = cfg.seg_chunks;
     prm.segs_per_row = cfg.segs_per_row;
     prm.warm_chunks = cfg.warm_chunks;
+    prm.tag_mask = ~kCodeMask;
     cudaError_t e = cudaErrorInvalidValue;
 #define SPD_LAUNCH(TT, KK) \
     if (cfg.K == KK) e = launch_tree<TT, KK>(cfg, prm, n_dm, stream);
