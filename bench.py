@@ -259,6 +259,9 @@ def run_b200(args):
     cap = 1 << 22
     plan = spd.Plan(w.n_dm, w.n_t, widths, w.max_width)
     info = plan.info
+    activity = torch.empty(info["activity_bytes"], dtype=torch.uint8, device=dev)
+    cand_list = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
+    cand_count = torch.zeros(1, dtype=torch.int64, device=dev)
     # planes smaller than L2 would be re-read from cache: flush between steps
     need_flush = 3 * n * 4 <= (512 << 20)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if need_flush else None
@@ -269,10 +272,11 @@ def run_b200(args):
             flush.fill_(1)
         if ev is not None:
             ev[0].record(stream)
-        plan.run(plane, mean, sigma, out_snr, out_width)
+        plan.run_flagged(plane, mean, sigma, thr, out_snr, out_width, activity)
         if ev is not None:
             ev[1].record(stream)
-        lst, n_found = plan.find_candidates(out_snr, out_width, thr, cap)
+        lst, n_found = plan.find_candidates_flagged(out_snr, out_width, activity, thr, cap,
+                                                    lst=cand_list, n_found=cand_count)
         if ev is not None:
             ev[2].record(stream)
         return lst, n_found

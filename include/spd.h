@@ -90,6 +90,9 @@ typedef struct spd_plan_info {
     int32_t segments_per_row;   /* independent streams per DM row (dyadic tree), else 0 */
     int64_t smem_bytes;         /* dynamic shared memory per block of the dominant kernel */
     int64_t workspace_bytes;    /* plan-owned device workspace */
+    int64_t activity_bytes;     /* size of the activity map of spd_run_flagged (multiple of 128) */
+    int32_t activity_block;     /* time samples of one row covered by one byte of that map */
+    int32_t activity_per_row;   /* bytes of that map per DM row */
 } spd_plan_info;
 
 /*
@@ -162,6 +165,32 @@ int spd_run(const spd_plan* plan, const float* plane, const float* mean, const f
 int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
                         float threshold, spd_candidate* list, int64_t capacity,
                         int64_t* n_found, void* cuda_stream);
+
+/*
+ * spd_run_flagged - spd_run with row a8's threshold test fused into the same pass.
+ * Besides Y and W it fills the caller's activity map: byte [d * activity_per_row + b]
+ * is non-zero if any Y[d, n] with b * activity_block <= n < (b+1) * activity_block may
+ * reach `threshold` (it is zero only if none does), so the candidate stage can skip the
+ * rest of the plane.  The plane is still read once and Y, W written once.
+ *   threshold : candidate threshold in SNR units (the value later given to
+ *               spd_find_candidates_flagged, or any lower one).
+ *   activity  : DEVICE, uint8 [spd_plan_info.activity_bytes], 16-byte aligned, fully overwritten.
+ * Other arguments, asynchrony and aliasing rules as spd_run.  A SPD_PATH_GENERIC plan
+ * marks every block active.
+ */
+int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                    float* out_snr, int32_t* out_width, float threshold, uint8_t* activity,
+                    void* cuda_stream);
+
+/*
+ * spd_find_candidates_flagged - spd_find_candidates restricted to the blocks marked in
+ * `activity` (written by spd_run_flagged on the same out_snr with a threshold <= this
+ * one).  Same rule, same outputs; samples of unmarked blocks are never candidates
+ * because their Y is below the threshold.
+ */
+int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+                                const uint8_t* activity, float threshold, spd_candidate* list,
+                                int64_t capacity, int64_t* n_found, void* cuda_stream);
 
 /*
  * spd_run_host - the same hot path on HOST buffers (end-to-end entry point):

@@ -14,7 +14,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-LIB_PATH = os.path.join(_HERE, "libspd_b200.so")
+# SPD_B200_LIB points the binding at another build of the same library (kernel-tuning sweeps).
+LIB_PATH = os.environ.get("SPD_B200_LIB") or os.path.join(_HERE, "libspd_b200.so")
 
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo", "--expt-relaxed-constexpr",
@@ -48,6 +49,8 @@ def nvcc_path() -> str:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every CUDA source for sm_100a into ``libspd_b200.so``; returns its path."""
+    if os.environ.get("SPD_B200_LIB"):
+        return LIB_PATH  # an explicitly chosen build is used as it is
     if force or needs_build():
         cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
             ["-o", LIB_PATH + ".tmp"] + sources()

@@ -31,6 +31,7 @@ SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC = 1, 2
 EXPORTS = (
     "spd_width_set_generate", "spd_plan_create", "spd_plan_create_ex", "spd_plan_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
+    "spd_run_flagged", "spd_find_candidates_flagged",
     "spd_run_host", "spd_last_error_string", "spd_version",
 )
 
@@ -55,7 +56,9 @@ class spd_plan_info(ctypes.Structure):
                 ("path", ctypes.c_int32), ("launches_per_run", ctypes.c_int32),
                 ("threads_per_block", ctypes.c_int32), ("blocks", ctypes.c_int32),
                 ("chunk", ctypes.c_int32), ("segments_per_row", ctypes.c_int32),
-                ("smem_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64)]
+                ("smem_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64),
+                ("activity_bytes", ctypes.c_int64), ("activity_block", ctypes.c_int32),
+                ("activity_per_row", ctypes.c_int32)]
 
 
 _lib: Optional[ctypes.CDLL] = None
@@ -95,6 +98,10 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_run.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.spd_find_candidates.restype = ctypes.c_int
     lib.spd_find_candidates.argtypes = [_vp, _vp, _vp, ctypes.c_float, _vp, _i64, _vp, _vp]
+    lib.spd_run_flagged.restype = ctypes.c_int
+    lib.spd_run_flagged.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp]
+    lib.spd_find_candidates_flagged.restype = ctypes.c_int
+    lib.spd_find_candidates_flagged.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_float, _vp, _i64, _vp, _vp]
     lib.spd_run_host.restype = ctypes.c_int
     lib.spd_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     _lib = lib
@@ -213,6 +220,44 @@ def spd_find_candidates(plan: int, out_snr, out_width, threshold: float, capacit
     return lst, n_found
 
 
+def spd_run_flagged(plan: int, plane, mean, sigma, out_snr, out_width, threshold: float, activity,
+                    stream=None) -> None:
+    """spd_run plus the fused threshold test: also fills the ``activity`` map (uint8 device tensor of
+    ``spd_plan_get_info(plan)["activity_bytes"]`` bytes)."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    _check(load().spd_run_flagged(
+        _vp(plan),
+        _dev_ptr(plane, torch.float32, n, "plane"),
+        _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
+        _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
+        _dev_ptr(out_snr, torch.float32, n, "out_snr"),
+        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        ctypes.c_float(threshold),
+        _dev_ptr(activity, torch.uint8, info["activity_bytes"], "activity"),
+        _vp(_stream_handle(stream))))
+
+
+def spd_find_candidates_flagged(plan: int, out_snr, out_width, activity, threshold: float, capacity: int,
+                                stream=None, lst=None, n_found=None):
+    """Candidate stage over the blocks marked in ``activity``; returns (list, n_found) as spd_find_candidates."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    if lst is None:
+        lst = torch.empty(max(int(capacity), 1) * ctypes.sizeof(spd_candidate), dtype=torch.uint8,
+                          device=out_snr.device)
+    if n_found is None:
+        n_found = torch.zeros(1, dtype=torch.int64, device=out_snr.device)
+    _check(load().spd_find_candidates_flagged(
+        _vp(plan), _dev_ptr(out_snr, torch.float32, n, "out_snr"),
+        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _dev_ptr(activity, torch.uint8, info["activity_bytes"], "activity"), ctypes.c_float(threshold),
+        _vp(lst.data_ptr()), int(capacity), _vp(n_found.data_ptr()), _vp(_stream_handle(stream))))
+    return lst, n_found
+
+
 def candidates_to_numpy(lst, n_found, capacity: int) -> Tuple[int, np.ndarray]:
     """Synchronising helper: (count, structured array of the stored candidates sorted by (dm, t))."""
     count = int(n_found.item())
@@ -274,6 +319,23 @@ class Plan:
 
     def find_candidates(self, out_snr, out_width, threshold: float, capacity: int, stream=None):
         return spd_find_candidates(self.handle, out_snr, out_width, threshold, capacity, stream)
+
+    def run_flagged(self, plane, mean, sigma, threshold: float, out_snr=None, out_width=None, activity=None,
+                    stream=None):
+        import torch
+        if out_snr is None:
+            out_snr = torch.empty((self.n_dm, self.n_t), dtype=torch.float32, device=plane.device)
+        if out_width is None:
+            out_width = torch.empty((self.n_dm, self.n_t), dtype=torch.int32, device=plane.device)
+        if activity is None:
+            activity = torch.empty(self.info["activity_bytes"], dtype=torch.uint8, device=plane.device)
+        spd_run_flagged(self.handle, plane, mean, sigma, out_snr, out_width, threshold, activity, stream)
+        return out_snr, out_width, activity
+
+    def find_candidates_flagged(self, out_snr, out_width, activity, threshold: float, capacity: int, stream=None,
+                                lst=None, n_found=None):
+        return spd_find_candidates_flagged(self.handle, out_snr, out_width, activity, threshold, capacity, stream,
+                                           lst, n_found)
 
     def run_host(self, plane, mean, sigma, out_snr, out_width):
         spd_run_host(self.handle, plane, mean, sigma, out_snr, out_width)

@@ -164,8 +164,16 @@ int prepare_host_staging(spd_plan* plan) {
 int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const float* mean, const float* sigma,
              float* out_snr, int32_t* out_width, cudaStream_t stream) {
     if (plan->path == SPD_PATH_DYADIC_TREE)
-        return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
+        return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
     return generic_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
+}
+
+size_t activity_bytes(const spd_plan* plan) {
+    return (static_cast<size_t>(plan->n_dm) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
+}
+
+bool misaligned16(const void* a, const void* b, const void* c) {
+    return ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(b) | reinterpret_cast<uintptr_t>(c)) & 15u) != 0;
 }
 
 }  // namespace
@@ -305,6 +313,9 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         info->blocks = static_cast<int32_t>(plan->n_dm * ((plan->n_t + 255) / 256));
     }
     info->workspace_bytes = plan->workspace_bytes;
+    info->activity_bytes = static_cast<int64_t>(activity_bytes(plan));
+    info->activity_block = static_cast<int32_t>(activity_block(plan));
+    info->activity_per_row = static_cast<int32_t>(activity_per_row(plan));
     return SPD_OK;
 }
 
@@ -314,8 +325,7 @@ int spd_run(const spd_plan* plan, const float* plane, const float* mean, const f
         set_error("spd_run: NULL argument");
         return SPD_ERR_INVALID_ARG;
     }
-    if ((reinterpret_cast<uintptr_t>(plane) | reinterpret_cast<uintptr_t>(out_snr) |
-         reinterpret_cast<uintptr_t>(out_width)) & 15u) {
+    if (misaligned16(plane, out_snr, out_width)) {
         set_error("spd_run: plane, out_snr and out_width must be 16-byte aligned");
         return SPD_ERR_INVALID_ARG;
     }
@@ -328,7 +338,42 @@ int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_
         set_error("spd_find_candidates: NULL argument or negative capacity");
         return SPD_ERR_INVALID_ARG;
     }
-    return candidates_run(plan, out_snr, out_width, threshold, list, capacity, n_found,
+    return candidates_run(plan, out_snr, out_width, nullptr, threshold, list, capacity, n_found,
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
+                    int32_t* out_width, float threshold, uint8_t* activity, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma || !out_snr || !out_width || !activity) {
+        set_error("spd_run_flagged: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (misaligned16(plane, out_snr, out_width) || misaligned16(activity, nullptr, nullptr)) {
+        set_error("spd_run_flagged: plane, out_snr, out_width and activity must be 16-byte aligned");
+        return SPD_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (plan->path == SPD_PATH_DYADIC_TREE)
+        return tree_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    // any-width-set path: no fused test, every block stays active (padding included: the
+    // candidate kernel bounds the flag index itself)
+    const cudaError_t e = cudaMemsetAsync(activity, 1, activity_bytes(plan), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "filling the activity map");
+    return generic_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, stream);
+}
+
+int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+                                const uint8_t* activity, float threshold, spd_candidate* list, int64_t capacity,
+                                int64_t* n_found, void* cuda_stream) {
+    if (!plan || !out_snr || !out_width || !activity || !n_found || capacity < 0 || (capacity > 0 && !list)) {
+        set_error("spd_find_candidates_flagged: NULL argument or negative capacity");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (misaligned16(out_snr, activity, nullptr)) {
+        set_error("spd_find_candidates_flagged: out_snr and activity must be 16-byte aligned");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return candidates_run(plan, out_snr, out_width, activity, threshold, list, capacity, n_found,
                           static_cast<cudaStream_t>(cuda_stream));
 }
 

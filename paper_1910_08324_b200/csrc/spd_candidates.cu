@@ -6,8 +6,19 @@
 // and Y[d,n] >= Y[d,n+1], row ends comparing against -inf, i.e. the first sample of
 // a local-maximum plateau.  Candidates are appended to a bounded list with one
 // atomic per warp; the count keeps running past the capacity (overflow report).
+//
+// Two kernels apply the same rule:
+//   * find_candidates_kernel visits every sample (any plane, any alignment);
+//   * find_candidates_flagged_kernel visits only the blocks of samples whose byte in the
+//     activity map is set.  The map is written by the kernel that produced Y (the
+//     threshold test is fused into spd_tree.cu), so on planes where detections are rare
+//     this stage reads a few per cent of Y instead of all of it.  A persistent grid of
+//     warps scans the map (128 blocks per warp step) and each warp walks its flagged blocks
+//     with 128-bit loads, neighbours coming from the adjacent lanes.
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <algorithm>
 
 #include "spd_internal.h"
 
@@ -17,6 +28,30 @@ namespace {
 constexpr int kCandThreads = 256;
 constexpr int kCandPerThread = 4;
 constexpr int kCandTile = kCandThreads * kCandPerThread;
+
+// Warp-aggregated append of the lanes with `hit` set.
+__device__ __forceinline__ void append_hits(bool hit, long long d, long long n, float c,
+                                            const int32_t* __restrict__ width, long long n_t,
+                                            spd_candidate* __restrict__ list, unsigned long long capacity,
+                                            unsigned long long* __restrict__ n_found, unsigned lane) {
+    const unsigned mask = __ballot_sync(0xffffffffu, hit);
+    if (mask == 0u) return;
+    unsigned long long base = 0;
+    const int leader = __ffs(mask) - 1;
+    if (static_cast<int>(lane) == leader) base = atomicAdd(n_found, static_cast<unsigned long long>(__popc(mask)));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (hit) {
+        const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
+        if (slot < capacity) {
+            spd_candidate cnd;
+            cnd.dm = static_cast<int32_t>(d);
+            cnd.t = static_cast<int32_t>(n);
+            cnd.snr = c;
+            cnd.width_idx = __ldg(width + d * n_t + n);
+            list[slot] = cnd;
+        }
+    }
+}
 
 __global__ void __launch_bounds__(kCandThreads) find_candidates_kernel(
     const float* __restrict__ snr, const int32_t* __restrict__ width, long long n_t, long long tiles_per_row,
@@ -40,21 +75,100 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_kernel(
         const long long n = n0 + i;
         const float c = v[i + 1];
         const bool hit = n < n_t && c >= thr && c > v[i] && c >= v[i + 2];
-        const unsigned mask = __ballot_sync(0xffffffffu, hit);
-        if (mask == 0u) continue;
-        unsigned long long base = 0;
-        const int leader = __ffs(mask) - 1;
-        if (static_cast<int>(lane) == leader) base = atomicAdd(n_found, static_cast<unsigned long long>(__popc(mask)));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (hit) {
-            const unsigned long long slot = base + __popc(mask & ((1u << lane) - 1u));
-            if (slot < capacity) {
-                spd_candidate cnd;
-                cnd.dm = static_cast<int32_t>(d);
-                cnd.t = static_cast<int32_t>(n);
-                cnd.snr = c;
-                cnd.width_idx = __ldg(width + d * n_t + n);
-                list[slot] = cnd;
+        append_hits(hit, d, n, c, width, n_t, list, capacity, n_found, lane);
+    }
+}
+
+// Peak test of the 4 samples a lane holds -> 4-bit mask (bit i: sample n + i is a candidate).
+__device__ __forceinline__ unsigned peak_bits(float4 v, float prev, float next, float thr) {
+    unsigned m = 0;
+    if (v.x >= thr && v.x > prev && v.x >= v.y) m |= 1u;
+    if (v.y >= thr && v.y > v.x && v.y >= v.z) m |= 2u;
+    if (v.z >= thr && v.z > v.y && v.z >= v.w) m |= 4u;
+    if (v.w >= thr && v.w > v.z && v.w >= next) m |= 8u;
+    return m;
+}
+
+// One warp per flagged block of `block` samples (block % 128 == 0, n_t % 4 == 0), walked in
+// pieces of kPiece samples: the piece's peaks are first collected as bits (4 per lane and
+// 128-sample step), counted across the warp, reserved with ONE atomic per piece, and then
+// written.  On planes that flood the threshold (config 5: baseline drift) this keeps the
+// single counter off the critical path.
+constexpr int kPiece = 2048;             // samples per reservation
+constexpr int kPieceSteps = kPiece / 128;  // 16 steps x 4 bits = 64 bits per lane
+
+__global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
+    const float* __restrict__ snr, const int32_t* __restrict__ width, const uint8_t* __restrict__ activity,
+    long long n_flags, long long flags_per_row, long long block, long long n_t, float thr,
+    spd_candidate* __restrict__ list, unsigned long long capacity, unsigned long long* __restrict__ n_found) {
+    const unsigned lane = threadIdx.x & 31u;
+    const long long warp = (static_cast<long long>(blockIdx.x) * kCandThreads + threadIdx.x) >> 5;
+    const long long n_warps = (static_cast<long long>(gridDim.x) * kCandThreads) >> 5;
+    const float ninf = __int_as_float(0xff800000);
+    // the map is padded to a multiple of 128 bytes, so 32-bit loads are in bounds
+    const uint32_t* __restrict__ act32 = reinterpret_cast<const uint32_t*>(activity);
+    const long long n_steps = (n_flags + 127) / 128;
+    for (long long step = warp; step < n_steps; step += n_warps) {
+        const uint32_t f4 = __ldg(act32 + step * 32 + lane);
+        unsigned pending = __ballot_sync(0xffffffffu, f4 != 0u);
+        while (pending) {
+            const int src = __ffs(pending) - 1;
+            pending &= pending - 1;
+            uint32_t word = __shfl_sync(0xffffffffu, f4, src);
+            while (word) {
+                const int byte = (__ffs(word) - 1) >> 3;
+                word &= ~(0xffu << (8 * byte));
+                const long long fi = step * 128 + src * 4 + byte;
+                if (fi >= n_flags) continue;
+                const long long d = fi / flags_per_row;
+                const long long b = fi - d * flags_per_row;
+                const float* __restrict__ y = snr + d * n_t;
+                const long long lo = b * block;
+                const long long hi = min(lo + block, n_t);  // multiples of 4
+                for (long long p0 = lo; p0 < hi; p0 += kPiece) {
+                    const long long p1 = min(p0 + kPiece, hi);
+                    // value before the first sample of the piece
+                    float carry = p0 > 0 ? __ldg(y + p0 - 1) : ninf;
+                    unsigned long long bits = 0ull;
+#pragma unroll 4
+                    for (int it = 0; it < kPieceSteps; ++it) {
+                        const long long n = p0 + 128ll * it + 4 * lane;
+                        const bool in = n < p1;
+                        float4 v = make_float4(ninf, ninf, ninf, ninf);
+                        if (in) v = __ldg(reinterpret_cast<const float4*>(y + n));
+                        float prev = __shfl_up_sync(0xffffffffu, v.w, 1);
+                        if (lane == 0) prev = carry;
+                        float next = __shfl_down_sync(0xffffffffu, v.x, 1);
+                        if (lane == 31) next = (in && n + 4 < n_t) ? __ldg(y + n + 4) : ninf;
+                        carry = __shfl_sync(0xffffffffu, v.w, 31);
+                        if (in) bits |= static_cast<unsigned long long>(peak_bits(v, prev, next, thr)) << (4 * it);
+                    }
+                    const unsigned mine = __popcll(bits);
+                    if (!__any_sync(0xffffffffu, mine != 0u)) continue;
+                    // exclusive scan of the per-lane counts, one reservation for the piece
+                    unsigned incl = mine;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const unsigned u = __shfl_up_sync(0xffffffffu, incl, o);
+                        if (lane >= static_cast<unsigned>(o)) incl += u;
+                    }
+                    const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
+                    unsigned long long base = 0;
+                    if (lane == 0) base = atomicAdd(n_found, static_cast<unsigned long long>(total));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    unsigned long long slot = base + (incl - mine);
+                    while (bits && slot < capacity) {
+                        const int bpos = __ffsll(static_cast<long long>(bits)) - 1;
+                        bits &= bits - 1;
+                        const long long n = p0 + 128ll * (bpos >> 2) + 4 * lane + (bpos & 3);
+                        spd_candidate cnd;
+                        cnd.dm = static_cast<int32_t>(d);
+                        cnd.t = static_cast<int32_t>(n);
+                        cnd.snr = __ldg(y + n);
+                        cnd.width_idx = __ldg(width + d * n_t + n);
+                        list[slot++] = cnd;
+                    }
+                }
             }
         }
     }
@@ -62,18 +176,38 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_kernel(
 
 }  // namespace
 
-int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* out_width, float threshold,
-                   spd_candidate* list, int64_t capacity, int64_t* n_found, cudaStream_t stream) {
+int64_t activity_block(const spd_plan* plan) {
+    return plan->path == SPD_PATH_DYADIC_TREE ? plan->tree.chunk : 4096;
+}
+int64_t activity_per_row(const spd_plan* plan) {
+    const int64_t b = activity_block(plan);
+    return (plan->n_t + b - 1) / b;
+}
+
+int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* out_width, const uint8_t* activity,
+                   float threshold, spd_candidate* list, int64_t capacity, int64_t* n_found, cudaStream_t stream) {
     cudaError_t e = cudaMemsetAsync(n_found, 0, sizeof(int64_t), stream);
     if (e != cudaSuccess) return cuda_fail(e, "clearing the candidate counter");
-    const long long tiles = (plan->n_t + kCandTile - 1) / kCandTile;
-    if (plan->n_dm * tiles > 0x7fffffffll) {
-        set_error("plane too large for the candidate grid");
-        return SPD_ERR_INVALID_ARG;
+    if (activity && plan->n_t % 4 == 0) {
+        const long long per_row = activity_per_row(plan);
+        const long long n_flags = plan->n_dm * per_row;
+        const long long steps = (n_flags + 127) / 128;
+        const long long warps_per_block = kCandThreads / 32;
+        long long blocks = (steps + warps_per_block - 1) / warps_per_block;
+        blocks = std::max<long long>(1, std::min<long long>(blocks, static_cast<long long>(plan->sm_count) * 8));
+        find_candidates_flagged_kernel<<<static_cast<unsigned>(blocks), kCandThreads, 0, stream>>>(
+            out_snr, out_width, activity, n_flags, per_row, activity_block(plan), plan->n_t, threshold, list,
+            static_cast<unsigned long long>(capacity), reinterpret_cast<unsigned long long*>(n_found));
+    } else {
+        const long long tiles = (plan->n_t + kCandTile - 1) / kCandTile;
+        if (plan->n_dm * tiles > 0x7fffffffll) {
+            set_error("plane too large for the candidate grid");
+            return SPD_ERR_INVALID_ARG;
+        }
+        find_candidates_kernel<<<static_cast<unsigned>(plan->n_dm * tiles), kCandThreads, 0, stream>>>(
+            out_snr, out_width, plan->n_t, tiles, threshold, list, static_cast<unsigned long long>(capacity),
+            reinterpret_cast<unsigned long long*>(n_found));
     }
-    find_candidates_kernel<<<static_cast<unsigned>(plan->n_dm * tiles), kCandThreads, 0, stream>>>(
-        out_snr, out_width, plan->n_t, tiles, threshold, list, static_cast<unsigned long long>(capacity),
-        reinterpret_cast<unsigned long long*>(n_found));
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launching the candidate kernel");
     return SPD_OK;

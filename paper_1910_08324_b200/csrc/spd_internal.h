@@ -13,15 +13,14 @@
 namespace spd {
 
 // Dyadic-tree geometry: a block of T threads owns "rows" of 4*T consecutive
-// samples, R = 4 rows per streaming step ("chunk").
-constexpr int kRowsPerChunk = 4;
+// samples, R rows per streaming step ("chunk"); T and R are chosen in spd_tree.cu.
 constexpr int kTreeMaxLevels = 16;  // widths 1 .. 32768
 constexpr int kStages = 3;          // bulk-copy ring depth
 
 struct TreeConfig {
     int K = 0;            // number of widths: 2^0 .. 2^(K-1)
     int T = 0;            // threads per block
-    int chunk = 0;        // 16 * T samples
+    int chunk = 0;        // 4 * T * R samples
     int warm_chunks = 0;  // look-ahead chunks an interior segment replays
     int segs_per_row = 1;
     int seg_chunks = 0;   // chunks per segment
@@ -71,8 +70,11 @@ int cuda_fail(cudaError_t e, const char* what);
 // spd_tree.cu
 bool tree_applicable(const std::vector<int32_t>& widths, int64_t n_t);
 int tree_configure(spd_plan* plan);
+// activity: nullptr, or [n_dm][chunks_per_row] bytes (cleared here, set by the kernel for
+// every chunk whose best SNR reaches `threshold`).
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
-             const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
+             const float* sigma, float* out_snr, int32_t* out_width, float threshold,
+             uint8_t* activity, cudaStream_t stream);
 
 // spd_generic.cu
 int generic_configure(spd_plan* plan);
@@ -81,8 +83,14 @@ int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const fl
                 const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
 
 // spd_candidates.cu
+// activity: nullptr (visit every sample) or the map written by spd_run_flagged, one byte
+// per `act_block` samples of each row (`act_per_row` bytes per row).
 int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
-                   float threshold, spd_candidate* list, int64_t capacity, int64_t* n_found,
-                   cudaStream_t stream);
+                   const uint8_t* activity, float threshold, spd_candidate* list, int64_t capacity,
+                   int64_t* n_found, cudaStream_t stream);
+
+// Activity-map geometry of a plan (both paths): samples per byte and bytes per row.
+int64_t activity_block(const spd_plan* plan);
+int64_t activity_per_row(const spd_plan* plan);
 
 }  // namespace spd

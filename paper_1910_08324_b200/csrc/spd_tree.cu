@@ -12,23 +12,31 @@
 //
 // Design (B200, not the paper's P100/Titan V kernel):
 //   * One block = one stream over a segment of one DM row, marching in REVERSE time in
-//     chunks of C = 16*T samples.  eq. (2) looks forward in time, so in reverse time the
-//     partner P_k[n + 2^k] has always been computed already; each level keeps a delay
-//     line instead of re-reading a (max_width - 1)-sample halo per tile.  The halo is
-//     paid once per segment (warm-up chunks), not once per tile.
-//   * Thread t owns, in each of the chunk's 4 "rows" of 4*T samples, the 4 consecutive
-//     samples 4t..4t+3 (one float4).  Widths 2, 4, 8: in the thread's own registers from
-//     three float4 of raw samples (the width-4 sums of the next float4 are recomputed
-//     rather than exchanged).  Levels 8 <= 2^k <= 2T: the partner belongs to another thread - exchanged through
-//     a ping-pong shared-memory buffer with 128-bit accesses, one __syncthreads() each.
-//     Levels 2^k >= 4T: the partner is the SAME thread's float4 1, 2, 4 or 8 rows later,
+//     chunks of C = 4*T*R samples (T threads, R "rows" of 4*T samples).  eq. (2) looks
+//     forward in time, so in reverse time the partner P_k[n + 2^k] has always been computed
+//     already; each level keeps a delay line instead of re-reading a (max_width - 1)-sample
+//     halo per tile.  The halo is paid once per segment (warm-up chunks), not once per tile.
+//   * Thread t owns, in each row, the 4 consecutive samples 4t..4t+3 (one float4).
+//     Widths 2, 4, 8: in the thread's own registers from three float4 of raw samples (the
+//     width-4 sums of the next float4 are recomputed rather than exchanged).
+//     Levels 8 <= 2^k <= 2T: the partner belongs to another thread - exchanged through a
+//     ping-pong shared-memory buffer with 128-bit accesses, one __syncthreads() each.
+//     Levels 2^k >= 4T: the partner is the SAME thread's float4 1, 2, 4, ... rows later,
 //     i.e. a register of this chunk or a delay register kept from the previous chunks.
+//     The shared-memory data pipe is the binding unit (profiles/r01b_*), so T is as small
+//     as the register file allows: T = 64 up to max_width 8192 (5 exchange levels,
+//     31 float4 of delay registers), doubling with max_width above that.
+//   * Delay lines deeper than one chunk are register FIFOs; the chunk loop is unrolled
+//     over the FIFO depth so that the FIFO slot is a compile-time constant (no moves).
 //   * Chunks are staged into shared memory by cp.async.bulk (TMA, 1-D) through a
 //     3-deep mbarrier ring; results leave as 128-bit streaming stores.
-//   * SNR scale 2^(-k/2) is a compile-time constant (data are divided by sigma on load);
-//     the width index rides in the 5 low mantissa bits of the SNR being maximised
-//     (relative perturbation <= 2^-18, inside the 1e-4 tolerance), stored inverted so
-//     that exact ties resolve to the smallest width; max is the 3-input FMNMX3.
+//   * SNR scale 2^(-k/2) is a compile-time constant (1/sigma is applied once per output
+//     sample at the store); the width index rides in the 5 low mantissa bits of the SNR
+//     being maximised (relative perturbation <= 2^-18, inside the 1e-4 tolerance), stored
+//     inverted so that exact ties resolve to the smallest width; max is the 3-input FMNMX3.
+//   * Row a8's threshold test is fused in: a chunk whose best SNR reaches the candidate
+//     threshold sets one byte of the caller's activity map, so that the candidate kernel
+//     only revisits those chunks (spd_candidates.cu).
 //   * Row tails (valid-windows-only rule, reading A3) and warm-up chunks run in a
 //     guarded variant of the same body; interior chunks run the unguarded one.
 #include <cuda_runtime.h>
@@ -36,6 +44,7 @@
 
 #include <algorithm>
 #include <cstdlib>
+#include <type_traits>
 
 #include "spd_internal.h"
 
@@ -48,6 +57,8 @@ struct TreeParams {
     const float* sigma;
     float* out_snr;
     int32_t* out_width;
+    uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr
+    float threshold;    // candidate threshold in SNR units (used only with activity)
     long long n_t;
     int chunks_per_row;
     int seg_chunks;
@@ -118,8 +129,8 @@ __device__ __forceinline__ float4 scale4(float4 a, float c) {
     const float2 hi = __fmul2_rn(make_float2(a.z, a.w), cc);
     return make_float4(lo.x, lo.y, hi.x, hi.y);
 }
-// x - mu (eq. 4 numerator per sample; exact-ish, no cancellation later).  The division by
-// sigma is applied once per output sample at the store, not per input sample here.
+// x - mu (eq. 4 numerator per sample; sums of mean-free data never cancel later).  The
+// division by sigma is applied once per output sample at the store, not per input sample.
 __device__ __forceinline__ float4 norm4(float4 a, float mu) {
     const float2 m = make_float2(-mu, -mu);
     const float2 lo = __fadd2_rn(make_float2(a.x, a.y), m);
@@ -188,30 +199,137 @@ __device__ __forceinline__ void fold(float4& best, float4 before, float4 now, in
     }
 }
 
-constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
+// Shared-memory store of a float4: as one 128-bit store, or as two 64-bit stores.  The sums
+// are produced by packed FADD2 into register PAIRS; a 128-bit store needs an aligned QUAD
+// and costs up to four register moves when the allocator cannot place the pairs together.
+#ifndef SPD_TREE_STS64
+#define SPD_TREE_STS64 1
+#endif
+template <int SPLIT>
+__device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
+    if constexpr (SPLIT) {
+        // inline PTX: as plain C++ the two halves are merged back into one 128-bit store
+        const uint32_t a = smem_u32(dst);
+        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
+        asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(a), "f"(v.z), "f"(v.w) : "memory");
+    } else {
+        *dst = v;
+    }
+}
 
-// Delay registers of the in-register levels: the first rows of the previous chunks.
-struct Delay {
-    float4 a;     // row offset 1
-    float4 b[2];  // row offset 2
-    float4 c[4];  // row offset 4 (= previous chunk)
-    float4 d0[4]; // row offset 8: two chunks ago
-    float4 d1[4]; //               previous chunk
+constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
+constexpr int imax(int a, int b) { return a > b ? a : b; }
+
+// Geometry of one kernel instantiation.
+template <int T, int R, int K>
+struct Geo {
+    static constexpr int LT = ilog2(T);
+    static constexpr int C4 = R * T;   // float4 per chunk
+    static constexpr int C = 4 * C4;   // samples per chunk
+    static constexpr int LAST = K - 1;  // highest level: width 2^LAST
+    // In-register levels j = 0 .. J-1: partner 2^j rows later, produces level LT + 3 + j.
+    static constexpr int J = imax(0, LAST - LT - 2);
+    static constexpr int ND = (1 << J) - 1;  // float4 of delay registers: sum of 2^j
+    // Depth, in chunks, of the deepest delay FIFO = unroll factor of the chunk loop.
+    static constexpr int U = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
 };
 
+struct ChunkCtx {
+    float mu, inv;
+    uint32_t tm;
+    float* __restrict__ out_snr;
+    int32_t* __restrict__ out_width;
+    long long n0, n_t;
+    bool do_out;
+    int tid;
+};
+
+// Exchange levels k = 3 .. LT+1: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner in another thread.
+template <int T, int R, int K, bool FAST, int k>
+__device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
+                                                float4* __restrict__ pp, float4* __restrict__ hr,
+                                                float4* __restrict__ hw, int& xsel, const ChunkCtx& cx) {
+    using G = Geo<T, R, K>;
+    if constexpr (k <= G::LT + 1 && k + 1 <= G::LAST) {
+        constexpr int d4 = (1 << k) / 4;  // partner distance in float4
+        constexpr int hoff = d4 - 2;      // sum of the halo sizes of the levels below
+        const int tid = cx.tid;
+        float4* const buf = pp + xsel * G::C4;
+        xsel ^= 1;
+#pragma unroll
+        for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
+        if (tid < d4) hw[hoff + tid] = P[0];
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4* src = buf + (tid + T * r + d4);
+            if (r == R - 1 && tid + d4 >= T) src = hr + (hoff + tid + d4 - T);
+            const float4 now = add4(P[r], *src);
+            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], now, lim[r], cx.tm);
+            P[r] = now;
+        }
+        exchange_levels<T, R, K, FAST, k + 1>(P, best, lim, pp, hr, hw, xsel, cx);
+    }
+}
+
+// In-register levels j = 0 .. J-1: partner 2^j rows later in the same thread.  Delay
+// registers of level j live at dl[2^j - 1 .. 2^(j+1) - 2].
+template <int T, int R, int K, bool FAST, int PH, int j>
+__device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
+                                                float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
+    using G = Geo<T, R, K>;
+    if constexpr (j < G::J) {
+        constexpr int D = 1 << j;   // partner distance in rows
+        constexpr int off = D - 1;  // first delay register of this level
+        constexpr int lvl = G::LT + 3 + j;
+        float4 now[R];
+        if constexpr (D < R) {
+            // partner in this chunk, or among the first D rows of the previous chunk
+#pragma unroll
+            for (int r = 0; r < R; ++r) now[r] = add4(P[r], r + D < R ? P[r + D] : dl[off + r + D - R]);
+#pragma unroll
+            for (int i = 0; i < D; ++i) dl[off + i] = P[i];
+        } else {
+            // partner D / R chunks back: FIFO of Q chunks.  Unguarded steps use slot PH % Q
+            // (the chunk loop is unrolled over the deepest FIFO); guarded steps keep the
+            // FIFO in canonical order (slot 0 oldest) by moving registers.
+            constexpr int Q = D / R;
+            constexpr int slot = FAST ? (PH % Q) : 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) now[r] = add4(P[r], dl[off + slot * R + r]);
+            if constexpr (FAST) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) dl[off + slot * R + r] = P[r];
+            } else {
+#pragma unroll
+                for (int s = 0; s + 1 < Q; ++s) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) dl[off + s * R + r] = dl[off + (s + 1) * R + r];
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) dl[off + (Q - 1) * R + r] = P[r];
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (FAST || cx.do_out) fold<lvl, K, FAST>(best[r], P[r], now[r], lim[r], cx.tm);
+            P[r] = now[r];
+        }
+        register_levels<T, R, K, FAST, PH, j + 1>(P, best, lim, dl, cx);
+    }
+}
+
 // One streaming step: the chunk staged at `st4` (C + 8 floats: the chunk and the first two
-// float4 of the following chunk) -> Y, W for its C samples.
-template <int T, int K, bool FAST>
-__device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float4* __restrict__ pp,
-                                           float4* __restrict__ halo, int& xsel, int& hsel, Delay& dl,
-                                           const float mu, const float inv, const uint32_t tm,
-                                           float* __restrict__ out_snr,
-                                           int32_t* __restrict__ out_width, const long long n0,
-                                           const long long n_t, const bool do_out, const int tid) {
-    constexpr int R = kRowsPerChunk;
-    constexpr int LT = ilog2(T);
-    constexpr int C4 = R * T;  // float4 per chunk
-    constexpr int LAST = K - 1;
+// float4 of the following chunk) -> Y, W for its C samples.  Returns the largest tagged,
+// sigma-unscaled key of the chunk's samples owned by this thread (for the activity map).
+template <int T, int R, int K, bool FAST, int PH>
+__device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, float4* __restrict__ pp,
+                                            float4* __restrict__ halo, int& xsel, int& hsel,
+                                            float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
+    using G = Geo<T, R, K>;
+    const int tid = cx.tid;
+    const float mu = cx.mu;
+    const uint32_t tm = cx.tm;
 
     float4 P[R], best[R];
     int lim[R];
@@ -222,163 +340,121 @@ __device__ __forceinline__ void tree_chunk(const float4* __restrict__ st4, float
         if constexpr (FAST) {
             lim[r] = 1 << 30;
         } else {
-            const long long left = n_t - (n0 + 4ll * (tid + T * r));
+            const long long left = cx.n_t - (cx.n0 + 4ll * (tid + T * r));
             lim[r] = left > (1ll << 30) ? (1 << 30) : (left < 0 ? 0 : static_cast<int>(left));
         }
         const float4 a = norm4(st4[tid + T * r], mu);
         if constexpr (K == 1) {
             P[r] = a;
-            if (FAST || do_out) best[r] = keyx<0, FAST>(a, lim[r], tm);
+            if (FAST || cx.do_out) best[r] = keyx<0, FAST>(a, lim[r], tm);
         } else {
             const float4 b = norm4(st4[tid + T * r + 1], mu);
             const float s01 = a.x + a.y, s12 = a.y + a.z, s23 = a.z + a.w, s34 = a.w + b.x;
             const float4 p1 = make_float4(s01, s12, s23, s34);
             if constexpr (K == 2) {
                 P[r] = p1;
-                if (FAST || do_out) best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm));
+                if (FAST || cx.do_out) best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm));
             } else {
                 const float s45 = b.x + b.y, s56 = b.y + b.z;
                 const float4 p2 = make_float4(s01 + s23, s12 + s34, s23 + s45, s34 + s56);
-                if (FAST || do_out)
-                    best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm), keyx<2, FAST>(p2, lim[r], tm));
+                if (FAST || cx.do_out)
+                    best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm),
+                                   keyx<2, FAST>(p2, lim[r], tm));
                 if constexpr (K == 3) {
                     P[r] = p2;
                 } else {
                     // Width 8 from a third float4 of raw samples: recomputing the width-4 sums of
-                    // the next float4 here costs 8 adds on an idle pipe and saves one whole
-                    // shared-memory exchange (the L1/shared data pipe is the binding unit).
+                    // the next float4 here costs 8 adds and saves one whole shared-memory
+                    // exchange (the L1/shared data pipe is the binding unit).
                     const float4 c = norm4(st4[tid + T * r + 2], mu);
                     const float s67 = b.z + b.w, s78 = b.w + c.x, s89 = c.x + c.y, s9a = c.y + c.z;
                     const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
                                                   (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
-                    if (FAST || do_out) fold<3, K, FAST>(best[r], p2, p3, lim[r], tm);
+                    if (FAST || cx.do_out) fold<3, K, FAST>(best[r], p2, p3, lim[r], tm);
                     P[r] = p3;
                 }
             }
         }
     }
 
-    // ---- exchange levels: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], 8 <= 2^k <= 2T -----------
+    // ---- exchange levels: 8 <= 2^k <= 2T ----------------------------------------------
     float4* const hr = halo + hsel * T;        // written by the previous (later-in-time) chunk
     float4* const hw = halo + (hsel ^ 1) * T;  // read by the next chunk
     hsel ^= 1;
-#pragma unroll
-    for (int k = 3; k <= LT + 1; ++k) {
-        if (k + 1 <= LAST) {
-            const int d4 = (1 << k) / 4;  // partner distance in float4
-            const int hoff = d4 - 2;      // sum of the halo sizes of the levels below
-            float4* const buf = pp + xsel * C4;
-            xsel ^= 1;
-#pragma unroll
-            for (int r = 0; r < R; ++r) buf[tid + T * r] = P[r];
-            if (tid < d4) hw[hoff + tid] = P[0];
-            __syncthreads();
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float4* src = buf + (tid + T * r + d4);
-                if (r == R - 1 && tid + d4 >= T) src = hr + (hoff + tid + d4 - T);
-                const float4 now = add4(P[r], *src);
-                if (FAST || do_out) {
-                    switch (k) {  // k is a compile-time constant after unrolling
-                        case 3: fold<4, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 4: fold<5, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 5: fold<6, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 6: fold<7, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 7: fold<8, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 8: fold<9, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 9: fold<10, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        case 10: fold<11, K, FAST>(best[r], P[r], now, lim[r], tm); break;
-                        default: break;
-                    }
-                }
-                P[r] = now;
-            }
-        }
-    }
+    exchange_levels<T, R, K, FAST, 3>(P, best, lim, pp, hr, hw, xsel, cx);
 
-    // ---- in-register levels: partner 1, 2, 4, 8 rows later (same thread) --------------
-    if constexpr (LAST >= LT + 3) {
-        float4 now[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) now[r] = add4(P[r], r + 1 < R ? P[r + 1] : dl.a);
-        dl.a = P[0];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            if (FAST || do_out) fold<LT + 3, K, FAST>(best[r], P[r], now[r], lim[r], tm);
-            P[r] = now[r];
-        }
-    }
-    if constexpr (LAST >= LT + 4) {
-        float4 now[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) now[r] = add4(P[r], r + 2 < R ? P[r + 2] : dl.b[r + 2 - R]);
-        dl.b[0] = P[0];
-        dl.b[1] = P[1];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            if (FAST || do_out) fold<LT + 4, K, FAST>(best[r], P[r], now[r], lim[r], tm);
-            P[r] = now[r];
-        }
-    }
-    if constexpr (LAST >= LT + 5) {
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 now = add4(P[r], dl.c[r]);
-            dl.c[r] = P[r];
-            if (FAST || do_out) fold<LT + 5, K, FAST>(best[r], P[r], now, lim[r], tm);
-            P[r] = now;
-        }
-    }
-    if constexpr (LAST >= LT + 6) {
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 now = add4(P[r], dl.d0[r]);
-            dl.d0[r] = dl.d1[r];
-            dl.d1[r] = P[r];
-            if (FAST || do_out) fold<LT + 6, K, FAST>(best[r], P[r], now, lim[r], tm);
-            P[r] = now;
-        }
-    }
+    // ---- in-register levels: partner 1, 2, 4, ... rows later (same thread) -------------
+    register_levels<T, R, K, FAST, PH, 0>(P, best, lim, dl, cx);
 
-    // ---- unpack and store: Y = key with the code bits cleared, W = inverted code --------
-    if (FAST || do_out) {
+    // ---- unpack and store: Y = key (code bits cleared) / sigma, W = inverted code ---------------------------
+    float top = __int_as_float(0xff800000);
+    if (FAST || cx.do_out) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (FAST || lim[r] > 0) {
-                const uint32_t kx = __float_as_uint(best[r].x), ky = __float_as_uint(best[r].y);
-                const uint32_t kz = __float_as_uint(best[r].z), kw = __float_as_uint(best[r].w);
-                const float4 y = make_float4(__uint_as_float(kx & tm) * inv, __uint_as_float(ky & tm) * inv,
-                                             __uint_as_float(kz & tm) * inv, __uint_as_float(kw & tm) * inv);
-                const int4 w = make_int4(static_cast<int>(~kx & kCodeMask), static_cast<int>(~ky & kCodeMask),
-                                         static_cast<int>(~kz & kCodeMask), static_cast<int>(~kw & kCodeMask));
-                const long long o = n0 + 4ll * (tid + T * r);
-                __stcs(reinterpret_cast<float4*>(out_snr + o), y);
-                __stcs(reinterpret_cast<int4*>(out_width + o), w);
+                const float4 kq = best[r];
+                top = fmax3(top, fmax3(kq.x, kq.y, kq.z), kq.w);
+                const float4 y = scale4(make_float4(__uint_as_float(__float_as_uint(kq.x) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.y) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.z) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.w) & tm)),
+                                        cx.inv);
+                const int4 w = make_int4(static_cast<int>(~__float_as_uint(kq.x) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.y) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.z) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
+                const long long o = cx.n0 + 4ll * (tid + T * r);
+                __stcs(reinterpret_cast<float4*>(cx.out_snr + o), y);
+                __stcs(reinterpret_cast<int4*>(cx.out_width + o), w);
             }
         }
     }
     // With no exchange level there is no barrier inside the step: add the one that
     // orders this step's stage reads before the next refill of the stage.
-    if constexpr (LAST < 4) __syncthreads();
+    if constexpr (G::LAST < 4) __syncthreads();
+    return top;
 }
 
-// Resident blocks per SM for T = 128.  3 (168 registers per thread, no spills) measured 3 %
-// faster than 4 (128 registers, 11 spilled delay registers): the kernel is bound by the
-// L1/shared data pipe, not by occupancy (profiles/r01b_*).
-#ifndef SPD_TREE_BPS128
-#define SPD_TREE_BPS128 3
-#endif
-constexpr int tree_blocks_per_sm(int T) { return T == 128 ? SPD_TREE_BPS128 : (T == 256 ? 2 : 1); }
+// Compile-time loop over the phases of the unrolled chunk loop.
+template <int PH, int U, typename F>
+__device__ __forceinline__ void static_phases(F&& f) {
+    if constexpr (PH < U) {
+        f(std::integral_constant<int, PH>{});
+        static_phases<PH + 1, U>(f);
+    }
+}
 
-template <int T>
+// Threads per block, rows per chunk and resident blocks per SM, per depth K.  Measured on
+// config 3 (K = 14; sweep of T in {64,128,256} x R in {1,2,4,8} x blocks):
+// T = 64 halves one exchange level away but leaves 2 warps per barrier group and cannot hide
+// the shared-memory latency (13.7-17.5 ms); T = 256 adds an exchange level (13.4 ms);
+// T = 128, R = 4, 3 blocks (168 registers, no spills) is fastest (11.5 ms).  Above
+// max_width 8192 the delay registers double: 2 blocks at K = 15, T = 256 and 1 block at K = 16.
+#ifndef SPD_TREE_ROWS
+#define SPD_TREE_ROWS 4
+#endif
+constexpr int kRows = SPD_TREE_ROWS;
+#ifdef SPD_TREE_T
+constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? imax(SPD_TREE_T, 128) : 256); }
+#else
+constexpr int tree_threads_for(int K) { return K <= 15 ? 128 : 256; }
+#endif
+#ifdef SPD_TREE_BPS
+constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 15 ? 2 : 1); }
+#else
+constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? 3 : (K == 15 ? 2 : 1); }
+#endif
+
+template <int T, int R>
 constexpr size_t tree_smem_bytes() {
-    constexpr size_t C = 16 * T;
+    constexpr size_t C = 4 * T * R;
     return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8;
 }
 
-template <int T, int K>
-__global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(const TreeParams p) {
-    constexpr int C = 16 * T;
+template <int T, int R, int K>
+__global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(const TreeParams p) {
+    using G = Geo<T, R, K>;
+    constexpr int C = G::C;
     constexpr int M = 1 << (K - 1);
     constexpr int GUARD = M > 8 ? M : 8;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -400,11 +476,23 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
     const int first_fast = max(c_lo, min(c_hi, c_fast_end));  // chunks [c_lo, first_fast) are fast
 
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
-    float* __restrict__ out_snr = p.out_snr + static_cast<long long>(d) * n_t;
-    int32_t* __restrict__ out_width = p.out_width + static_cast<long long>(d) * n_t;
-    const float mu = p.mean[d];
-    const float inv = 1.0f / p.sigma[d];
-    const uint32_t tm = p.tag_mask;
+    ChunkCtx cx;
+    cx.mu = p.mean[d];
+    const float sg = p.sigma[d];
+    cx.inv = 1.0f / sg;
+    cx.tm = p.tag_mask;
+    cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
+    cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
+    cx.n_t = n_t;
+    cx.tid = tid;
+    // Activity threshold on the sigma-unscaled key: Y = key / sigma >= thr  <=  key >= thr * sigma
+    // lowered by a few ulp so that rounding can only add chunks to the map, never drop one.
+    uint8_t* const act = p.activity ? p.activity + static_cast<long long>(d) * p.chunks_per_row : nullptr;
+    float thr_key = __int_as_float(0x7f800000);
+    if (act) {
+        const float t = p.threshold * sg;
+        thr_key = t - fabsf(t) * 2e-6f;
+    }
 
     for (int i = tid; i < 2 * T; i += T) halo[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (tid == 0) {
@@ -412,14 +500,9 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
         for (int i = 0; i < kStages; ++i) mbar_init(&bars[i], 1);
         fence_mbar_init();
     }
-    Delay dl;
-    {
-        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-        dl.a = z;
-        dl.b[0] = dl.b[1] = z;
+    float4 dl[G::ND + 1];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) dl.c[r] = dl.d0[r] = dl.d1[r] = z;
-    }
+    for (int i = 0; i < G::ND + 1; ++i) dl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     int xsel = 0, hsel = 0;
     __syncthreads();
 
@@ -428,11 +511,14 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
         const long long n0 = static_cast<long long>(c) * C;
         for (int i = tid; i < C + 8; i += T) {
             const long long n = n0 + i;
-            stages[i] = n < n_t ? __ldg(row + n) : mu;
+            stages[i] = n < n_t ? __ldg(row + n) : cx.mu;
         }
         __syncthreads();
-        tree_chunk<T, K, false>(reinterpret_cast<const float4*>(stages), pp, halo, xsel, hsel, dl, mu, inv, tm,
-                                out_snr, out_width, n0, n_t, c < c_hi, tid);
+        cx.n0 = n0;
+        cx.do_out = c < c_hi;
+        const float top = tree_chunk<T, R, K, false, 0>(reinterpret_cast<const float4*>(stages), pp, halo, xsel,
+                                                        hsel, dl, cx);
+        if (act && cx.do_out && top >= thr_key) act[c] = 1;
         __syncthreads();
     }
 
@@ -454,67 +540,73 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(T)) spd_tree_kernel(cons
     }
     int stage = 0;
     uint32_t phase = 0;
-    for (int it = 0; it < n_fast; ++it) {
-        if (tid == 0) {
-            const int nx = it + kStages - 1;
-            if (nx < n_fast) {
-                const int sx = stage == 0 ? kStages - 1 : stage - 1;  // (it + kStages - 1) % kStages
-                mbar_arrive_expect_tx(&bars[sx], kBytes);
-                bulk_g2s(stages + sx * (C + 8), row + static_cast<long long>(first_fast - 1 - nx) * C, kBytes,
-                         &bars[sx]);
+    cx.do_out = true;
+    int it = 0;
+    while (it < n_fast) {
+        static_phases<0, G::U>([&](auto ph) {
+            if (it < n_fast) {
+                if (tid == 0) {
+                    const int nx = it + kStages - 1;
+                    if (nx < n_fast) {
+                        const int sx = stage == 0 ? kStages - 1 : stage - 1;  // (it + kStages - 1) % kStages
+                        mbar_arrive_expect_tx(&bars[sx], kBytes);
+                        bulk_g2s(stages + sx * (C + 8), row + static_cast<long long>(first_fast - 1 - nx) * C,
+                                 kBytes, &bars[sx]);
+                    }
+                }
+                mbar_wait(&bars[stage], phase);
+                const int c = first_fast - 1 - it;
+                cx.n0 = static_cast<long long>(c) * C;
+                const float top = tree_chunk<T, R, K, true, decltype(ph)::value>(
+                    reinterpret_cast<const float4*>(stages + stage * (C + 8)), pp, halo, xsel, hsel, dl, cx);
+                if (act && top >= thr_key) act[c] = 1;
+                if (++stage == kStages) {
+                    stage = 0;
+                    phase ^= 1;
+                }
+                ++it;
             }
-        }
-        mbar_wait(&bars[stage], phase);
-        const long long n0 = static_cast<long long>(first_fast - 1 - it) * C;
-        tree_chunk<T, K, true>(reinterpret_cast<const float4*>(stages + stage * (C + 8)), pp, halo, xsel, hsel,
-                               dl, mu, inv, tm, out_snr, out_width, n0, n_t, true, tid);
-        if (++stage == kStages) {
-            stage = 0;
-            phase ^= 1;
-        }
+        });
     }
 }
 
-template <int T, int K>
+template <int T, int R, int K>
 cudaError_t launch_tree(const TreeConfig& cfg, const TreeParams& prm, int64_t n_dm, cudaStream_t stream) {
     const dim3 grid(static_cast<unsigned>(n_dm * cfg.segs_per_row));
-    spd_tree_kernel<T, K><<<grid, T, cfg.smem_bytes, stream>>>(prm);
+    spd_tree_kernel<T, R, K><<<grid, T, cfg.smem_bytes, stream>>>(prm);
     return cudaGetLastError();
 }
 
-template <int T, int K>
+template <int T, int R, int K>
 cudaError_t prepare_tree(TreeConfig& cfg) {
-    cfg.smem_bytes = tree_smem_bytes<T>();
-    if (const char* env = std::getenv("SPD_TREE_PAD_SMEM")) cfg.smem_bytes += static_cast<size_t>(std::atoll(env));
-    cudaError_t e = cudaFuncSetAttribute(spd_tree_kernel<T, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cfg.smem_bytes = tree_smem_bytes<T, R>();
+    cudaError_t e = cudaFuncSetAttribute(spd_tree_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(cfg.smem_bytes));
     if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, K>, T, cfg.smem_bytes);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, R, K>, T, cfg.smem_bytes);
     if (e != cudaSuccess) return e;
     cfg.blocks_per_sm = nb;
     return cudaSuccess;
 }
 
-#define SPD_TREE_CASES(OP)      \
-    OP(128, 1)                  \
-    OP(128, 2)                  \
-    OP(128, 3)                  \
-    OP(128, 4)                  \
-    OP(128, 5)                  \
-    OP(128, 6)                  \
-    OP(128, 7)                  \
-    OP(128, 8)                  \
-    OP(128, 9)                  \
-    OP(128, 10)                 \
-    OP(128, 11)                 \
-    OP(128, 12)                 \
-    OP(128, 13)                 \
-    OP(128, 14)                 \
-    OP(256, 15)                 \
-    OP(512, 16)
-
-constexpr int tree_threads_for(int K) { return K <= 14 ? 128 : (K == 15 ? 256 : 512); }
+#define SPD_TREE_CASES(OP) \
+    OP(1)                  \
+    OP(2)                  \
+    OP(3)                  \
+    OP(4)                  \
+    OP(5)                  \
+    OP(6)                  \
+    OP(7)                  \
+    OP(8)                  \
+    OP(9)                  \
+    OP(10)                 \
+    OP(11)                 \
+    OP(12)                 \
+    OP(13)                 \
+    OP(14)                 \
+    OP(15)                 \
+    OP(16)
 
 }  // namespace
 
@@ -531,10 +623,10 @@ int tree_configure(spd_plan* plan) {
     TreeConfig& cfg = plan->tree;
     cfg.K = static_cast<int>(plan->widths.size());
     cfg.T = tree_threads_for(cfg.K);
-    cfg.chunk = 16 * cfg.T;
+    cfg.chunk = 4 * cfg.T * kRows;
     cudaError_t e = cudaErrorInvalidValue;
-#define SPD_PREP(TT, KK) \
-    if (cfg.K == KK) e = prepare_tree<TT, KK>(cfg);
+#define SPD_PREP(KK) \
+    if (cfg.K == KK) e = prepare_tree<tree_threads_for(KK), kRows, KK>(cfg);
     SPD_TREE_CASES(SPD_PREP)
 #undef SPD_PREP
     if (e != cudaSuccess) return cuda_fail(e, "configuring the dyadic-tree kernel");
@@ -568,7 +660,7 @@ int tree_configure(spd_plan* plan) {
 }
 
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-             float* out_snr, int32_t* out_width, cudaStream_t stream) {
+             float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
     const TreeConfig& cfg = plan->tree;
     TreeParams prm;
     prm.plane = plane;
@@ -576,15 +668,24 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     prm.sigma = sigma;
     prm.out_snr = out_snr;
     prm.out_width = out_width;
+    prm.activity = activity;
+    prm.threshold = threshold;
     prm.n_t = plan->n_t;
     prm.chunks_per_row = cfg.chunks_per_row;
     prm.seg_chunks = cfg.seg_chunks;
     prm.segs_per_row = cfg.segs_per_row;
     prm.warm_chunks = cfg.warm_chunks;
     prm.tag_mask = ~kCodeMask;
-    cudaError_t e = cudaErrorInvalidValue;
-#define SPD_LAUNCH(TT, KK) \
-    if (cfg.K == KK) e = launch_tree<TT, KK>(cfg, prm, n_dm, stream);
+    cudaError_t e = cudaSuccess;
+    if (activity) {
+        // the map is padded to a multiple of 128 bytes; the padding is cleared too
+        const size_t bytes = (static_cast<size_t>(n_dm) * cfg.chunks_per_row + 127) / 128 * 128;
+        e = cudaMemsetAsync(activity, 0, bytes, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "clearing the activity map");
+    }
+    e = cudaErrorInvalidValue;
+#define SPD_LAUNCH(KK) \
+    if (cfg.K == KK) e = launch_tree<tree_threads_for(KK), kRows, KK>(cfg, prm, n_dm, stream);
     SPD_TREE_CASES(SPD_LAUNCH)
 #undef SPD_LAUNCH
     if (e != cudaSuccess) return cuda_fail(e, "launching the dyadic-tree kernel");

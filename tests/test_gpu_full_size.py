@@ -1,0 +1,187 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(spd_run_flagged + spd_find_candidates_flagged through the C ABI).
+
+The planes (up to 16 GiB) never leave the device; the oracle is run on sampled windows it can
+compute one by one - around injected pulses, at row starts and row tails, across the kernel's
+chunk and segment boundaries, and at random places - by direct summation (oracle A) and, on
+longer windows, by the double-precision running sum (oracle B).  A window is a piece of one row
+copied to the host together with the max_width - 1 samples that follow it, so every boxcar of
+every compared sample lies inside the piece (windows that reach the end of the row exercise the
+valid-windows-only rule instead).  Properties that hold at any size are checked on the whole
+plane with integer / comparison tensor ops: width indices in range, Y finite, Y >= SNR of width 1
+(width 1 is in every set used here), last sample of each row takes width 1, and the candidate list
+equals the reading-A9 rule applied to the CUDA plane (exact integer comparison).
+"""
+import numpy as np
+import pytest
+
+import parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def spd():
+    import paper_1910_08324_b200 as spd
+    spd.build()
+    spd.load()
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return spd
+
+
+def _window_list(w, info, pulses, rng, n_random):
+    """(row, t0, span, kind) windows; span samples are compared."""
+    M, n_t, n_dm = w.max_width, w.n_t, w.n_dm
+    chunk = max(info["chunk"], 1)
+    segs = max(info["segments_per_row"], 1)
+    out = []
+    direct_span = 1536 if M <= 8192 else 512
+    # injected pulses: start of the pulse, its matched boxcars begin up to M samples earlier
+    for p in pulses[:: max(1, len(pulses) // 12)]:
+        t0 = max(0, p.t0 - direct_span // 2)
+        out.append((p.dm, t0, min(direct_span, n_t - t0), "pulse"))
+    # row starts and row tails (tail rule A3)
+    for d in (0, n_dm - 1, int(rng.integers(0, n_dm))):
+        out.append((d, 0, direct_span, "row-start"))
+        out.append((d, n_t - direct_span, direct_span, "row-tail"))
+        out.append((d, n_t - M - direct_span // 2, direct_span, "tail-onset"))
+    # segment and chunk boundaries of the launch configuration
+    chunks_per_row = (n_t + chunk - 1) // chunk
+    seg_chunks = (chunks_per_row + segs - 1) // segs
+    for s in range(1, segs)[:3]:
+        b = s * seg_chunks * chunk
+        out.append((int(rng.integers(0, n_dm)), b - direct_span // 2, direct_span, "segment-boundary"))
+    for _ in range(3):
+        b = int(rng.integers(1, chunks_per_row)) * chunk
+        out.append((int(rng.integers(0, n_dm)), b - direct_span // 2, direct_span, "chunk-boundary"))
+    for _ in range(n_random):
+        t0 = int(rng.integers(0, n_t - direct_span))
+        out.append((int(rng.integers(0, n_dm)), t0, direct_span, "random"))
+    return out
+
+
+def _check_window(oracle, plane, snr, idx, mean_h, sigma_h, widths, M, row, t0, span, direct, what):
+    n_t = plane.shape[1]
+    t0 = max(0, min(int(t0), n_t - 1))
+    span = int(min(span, n_t - t0))
+    t_end = min(n_t, t0 + span + M - 1)
+    seg = plane[row, t0:t_end].cpu().numpy()[None, :]
+    got_snr = snr[row, t0:t0 + span].cpu().numpy()[None, :]
+    got_idx = idx[row, t0:t0 + span].cpu().numpy()[None, :]
+    mu, sg = float(mean_h[row]), float(sigma_h[row])
+    if direct:
+        ref_snr, ref_idx, ref_sec = oracle.spd_direct(seg, mu, sg, widths, 0, span)
+    else:
+        ref_snr, ref_idx, ref_sec = oracle.spd_prefix(seg, mu, sg, widths)
+        ref_snr, ref_idx, ref_sec = ref_snr[:, :span], ref_idx[:, :span], ref_sec[:, :span]
+    return parity.assert_parity(oracle, seg, mu, sg, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                                what=f"{what} row {row} t0 {t0}")
+
+
+def _whole_plane_properties(plane, mean, sigma, snr, idx, n_widths, rows_per_block=64):
+    n_dm, n_t = plane.shape
+    for r0 in range(0, n_dm, rows_per_block):
+        r1 = min(n_dm, r0 + rows_per_block)
+        y, k = snr[r0:r1], idx[r0:r1]
+        assert bool(torch.isfinite(y).all()), "non-finite SNR"
+        assert int(k.min()) >= 0 and int(k.max()) < n_widths, "width index out of range"
+        # width 1 is in the set: Y >= (x - mu) / sigma within the tolerance
+        s1 = (plane[r0:r1] - mean[r0:r1, None]) / sigma[r0:r1, None]
+        tol = parity.SNR_RTOL * torch.clamp(s1.abs(), min=1.0)
+        assert bool((y >= s1 - tol).all()), "best SNR below the width-1 SNR"
+        del s1, tol
+        assert bool((k[:, -1] == 0).all()), "last sample of a row must take width 1 (reading A3)"
+
+
+def _rule_candidates(snr, thr, rows_per_block=64):
+    """Reading A9 on the CUDA plane with comparison ops only -> sorted int64 keys dm * n_t + t."""
+    n_dm, n_t = snr.shape
+    keys = []
+    ninf = torch.full((1,), float("-inf"), device=snr.device)
+    for r0 in range(0, n_dm, rows_per_block):
+        y = snr[r0:r0 + rows_per_block]
+        prev = torch.cat([ninf.expand(y.shape[0], 1), y[:, :-1]], dim=1)
+        nxt = torch.cat([y[:, 1:], ninf.expand(y.shape[0], 1)], dim=1)
+        hit = (y >= thr) & (y > prev) & (y >= nxt)
+        del prev, nxt
+        rr, tt = torch.nonzero(hit, as_tuple=True)
+        keys.append((rr + r0) * n_t + tt)
+    return torch.sort(torch.cat(keys))[0]
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_config(spd, oracle_lib, cfg):
+    import ctypes
+    from workloads import get_workload, make_plane_torch
+    w = get_workload(cfg)
+    dev = torch.device("cuda:0")
+    free, _ = torch.cuda.mem_get_info(dev)
+    need = 13 * w.n_samples + (6 << 30)
+    if free < need:
+        pytest.skip(f"config {cfg} needs {need >> 30} GiB of device memory, {free >> 30} GiB free")
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    plane, pulses = make_plane_torch(w, dev)
+    if w.stats == "measured":  # reading A6: per-row mean and population sigma, in double
+        mean = torch.cat([plane[r:r + 64].double().mean(dim=1) for r in range(0, w.n_dm, 64)]).float()
+        sigma = torch.cat([plane[r:r + 64].double().std(dim=1, unbiased=False)
+                           for r in range(0, w.n_dm, 64)]).float()
+    else:
+        mean = torch.zeros(w.n_dm, device=dev)
+        sigma = torch.ones(w.n_dm, device=dev)
+    thr = w.candidate_threshold if w.candidate_threshold is not None else 6.0
+    cap = 1 << 22
+    with spd.Plan(w.n_dm, w.n_t, widths, w.max_width) as plan:
+        info = dict(plan.info)
+        assert info["path"] == spd.SPD_PATH_DYADIC_TREE
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, thr)
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, thr, cap)
+        torch.cuda.synchronize()
+        count, cands = spd.candidates_to_numpy(lst, n_found, cap)
+
+    # ---- sampled windows against the oracle ------------------------------------------------
+    mean_h, sigma_h = mean.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+    rng = np.random.default_rng(w.seed + 17)
+    worst, n_cmp = 0.0, 0
+    for row, t0, span, kind in _window_list(w, info, pulses, rng, n_random=6):
+        st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, w.max_width, row, t0, span,
+                           direct=True, what=f"config {cfg} {kind}")
+        worst, n_cmp = max(worst, st.max_err_over_tol), n_cmp + st.n
+    # longer windows with the running-sum oracle (itself pinned to direct summation)
+    for _ in range(4):
+        row = int(rng.integers(0, w.n_dm))
+        span = min(1 << 18, w.n_t - w.max_width)
+        t0 = int(rng.integers(0, w.n_t - span - w.max_width + 1))
+        st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, w.max_width, row, t0, span,
+                           direct=False, what=f"config {cfg} long")
+        worst, n_cmp = max(worst, st.max_err_over_tol), n_cmp + st.n
+    row = int(rng.integers(0, w.n_dm))
+    span = min(1 << 18, w.n_t)
+    st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, w.max_width, row, w.n_t - span, span,
+                       direct=False, what=f"config {cfg} long-tail")
+    worst, n_cmp = max(worst, st.max_err_over_tol), n_cmp + st.n
+    assert worst <= 1.0 and n_cmp > 1 << 19
+
+    # ---- properties of the whole plane ------------------------------------------------------
+    _whole_plane_properties(plane, mean, sigma, snr, idx, len(widths))
+
+    # ---- candidate list = the rule on the CUDA plane (exact) --------------------------------
+    ref_keys = _rule_candidates(snr, thr)
+    assert count == int(ref_keys.numel()), f"config {cfg}: {count} candidates, rule gives {ref_keys.numel()}"
+    if count <= cap:
+        got_keys = torch.from_numpy(cands["dm"].astype(np.int64) * w.n_t + cands["t"].astype(np.int64)).to(dev)
+        assert torch.equal(torch.sort(got_keys)[0], ref_keys)
+        sel = torch.from_numpy(cands["dm"].astype(np.int64)).to(dev), torch.from_numpy(cands["t"].astype(np.int64)).to(dev)
+        assert torch.equal(snr[sel], torch.from_numpy(cands["snr"]).to(dev))
+        assert torch.equal(idx[sel], torch.from_numpy(cands["width_idx"]).to(dev))
+    else:
+        assert len(cands) == cap
+    # every injected pulse clear of the threshold is detected near its start
+    if count <= cap:
+        hit = 0
+        strong = [p for p in pulses if p.snr_t >= thr + 4.0]
+        for p in strong:
+            m = (cands["dm"] == p.dm) & (np.abs(cands["t"].astype(np.int64) - p.t0) <= 2 * p.width + 4)
+            hit += bool(m.any())
+        assert hit >= 0.95 * len(strong), f"config {cfg}: only {hit} of {len(strong)} strong pulses detected"

@@ -265,6 +265,107 @@ def test_candidates_against_oracle_plane_tolerance_aware(spd, oracle_lib):
     covered(got["dm"], got["t"], got["snr"], got["width_idx"], o_dm, o_t, o_snr)
 
 
+def _activity_truth(snr_h, block, per_row, thr):
+    """Per-block 'some Y >= thr' map of a host SNR plane."""
+    n_dm, n_t = snr_h.shape
+    pad = per_row * block - n_t
+    y = np.pad(snr_h, ((0, 0), (0, pad)), constant_values=-np.inf) if pad else snr_h
+    return (y.reshape(n_dm, per_row, block) >= thr).any(axis=2)
+
+
+@pytest.mark.parametrize("cfg,n_dm,n_t,thr,segs", [(3, 6, 262144 + 4 * 11, 6.0, None), (5, 4, 262144, 6.0, "3"),
+                                                     (2, 8, 65536, 4.5, None), (3, 3, 40000, 3.0, "2")])
+def test_flagged_run_equals_plain_run_and_dense_candidates(spd, oracle_lib, cfg, n_dm, n_t, thr, segs,
+                                                           monkeypatch):
+    """Row a8 fused: spd_run_flagged writes the same Y, W as spd_run; its activity map marks every block
+    that holds a sample >= threshold (and may mark no block whose samples are all clearly below it);
+    spd_find_candidates_flagged returns exactly the list of the visit-everything kernel, which equals
+    the reading-A9 rule evaluated by the oracle on that plane."""
+    from workloads import get_workload, make_plane_numpy
+    if segs:
+        monkeypatch.setenv("SPD_SEGS_PER_ROW", segs)
+    w = get_workload(cfg).scaled(n_dm, n_t, 12)
+    x, _ = make_plane_numpy(w)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, min(w.max_width, 8192))
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    rng = np.random.default_rng(3)
+    mean = torch.from_numpy((0.01 * rng.standard_normal(n_dm)).astype(np.float32)).to(dev)
+    sigma = torch.from_numpy((1.0 + 0.3 * rng.random(n_dm)).astype(np.float32)).to(dev)
+    cap = 1 << 20
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_DYADIC_TREE
+        snr0, idx0 = plan.run(plane, mean, sigma)
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, thr)
+        assert torch.equal(snr0, snr) and torch.equal(idx0, idx)
+        block, per_row = plan.info["activity_block"], plan.info["activity_per_row"]
+        assert plan.info["activity_bytes"] % 128 == 0 and plan.info["activity_bytes"] >= n_dm * per_row
+        snr_h = snr.cpu().numpy()
+        act_h = act.cpu().numpy()
+        assert not act_h[n_dm * per_row:].any(), "padding of the activity map must be cleared"
+        got_map = act_h[: n_dm * per_row].reshape(n_dm, per_row) != 0
+        must = _activity_truth(snr_h, block, per_row, thr)
+        may = _activity_truth(snr_h, block, per_row, thr * (1 - 1e-5) - 1e-5)
+        assert not (must & ~got_map).any(), "a block holding a sample >= threshold is not marked"
+        assert not (got_map & ~may).any(), "a block clearly below the threshold is marked"
+        lst_d, n_d = plan.find_candidates(snr, idx, thr, cap)
+        count_d, dense = spd.candidates_to_numpy(lst_d, n_d, cap)
+        lst_f, n_f = plan.find_candidates_flagged(snr, idx, act, thr, cap)
+        count_f, flagged = spd.candidates_to_numpy(lst_f, n_f, cap)
+        assert count_f == count_d and count_d > 0
+        assert np.array_equal(dense, flagged)
+        ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr_h, idx.cpu().numpy(), thr)
+        assert count_f == ref_count
+        assert np.array_equal(flagged["dm"], c_dm) and np.array_equal(flagged["t"], c_t)
+        assert np.array_equal(flagged["snr"], c_snr) and np.array_equal(flagged["width_idx"], c_w)
+        # a higher threshold with the same (lower-threshold) map is allowed
+        lst_h, n_h = plan.find_candidates_flagged(snr, idx, act, thr + 2.0, cap)
+        count_h, _ = spd.candidates_to_numpy(lst_h, n_h, cap)
+        assert count_h == oracle_lib.find_candidates(snr_h, idx.cpu().numpy(), thr + 2.0)[0]
+        # overflow keeps counting
+        lst_o, n_o = plan.find_candidates_flagged(snr, idx, act, thr, 3)
+        count_o, got_o = spd.candidates_to_numpy(lst_o, n_o, 3)
+        assert count_o == ref_count and len(got_o) == min(3, ref_count)
+
+
+def test_flagged_run_generic_path_marks_everything(spd, oracle_lib):
+    rng = np.random.default_rng(21)
+    x = rng.standard_normal((3, 20000), dtype=np.float32)
+    x[1, 7000:7030] += np.float32(2.0)
+    widths = spd.spd_width_set_generate("IGRID", 1, 64)
+    dev = torch.device("cuda:0")
+    with spd.Plan(3, 20000, widths) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GENERIC
+        snr, idx, act = plan.run_flagged(torch.from_numpy(x).to(dev), torch.zeros(3, device=dev),
+                                         torch.ones(3, device=dev), 5.0)
+        assert bool((act != 0).all())
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, 5.0, 1 << 16)
+        count, got = spd.candidates_to_numpy(lst, n_found, 1 << 16)
+        ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.cpu().numpy(), idx.cpu().numpy(), 5.0)
+        assert count == ref_count and count > 0
+        assert np.array_equal(got["dm"], c_dm) and np.array_equal(got["t"], c_t)
+
+
+def test_flagged_no_detections_and_all_detections(spd):
+    """Degenerate maps: nothing above the threshold (empty list, empty map) and everything above it."""
+    rng = np.random.default_rng(22)
+    x = (0.01 * rng.standard_normal((2, 32768))).astype(np.float32)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(2, device=dev), torch.ones(2, device=dev)
+    with spd.Plan(2, 32768, [1 << k for k in range(8)]) as plan:
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 6.0)
+        assert not bool(act.any())
+        _, n0 = plan.find_candidates_flagged(snr, idx, act, 6.0, 16)
+        assert int(n0.item()) == 0
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, -1e30)
+        per_row = plan.info["activity_per_row"]
+        assert bool((act[: 2 * per_row] != 0).all())
+        _, n1 = plan.find_candidates_flagged(snr, idx, act, -1e30, 16)
+        lst_d, n_d = plan.find_candidates(snr, idx, -1e30, 16)
+        assert int(n1.item()) == int(n_d.item()) > 0
+
+
 def test_run_host_equals_device_run(spd):
     """The end-to-end host entry point (several row blocks) returns exactly what spd_run does."""
     rng = np.random.default_rng(11)
