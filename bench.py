@@ -56,6 +56,29 @@ def dist_env():
         int(os.environ.get("WORLD_SIZE", "1"))
 
 
+def rank_workload(w, rank):
+    """Weak scaling: every rank holds its own n_dm DM trials of the same recipe (its own seed);
+    DM trials are independent, so there is no data-path exchange."""
+    from dataclasses import replace
+    return replace(w, seed=w.seed + 1000003 * rank)
+
+
+def max_over_ranks(ms, device=None):
+    """Device-timed milliseconds -> max over the ranks of the job (identity without a process group)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, samples_per_rank, ms_per_step):
+    """DM-time samples/s of the whole job: all ranks' samples over the slowest rank's step time."""
+    return world * samples_per_rank / (ms_per_step * 1e-3)
+
+
 def workload_config(w, widths, extra=None):
     cfg = {
         "workload": f"configs[{w.index - 1}] {w.name}: {w.n_dm} DM trials x {w.n_t} samples float32 per GPU",
@@ -242,8 +265,7 @@ def run_b200(args):
     if args.n_dm:
         w = w.scaled(args.n_dm, w.n_t)
     # weak scaling: every rank holds its own n_dm DM trials (different seed per rank)
-    from dataclasses import replace
-    w_rank = replace(w, seed=w.seed + 1000003 * rank)
+    w_rank = rank_workload(w, rank)
     widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
     n = w.n_samples
 
@@ -316,12 +338,9 @@ def run_b200(args):
     if flush is not None:  # the flush is not part of the path: take it out of the step time
         flush_ms = total_ms - sum(run_ms) - sum(cand_ms)
         total_ms = sum(run_ms) + sum(cand_ms)
-    if distributed:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
+    value = whole_job_value(world, n, ms_per_step)
     n_cand = int(n_found.item())
 
     # ---- roofline of the dominant kernel (the spd_run kernel) ---------------------------
@@ -430,10 +449,7 @@ def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
             if i > 0:
                 times.append(dt)
     dt = sum(times) / len(times)
-    if distributed:
-        t = torch.tensor([dt], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        dt = float(t.item())
+    dt = max_over_ranks(dt, dev)
     checksum = float(h_snr[0, :1024].double().sum().item())
     return {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": 4 * n + 8 * rows,
             "d2h_bytes_per_step": 8 * n, "ms_per_step": 1e3 * dt, "steps": len(times), "rows": rows,

@@ -24,8 +24,7 @@
 //     Levels 2^k >= 4T: the partner is the SAME thread's float4 1, 2, 4, ... rows later,
 //     i.e. a register of this chunk or a delay register kept from the previous chunks.
 //     The shared-memory data pipe is the binding unit (profiles/r01b_*), so T is as small
-//     as the register file allows: T = 64 up to max_width 8192 (5 exchange levels,
-//     31 float4 of delay registers), doubling with max_width above that.
+//     as the register file and the instruction cache allow (geometry table below).
 //   * Delay lines deeper than one chunk are register FIFOs; the chunk loop is unrolled
 //     over the FIFO depth so that the FIFO slot is a compile-time constant (no moves).
 //   * Chunks are staged into shared memory by cp.async.bulk (TMA, 1-D) through a
@@ -217,6 +216,14 @@ __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
     }
 }
 
+// The chunk loop is unrolled over the delay FIFOs up to this factor: a FIFO no deeper than
+// the unroll gets a compile-time slot (no register moves), a deeper one is rotated by moves.
+// Code size grows with the factor; past the instruction cache the kernel stalls on fetch
+// (T = 64, R = 4 unrolled x4: smsp stall_no_instruction 2.6 per issue).
+#ifndef SPD_TREE_MAX_UNROLL
+#define SPD_TREE_MAX_UNROLL 2
+#endif
+
 constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
 constexpr int imax(int a, int b) { return a > b ? a : b; }
 
@@ -231,7 +238,8 @@ struct Geo {
     static constexpr int J = imax(0, LAST - LT - 2);
     static constexpr int ND = (1 << J) - 1;  // float4 of delay registers: sum of 2^j
     // Depth, in chunks, of the deepest delay FIFO = unroll factor of the chunk loop.
-    static constexpr int U = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
+    static constexpr int TOPQ = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
+    static constexpr int U = TOPQ < SPD_TREE_MAX_UNROLL ? TOPQ : SPD_TREE_MAX_UNROLL;
 };
 
 struct ChunkCtx {
@@ -294,10 +302,11 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
             // (the chunk loop is unrolled over the deepest FIFO); guarded steps keep the
             // FIFO in canonical order (slot 0 oldest) by moving registers.
             constexpr int Q = D / R;
-            constexpr int slot = FAST ? (PH % Q) : 0;
+            constexpr bool kSlotted = FAST && G::U >= Q;  // slot known at compile time
+            constexpr int slot = kSlotted ? (PH % Q) : 0;
 #pragma unroll
             for (int r = 0; r < R; ++r) now[r] = add4(P[r], dl[off + slot * R + r]);
-            if constexpr (FAST) {
+            if constexpr (kSlotted) {
 #pragma unroll
                 for (int r = 0; r < R; ++r) dl[off + slot * R + r] = P[r];
             } else {
