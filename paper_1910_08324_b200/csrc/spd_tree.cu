@@ -105,6 +105,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
         "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem),
+                 "r"(smem_u32(src_smem)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -216,6 +224,10 @@ __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
     }
 }
 
+#ifndef SPD_TREE_TMA_STORE
+#define SPD_TREE_TMA_STORE 0  // measured: 11.87 ms vs 11.41 ms with direct 128-bit stores (config 3)
+#endif
+
 // The chunk loop is unrolled over the delay FIFOs up to this factor: a FIFO no deeper than
 // the unroll gets a compile-time slot (no register moves), a deeper one is rotated by moves.
 // Code size grows with the factor; past the instruction cache the kernel stalls on fetch
@@ -223,6 +235,7 @@ __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
 #ifndef SPD_TREE_MAX_UNROLL
 #define SPD_TREE_MAX_UNROLL 2
 #endif
+constexpr int tree_max_unroll(int K) { return K == 16 ? 4 : SPD_TREE_MAX_UNROLL; }
 
 constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
 constexpr int imax(int a, int b) { return a > b ? a : b; }
@@ -238,11 +251,17 @@ struct Geo {
     static constexpr int J = imax(0, LAST - LT - 2);
     static constexpr int ND = (1 << J) - 1;  // float4 of delay registers: sum of 2^j
     // Depth, in chunks, of the deepest delay FIFO = unroll factor of the chunk loop.
+    // Optional: unguarded chunks leave through a shared-memory staging buffer and two bulk
+    // stores (Y, W) instead of 128-bit global stores.  Off by default: the extra barrier and
+    // shared-memory stores cost more than the global stores they replace (DESIGN.md "Tuning
+    // log").  Needs an exchange level (its barrier orders the reuse of the staging buffer).
+    static constexpr bool TMA_STORE = SPD_TREE_TMA_STORE && LAST >= 4;
     static constexpr int TOPQ = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
-    static constexpr int U = TOPQ < SPD_TREE_MAX_UNROLL ? TOPQ : SPD_TREE_MAX_UNROLL;
+    static constexpr int U = TOPQ < tree_max_unroll(K) ? TOPQ : tree_max_unroll(K);
 };
 
 struct ChunkCtx {
+    float4* sout;  // staging of one chunk's Y (C floats) then W (C ints)
     float mu, inv;
     uint32_t tm;
     float* __restrict__ out_snr;
@@ -267,6 +286,11 @@ __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R
 #pragma unroll
         for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
         if (tid < d4) hw[hoff + tid] = P[0];
+        // the previous chunk's bulk stores must have read the staging buffer before any
+        // thread passes this barrier on its way to refilling it
+        if constexpr (FAST && G::TMA_STORE && k == 3) {
+            if (tid == 0) bulk_wait_read0();
+        }
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -412,10 +436,24 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
                                          static_cast<int>(~__float_as_uint(kq.y) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.z) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
-                const long long o = cx.n0 + 4ll * (tid + T * r);
-                __stcs(reinterpret_cast<float4*>(cx.out_snr + o), y);
-                __stcs(reinterpret_cast<int4*>(cx.out_width + o), w);
+                if constexpr (FAST && G::TMA_STORE) {
+                    cx.sout[tid + T * r] = y;
+                    reinterpret_cast<int4*>(cx.sout + G::C4)[tid + T * r] = w;
+                } else {
+                    const long long o = cx.n0 + 4ll * (tid + T * r);
+                    *reinterpret_cast<float4*>(cx.out_snr + o) = y;
+                    *reinterpret_cast<int4*>(cx.out_width + o) = w;
+                }
             }
+        }
+    }
+    if constexpr (FAST && G::TMA_STORE) {
+        fence_proxy_async();
+        __syncthreads();
+        if (tid == 0) {
+            bulk_s2g(cx.out_snr + cx.n0, cx.sout, G::C * 4);
+            bulk_s2g(cx.out_width + cx.n0, cx.sout + G::C4, G::C * 4);
+            bulk_commit();
         }
     }
     // With no exchange level there is no barrier inside the step: add the one that
@@ -433,31 +471,29 @@ __device__ __forceinline__ void static_phases(F&& f) {
     }
 }
 
-// Threads per block, rows per chunk and resident blocks per SM, per depth K.  Measured on
-// config 3 (K = 14; sweep of T in {64,128,256} x R in {1,2,4,8} x blocks):
-// T = 64 halves one exchange level away but leaves 2 warps per barrier group and cannot hide
-// the shared-memory latency (13.7-17.5 ms); T = 256 adds an exchange level (13.4 ms);
-// T = 128, R = 4, 3 blocks (168 registers, no spills) is fastest (11.5 ms).  Above
-// max_width 8192 the delay registers double: 2 blocks at K = 15, T = 256 and 1 block at K = 16.
+// Threads per block T, rows per chunk R and resident blocks per SM, per depth K (measured
+// sweeps in DESIGN.md "Tuning log").  K <= 14: T = 128, R = 4, 3 blocks (165 registers, no
+// spills): 11.5 ms on config 3.  T = 64 (one exchange level fewer) ties at 11.7 ms once its
+// chunk loop is not unrolled past the instruction cache, T = 256 (one more) is at 13.4 ms.
+// Above max_width 8192 the delay registers double: K = 15 runs 2 blocks of 128 threads
+// (247 registers), K = 16 one block of 512 threads with R = 2.
+#ifndef SPD_TREE_T
+#define SPD_TREE_T 128  // K <= 14
+#endif
 #ifndef SPD_TREE_ROWS
 #define SPD_TREE_ROWS 4
 #endif
-constexpr int kRows = SPD_TREE_ROWS;
-#ifdef SPD_TREE_T
-constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? imax(SPD_TREE_T, 128) : 256); }
-#else
-constexpr int tree_threads_for(int K) { return K <= 15 ? 128 : 256; }
+#ifndef SPD_TREE_BPS
+#define SPD_TREE_BPS 3
 #endif
-#ifdef SPD_TREE_BPS
+constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? 128 : 512); }
+constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : (K == 15 ? 4 : 2); }
 constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 15 ? 2 : 1); }
-#else
-constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? 3 : (K == 15 ? 2 : 1); }
-#endif
 
-template <int T, int R>
+template <int T, int R, int K>
 constexpr size_t tree_smem_bytes() {
     constexpr size_t C = 4 * T * R;
-    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8;
+    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + (Geo<T, R, K>::TMA_STORE ? 2 * C * 4 : 0) + kStages * 8;
 }
 
 template <int T, int R, int K>
@@ -470,7 +506,8 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     float4* const pp = reinterpret_cast<float4*>(smem_raw);
     float* const stages = reinterpret_cast<float*>(smem_raw + 2 * C * 4);
     float4* const halo = reinterpret_cast<float4*>(stages + kStages * (C + 8));
-    uint64_t* const bars = reinterpret_cast<uint64_t*>(halo + 2 * T);
+    float4* const sout = halo + 2 * T;
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sout + (G::TMA_STORE ? 2 * G::C4 : 0));
 
     const int tid = threadIdx.x;
     const int d = blockIdx.x / p.segs_per_row;
@@ -486,6 +523,7 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
 
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
     ChunkCtx cx;
+    cx.sout = sout;
     cx.mu = p.mean[d];
     const float sg = p.sigma[d];
     cx.inv = 1.0f / sg;
@@ -577,6 +615,10 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
             }
         });
     }
+    // the staging buffer must outlive the last bulk stores
+    if constexpr (G::TMA_STORE) {
+        if (tid == 0) bulk_wait0();
+    }
 }
 
 template <int T, int R, int K>
@@ -588,7 +630,7 @@ cudaError_t launch_tree(const TreeConfig& cfg, const TreeParams& prm, int64_t n_
 
 template <int T, int R, int K>
 cudaError_t prepare_tree(TreeConfig& cfg) {
-    cfg.smem_bytes = tree_smem_bytes<T, R>();
+    cfg.smem_bytes = tree_smem_bytes<T, R, K>();
     cudaError_t e = cudaFuncSetAttribute(spd_tree_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(cfg.smem_bytes));
     if (e != cudaSuccess) return e;
@@ -632,10 +674,10 @@ int tree_configure(spd_plan* plan) {
     TreeConfig& cfg = plan->tree;
     cfg.K = static_cast<int>(plan->widths.size());
     cfg.T = tree_threads_for(cfg.K);
-    cfg.chunk = 4 * cfg.T * kRows;
+    cfg.chunk = 4 * cfg.T * tree_rows_for(cfg.K);
     cudaError_t e = cudaErrorInvalidValue;
 #define SPD_PREP(KK) \
-    if (cfg.K == KK) e = prepare_tree<tree_threads_for(KK), kRows, KK>(cfg);
+    if (cfg.K == KK) e = prepare_tree<tree_threads_for(KK), tree_rows_for(KK), KK>(cfg);
     SPD_TREE_CASES(SPD_PREP)
 #undef SPD_PREP
     if (e != cudaSuccess) return cuda_fail(e, "configuring the dyadic-tree kernel");
@@ -694,7 +736,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     }
     e = cudaErrorInvalidValue;
 #define SPD_LAUNCH(KK) \
-    if (cfg.K == KK) e = launch_tree<tree_threads_for(KK), kRows, KK>(cfg, prm, n_dm, stream);
+    if (cfg.K == KK) e = launch_tree<tree_threads_for(KK), tree_rows_for(KK), KK>(cfg, prm, n_dm, stream);
     SPD_TREE_CASES(SPD_LAUNCH)
 #undef SPD_LAUNCH
     if (e != cudaSuccess) return cuda_fail(e, "launching the dyadic-tree kernel");
