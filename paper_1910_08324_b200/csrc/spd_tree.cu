@@ -224,6 +224,9 @@ __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
     }
 }
 
+#ifndef SPD_TREE_RADIX4
+#define SPD_TREE_RADIX4 0  // two exchange levels per barrier; measured 11.99 ms vs 11.41 ms (config 3)
+#endif
 #ifndef SPD_TREE_TMA_STORE
 #define SPD_TREE_TMA_STORE 0  // measured: 11.87 ms vs 11.41 ms with direct 128-bit stores (config 3)
 #endif
@@ -272,20 +275,25 @@ struct ChunkCtx {
 };
 
 // Exchange levels k = 3 .. LT+1: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner in another thread.
-template <int T, int R, int K, bool FAST, int k>
+template <int T, int R, int K, bool FAST, int k, int hoff>
 __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
                                                 float4* __restrict__ pp, float4* __restrict__ hr,
                                                 float4* __restrict__ hw, int& xsel, const ChunkCtx& cx) {
     using G = Geo<T, R, K>;
     if constexpr (k <= G::LT + 1 && k + 1 <= G::LAST) {
         constexpr int d4 = (1 << k) / 4;  // partner distance in float4
-        constexpr int hoff = d4 - 2;      // sum of the halo sizes of the levels below
+        // Optional (off: slower, the loads bind, not the barriers) - two levels per barrier: with P_k stored once, P_{k+1}[n] = P_k[n] + P_k[n+d] and
+        // P_{k+2}[n] = P_{k+1}[n] + (P_k[n+2d] + P_k[n+3d]) - the same shared-memory bytes as
+        // two single exchanges, one add more, one barrier fewer.
+        constexpr bool PAIR = SPD_TREE_RADIX4 && k + 1 <= G::LT + 1 && k + 2 <= G::LAST;
+        constexpr int nh = PAIR ? 3 * d4 : d4;  // row-0 slots the next chunk's last row wraps into
+        static_assert(hoff + nh <= T, "halo buffer overflow");
         const int tid = cx.tid;
         float4* const buf = pp + xsel * G::C4;
         xsel ^= 1;
 #pragma unroll
         for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
-        if (tid < d4) hw[hoff + tid] = P[0];
+        if (tid < nh) hw[hoff + tid] = P[0];
         // the previous chunk's bulk stores must have read the staging buffer before any
         // thread passes this barrier on its way to refilling it
         if constexpr (FAST && G::TMA_STORE && k == 3) {
@@ -294,13 +302,23 @@ __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float4* src = buf + (tid + T * r + d4);
-            if (r == R - 1 && tid + d4 >= T) src = hr + (hoff + tid + d4 - T);
-            const float4 now = add4(P[r], *src);
-            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], now, lim[r], cx.tm);
-            P[r] = now;
+            // partner m*d4 slots later: in this chunk, or (last row only) in the halo
+            auto partner = [&](int m) -> float4 {
+                const float4* src = buf + (tid + T * r + m * d4);
+                if (r == R - 1 && tid + m * d4 >= T) src = hr + (hoff + tid + m * d4 - T);
+                return *src;
+            };
+            const float4 p1 = add4(P[r], partner(1));
+            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], p1, lim[r], cx.tm);
+            if constexpr (PAIR) {
+                const float4 p2 = add4(p1, add4(partner(2), partner(3)));
+                if (FAST || cx.do_out) fold<k + 2, K, FAST>(best[r], p1, p2, lim[r], cx.tm);
+                P[r] = p2;
+            } else {
+                P[r] = p1;
+            }
         }
-        exchange_levels<T, R, K, FAST, k + 1>(P, best, lim, pp, hr, hw, xsel, cx);
+        exchange_levels<T, R, K, FAST, k + (PAIR ? 2 : 1), hoff + nh>(P, best, lim, pp, hr, hw, xsel, cx);
     }
 }
 
@@ -414,7 +432,7 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
     float4* const hr = halo + hsel * T;        // written by the previous (later-in-time) chunk
     float4* const hw = halo + (hsel ^ 1) * T;  // read by the next chunk
     hsel ^= 1;
-    exchange_levels<T, R, K, FAST, 3>(P, best, lim, pp, hr, hw, xsel, cx);
+    exchange_levels<T, R, K, FAST, 3, 0>(P, best, lim, pp, hr, hw, xsel, cx);
 
     // ---- in-register levels: partner 1, 2, 4, ... rows later (same thread) -------------
     register_levels<T, R, K, FAST, PH, 0>(P, best, lim, dl, cx);
