@@ -193,6 +193,24 @@ int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, cons
                                 int64_t capacity, int64_t* n_found, void* cuda_stream);
 
 /*
+ * spd_row_stats - per-DM mean and standard deviation of the plane, the inputs of eq. (4)/(5)
+ * (sec. 4.6.2: Chan et al. streaming algorithm with point-wise outlier
+ * rejection).  Pass 0 uses every sample of a row; each of the n_reject_passes further passes
+ * uses the samples with |x - mean| <= clip_sigma * sigma of the previous pass (float32
+ * comparison).  sigma is the population standard deviation (ddof 0).  With
+ * n_reject_passes == 0 this is the plain per-row mean / sigma of reading A6.
+ *   plane       : DEVICE, float32 [n_dm][n_t] (any alignment; 16-byte aligned rows are faster).
+ *   clip_sigma  : rejection threshold in sigmas (> 0 when n_reject_passes > 0; the paper's
+ *                 comparison used 2).
+ *   mean, sigma : DEVICE, float32 [n_dm], overwritten.  A row whose samples are all rejected
+ *                 keeps its previous estimate.
+ * Asynchronous on cuda_stream; uses a plan-owned workspace (one call at a time per plan).
+ * Each pass reads the plane once.
+ */
+int spd_row_stats(const spd_plan* plan, const float* plane, float clip_sigma, int32_t n_reject_passes,
+                  float* mean, float* sigma, void* cuda_stream);
+
+/*
  * spd_run_host - the same hot path on HOST buffers (end-to-end entry point):
  * copies row blocks of the plane to the device, runs the kernels and copies
  * Y and W back, overlapping copies and kernels on internal streams.

@@ -11,6 +11,7 @@ from .core import (  # noqa: F401
     find_candidates,
     num_threads,
     row_stats,
+    row_stats_clipped,
     snr_of_width,
     spd_direct,
     spd_prefix,

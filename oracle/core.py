@@ -47,6 +47,8 @@ def _load() -> ctypes.CDLL:
         lib.oracle_snr_of_width.argtypes = [_vp, _i64, _f64, _f64, _i64, _vp, _i64, _vp]
         lib.oracle_row_stats.restype = None
         lib.oracle_row_stats.argtypes = [_vp, _i64, _i64, _vp, _vp]
+        lib.oracle_row_stats_clipped.restype = None
+        lib.oracle_row_stats_clipped.argtypes = [_vp, _i64, _i64, ctypes.c_float, _i32, _vp, _vp]
         lib.oracle_find_candidates.restype = _i64
         lib.oracle_find_candidates.argtypes = [_vp, _vp, _i64, _i64, ctypes.c_float, _i64, _vp, _vp, _vp, _vp]
         _lib = lib
@@ -128,6 +130,18 @@ def row_stats(x) -> Tuple[np.ndarray, np.ndarray]:
     mu = np.empty(n_dm, dtype=np.float64)
     sg = np.empty(n_dm, dtype=np.float64)
     _load().oracle_row_stats(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data)
+    return mu, sg
+
+
+def row_stats_clipped(x, clip: float, n_reject_passes: int) -> Tuple[np.ndarray, np.ndarray]:
+    """Per-row mean and population sigma after ``n_reject_passes`` rounds of point-wise outlier
+    rejection at ``clip`` sigmas (reading A14); float32-rounded values as float64."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    mu = np.empty(n_dm, dtype=np.float64)
+    sg = np.empty(n_dm, dtype=np.float64)
+    _load().oracle_row_stats_clipped(x.ctypes.data, n_dm, n_t, ctypes.c_float(clip), int(n_reject_passes),
+                                     mu.ctypes.data, sg.ctypes.data)
     return mu, sg
 
 

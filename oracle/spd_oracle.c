@@ -29,12 +29,16 @@
  *                        oracle_spd_direct in tests (<= 1e-9).
  *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
  *   oracle_row_stats   : per-row mean and population standard deviation (reading A6).
+ *   oracle_row_stats_clipped: mean / sigma with point-wise outlier rejection
+ *                        repeated a given number of times (reading A14).
  *   oracle_find_candidates: threshold + 1-D local-peak rule (reading A9).
  *
  * Pins: tests/test_oracle_pins.py (closed form eq. 22 on single-pulse planes,
  * numpy.convolve for single widths, constant / ramp / impulse closed forms,
  * affine and shift invariances, white-noise statistics, brute force, the
  * Fig. 17 worked example PAPER.md:587,605, eq. 24 on noise-free twins).
+ * oracle_row_stats(_clipped): numpy mean / std; exact two-valued rows with outliers;
+ * the textbook variance of a normal distribution truncated at +-c sigma.
  * oracle_find_candidates: the rule is this project's reading A9 (the paper
  * names "peak-finding" only) - pinned by closed form on
  * isolated pulses; otherwise "parity unpinned by the paper".
@@ -157,6 +161,48 @@ void oracle_row_stats(const float* x, int64_t n_dm, int64_t n_t, double* mean, d
         }
         mean[d] = m;
         sigma[d] = sqrt(v / (double)n_t);
+    }
+}
+
+/* Mean and standard deviation with point-wise outlier rejection (PAPER.md:720-726,
+ * sec. 4.6.2; reading A14).  Pass 0: mean and population sigma of all samples of the row.
+ * Pass i = 1..n_reject_passes: "each point is compared with the current estimate of the mean
+ * and standard deviation and rejected if it is significantly different (the threshold is
+ * user defined)": keep x iff |x - mu| <= clip * sigma, with mu, sigma the float32-rounded
+ * estimates of pass i-1 and the comparison in float32 (the precision the CUDA path takes
+ * this decision in); mean and sigma of the kept samples by the plain two-pass definition in
+ * double.  A pass that rejects every sample keeps the previous estimate.  Outputs are the
+ * float32-rounded estimates widened to double. */
+void oracle_row_stats_clipped(const float* x, int64_t n_dm, int64_t n_t, float clip, int32_t n_reject_passes,
+                              double* mean, double* sigma) {
+#pragma omp parallel for schedule(static)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float* row = x + d * n_t;
+        float mu = 0.0f, sg = 0.0f;
+        for (int32_t pass = 0; pass <= n_reject_passes; ++pass) {
+            const float lim = clip * sg;
+            double s = 0.0;
+            int64_t cnt = 0;
+            for (int64_t n = 0; n < n_t; ++n) {
+                if (pass == 0 || fabsf(row[n] - mu) <= lim) {
+                    s += (double)row[n];
+                    ++cnt;
+                }
+            }
+            if (cnt == 0) break;
+            const double m = s / (double)cnt;
+            double v = 0.0;
+            for (int64_t n = 0; n < n_t; ++n) {
+                if (pass == 0 || fabsf(row[n] - mu) <= lim) {
+                    const double e = (double)row[n] - m;
+                    v += e * e;
+                }
+            }
+            mu = (float)m;
+            sg = (float)sqrt(v / (double)cnt);
+        }
+        mean[d] = (double)mu;
+        sigma[d] = (double)sg;
     }
 }
 

@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     SPD_FLAG_FORCE_GENERIC, SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC,
     candidates_to_numpy, load, spd_destroy, spd_find_candidates, spd_last_error_string,
     spd_plan_create, spd_plan_destroy, spd_plan_get_info, spd_plan_get_widths, spd_run,
-    spd_run_flagged, spd_find_candidates_flagged,
+    spd_run_flagged, spd_find_candidates_flagged, spd_row_stats,
     spd_run_host, spd_version, spd_width_set_generate,
 )
 
@@ -20,6 +20,6 @@ __all__ = [
     "SPD_FLAG_FORCE_GENERIC", "SPD_PATH_DYADIC_TREE", "SPD_PATH_GENERIC",
     "spd_width_set_generate", "spd_plan_create", "spd_plan_destroy", "spd_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
-    "spd_run_flagged", "spd_find_candidates_flagged",
+    "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
     "spd_run_host", "spd_last_error_string", "spd_version", "candidates_to_numpy",
 ]

@@ -31,7 +31,7 @@ SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC = 1, 2
 EXPORTS = (
     "spd_width_set_generate", "spd_plan_create", "spd_plan_create_ex", "spd_plan_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
-    "spd_run_flagged", "spd_find_candidates_flagged",
+    "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
     "spd_run_host", "spd_last_error_string", "spd_version",
 )
 
@@ -102,6 +102,8 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_run_flagged.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_float, _vp, _vp]
     lib.spd_find_candidates_flagged.restype = ctypes.c_int
     lib.spd_find_candidates_flagged.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_float, _vp, _i64, _vp, _vp]
+    lib.spd_row_stats.restype = ctypes.c_int
+    lib.spd_row_stats.argtypes = [_vp, _vp, ctypes.c_float, _i32, _vp, _vp, _vp]
     lib.spd_run_host.restype = ctypes.c_int
     lib.spd_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     _lib = lib
@@ -258,6 +260,23 @@ def spd_find_candidates_flagged(plan: int, out_snr, out_width, activity, thresho
     return lst, n_found
 
 
+def spd_row_stats(plan: int, plane, clip_sigma: float = 0.0, n_reject_passes: int = 0, mean=None, sigma=None,
+                  stream=None):
+    """Per-DM mean and population sigma of ``plane`` (device tensors); returns (mean, sigma)."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    if mean is None:
+        mean = torch.empty(info["n_dm"], dtype=torch.float32, device=plane.device)
+    if sigma is None:
+        sigma = torch.empty(info["n_dm"], dtype=torch.float32, device=plane.device)
+    _check(load().spd_row_stats(
+        _vp(plan), _dev_ptr(plane, torch.float32, n, "plane"), ctypes.c_float(clip_sigma), int(n_reject_passes),
+        _dev_ptr(mean, torch.float32, info["n_dm"], "mean"), _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
+        _vp(_stream_handle(stream))))
+    return mean, sigma
+
+
 def candidates_to_numpy(lst, n_found, capacity: int) -> Tuple[int, np.ndarray]:
     """Synchronising helper: (count, structured array of the stored candidates sorted by (dm, t))."""
     count = int(n_found.item())
@@ -336,6 +355,10 @@ class Plan:
                                 lst=None, n_found=None):
         return spd_find_candidates_flagged(self.handle, out_snr, out_width, activity, threshold, capacity, stream,
                                            lst, n_found)
+
+    def row_stats(self, plane, clip_sigma: float = 0.0, n_reject_passes: int = 0, mean=None, sigma=None,
+                  stream=None):
+        return spd_row_stats(self.handle, plane, clip_sigma, n_reject_passes, mean, sigma, stream)
 
     def run_host(self, plane, mean, sigma, out_snr, out_width):
         spd_run_host(self.handle, plane, mean, sigma, out_snr, out_width)

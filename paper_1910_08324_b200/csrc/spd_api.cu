@@ -264,7 +264,10 @@ int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
         plan->path = SPD_PATH_GENERIC;
         rc = generic_configure(plan);
     }
+    if (rc == SPD_OK) rc = stats_configure(plan);
     if (rc != SPD_OK) {
+        generic_release(plan);
+        stats_release(plan);
         delete plan;
         return rc;
     }
@@ -276,6 +279,7 @@ void spd_plan_destroy(spd_plan* plan) {
     if (!plan) return;
     release_host_staging(plan);
     generic_release(plan);
+    stats_release(plan);
     delete plan;
 }
 
@@ -375,6 +379,20 @@ int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, cons
     }
     return candidates_run(plan, out_snr, out_width, activity, threshold, list, capacity, n_found,
                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_row_stats(const spd_plan* plan, const float* plane, float clip_sigma, int32_t n_reject_passes, float* mean,
+                  float* sigma, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma) {
+        set_error("spd_row_stats: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (n_reject_passes < 0 || n_reject_passes > 64 || (n_reject_passes > 0 && !(clip_sigma > 0.0f))) {
+        set_error("spd_row_stats: need 0 <= n_reject_passes <= 64 and clip_sigma > 0 when rejecting (got %d, %g)",
+                  n_reject_passes, static_cast<double>(clip_sigma));
+        return SPD_ERR_INVALID_ARG;
+    }
+    return stats_run(plan, plane, clip_sigma, n_reject_passes, mean, sigma, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,

@@ -130,12 +130,19 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
                     // value before the first sample of the piece
                     float carry = p0 > 0 ? __ldg(y + p0 - 1) : ninf;
                     unsigned long long bits = 0ull;
-#pragma unroll 4
+                    // all loads of the piece first: one memory latency per piece, not per step
+                    float4 pv[kPieceSteps];
+#pragma unroll
+                    for (int it = 0; it < kPieceSteps; ++it) {
+                        const long long n = p0 + 128ll * it + 4 * lane;
+                        pv[it] = n < p1 ? __ldg(reinterpret_cast<const float4*>(y + n))
+                                        : make_float4(ninf, ninf, ninf, ninf);
+                    }
+#pragma unroll
                     for (int it = 0; it < kPieceSteps; ++it) {
                         const long long n = p0 + 128ll * it + 4 * lane;
                         const bool in = n < p1;
-                        float4 v = make_float4(ninf, ninf, ninf, ninf);
-                        if (in) v = __ldg(reinterpret_cast<const float4*>(y + n));
+                        const float4 v = pv[it];
                         float prev = __shfl_up_sync(0xffffffffu, v.w, 1);
                         if (lane == 0) prev = carry;
                         float next = __shfl_down_sync(0xffffffffu, v.x, 1);
@@ -194,7 +201,7 @@ int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* ou
         const long long steps = (n_flags + 127) / 128;
         const long long warps_per_block = kCandThreads / 32;
         long long blocks = (steps + warps_per_block - 1) / warps_per_block;
-        blocks = std::max<long long>(1, std::min<long long>(blocks, static_cast<long long>(plan->sm_count) * 8));
+        blocks = std::max<long long>(1, std::min<long long>(blocks, static_cast<long long>(plan->sm_count) * 16));
         find_candidates_flagged_kernel<<<static_cast<unsigned>(blocks), kCandThreads, 0, stream>>>(
             out_snr, out_width, activity, n_flags, per_row, activity_block(plan), plan->n_t, threshold, list,
             static_cast<unsigned long long>(capacity), reinterpret_cast<unsigned long long*>(n_found));

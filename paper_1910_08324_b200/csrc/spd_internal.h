@@ -58,6 +58,10 @@ struct spd_plan {
     double* d_blocksum = nullptr;  // [n_dm][blocks_per_row]
     int64_t generic_blocks_per_row = 0;
     int64_t workspace_bytes = 0;
+    // spd_row_stats
+    void* d_stats = nullptr;  // [n_dm][stats_parts] partial moments
+    int stats_parts = 0;
+    int64_t stats_part = 0;   // samples per part
     // spd_run_host
     spd::HostStaging host;
 };
@@ -81,6 +85,12 @@ int generic_configure(spd_plan* plan);
 void generic_release(spd_plan* plan);
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
                 const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
+
+// spd_stats.cu
+int stats_configure(spd_plan* plan);
+void stats_release(spd_plan* plan);
+int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float* mean,
+              float* sigma, cudaStream_t stream);
 
 // spd_candidates.cu
 // activity: nullptr (visit every sample) or the map written by spd_run_flagged, one byte

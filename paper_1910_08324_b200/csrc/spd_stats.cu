@@ -1,0 +1,191 @@
+// Per-DM mean and standard deviation of the plane (the step that
+// feeds mu, sigma of eq. (4)/(5) into the hot path).
+//
+// PAPER.md:720-726 (sec. 4.6.2): "a streaming algorithm by Chan et al. [1983]" for the mean and
+// the standard deviation, and "point-wise outlier rejection. Each point is compared with the
+// current estimate of the mean and standard deviation and rejected if it is significantly
+// different (the threshold is user defined). This is repeated until convergence."
+//
+// Reading (A14): pass 0 takes every sample; each further pass takes the samples with
+// |x - mu| <= clip * sigma of the previous pass (comparison in float32 on the float32 mu, sigma
+// the caller receives); sigma is the population standard deviation (ddof 0, as reading A6); the
+// caller fixes the number of rejection passes (the paper's convergence rule is not given).
+//
+// Partial statistics (n, mean, M2) are combined with the pairwise update of Chan, Golub &
+// LeVeque: delta = mean_b - mean_a, mean = mean_a + delta n_b / n,
+// M2 = M2_a + M2_b + delta^2 n_a n_b / n.  A thread accumulates its samples as shifted sums
+// (shift = first sample of its block's part; four samples at a time in float32, then double), threads and parts are then merged
+// pairwise in a fixed order, so the result does not depend on scheduling.
+// One pass reads the plane once: 4 B per sample, HBM-bound.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <algorithm>
+
+#include "spd_internal.h"
+
+namespace spd {
+namespace {
+
+constexpr int kStatThreads = 256;
+
+struct Moments {
+    double n, mean, m2;
+};
+
+__device__ __forceinline__ Moments merge(const Moments a, const Moments b) {
+    if (b.n == 0.0) return a;
+    if (a.n == 0.0) return b;
+    Moments r;
+    r.n = a.n + b.n;
+    const double delta = b.mean - a.mean;
+    const double f = b.n / r.n;
+    r.mean = a.mean + delta * f;
+    r.m2 = a.m2 + b.m2 + delta * delta * a.n * f;
+    return r;
+}
+
+__device__ __forceinline__ Moments shfl_down(const Moments v, int o) {
+    Moments r;
+    r.n = __shfl_down_sync(0xffffffffu, v.n, o);
+    r.mean = __shfl_down_sync(0xffffffffu, v.mean, o);
+    r.m2 = __shfl_down_sync(0xffffffffu, v.m2, o);
+    return r;
+}
+
+// Block b of row d reduces samples [b * part, min((b+1) * part, n_t)) to one Moments.
+// clip_on: keep only |x - mu[d]| <= clip * sigma[d] (float32 comparison).
+template <bool VEC>
+__global__ void __launch_bounds__(kStatThreads) row_moments_kernel(const float* __restrict__ plane, long long n_t,
+                                                                   long long part, int parts, int clip_on,
+                                                                   float clip, const float* __restrict__ mean,
+                                                                   const float* __restrict__ sigma,
+                                                                   Moments* __restrict__ out) {
+    __shared__ Moments warp_m[kStatThreads / 32];
+    const long long d = blockIdx.x / parts;
+    const int b = blockIdx.x - static_cast<int>(d) * parts;
+    const float* __restrict__ row = plane + d * n_t;
+    const long long lo = static_cast<long long>(b) * part;
+    const long long hi = min(lo + part, n_t);
+    float mu = 0.f, lim = 0.f;
+    if (clip_on) {
+        mu = mean[d];
+        lim = clip * sigma[d];
+    }
+    const float shift = lo < hi ? __ldg(row + lo) : 0.f;
+    // Shifted sums: x - shift and the sums over one float4 in float32 (a sum of 4 terms each
+    // rounded to 2^-24 relative), everything longer in double.
+    double s1 = 0.0, s2 = 0.0;
+    unsigned int cnt = 0;
+    auto keep = [&](float x) { return !clip_on || fabsf(x - mu) <= lim; };
+    if constexpr (VEC) {  // n_t % 4 == 0, part % 4 == 0 and an aligned plane: float4 loads
+#pragma unroll 4
+        for (long long n = lo + 4ll * threadIdx.x; n < hi; n += 4ll * kStatThreads) {
+            const float4 v = __ldg(reinterpret_cast<const float4*>(row + n));
+            const bool k0 = keep(v.x), k1 = keep(v.y), k2 = keep(v.z), k3 = keep(v.w);
+            const float a0 = k0 ? v.x - shift : 0.f, a1 = k1 ? v.y - shift : 0.f;
+            const float a2 = k2 ? v.z - shift : 0.f, a3 = k3 ? v.w - shift : 0.f;
+            s1 += static_cast<double>((a0 + a1) + (a2 + a3));
+            s2 += static_cast<double>((a0 * a0 + a1 * a1) + (a2 * a2 + a3 * a3));
+            cnt += static_cast<unsigned>(k0) + k1 + k2 + k3;
+        }
+    } else {
+        for (long long n = lo + threadIdx.x; n < hi; n += kStatThreads) {
+            const float x = __ldg(row + n);
+            if (keep(x)) {
+                const float a = x - shift;
+                s1 += static_cast<double>(a);
+                s2 += static_cast<double>(a * a);
+                ++cnt;
+            }
+        }
+    }
+    Moments m;
+    m.n = static_cast<double>(cnt);
+    m.mean = cnt ? static_cast<double>(shift) + s1 / m.n : 0.0;
+    m.m2 = cnt ? fmax(s2 - s1 * s1 / m.n, 0.0) : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const Moments other = shfl_down(m, o);
+        m = merge(m, other);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) warp_m[warp] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        Moments t = warp_m[0];
+#pragma unroll
+        for (int w = 1; w < kStatThreads / 32; ++w) t = merge(t, warp_m[w]);
+        out[blockIdx.x] = t;
+    }
+}
+
+// One thread per row: merge its parts in order, write float32 mean and population sigma.
+__global__ void row_moments_finish_kernel(const Moments* __restrict__ parts_m, int parts, long long n_dm,
+                                          float* __restrict__ mean, float* __restrict__ sigma) {
+    const long long d = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (d >= n_dm) return;
+    Moments t = parts_m[d * parts];
+    for (int b = 1; b < parts; ++b) t = merge(t, parts_m[d * parts + b]);
+    // no sample survived the rejection: keep the previous estimate
+    if (t.n == 0.0) return;
+    mean[d] = static_cast<float>(t.mean);
+    sigma[d] = static_cast<float>(sqrt(t.m2 / t.n));
+}
+
+}  // namespace
+
+int stats_configure(spd_plan* plan) {
+    // enough blocks to fill the machine, parts a multiple of 1024 samples
+    const long long want = 16ll * plan->sm_count;
+    long long parts = std::max<long long>(1, std::min<long long>(256, (want + plan->n_dm - 1) / plan->n_dm));
+    long long part = (plan->n_t + parts - 1) / parts;
+    part = (part + 1023) / 1024 * 1024;
+    parts = (plan->n_t + part - 1) / part;
+    plan->stats_parts = static_cast<int>(parts);
+    plan->stats_part = part;
+    if (plan->n_dm * parts > 0x7fffffffll) {
+        set_error("plane too large for the statistics grid");
+        return SPD_ERR_INVALID_ARG;
+    }
+    const size_t bytes = sizeof(Moments) * static_cast<size_t>(plan->n_dm) * static_cast<size_t>(parts);
+    const cudaError_t e = cudaMalloc(&plan->d_stats, bytes);
+    if (e != cudaSuccess) {
+        set_error("device allocation of the statistics workspace (%zu bytes) failed: %s", bytes,
+                  cudaGetErrorString(e));
+        cudaGetLastError();
+        return SPD_ERR_ALLOC;
+    }
+    plan->workspace_bytes += static_cast<int64_t>(bytes);
+    return SPD_OK;
+}
+
+void stats_release(spd_plan* plan) {
+    cudaFree(plan->d_stats);
+    plan->d_stats = nullptr;
+}
+
+int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float* mean, float* sigma,
+              cudaStream_t stream) {
+    Moments* ws = static_cast<Moments*>(plan->d_stats);
+    const int parts = plan->stats_parts;
+    const unsigned grid = static_cast<unsigned>(plan->n_dm * parts);
+    const bool vec = plan->n_t % 4 == 0 && (reinterpret_cast<uintptr_t>(plane) & 15u) == 0;
+    const unsigned fin_grid = static_cast<unsigned>((plan->n_dm + 127) / 128);
+    for (int pass = 0; pass <= n_iter; ++pass) {
+        const int clip_on = pass > 0;
+        if (vec)
+            row_moments_kernel<true><<<grid, kStatThreads, 0, stream>>>(plane, plan->n_t, plan->stats_part, parts,
+                                                                        clip_on, clip, mean, sigma, ws);
+        else
+            row_moments_kernel<false><<<grid, kStatThreads, 0, stream>>>(plane, plan->n_t, plan->stats_part, parts,
+                                                                         clip_on, clip, mean, sigma, ws);
+        row_moments_finish_kernel<<<fin_grid, 128, 0, stream>>>(ws, parts, plan->n_dm, mean, sigma);
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "launching the statistics kernels");
+    return SPD_OK;
+}
+
+}  // namespace spd

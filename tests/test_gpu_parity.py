@@ -366,6 +366,59 @@ def test_flagged_no_detections_and_all_detections(spd):
         assert int(n1.item()) == int(n_d.item()) > 0
 
 
+@pytest.mark.parametrize("n_dm,n_t", [(16, 65536), (5, 10007), (300, 4096 + 4), (2, 1 << 21)])
+@pytest.mark.parametrize("clip,passes", [(0.0, 0), (2.0, 1), (2.5, 4), (3.0, 8)])
+def test_row_stats_against_oracle(spd, oracle_lib, n_dm, n_t, clip, passes):
+    """Row f1: per-DM mean / sigma with point-wise outlier rejection (reading A14).
+    Tolerance 2e-6 * sigma: the kept set is decided in float32 on both sides; a sample within an ulp
+    of the rejection limit may fall on the other side when the previous pass's float32 estimate
+    differs in its last bit."""
+    rng = np.random.default_rng(n_dm * 31 + passes)
+    x = (rng.standard_normal((n_dm, n_t)) * 2.5 + 11.0).astype(np.float32)
+    x[0, n_t // 4: n_t // 4 + max(4, n_t // 50)] += np.float32(40.0)  # a strong wide pulse
+    x[n_dm - 1, ::97] -= np.float32(25.0)                             # scattered outliers
+    dev = torch.device("cuda:0")
+    widths = [1, 2, 4] if n_t % 4 == 0 else [1, 3]
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        mean, sigma = plan.row_stats(torch.from_numpy(x).to(dev), clip, passes)
+        got_mu, got_sg = mean.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+    ref_mu, ref_sg = oracle_lib.row_stats_clipped(x, clip, passes)
+    tol = 2e-6 * ref_sg + 1e-7 * np.abs(ref_mu)
+    assert np.all(np.abs(got_mu - ref_mu) <= tol), float(np.max(np.abs(got_mu - ref_mu) / tol))
+    assert np.all(np.abs(got_sg - ref_sg) <= tol), float(np.max(np.abs(got_sg - ref_sg) / tol))
+
+
+def test_row_stats_feed_the_hot_path(spd, oracle_lib):
+    """mu, sigma from spd_row_stats (no rejection = reading A6) go straight into spd_run on the device."""
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(2).scaled(8, 65536, 8)
+    x, _ = make_plane_numpy(w)
+    x = (x * np.float32(1.9) - np.float32(7.0)).astype(np.float32)
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(8, 65536, widths) as plan:
+        mean, sigma = plan.row_stats(plane)
+        snr, idx = plan.run(plane, mean, sigma)
+        got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+        mu64, sg64 = mean.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+    ref_mu, ref_sg = oracle_lib.row_stats(x)
+    assert np.allclose(mu64, ref_mu, rtol=0, atol=2e-6 * ref_sg.max()) and np.allclose(sg64, ref_sg, rtol=2e-6)
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_prefix(x, mu64, sg64, widths)
+    parity.assert_parity(oracle_lib, x, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                         what="row_stats -> spd_run")
+
+
+def test_row_stats_argument_checks(spd):
+    dev = torch.device("cuda:0")
+    plane = torch.zeros((2, 1024), device=dev)
+    with spd.Plan(2, 1024, [1, 2]) as plan:
+        with pytest.raises(spd.SpdError):
+            plan.row_stats(plane, 0.0, 2)      # rejection needs a positive threshold
+        with pytest.raises(spd.SpdError):
+            plan.row_stats(plane, 2.0, -1)
+
+
 def test_run_host_equals_device_run(spd):
     """The end-to-end host entry point (several row blocks) returns exactly what spd_run does."""
     rng = np.random.default_rng(11)

@@ -109,6 +109,75 @@ def test_row_stats_is_numpy_mean_std(oracle_lib):
     assert np.allclose(sg, x64.std(axis=1, ddof=0), rtol=1e-12)
 
 
+# --- reading A14: mean / sigma with point-wise outlier rejection -----
+
+def test_clipped_stats_zero_passes_is_plain_stats(oracle_lib):
+    rng = np.random.default_rng(12)
+    x = (rng.standard_normal((4, 5000)) * 1.7 - 0.4).astype(np.float32)
+    mu0, sg0 = oracle_lib.row_stats(x)
+    mu, sg = oracle_lib.row_stats_clipped(x, 2.0, 0)
+    assert np.array_equal(mu, mu0.astype(np.float32).astype(np.float64))
+    assert np.array_equal(sg, sg0.astype(np.float32).astype(np.float64))
+
+
+def test_clipped_stats_two_valued_row_with_outliers_exact(oracle_lib):
+    """A row of +-1 (mean 0, sigma 1 exactly) plus k outliers of height V: the plain estimate is
+    (kV/n, sqrt(...)) in closed form; one 3-sigma rejection removes exactly the outliers and gives
+    (0, 1); further passes change nothing."""
+    n, k, V = 4000, 8, 50.0
+    row = np.tile(np.array([1.0, -1.0], dtype=np.float32), n // 2)
+    pos = np.arange(k) * 401 + 7
+    row_out = row.copy()
+    base_sum = float(row.sum()) - float(row[pos].sum())
+    row_out[pos] = V
+    x = np.stack([row, row_out])
+    mu, sg = oracle_lib.row_stats_clipped(x, 3.0, 0)
+    m1 = (base_sum + k * V) / n
+    v1 = ((n - k) * 1.0 + k * V * V) / n - m1 * m1
+    assert mu[0] == 0.0 and sg[0] == 1.0
+    assert abs(mu[1] - m1) < 1e-6 and abs(sg[1] - math.sqrt(v1)) < 1e-5
+    assert abs(m1) + 3.0 * math.sqrt(v1) < V  # the outliers are beyond 3 sigma of the plain estimate
+    for passes in (1, 2, 5):
+        mu, sg = oracle_lib.row_stats_clipped(x, 3.0, passes)
+        kept_mean = base_sum / (n - k)
+        kept_sigma = math.sqrt(1.0 - kept_mean * kept_mean)
+        assert mu[0] == 0.0 and sg[0] == 1.0
+        assert abs(mu[1] - kept_mean) < 1e-7 and abs(sg[1] - kept_sigma) < 1e-7
+
+
+def test_clipped_stats_truncated_normal_variance(oracle_lib):
+    """One rejection pass at c sigma on N(0,1) data leaves a normal truncated at +-c:
+    variance 1 - 2 c phi(c) / (2 Phi(c) - 1) (textbook)."""
+    rng = np.random.default_rng(13)
+    x = rng.standard_normal((2, 1 << 20)).astype(np.float32)
+    for c in (2.0, 3.0):
+        mu, sg = oracle_lib.row_stats_clipped(x, c, 1)
+        phi = math.exp(-0.5 * c * c) / math.sqrt(2.0 * math.pi)
+        Phi = 0.5 * (1.0 + math.erf(c / math.sqrt(2.0)))
+        want = math.sqrt(1.0 - 2.0 * c * phi / (2.0 * Phi - 1.0))
+        assert np.all(np.abs(sg - want) < 4e-3) and np.all(np.abs(mu) < 4e-3)
+
+
+def test_clipped_stats_rejection_is_monotone_and_affine(oracle_lib):
+    rng = np.random.default_rng(14)
+    x = rng.standard_normal((3, 20000)).astype(np.float32)
+    x[1, 5000:5200] += 30.0   # a strong pulse
+    sgs = [oracle_lib.row_stats_clipped(x, 2.5, p)[1] for p in range(4)]
+    for a, b in zip(sgs, sgs[1:]):
+        assert np.all(b <= a + 1e-12)              # rejecting outliers never raises sigma
+    assert sgs[0][1] > 2.0 and abs(sgs[3][1] - sgs[3][0]) < 0.05  # the pulse is gone after a few passes
+    # power-of-two scaling and integer shift commute exactly with the float32 comparison
+    mu, sg = oracle_lib.row_stats_clipped(x, 2.5, 2)
+    mu2, sg2 = oracle_lib.row_stats_clipped((x * np.float32(4.0)), 2.5, 2)
+    assert np.allclose(mu2, 4.0 * mu, rtol=0, atol=1e-6) and np.allclose(sg2, 4.0 * sg, rtol=1e-6)
+
+
+def test_clipped_stats_everything_rejected_keeps_estimate(oracle_lib):
+    x = np.array([[0.0, 0.0, 10.0, 10.0]], dtype=np.float32)  # mean 5, sigma 5: clip 0.5 rejects all
+    mu, sg = oracle_lib.row_stats_clipped(x, 0.5, 3)
+    assert mu[0] == 5.0 and sg[0] == 5.0
+
+
 # --- P9: brute force written out here, tiny planes ------------------------------------
 
 def _brute(x, mu, sg, widths):
