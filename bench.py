@@ -412,14 +412,16 @@ def run_b200(args):
     return 0
 
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of the dominant
-# kernel from the committed `ncu --set full` capture, per workload; None until captured.
-# Source files: profiles/ (see profiles/README.md).
-NCU_TRAFFIC_BYTES = {}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per sample of the dominant kernel from
+# the committed `ncu --set full` capture (taken on 1024 of the workload's DM trials: the kernel
+# streams rows independently, so traffic scales with the sample count); None where not captured.
+# profiles/r01c_tree_kernel_full.md: 4.397637 + 8.536988 GB for 2^30 samples of the config-3 recipe.
+NCU_DRAM_BYTES_PER_SAMPLE = {3: (4.397637e9 + 8.536988e9) / float(1 << 30)}
 
 
 def ncu_traffic_bytes(w):
-    return NCU_TRAFFIC_BYTES.get((w.index, w.n_dm))
+    per_sample = NCU_DRAM_BYTES_PER_SAMPLE.get(w.index)
+    return None if per_sample is None else per_sample * w.n_samples
 
 
 def host_mem_available_bytes():
