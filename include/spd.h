@@ -66,7 +66,7 @@ typedef enum spd_width_kind {
 
 /* Which kernels a plan dispatches to (spd_plan_info.path). */
 #define SPD_PATH_DYADIC_TREE 1 /* streaming partial-sum tree, widths {1,2,4,...,2^(K-1)} */
-#define SPD_PATH_GENERIC 2     /* any width set: per-row running partial sums in a plan-owned workspace */
+#define SPD_PATH_GENERIC 2     /* any width set: per-row running partial sums, staged per tile in shared memory */
 
 typedef struct spd_plan spd_plan; /* opaque */
 
@@ -115,8 +115,10 @@ int spd_width_set_generate(int32_t kind, int32_t param, int32_t max_width,
  *                ascending, de-duplicated).  Error if empty, any width < 1,
  *                any width > max_width, or more than 32768 distinct widths.
  *   max_width  : L_end; must satisfy max_width <= n_t.
- * The plan owns small device tables and, for SPD_PATH_GENERIC, a workspace of
- * n_dm*(n_t+1) doubles allocated here.  Uses the current CUDA device.
+ * The plan owns small device tables, the workspace of spd_row_stats and - only for a
+ * SPD_PATH_GENERIC plan whose max_width exceeds what a shared-memory tile holds (about
+ * 45 000 samples) - a workspace of n_dm*(n_t+1) doubles; spd_plan_info.workspace_bytes
+ * reports the total.  Uses the current CUDA device.
  */
 int spd_plan_create(spd_plan** out, int64_t n_dm, int64_t n_t,
                     const int32_t* width_set, int32_t n_widths, int32_t max_width);
@@ -147,7 +149,8 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info);
  *                enqueues work; it never synchronises.
  * Buffers are owned by the caller and must not alias.  A SPD_PATH_DYADIC_TREE
  * plan is read-only during the call (concurrent runs on different streams are
- * allowed); a SPD_PATH_GENERIC plan uses its workspace (one run at a time).
+ * allowed); a SPD_PATH_GENERIC plan with a workspace (see spd_plan_create) runs one call
+ * at a time.
  */
 int spd_run(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
             float* out_snr, int32_t* out_width, void* cuda_stream);

@@ -312,9 +312,17 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         info->segments_per_row = plan->tree.segs_per_row;
         info->smem_bytes = static_cast<int64_t>(plan->tree.smem_bytes);
     } else {
-        info->launches_per_run = 4;
-        info->threads_per_block = 256;
-        info->blocks = static_cast<int32_t>(plan->n_dm * ((plan->n_t + 255) / 256));
+        if (plan->generic_tile > 0) {
+            info->launches_per_run = 1;
+            info->threads_per_block = 1024;
+            info->blocks = static_cast<int32_t>(plan->n_dm * plan->generic_tiles_per_row);
+            info->chunk = plan->generic_tile;
+            info->smem_bytes = static_cast<int64_t>(plan->generic_smem);
+        } else {
+            info->launches_per_run = 4;
+            info->threads_per_block = 256;
+            info->blocks = static_cast<int32_t>(plan->n_dm * ((plan->n_t + 255) / 256));
+        }
     }
     info->workspace_bytes = plan->workspace_bytes;
     info->activity_bytes = static_cast<int64_t>(activity_bytes(plan));
@@ -411,8 +419,8 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
             cudaSuccess ||
         (e = cudaStreamSynchronize(h.stream[0])) != cudaSuccess)
         return cuda_fail(e, "copying mean / sigma to the device");
-    // The generic path shares one workspace, so its blocks run on one stream.
-    const int n_streams = plan->path == SPD_PATH_DYADIC_TREE ? 2 : 1;
+    // The workspace variant of the any-width-set path shares one workspace: one stream.
+    const int n_streams = (plan->path == SPD_PATH_DYADIC_TREE || plan->generic_tile > 0) ? 2 : 1;
     int64_t blk = 0;
     for (int64_t r0 = 0; r0 < plan->n_dm; r0 += h.rows_per_block, ++blk) {
         const int64_t rows = std::min<int64_t>(h.rows_per_block, plan->n_dm - r0);

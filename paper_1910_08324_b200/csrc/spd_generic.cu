@@ -1,15 +1,27 @@
 // Any-width-set path (SURVEY.md sec. 8(a) rows a2-a7 for width sets the dyadic tree does
 // not cover: the "ideal" set 1..L_max of PAPER.md:193, BoxDIT eq. (14), IGRID eq. (18), ...).
 //
-// Partial sums are reused through one running sum per DM row, kept in double precision in a
-// plan-owned workspace:  C_d[n] = sum_{j<n} (x[d,j] - mu_d),  X_L[n] - L mu_d = C_d[n+L] - C_d[n]
-// (eq. 2 with eq. 5).  Three small kernels build C (block sums, scan of the
-// block sums, in-block scan); the fourth evaluates eq. (4) and the max / arg-max of eq. (12)
-// for every sample, visiting the widths in ascending order with a strict '>'.
-// This path favours generality over speed; the dyadic tree (spd_tree.cu) is the fast path.
+// Partial sums are reused through one running sum per DM row,
+//   C_d[n] = sum_{j<n} (x[d,j] - mu_d),  X_L[n] - L mu_d = C_d[n+L] - C_d[n]
+// (eq. 2 with eq. 5); eq. (4) and the max / arg-max of eq. (12) then visit
+// the widths in ascending order with a strict '>'.
+//
+// Tile kernel (max_width up to ~40 K): a block stages one time tile of a row plus its
+// max_width - 1 look-ahead in shared memory as a two-level running sum - a float32
+// exclusive sum inside 64-sample sub-blocks (magnitude of a few sigma, so differences keep
+// ~1e-6 sigma) and a double running sum of the sub-block totals - and evaluates every width
+// of every sample of the tile from it.  Nothing but x is read and Y, W written; the work is
+// O(|B|) shared-memory loads per sample, so this path is bound by the L1/issue pipes, not by
+// HBM, and is not the tuned path (the dyadic tree, spd_tree.cu, is).
+//
+// Workspace kernels (fallback for larger max_width): the same running sum kept in double in
+// a plan-owned device workspace, built by three scan kernels and read by an evaluation kernel.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+
+#include <algorithm>
+#include <cstdlib>
 
 #include "spd_internal.h"
 
@@ -149,24 +161,187 @@ __global__ void __launch_bounds__(256) generic_eval(const double* __restrict__ p
     out_width[d * n_t + n] = idx;
 }
 
+// ---- tile kernel --------------------------------------------------------------------
+constexpr int kTileThreads = 1024;
+constexpr int kSub = 64;                 // samples per float32 sub-block
+constexpr int kTileSpanMax = 48 * 1024;  // floats of shared memory for tile + look-ahead
+constexpr int kTileWidthsMax = 1024;     // width table kept in shared memory up to this many widths
+
+__global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
+    const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
+    const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, long long n_t, int tile,
+    int span, long long tiles_per_row, float* __restrict__ out_snr, int32_t* __restrict__ out_width) {
+    extern __shared__ __align__(16) unsigned char gsm[];
+    const int n_sub = span / kSub;  // span is a multiple of kSub
+    double* const B = reinterpret_cast<double*>(gsm);                        // [n_sub + 1] running sum of sub-block totals
+    float* const c = reinterpret_cast<float*>(gsm + (n_sub + 2) / 2 * 16);  // [span + 1] exclusive sum inside a sub-block
+    int32_t* const sw = reinterpret_cast<int32_t*>(c + (span + 4) / 4 * 4);   // [kTileWidthsMax] widths
+    float* const ss = reinterpret_cast<float*>(sw + kTileWidthsMax);          // [kTileWidthsMax] 1 / (sqrt(L) sigma)
+    const long long d = blockIdx.x / tiles_per_row;
+    const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
+    const float* __restrict__ row = plane + d * n_t;
+    const float mu = mean[d];
+    const float inv = 1.0f / sigma[d];
+    const long long avail = n_t - t0;  // samples of the row from t0 on
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool table_in_smem = n_w <= kTileWidthsMax;
+    if (table_in_smem) {
+        for (int k = threadIdx.x; k < n_w; k += kTileThreads) {
+            sw[k] = __ldg(widths + k);
+            ss[k] = __ldg(wscale + k) * inv;
+        }
+    }
+    const int32_t* __restrict__ wp = table_in_smem ? sw : widths;
+    const float* __restrict__ sp = table_in_smem ? ss : wscale;
+    const float post = table_in_smem ? 1.0f : inv;  // 1/sigma already folded into ss
+
+    // phase 1: sub-block sums; samples beyond the row count as x = mu (never used by a valid window)
+    for (int sb = warp; sb < n_sub; sb += kTileThreads / 32) {
+        const int i = sb * kSub + 2 * lane;
+        const float x0 = i < avail ? __ldg(row + t0 + i) - mu : 0.f;
+        const float x1 = i + 1 < avail ? __ldg(row + t0 + i + 1) - mu : 0.f;
+        const float s = x0 + x1;
+        float incl = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const float u = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += u;
+        }
+        c[i] = incl - s;
+        c[i + 1] = incl - s + x0;
+        // sub-block total in double (pairwise over the lanes)
+        double tot = static_cast<double>(x0) + static_cast<double>(x1);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+        if (lane == 0) B[sb + 1] = tot;
+    }
+    __syncthreads();
+    // phase 2: running sum of the totals (one warp, consecutive runs per lane)
+    if (warp == 0) {
+        const int per = (n_sub + 31) / 32;
+        const int lo = min(lane * per, n_sub), hi = min(lo + per, n_sub);
+        double run = 0.0;
+        for (int j = lo; j < hi; ++j) run += B[j + 1];
+        double incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double u = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += u;
+        }
+        double acc = incl - run;
+        for (int j = lo; j < hi; ++j) {
+            const double t = B[j + 1];
+            B[j + 1] = acc + t;
+            acc += t;
+        }
+        if (lane == 0) {
+            B[0] = 0.0;
+            c[span] = 0.f;  // C at the end of the last sub-block = B[n_sub] + 0
+        }
+    }
+    __syncthreads();
+    // phase 3: every width of every sample of the tile.  C[i] = B[i / kSub] + c[i].
+    const int n_out = static_cast<int>(min(static_cast<long long>(tile), avail));
+    const int max_w = __ldg(widths + n_w - 1);
+    for (int i = threadIdx.x; i < n_out; i += kTileThreads) {
+        const long long room = avail - i;
+        const float c0 = c[i];
+        const double b0 = B[i / kSub];
+        float best = __int_as_float(0xff800000);
+        int idx = -1;
+        auto visit = [&](int k, int L) {
+            const int e = i + L;
+            const float x = static_cast<float>(B[e / kSub] - b0) + (c[e] - c0);
+            const float snr = x * sp[k] * post;  // eq. (4) with eq. (5)
+            if (snr > best) {                    // strict '>'
+                best = snr;
+                idx = k;
+            }
+        };
+        if (room >= max_w) {  // every width fits: no test inside the loop, loads of 4 widths in flight
+            int k = 0;
+            for (; k + 4 <= n_w; k += 4) {
+                const int L0 = wp[k], L1 = wp[k + 1], L2 = wp[k + 2], L3 = wp[k + 3];
+                visit(k, L0);
+                visit(k + 1, L1);
+                visit(k + 2, L2);
+                visit(k + 3, L3);
+            }
+            for (; k < n_w; ++k) visit(k, wp[k]);
+        } else {
+            for (int k = 0; k < n_w; ++k) {
+                const int L = wp[k];
+                if (L > room) break;  // valid windows only (reading A3); widths ascend
+                visit(k, L);
+            }
+        }
+        out_snr[d * n_t + t0 + i] = best;
+        out_width[d * n_t + t0 + i] = idx;
+    }
+}
+
 }  // namespace
 
 int generic_configure(spd_plan* plan) {
     const int n_w = static_cast<int>(plan->widths.size());
     std::vector<float> scale(n_w);
     for (int k = 0; k < n_w; ++k) scale[k] = static_cast<float>(1.0 / sqrt(static_cast<double>(plan->widths[k])));
+    cudaError_t e;
+    if ((e = cudaMalloc(&plan->d_widths, sizeof(int32_t) * n_w)) != cudaSuccess ||
+        (e = cudaMalloc(&plan->d_wscale, sizeof(float) * n_w)) != cudaSuccess) {
+        set_error("device allocation of the width table failed: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        generic_release(plan);
+        return SPD_ERR_ALLOC;
+    }
+    if ((e = cudaMemcpy(plan->d_widths, plan->widths.data(), sizeof(int32_t) * n_w, cudaMemcpyHostToDevice)) !=
+            cudaSuccess ||
+        (e = cudaMemcpy(plan->d_wscale, scale.data(), sizeof(float) * n_w, cudaMemcpyHostToDevice)) != cudaSuccess) {
+        generic_release(plan);
+        return cuda_fail(e, "uploading the width table");
+    }
+
+    // ---- tile kernel: no workspace -------------------------------------------------------
+    const int64_t M = plan->max_width;
+    plan->generic_tile = 0;
+    if (M - 1 + 4096 <= kTileSpanMax && !std::getenv("SPD_GENERIC_WORKSPACE")) {
+        const int64_t tile_max = (kTileSpanMax - (M - 1)) / kSub * kSub;
+        // enough tiles to fill the machine, but none so short that its look-ahead dominates
+        const int64_t tiles_wanted = std::max<int64_t>(1, (2 * plan->sm_count + plan->n_dm - 1) / plan->n_dm);
+        int64_t tile = ((plan->n_t + tiles_wanted - 1) / tiles_wanted + 1023) / 1024 * 1024;
+        tile = std::max<int64_t>(tile, std::min<int64_t>(tile_max, (M + 1023) / 1024 * 1024));
+        tile = std::min<int64_t>(tile, tile_max);
+        const int64_t span = (tile + M - 1 + kSub - 1) / kSub * kSub;
+        const int64_t n_sub = span / kSub;
+        plan->generic_tile = static_cast<int>(tile);
+        plan->generic_span = static_cast<int>(span);
+        plan->generic_smem = static_cast<size_t>((n_sub + 2) / 2 * 16 + (span + 4) / 4 * 16 + kTileWidthsMax * 8);
+        plan->generic_tiles_per_row = (plan->n_t + tile - 1) / tile;
+        if (plan->n_dm * plan->generic_tiles_per_row > 0x7fffffffll) {
+            set_error("plane too large for the generic path's 1-D grid");
+            generic_release(plan);
+            return SPD_ERR_INVALID_ARG;
+        }
+        e = cudaFuncSetAttribute(generic_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 static_cast<int>(plan->generic_smem));
+        if (e != cudaSuccess) {
+            generic_release(plan);
+            return cuda_fail(e, "configuring the any-width-set tile kernel");
+        }
+        return SPD_OK;
+    }
+
+    // ---- workspace kernels (max_width too large for a shared-memory tile) -----------------
     plan->generic_blocks_per_row = (plan->n_t + kScanBlock - 1) / kScanBlock;
     const size_t prefix_bytes = sizeof(double) * static_cast<size_t>(plan->n_dm) * static_cast<size_t>(plan->n_t + 1);
     const size_t bs_bytes = sizeof(double) * static_cast<size_t>(plan->n_dm) * plan->generic_blocks_per_row;
     if (plan->n_dm * plan->generic_blocks_per_row > 0x7fffffffll ||
         plan->n_dm * ((plan->n_t + 255) / 256) > 0x7fffffffll) {
         set_error("plane too large for the generic path's 1-D grids");
+        generic_release(plan);
         return SPD_ERR_INVALID_ARG;
     }
-    cudaError_t e;
-    if ((e = cudaMalloc(&plan->d_widths, sizeof(int32_t) * n_w)) != cudaSuccess ||
-        (e = cudaMalloc(&plan->d_wscale, sizeof(float) * n_w)) != cudaSuccess ||
-        (e = cudaMalloc(&plan->d_prefix, prefix_bytes)) != cudaSuccess ||
+    if ((e = cudaMalloc(&plan->d_prefix, prefix_bytes)) != cudaSuccess ||
         (e = cudaMalloc(&plan->d_blocksum, bs_bytes)) != cudaSuccess) {
         set_error("device allocation of the generic workspace (%zu bytes) failed: %s", prefix_bytes + bs_bytes,
                   cudaGetErrorString(e));
@@ -175,12 +350,6 @@ int generic_configure(spd_plan* plan) {
         return SPD_ERR_ALLOC;
     }
     plan->workspace_bytes = static_cast<int64_t>(prefix_bytes + bs_bytes);
-    if ((e = cudaMemcpy(plan->d_widths, plan->widths.data(), sizeof(int32_t) * n_w, cudaMemcpyHostToDevice)) !=
-            cudaSuccess ||
-        (e = cudaMemcpy(plan->d_wscale, scale.data(), sizeof(float) * n_w, cudaMemcpyHostToDevice)) != cudaSuccess) {
-        generic_release(plan);
-        return cuda_fail(e, "uploading the width table");
-    }
     return SPD_OK;
 }
 
@@ -198,6 +367,15 @@ void generic_release(spd_plan* plan) {
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                 float* out_snr, int32_t* out_width, cudaStream_t stream) {
     const long long n_t = plan->n_t;
+    if (plan->generic_tile > 0) {
+        generic_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads,
+                              plan->generic_smem, stream>>>(
+            plane, mean, sigma, plan->d_widths, plan->d_wscale, static_cast<int>(plan->widths.size()), n_t,
+            plan->generic_tile, plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "launching the any-width-set tile kernel");
+        return SPD_OK;
+    }
     const long long bpr = plan->generic_blocks_per_row;
     const unsigned scan_grid = static_cast<unsigned>(n_dm * bpr);
     generic_block_sums<<<scan_grid, kScanThreads, 0, stream>>>(plane, mean, n_t, bpr, plan->d_blocksum);

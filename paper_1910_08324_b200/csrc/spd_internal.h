@@ -57,6 +57,10 @@ struct spd_plan {
     double* d_prefix = nullptr;    // [n_dm][n_t + 1] running sums of (x - mu)
     double* d_blocksum = nullptr;  // [n_dm][blocks_per_row]
     int64_t generic_blocks_per_row = 0;
+    int generic_tile = 0;  // > 0: tile kernel (time samples per block); 0: workspace kernels
+    int generic_span = 0;  // tile + look-ahead, multiple of 64
+    size_t generic_smem = 0;
+    int64_t generic_tiles_per_row = 0;
     int64_t workspace_bytes = 0;
     // spd_row_stats
     void* d_stats = nullptr;  // [n_dm][stats_parts] partial moments

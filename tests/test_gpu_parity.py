@@ -118,6 +118,39 @@ def test_generic_width_sets(spd, oracle_lib, kind, param, max_width):
           expect_path=spd.SPD_PATH_GENERIC)
 
 
+def test_generic_tile_kernel_wide_sets_and_tile_boundaries(spd, oracle_lib):
+    """Any-width-set tile kernel: max_width in the thousands (several tiles per row, ragged last tile,
+    look-ahead longer than the tile's remainder), on drifting data with a large offset."""
+    rng = np.random.default_rng(31)
+    n_dm, n_t = 3, 150001
+    x = (rng.standard_normal((n_dm, n_t)) + 0.2 * np.sin(np.arange(n_t) / 9000.0) + 25.0).astype(np.float32)
+    x[1, 60000:63000] += np.float32(0.4)
+    x[2, n_t - 2500:] += np.float32(0.3)  # runs off the end of the row
+    mu, sg = oracle_lib.row_stats(x)
+    for kind, param, mw in [("IGRID", 1, 8192), ("BOXDIT", 16, 3000), ("GEOMETRIC", 1500, 20000)]:
+        widths = spd.spd_width_set_generate(kind, param, mw)
+        st = check(spd, oracle_lib, x, mu, sg, widths, f"tile {kind}({param})<= {mw}",
+                   expect_path=spd.SPD_PATH_GENERIC)
+        assert st.max_err_over_tol < 0.5
+
+
+def test_generic_workspace_fallback(spd, oracle_lib, monkeypatch):
+    """The running-sum-in-device-memory kernels (used when max_width does not fit a shared-memory tile)."""
+    rng = np.random.default_rng(32)
+    x = rng.standard_normal((4, 30011), dtype=np.float32)
+    x[3, 1000:1400] += np.float32(0.8)
+    widths = spd.spd_width_set_generate("IGRID", 2, 1024)
+    monkeypatch.setenv("SPD_GENERIC_WORKSPACE", "1")
+    got_snr, got_idx, info = run_gpu(spd, x, 0.0, 1.0, widths)
+    assert info["launches_per_run"] == 4 and info["workspace_bytes"] > 8 * 4 * 30011
+    monkeypatch.delenv("SPD_GENERIC_WORKSPACE")
+    got_snr2, got_idx2, info2 = run_gpu(spd, x, 0.0, 1.0, widths)
+    assert info2["launches_per_run"] == 1
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    for gs, gi, what in ((got_snr, got_idx, "workspace"), (got_snr2, got_idx2, "tile")):
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, gs, gi, ref_snr, ref_idx, ref_sec, what=what)
+
+
 def test_width_set_generators_agree_with_formula_module(spd):
     from oracle import formulas
     for kind, param, mw in [("ALL", 0, 64), ("POW2", 0, 8192), ("BOXDIT", 4, 12), ("BOXDIT", 8, 8192),
