@@ -42,7 +42,9 @@ def test_two_gloo_ranks_max_time_and_aggregate(tmp_path):
     script.write_text(_WORKER.format(root=ROOT))
     res = _torchrun([str(script)], 29541)
     assert res.returncode == 0, res.stdout[-2000:] + res.stderr[-4000:]
-    rows = [json.loads(ln.split("RESULT ", 1)[1]) for ln in res.stdout.splitlines() if "RESULT " in ln]
+    # the two ranks share stdout: their lines may run together
+    dec = json.JSONDecoder()
+    rows = [dec.raw_decode(part)[0] for part in res.stdout.split("RESULT ")[1:]]
     assert sorted(r["rank"] for r in rows) == [0, 1]
     r0, r1 = sorted(rows, key=lambda r: r["rank"])
     assert r0["world"] == r1["world"] == 2
