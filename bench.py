@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config number (1-based)")
     ap.add_argument("--n-dm", type=int, default=0, help="override the number of DM trials (debugging)")
+    ap.add_argument("--width-set", default="", help="override the workload's width set, e.g. IGRID:1 "
+                    "(widths 2^k and 3*2^m, the paper's IG(1) set) - not the BASELINE configuration")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -152,7 +154,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from workloads import get_workload
-    w = get_workload(args.workload)
+    w = apply_overrides(get_workload(args.workload), args)
     widths = oracle_widths(w)
     # bounded: the whole --steps/--warmup run is sized to about 4 * cpu_seconds
     res = time_oracle(w, widths, 4.0 * args.cpu_seconds, steps=args.steps, warmup=args.warmup)
@@ -261,7 +263,7 @@ def run_b200(args):
         dist.init_process_group("nccl", device_id=dev)
 
     spd.build()
-    w = get_workload(args.workload)
+    w = apply_overrides(get_workload(args.workload), args)
     if args.n_dm:
         w = w.scaled(args.n_dm, w.n_t)
     # weak scaling: every rank holds its own n_dm DM trials (different seed per rank)
@@ -358,7 +360,8 @@ def run_b200(args):
     k_ms = sum(run_ms) / len(run_ms)
     achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
     roofline = {
-        "bound": "hbm", "kernel": "spd_tree_kernel" if info["path"] == spd.SPD_PATH_DYADIC_TREE else "generic_eval",
+        "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_kernel", spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel"}.get(
+            info["path"], "generic_tile_kernel"),
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),
         "algorithmic_bytes_per_launch": BYTES_PER_SAMPLE * n, "bytes_per_sample": BYTES_PER_SAMPLE,
@@ -372,7 +375,8 @@ def run_b200(args):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": workload_config(w, widths, {
             "parallelism": f"dm-rows x{world} (independent DM trials per GPU, no collective)",
-            "path": "dyadic_tree" if info["path"] == spd.SPD_PATH_DYADIC_TREE else "generic",
+            "path": {spd.SPD_PATH_DYADIC_TREE: "dyadic_tree", spd.SPD_PATH_IGRID_TREE: "igrid_tree"}.get(
+                info["path"], "generic"),
             "blocks": info["blocks"], "threads_per_block": info["threads_per_block"],
             "segments_per_row": info["segments_per_row"], "chunk": info["chunk"], "smem_bytes": info["smem_bytes"],
             "candidate_threshold": thr, "candidates_found": n_cand}),
@@ -420,7 +424,7 @@ NCU_DRAM_BYTES_PER_SAMPLE = {3: (4.397637e9 + 8.536988e9) / float(1 << 30)}
 
 
 def ncu_traffic_bytes(w):
-    per_sample = NCU_DRAM_BYTES_PER_SAMPLE.get(w.index)
+    per_sample = NCU_DRAM_BYTES_PER_SAMPLE.get(w.index) if w.width_kind == "POW2" else None
     return None if per_sample is None else per_sample * w.n_samples
 
 
@@ -469,6 +473,14 @@ def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
             "api": "spd_run_host (pinned host buffers; H2D, kernels and D2H of Y and W inside the call)",
             "note": "whole plane" if rows == w.n_dm else f"first {rows} of {w.n_dm} DM trials (host memory bound)",
             "checksum": checksum}
+
+
+def apply_overrides(w, args):
+    from dataclasses import replace
+    if args.width_set:
+        kind, _, param = args.width_set.partition(":")
+        w = replace(w, width_kind=kind.upper(), width_param=int(param or 0))
+    return w
 
 
 def main():

@@ -62,10 +62,11 @@ typedef enum spd_width_kind {
 } spd_width_kind;
 
 /* Plan creation flags (spd_plan_create_ex). */
-#define SPD_FLAG_FORCE_GENERIC 0x1u /* use the any-width-set kernels even where the dyadic tree applies */
+#define SPD_FLAG_FORCE_GENERIC 0x1u /* use the any-width-set kernels even where a streaming tree applies */
 
 /* Which kernels a plan dispatches to (spd_plan_info.path). */
 #define SPD_PATH_DYADIC_TREE 1 /* streaming partial-sum tree, widths {1,2,4,...,2^(K-1)} */
+#define SPD_PATH_IGRID_TREE 3  /* the same streaming tree for widths {2^k} U {3 * 2^m} (IGRID depth 1, eq. 18) */
 #define SPD_PATH_GENERIC 2     /* any width set: per-row running partial sums, staged per tile in shared memory */
 
 typedef struct spd_plan spd_plan; /* opaque */

@@ -25,7 +25,7 @@ SPD_ERR_CUDA = -4
 SPD_WIDTHS_ALL, SPD_WIDTHS_POW2, SPD_WIDTHS_BOXDIT, SPD_WIDTHS_IGRID, SPD_WIDTHS_GEOMETRIC = range(5)
 WIDTH_KINDS = {"ALL": 0, "POW2": 1, "BOXDIT": 2, "IGRID": 3, "GEOMETRIC": 4}
 SPD_FLAG_FORCE_GENERIC = 0x1
-SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC = 1, 2
+SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC, SPD_PATH_IGRID_TREE = 1, 2, 3
 
 # every symbol include/spd.h declares
 EXPORTS = (

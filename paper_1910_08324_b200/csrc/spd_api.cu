@@ -165,6 +165,8 @@ int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const flo
              float* out_snr, int32_t* out_width, cudaStream_t stream) {
     if (plan->path == SPD_PATH_DYADIC_TREE)
         return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
+    if (plan->path == SPD_PATH_IGRID_TREE)
+        return ig_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
     return generic_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
 }
 
@@ -257,9 +259,14 @@ int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     plan->max_width = max_width;
     plan->device = device;
     plan->sm_count = sm_count;
+    int ig_levels = 0;
     if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
         plan->path = SPD_PATH_DYADIC_TREE;
         rc = tree_configure(plan);
+    } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && (ig_levels = ig_applicable(w, n_t)) > 0) {
+        plan->path = SPD_PATH_IGRID_TREE;
+        plan->tree.K = ig_levels;
+        rc = ig_configure(plan);
     } else {
         plan->path = SPD_PATH_GENERIC;
         rc = generic_configure(plan);
@@ -304,7 +311,7 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
     info->n_widths = static_cast<int32_t>(plan->widths.size());
     info->max_width = plan->max_width;
     info->path = plan->path;
-    if (plan->path == SPD_PATH_DYADIC_TREE) {
+    if (is_tree_path(plan)) {
         info->launches_per_run = 1;
         info->threads_per_block = plan->tree.T;
         info->blocks = static_cast<int32_t>(plan->n_dm * plan->tree.segs_per_row);
@@ -367,6 +374,8 @@ int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean,
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (plan->path == SPD_PATH_DYADIC_TREE)
         return tree_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (plan->path == SPD_PATH_IGRID_TREE)
+        return ig_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     // any-width-set path: no fused test, every block stays active (padding included: the
     // candidate kernel bounds the flag index itself)
     const cudaError_t e = cudaMemsetAsync(activity, 1, activity_bytes(plan), stream);
@@ -420,7 +429,7 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
         (e = cudaStreamSynchronize(h.stream[0])) != cudaSuccess)
         return cuda_fail(e, "copying mean / sigma to the device");
     // The workspace variant of the any-width-set path shares one workspace: one stream.
-    const int n_streams = (plan->path == SPD_PATH_DYADIC_TREE || plan->generic_tile > 0) ? 2 : 1;
+    const int n_streams = (is_tree_path(plan) || plan->generic_tile > 0) ? 2 : 1;
     int64_t blk = 0;
     for (int64_t r0 = 0; r0 < plan->n_dm; r0 += h.rows_per_block, ++blk) {
         const int64_t rows = std::min<int64_t>(h.rows_per_block, plan->n_dm - r0);

@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
 }  // namespace
 
 int64_t activity_block(const spd_plan* plan) {
-    return plan->path == SPD_PATH_DYADIC_TREE ? plan->tree.chunk : 4096;
+    return is_tree_path(plan) ? plan->tree.chunk : 4096;
 }
 int64_t activity_per_row(const spd_plan* plan) {
     const int64_t b = activity_block(plan);

@@ -78,11 +78,23 @@ int cuda_fail(cudaError_t e, const char* what);
 // spd_tree.cu
 bool tree_applicable(const std::vector<int32_t>& widths, int64_t n_t);
 int tree_configure(spd_plan* plan);
+int tree_configure_segments(spd_plan* plan);
 // activity: nullptr, or [n_dm][chunks_per_row] bytes (cleared here, set by the kernel for
 // every chunk whose best SNR reaches `threshold`).
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
              const float* sigma, float* out_snr, int32_t* out_width, float threshold,
              uint8_t* activity, cudaStream_t stream);
+
+// spd_tree_ig.cu: widths 2^k and 3 * 2^m (IGRID depth 1)
+int ig_applicable(const std::vector<int32_t>& widths, int64_t n_t);  // K (pow-2 levels) or 0
+int ig_configure(spd_plan* plan);
+int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
+           const float* sigma, float* out_snr, int32_t* out_width, float threshold,
+           uint8_t* activity, cudaStream_t stream);
+
+inline bool is_tree_path(const spd_plan* plan) {
+    return plan->path == SPD_PATH_DYADIC_TREE || plan->path == SPD_PATH_IGRID_TREE;
+}
 
 // spd_generic.cu
 int generic_configure(spd_plan* plan);

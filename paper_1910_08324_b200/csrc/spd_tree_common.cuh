@@ -1,0 +1,251 @@
+// Shared by the streaming-tree kernels (spd_tree.cu: widths 2^k; spd_tree_ig.cu: widths 2^k and
+// 3 * 2^m): launch parameters, PTX helpers (mbarrier, 1-D bulk copy, 3-input max), packed
+// float4 arithmetic, width-index tags, geometry.  Internal to libspd_b200.so.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <type_traits>
+
+#include "spd_internal.h"
+
+namespace spd {
+namespace {
+
+struct TreeParams {
+    const float* plane;
+    const float* mean;
+    const float* sigma;
+    float* out_snr;
+    int32_t* out_width;
+    uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr
+    float threshold;    // candidate threshold in SNR units (used only with activity)
+    long long n_t;
+    int chunks_per_row;
+    int seg_chunks;
+    int segs_per_row;
+    int warm_chunks;
+    // ~kCodeMask, passed at run time on purpose: as a compile-time constant the tag
+    // (v & mask) | code has two immediates and costs two LOP3 per value instead of one.
+    uint32_t tag_mask;
+};
+
+// ------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D bulk copy (TMA), 3-input max.
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        " .reg .pred p;\n"
+        " mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        " selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem),
+                 "r"(smem_u32(src_smem)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+
+// ------------------------------------------------------------------------------------
+// float4 arithmetic on the packed FP32x2 pipe.
+// ------------------------------------------------------------------------------------
+__device__ __forceinline__ float4 add4(float4 a, float4 b) {
+    const float2 lo = __fadd2_rn(make_float2(a.x, a.y), make_float2(b.x, b.y));
+    const float2 hi = __fadd2_rn(make_float2(a.z, a.w), make_float2(b.z, b.w));
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
+}
+__device__ __forceinline__ float4 scale4(float4 a, float c) {
+    const float2 cc = make_float2(c, c);
+    const float2 lo = __fmul2_rn(make_float2(a.x, a.y), cc);
+    const float2 hi = __fmul2_rn(make_float2(a.z, a.w), cc);
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
+}
+// x - mu (eq. 4 numerator per sample; sums of mean-free data never cancel later).  The
+// division by sigma is applied once per output sample at the store, not per input sample.
+__device__ __forceinline__ float4 norm4(float4 a, float mu) {
+    const float2 m = make_float2(-mu, -mu);
+    const float2 lo = __fadd2_rn(make_float2(a.x, a.y), m);
+    const float2 hi = __fadd2_rn(make_float2(a.z, a.w), m);
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
+}
+
+// 2^(-k/2): SNR scale of width 2^k on unit-variance data (eq. 5).
+template <int k>
+__device__ __forceinline__ constexpr float level_scale() {
+    return ((k & 1) ? 0.70710678118654752440f : 1.0f) / static_cast<float>(1 << (k / 2));
+}
+
+constexpr uint32_t kCodeBits = 5;
+constexpr uint32_t kCodeMask = (1u << kCodeBits) - 1u;
+
+// SNR of level k with the inverted width index in the low mantissa bits.
+template <int k>
+__device__ __forceinline__ float pack1(float v, uint32_t tm) {
+    return __uint_as_float((__float_as_uint(v) & tm) | (kCodeMask - static_cast<uint32_t>(k)));
+}
+template <int k>
+__device__ __forceinline__ float4 key4(float4 p, uint32_t tm) {
+    const float4 v = scale4(p, level_scale<k>());
+    return make_float4(pack1<k>(v.x, tm), pack1<k>(v.y, tm), pack1<k>(v.z, tm), pack1<k>(v.w, tm));
+}
+// Guarded variant: element v of the float4 is valid iff 2^k <= lim - v (reading A3).
+template <int k>
+__device__ __forceinline__ float4 key4_masked(float4 p, int lim, uint32_t tm) {
+    float4 q = key4<k>(p, tm);
+    const int w = 1 << k;
+    const float ninf = __int_as_float(0xff800000);
+    if (w > lim) q.x = ninf;
+    if (w > lim - 1) q.y = ninf;
+    if (w > lim - 2) q.z = ninf;
+    if (w > lim - 3) q.w = ninf;
+    return q;
+}
+__device__ __forceinline__ float4 max4(float4 a, float4 b) {
+    return make_float4(fmaxf(a.x, b.x), fmaxf(a.y, b.y), fmaxf(a.z, b.z), fmaxf(a.w, b.w));
+}
+__device__ __forceinline__ float4 max4(float4 a, float4 b, float4 c) {
+    return make_float4(fmax3(a.x, b.x, c.x), fmax3(a.y, b.y, c.y), fmax3(a.z, b.z, c.z), fmax3(a.w, b.w, c.w));
+}
+
+template <int k, bool FAST>
+__device__ __forceinline__ float4 keyx(float4 p, int lim, uint32_t tm) {
+    if constexpr (FAST) {
+        return key4<k>(p, tm);
+    } else {
+        return key4_masked<k>(p, lim, tm);
+    }
+}
+
+// Fold the SNR of level j (just produced as `now` from `before` = level j-1) into best.
+// Levels 0..2 are folded by the caller; above, levels are folded in pairs (j-1, j) when
+// j is even so that one FMNMX3 serves two widths; a trailing odd level is folded alone.
+template <int j, int K, bool FAST>
+__device__ __forceinline__ void fold(float4& best, float4 before, float4 now, int lim, uint32_t tm) {
+    if constexpr (j >= 3) {
+        if constexpr ((j & 1) == 0) {
+            best = max4(best, keyx<j - 1, FAST>(before, lim, tm), keyx<j, FAST>(now, lim, tm));
+        } else if constexpr (j == K - 1) {
+            best = max4(best, keyx<j, FAST>(now, lim, tm));
+        }
+    }
+}
+
+// Shared-memory store of a float4: as one 128-bit store, or as two 64-bit stores.  The sums
+// are produced by packed FADD2 into register PAIRS; a 128-bit store needs an aligned QUAD
+// and costs up to four register moves when the allocator cannot place the pairs together.
+#ifndef SPD_TREE_STS64
+#define SPD_TREE_STS64 1
+#endif
+template <int SPLIT>
+__device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
+    if constexpr (SPLIT) {
+        // inline PTX: as plain C++ the two halves are merged back into one 128-bit store
+        const uint32_t a = smem_u32(dst);
+        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
+        asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(a), "f"(v.z), "f"(v.w) : "memory");
+    } else {
+        *dst = v;
+    }
+}
+
+#ifndef SPD_TREE_RADIX4
+#define SPD_TREE_RADIX4 0  // two exchange levels per barrier; measured 11.99 ms vs 11.41 ms (config 3)
+#endif
+#ifndef SPD_TREE_TMA_STORE
+#define SPD_TREE_TMA_STORE 0  // measured: 11.87 ms vs 11.41 ms with direct 128-bit stores (config 3)
+#endif
+
+// The chunk loop is unrolled over the delay FIFOs up to this factor: a FIFO no deeper than
+// the unroll gets a compile-time slot (no register moves), a deeper one is rotated by moves.
+// Code size grows with the factor; past the instruction cache the kernel stalls on fetch
+// (T = 64, R = 4 unrolled x4: smsp stall_no_instruction 2.6 per issue).
+#ifndef SPD_TREE_MAX_UNROLL
+#define SPD_TREE_MAX_UNROLL 2
+#endif
+constexpr int tree_max_unroll(int K) { return K == 16 ? 4 : SPD_TREE_MAX_UNROLL; }
+
+constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
+constexpr int imax(int a, int b) { return a > b ? a : b; }
+
+// Geometry of one kernel instantiation.
+template <int T, int R, int K>
+struct Geo {
+    static constexpr int LT = ilog2(T);
+    static constexpr int C4 = R * T;   // float4 per chunk
+    static constexpr int C = 4 * C4;   // samples per chunk
+    static constexpr int LAST = K - 1;  // highest level: width 2^LAST
+    // In-register levels j = 0 .. J-1: partner 2^j rows later, produces level LT + 3 + j.
+    static constexpr int J = imax(0, LAST - LT - 2);
+    static constexpr int ND = (1 << J) - 1;  // float4 of delay registers: sum of 2^j
+    // Depth, in chunks, of the deepest delay FIFO = unroll factor of the chunk loop.
+    // Optional: unguarded chunks leave through a shared-memory staging buffer and two bulk
+    // stores (Y, W) instead of 128-bit global stores.  Off by default: the extra barrier and
+    // shared-memory stores cost more than the global stores they replace (DESIGN.md "Tuning
+    // log").  Needs an exchange level (its barrier orders the reuse of the staging buffer).
+    static constexpr bool TMA_STORE = SPD_TREE_TMA_STORE && LAST >= 4;
+    static constexpr int TOPQ = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
+    static constexpr int U = TOPQ < tree_max_unroll(K) ? TOPQ : tree_max_unroll(K);
+};
+
+struct ChunkCtx {
+    float4* sout;  // staging of one chunk's Y (C floats) then W (C ints)
+    float mu, inv;
+    uint32_t tm;
+    float* __restrict__ out_snr;
+    int32_t* __restrict__ out_width;
+    long long n0, n_t;
+    bool do_out;
+    int tid;
+};
+
+// Compile-time loop over the phases of the unrolled chunk loop.
+template <int PH, int U, typename F>
+__device__ __forceinline__ void static_phases(F&& f) {
+    if constexpr (PH < U) {
+        f(std::integral_constant<int, PH>{});
+        static_phases<PH + 1, U>(f);
+    }
+}
+
+
+}  // namespace
+}  // namespace spd

@@ -84,6 +84,70 @@ def test_dyadic_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
     check(spd, oracle_lib, x, 0.0, 1.0, widths, f"tree K={K}", expect_path=spd.SPD_PATH_DYADIC_TREE)
 
 
+@pytest.mark.parametrize("K", list(range(5, 17)))
+def test_igrid_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
+    """Every instantiation of the IGRID depth-1 streaming tree (widths 2^k and 3 * 2^m up to 2^(K-1)):
+    several chunks, ragged tail, several segments per row, pulses of non-power-of-two widths."""
+    M = 1 << (K - 1)
+    chunk = 4096
+    n_t = max(5 * chunk + 4 * 37, 2 * M + chunk + 4 * 5)
+    rng = np.random.default_rng(2000 + K)
+    x = rng.standard_normal((3, n_t), dtype=np.float32)
+    S = max(1, 3 * M // 8)
+    x[1, n_t // 3: n_t // 3 + S] += np.float32(12.0 / np.sqrt(S))
+    x[2, n_t - M // 2 - 3:] += np.float32(0.7)  # a pulse running off the end of the row
+    monkeypatch.setenv("SPD_SEGS_PER_ROW", "3")
+    widths = spd.spd_width_set_generate("IGRID", 1, M)
+    assert len(widths) == 2 * K - 2
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"igrid tree K={K}", expect_path=spd.SPD_PATH_IGRID_TREE)
+
+
+@pytest.mark.parametrize("segs", [1, 2, 5])
+def test_igrid_tree_segmentation_and_statistics(spd, oracle_lib, segs, monkeypatch):
+    rng = np.random.default_rng(78)
+    n_t = 2048 * 19 + 4 * 3
+    x = (rng.standard_normal((2, n_t)) * 3.1 - 17.0).astype(np.float32)
+    x[0, 9000:9000 + 96] += np.float32(4.0)  # width 96 = 3 * 32 is in the set
+    mu, sg = oracle_lib.row_stats(x)
+    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(segs))
+    widths = spd.spd_width_set_generate("IGRID", 1, 4096)
+    check(spd, oracle_lib, x, mu, sg, widths, f"igrid tree segs={segs}", expect_path=spd.SPD_PATH_IGRID_TREE)
+
+
+def test_igrid_tree_exact_ties_and_plateau(spd, oracle_lib):
+    """Zero background: exact ties resolve to the smallest width; a width-24 pulse is recovered exactly
+    by the width-24 boxcar (index 8 of 1,2,3,4,6,8,12,16,24)."""
+    n_t = 8192
+    x = np.zeros((2, n_t), dtype=np.float32)
+    x[1, 1000:1024] = np.float32(2.0)
+    widths = list(spd.spd_width_set_generate("IGRID", 1, 64))
+    got_snr, got_idx, info = run_gpu(spd, x, 0.0, 1.0, widths)
+    assert info["path"] == spd.SPD_PATH_IGRID_TREE
+    assert np.all(got_snr[0] == 0.0) and np.all(got_idx[0, : n_t - 64] == 0)
+    assert got_idx[1, 1000] == widths.index(24)
+    assert abs(got_snr[1, 1000] - 2.0 * np.sqrt(24.0)) < 1e-4 * 2.0 * np.sqrt(24.0)
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec, what="ig ties")
+
+
+def test_igrid_tree_flagged_candidates(spd, oracle_lib):
+    from workloads import get_workload, make_plane_numpy
+    w = get_workload(3).scaled(4, 131072, 10)
+    x, _ = make_plane_numpy(w)
+    widths = spd.spd_width_set_generate("IGRID", 1, 8192)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(4, device=dev), torch.ones(4, device=dev)
+    with spd.Plan(4, 131072, widths) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_IGRID_TREE
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 6.0)
+        lst, n_f = plan.find_candidates_flagged(snr, idx, act, 6.0, 1 << 16)
+        count, got = spd.candidates_to_numpy(lst, n_f, 1 << 16)
+        ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.cpu().numpy(), idx.cpu().numpy(), 6.0)
+        assert count == ref_count and count > 0
+        assert np.array_equal(got["dm"], c_dm) and np.array_equal(got["t"], c_t)
+
+
 @pytest.mark.parametrize("segs", [1, 2, 7])
 def test_dyadic_tree_segmentation_is_invisible(spd, oracle_lib, segs, monkeypatch):
     rng = np.random.default_rng(77)
@@ -363,11 +427,11 @@ def test_flagged_run_equals_plain_run_and_dense_candidates(spd, oracle_lib, cfg,
 
 def test_flagged_run_generic_path_marks_everything(spd, oracle_lib):
     rng = np.random.default_rng(21)
-    x = rng.standard_normal((3, 20000), dtype=np.float32)
+    x = rng.standard_normal((3, 20001), dtype=np.float32)
     x[1, 7000:7030] += np.float32(2.0)
     widths = spd.spd_width_set_generate("IGRID", 1, 64)
     dev = torch.device("cuda:0")
-    with spd.Plan(3, 20000, widths) as plan:
+    with spd.Plan(3, 20001, widths) as plan:
         assert plan.info["path"] == spd.SPD_PATH_GENERIC
         snr, idx, act = plan.run_flagged(torch.from_numpy(x).to(dev), torch.zeros(3, device=dev),
                                          torch.ones(3, device=dev), 5.0)
