@@ -111,11 +111,13 @@ def _rule_candidates(snr, thr, rows_per_block=64):
     return torch.sort(torch.cat(keys))[0]
 
 
-@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
-def test_full_size_config(spd, oracle_lib, cfg):
-    import ctypes
+@pytest.mark.parametrize("cfg,width_kind", [(2, None), (3, None), (4, None), (5, None), (3, "IGRID"), (4, "IGRID")])
+def test_full_size_config(spd, oracle_lib, cfg, width_kind):
+    from dataclasses import replace
     from workloads import get_workload, make_plane_torch
     w = get_workload(cfg)
+    if width_kind:  # the paper's IG(1) width set (IGRID streaming tree) on the same plane
+        w = replace(w, width_kind=width_kind, width_param=1)
     dev = torch.device("cuda:0")
     free, _ = torch.cuda.mem_get_info(dev)
     need = 13 * w.n_samples + (6 << 30)
@@ -134,7 +136,7 @@ def test_full_size_config(spd, oracle_lib, cfg):
     cap = 1 << 22
     with spd.Plan(w.n_dm, w.n_t, widths, w.max_width) as plan:
         info = dict(plan.info)
-        assert info["path"] == spd.SPD_PATH_DYADIC_TREE
+        assert info["path"] == (spd.SPD_PATH_IGRID_TREE if width_kind else spd.SPD_PATH_DYADIC_TREE)
         snr, idx, act = plan.run_flagged(plane, mean, sigma, thr)
         lst, n_found = plan.find_candidates_flagged(snr, idx, act, thr, cap)
         torch.cuda.synchronize()

@@ -277,8 +277,9 @@ def test_constant_offset_closed_form(spd):
     assert np.all(np.abs(got_snr[0] - exp_snr) <= 1e-4 * np.maximum(1, exp_snr))
 
 
+@pytest.mark.parametrize("kind", ["config", "IGRID1"])
 @pytest.mark.parametrize("cfg,n_dm,n_t,n_pulses", [(2, 8, 32768, 16), (3, 4, 262144, 12), (4, 2, 524288, 6)])
-def test_noise_free_twin_loss_matches_eq24(spd, cfg, n_dm, n_t, n_pulses):
+def test_noise_free_twin_loss_matches_eq24(spd, cfg, n_dm, n_t, n_pulses, kind):
     """Pin P14 through the CUDA path: on a zero-background plane each injected rectangular
     pulse is recovered at exactly eq. (24)'s fraction of its true SNR,
     and the mean loss equals the formula's mean over the injected widths."""
@@ -286,8 +287,12 @@ def test_noise_free_twin_loss_matches_eq24(spd, cfg, n_dm, n_t, n_pulses):
     from workloads import get_workload, make_pulse_only_plane_numpy
     w = get_workload(cfg).scaled(n_dm, n_t, n_pulses)
     x, pulses = make_pulse_only_plane_numpy(w)
-    widths = list(spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width))
-    got_snr, _, _ = run_gpu(spd, x, 0.0, 1.0, widths)
+    if kind == "IGRID1":  # the paper's IG(1) width set on the same pulses (IGRID streaming tree)
+        widths = list(spd.spd_width_set_generate("IGRID", 1, w.max_width))
+    else:
+        widths = list(spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width))
+    got_snr, _, info = run_gpu(spd, x, 0.0, 1.0, widths)
+    assert info["path"] == (spd.SPD_PATH_IGRID_TREE if kind == "IGRID1" else spd.SPD_PATH_DYADIC_TREE)
     losses, predicted = [], []
     for p in pulses:
         others = [q for q in pulses if q is not p and q.dm == p.dm and
