@@ -178,6 +178,40 @@ def test_clipped_stats_everything_rejected_keeps_estimate(oracle_lib):
     assert mu[0] == 5.0 and sg[0] == 5.0
 
 
+# --- sec. 4.3: other pulse shapes (reading A15) ---------------------
+
+def test_gaussian_pulse_worked_example(oracle_lib, paper_pins):
+    """The ideal algorithm (all widths) on a zero plane with one Gaussian pulse of 20 samples, C = 16:
+    best boxcar 11 samples wide, 4 or 5 samples late, RSNR above C."""
+    from workloads.generate import pulse_profile
+    pin = paper_pins["gaussian_pulse_example"]
+    S, C, t0 = pin["pulse_width"], pin["C"], 100
+    x = np.zeros((1, 400), dtype=np.float32)
+    x[0, t0:t0 + S] += pulse_profile("gauss", S, C).astype(np.float32)
+    assert abs(float(x[0].sum()) / math.sqrt(S) - C) < 1e-4           # boxcar of the signal width gives C
+    widths = list(range(1, 2 * S + 1))
+    snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+    n = int(np.argmax(snr[0]))
+    assert widths[idx[0, n]] == pin["detected_width"]
+    assert (n - t0) in pin["time_delay"]
+    assert snr[0, n] > C
+
+
+def test_gaussian_pulse_width_error_and_recovered_power(oracle_lib, paper_pins):
+    """Wide Gaussian pulses: width under-estimated by about 40 %, about 85 % of the power summed."""
+    from workloads.generate import pulse_profile
+    pin = paper_pins["gaussian_pulse_example"]
+    for S in (100, 200):
+        x = np.zeros((1, 4 * S), dtype=np.float32)
+        x[0, S:2 * S] += pulse_profile("gauss", S, pin["C"]).astype(np.float32)
+        widths = list(range(1, S + 1))
+        snr, idx, _ = oracle_lib.spd_direct(x, 0.0, 1.0, widths)
+        n = int(np.argmax(snr[0]))
+        L = widths[idx[0, n]]
+        assert abs((L - S) / S - pin["width_error"]) < 0.02
+        assert abs(float(x[0, n:n + L].sum() / x[0].sum()) - pin["recovered_power"]) < 0.01
+
+
 # --- P9: brute force written out here, tiny planes ------------------------------------
 
 def _brute(x, mu, sg, widths):

@@ -17,7 +17,9 @@ from .generate import (
     make_plane_numpy,
     make_plane_torch,
     make_pulse_only_plane_numpy,
+    make_shaped_pulse_plane_numpy,
     pulse_amplitude,
+    pulse_profile,
 )
 
 __all__ = [
@@ -29,5 +31,7 @@ __all__ = [
     "make_plane_numpy",
     "make_plane_torch",
     "make_pulse_only_plane_numpy",
+    "make_shaped_pulse_plane_numpy",
     "pulse_amplitude",
+    "pulse_profile",
 ]

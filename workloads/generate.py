@@ -37,6 +37,47 @@ def pulse_amplitude(snr_t: float, width: int) -> float:
     return float(snr_t) / math.sqrt(float(width))
 
 
+def pulse_profile(shape: str, width: int, snr_t: float) -> np.ndarray:
+    """Samples of one pulse of ``width`` samples (float64), normalised as PAPER.md:553: "when all its
+    samples are summed together, i.e. a boxcar of signal width is applied to it, it will produce
+    RSNR = C" on unit noise, i.e. sum = snr_t * sqrt(width).
+
+    shape "rect": eq. (6).  "gauss" / "double_gauss": eq. (20), sampled at
+    the integers 0 .. width-1 with mean width/2 (reading A15: the printed variances S/(8 ln 2),
+    (S/4)/(8 ln 2), (S/5)/(8 ln 2) are taken as FWHM^2/(8 ln 2) with FWHM = S/2, S/4, S/5 - the
+    reading that reproduces the worked example of PAPER.md:577, a 20-sample Gaussian best matched by
+    an 11-sample boxcar 4-5 samples late; the two components of the double Gaussian sit at S/3 and
+    2S/3 with equal weight - the paper does not say where)."""
+    n = np.arange(width, dtype=np.float64)
+    k = 8.0 * math.log(2.0)
+    if shape == "rect":
+        prof = np.ones(width, dtype=np.float64)
+    elif shape == "gauss":
+        var = (width / 2.0) ** 2 / k
+        prof = np.exp(-((n - width / 2.0) ** 2) / (2.0 * var))
+    elif shape == "double_gauss":
+        v1, v2 = (width / 4.0) ** 2 / k, (width / 5.0) ** 2 / k
+        prof = (np.exp(-((n - width / 3.0) ** 2) / (2.0 * v1)) / math.sqrt(v1)
+                + np.exp(-((n - 2.0 * width / 3.0) ** 2) / (2.0 * v2)) / math.sqrt(v2))
+    else:
+        raise ValueError(f"unknown pulse shape {shape!r}")
+    return prof * (float(snr_t) * math.sqrt(float(width)) / prof.sum())
+
+
+def make_shaped_pulse_plane_numpy(w: Workload, shape: str, noise: bool = False) -> Tuple[np.ndarray, List[Pulse]]:
+    """The workload's pulses drawn with another profile (sec. 4.3) on a zero
+    background ("The input time-series is zeroed") or on the workload's noise."""
+    if noise:
+        rng = np.random.default_rng(w.seed + 104729)
+        plane = rng.standard_normal(size=(w.n_dm, w.n_t), dtype=np.float32)
+    else:
+        plane = np.zeros((w.n_dm, w.n_t), dtype=np.float32)
+    pulses = draw_pulses(w)
+    for p in pulses:
+        plane[p.dm, p.t0:p.t0 + p.width] += pulse_profile(shape, p.width, p.snr_t).astype(np.float32)
+    return plane, pulses
+
+
 def draw_pulses(w: Workload) -> List[Pulse]:
     """Draw the injected-pulse population of a workload from its seed."""
     rng = np.random.default_rng(w.seed)
