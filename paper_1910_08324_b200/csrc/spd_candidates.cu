@@ -13,7 +13,7 @@
 //     activity map is set.  The map is written by the kernel that produced Y (the
 //     threshold test is fused into spd_tree.cu), so on planes where detections are rare
 //     this stage reads a few per cent of Y instead of all of it.  A persistent grid of
-//     warps scans the map (128 blocks per warp step) and each warp walks its flagged blocks
+//     warps scans the map (32 blocks per warp step) and each warp walks its flagged blocks
 //     with 128-bit loads, neighbours coming from the adjacent lanes.
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -105,21 +105,17 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
     const long long warp = (static_cast<long long>(blockIdx.x) * kCandThreads + threadIdx.x) >> 5;
     const long long n_warps = (static_cast<long long>(gridDim.x) * kCandThreads) >> 5;
     const float ninf = __int_as_float(0xff800000);
-    // the map is padded to a multiple of 128 bytes, so 32-bit loads are in bounds
-    const uint32_t* __restrict__ act32 = reinterpret_cast<const uint32_t*>(activity);
-    const long long n_steps = (n_flags + 127) / 128;
+    // 32 flags per warp step (one per lane): marked blocks spread over as many warps as possible
+    const long long n_steps = (n_flags + 31) / 32;
     for (long long step = warp; step < n_steps; step += n_warps) {
-        const uint32_t f4 = __ldg(act32 + step * 32 + lane);
-        unsigned pending = __ballot_sync(0xffffffffu, f4 != 0u);
+        const long long mine = step * 32 + lane;
+        const unsigned flag = mine < n_flags ? __ldg(activity + mine) : 0u;
+        unsigned pending = __ballot_sync(0xffffffffu, flag != 0u);
         while (pending) {
             const int src = __ffs(pending) - 1;
             pending &= pending - 1;
-            uint32_t word = __shfl_sync(0xffffffffu, f4, src);
-            while (word) {
-                const int byte = (__ffs(word) - 1) >> 3;
-                word &= ~(0xffu << (8 * byte));
-                const long long fi = step * 128 + src * 4 + byte;
-                if (fi >= n_flags) continue;
+            {
+                const long long fi = step * 32 + src;
                 const long long d = fi / flags_per_row;
                 const long long b = fi - d * flags_per_row;
                 const float* __restrict__ y = snr + d * n_t;
@@ -195,10 +191,12 @@ int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* ou
                    float threshold, spd_candidate* list, int64_t capacity, int64_t* n_found, cudaStream_t stream) {
     cudaError_t e = cudaMemsetAsync(n_found, 0, sizeof(int64_t), stream);
     if (e != cudaSuccess) return cuda_fail(e, "clearing the candidate counter");
-    if (activity && plan->n_t % 4 == 0) {
+    // the any-width-set path marks everything: visiting every sample with the dense kernel is
+    // the same work with more parallelism
+    if (activity && is_tree_path(plan)) {
         const long long per_row = activity_per_row(plan);
         const long long n_flags = plan->n_dm * per_row;
-        const long long steps = (n_flags + 127) / 128;
+        const long long steps = (n_flags + 31) / 32;
         const long long warps_per_block = kCandThreads / 32;
         long long blocks = (steps + warps_per_block - 1) / warps_per_block;
         blocks = std::max<long long>(1, std::min<long long>(blocks, static_cast<long long>(plan->sm_count) * 16));

@@ -545,6 +545,33 @@ def test_row_stats_argument_checks(spd):
             plan.row_stats(plane, 2.0, -1)
 
 
+@pytest.mark.parametrize("kind,param,max_width", [("POW2", 0, 8192), ("IGRID", 1, 8192), ("POW2", 0, 32768)])
+def test_repeated_runs_are_bit_identical(spd, kind, param, max_width):
+    """Race check by repetition (compute-sanitizer is not available on this pool): the kernels have
+    no atomics on the data path, so every run of the same plan on the same input must give the same
+    bits - a shared-memory or halo race would show up as a difference between runs."""
+    rng = np.random.default_rng(41)
+    n_dm, n_t = 24, 1 << 19
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(rng.standard_normal((n_dm, n_t), dtype=np.float32)).to(dev)
+    mean = torch.from_numpy((0.1 * rng.standard_normal(n_dm)).astype(np.float32)).to(dev)
+    sigma = torch.from_numpy((1.0 + rng.random(n_dm)).astype(np.float32)).to(dev)
+    widths = spd.spd_width_set_generate(kind, param, max_width)
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        ref = plan.run_flagged(plane, mean, sigma, 4.0)
+        ref = [t.clone() for t in ref]
+        streams = [torch.cuda.Stream() for _ in range(2)]
+        torch.cuda.synchronize()
+        for i in range(8):
+            st = streams[i % 2]
+            with torch.cuda.stream(st):
+                act = torch.empty_like(ref[2])
+                got = plan.run_flagged(plane, mean, sigma, 4.0, activity=act, stream=st)
+            st.synchronize()
+            for a, b in zip(ref, got):
+                assert torch.equal(a, b), f"run {i} differs"
+
+
 def test_run_host_equals_device_run(spd):
     """The end-to-end host entry point (several row blocks) returns exactly what spd_run does."""
     rng = np.random.default_rng(11)
