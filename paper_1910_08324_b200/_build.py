@@ -48,16 +48,33 @@ def nvcc_path() -> str:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every CUDA source for sm_100a into ``libspd_b200.so``; returns its path."""
+    """Compile every CUDA source for sm_100a into ``libspd_b200.so``; returns its path.
+    The translation units are compiled in parallel (one nvcc per file), then linked."""
     if os.environ.get("SPD_B200_LIB"):
         return LIB_PATH  # an explicitly chosen build is used as it is
     if force or needs_build():
-        cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-            ["-o", LIB_PATH + ".tmp"] + sources()
-        res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed:\n" + res.stdout[-4000:] + res.stderr[-8000:])
+        from concurrent.futures import ThreadPoolExecutor
+        nvcc = nvcc_path()
+        objdir = os.path.join(_HERE, "build")
+        os.makedirs(objdir, exist_ok=True)
+        compile_flags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else [])
+
+        def compile_one(src):
+            obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+            res = subprocess.run([nvcc] + compile_flags + ["-c", "-o", obj, src], cwd=CSRC,
+                                 capture_output=True, text=True)
+            if res.returncode != 0:
+                raise RuntimeError(f"nvcc failed on {src}:\n" + res.stdout[-4000:] + res.stderr[-8000:])
+            return obj, res.stderr
+
+        with ThreadPoolExecutor(max_workers=min(8, len(sources()))) as pool:
+            done = list(pool.map(compile_one, sources()))
         if verbose:
-            print(res.stderr)
+            print("".join(err for _, err in done))
+        link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB_PATH + ".tmp"] + \
+            [obj for obj, _ in done]
+        res = subprocess.run(link, cwd=CSRC, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc link failed:\n" + res.stdout[-4000:] + res.stderr[-8000:])
         os.replace(LIB_PATH + ".tmp", LIB_PATH)
     return LIB_PATH
