@@ -28,7 +28,7 @@
 //   * Delay lines deeper than one chunk are register FIFOs; the chunk loop is unrolled
 //     over the FIFO depth so that the FIFO slot is a compile-time constant (no moves).
 //   * Chunks are staged into shared memory by cp.async.bulk (TMA, 1-D) through a
-//     3-deep mbarrier ring; results leave as 128-bit streaming stores.
+//     3-deep mbarrier ring; results leave as 128-bit stores.
 //   * SNR scale 2^(-k/2) is a compile-time constant (1/sigma is applied once per output
 //     sample at the store); the width index rides in the 5 low mantissa bits of the SNR
 //     being maximised (relative perturbation <= 2^-18, inside the 1e-4 tolerance), stored
@@ -50,6 +50,8 @@ namespace spd {
 namespace {
 
 // Exchange levels k = 3 .. LT+1: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner in another thread.
+// hoff: halo slots used by the levels below (d4 slots each: the row-0 values that the next
+// chunk's last row wraps into).
 template <int T, int R, int K, bool FAST, int k, int hoff>
 __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
                                                 float4* __restrict__ pp, float4* __restrict__ hr,
@@ -57,43 +59,23 @@ __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R
     using G = Geo<T, R, K>;
     if constexpr (k <= G::LT + 1 && k + 1 <= G::LAST) {
         constexpr int d4 = (1 << k) / 4;  // partner distance in float4
-        // Optional (off: slower, the loads bind, not the barriers) - two levels per barrier: with P_k stored once, P_{k+1}[n] = P_k[n] + P_k[n+d] and
-        // P_{k+2}[n] = P_{k+1}[n] + (P_k[n+2d] + P_k[n+3d]) - the same shared-memory bytes as
-        // two single exchanges, one add more, one barrier fewer.
-        constexpr bool PAIR = SPD_TREE_RADIX4 && k + 1 <= G::LT + 1 && k + 2 <= G::LAST;
-        constexpr int nh = PAIR ? 3 * d4 : d4;  // row-0 slots the next chunk's last row wraps into
-        static_assert(hoff + nh <= T, "halo buffer overflow");
+        static_assert(hoff + d4 <= T, "halo buffer overflow");
         const int tid = cx.tid;
         float4* const buf = pp + xsel * G::C4;
         xsel ^= 1;
 #pragma unroll
-        for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
-        if (tid < nh) hw[hoff + tid] = P[0];
-        // the previous chunk's bulk stores must have read the staging buffer before any
-        // thread passes this barrier on its way to refilling it
-        if constexpr (FAST && G::TMA_STORE && k == 3) {
-            if (tid == 0) bulk_wait_read0();
-        }
+        for (int r = 0; r < R; ++r) st_shared4(buf + tid + T * r, P[r]);
+        if (tid < d4) hw[hoff + tid] = P[0];
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            // partner m*d4 slots later: in this chunk, or (last row only) in the halo
-            auto partner = [&](int m) -> float4 {
-                const float4* src = buf + (tid + T * r + m * d4);
-                if (r == R - 1 && tid + m * d4 >= T) src = hr + (hoff + tid + m * d4 - T);
-                return *src;
-            };
-            const float4 p1 = add4(P[r], partner(1));
-            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], p1, lim[r], cx.tm);
-            if constexpr (PAIR) {
-                const float4 p2 = add4(p1, add4(partner(2), partner(3)));
-                if (FAST || cx.do_out) fold<k + 2, K, FAST>(best[r], p1, p2, lim[r], cx.tm);
-                P[r] = p2;
-            } else {
-                P[r] = p1;
-            }
+            const float4* src = buf + (tid + T * r + d4);
+            if (r == R - 1 && tid + d4 >= T) src = hr + (hoff + tid + d4 - T);
+            const float4 now = add4(P[r], *src);
+            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], now, lim[r], cx.tm);
+            P[r] = now;
         }
-        exchange_levels<T, R, K, FAST, k + (PAIR ? 2 : 1), hoff + nh>(P, best, lim, pp, hr, hw, xsel, cx);
+        exchange_levels<T, R, K, FAST, k + 1, hoff + d4>(P, best, lim, pp, hr, hw, xsel, cx);
     }
 }
 
@@ -229,24 +211,10 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
                                          static_cast<int>(~__float_as_uint(kq.y) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.z) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
-                if constexpr (FAST && G::TMA_STORE) {
-                    cx.sout[tid + T * r] = y;
-                    reinterpret_cast<int4*>(cx.sout + G::C4)[tid + T * r] = w;
-                } else {
-                    const long long o = cx.n0 + 4ll * (tid + T * r);
-                    *reinterpret_cast<float4*>(cx.out_snr + o) = y;
-                    *reinterpret_cast<int4*>(cx.out_width + o) = w;
-                }
+                const long long o = cx.n0 + 4ll * (tid + T * r);
+                *reinterpret_cast<float4*>(cx.out_snr + o) = y;
+                *reinterpret_cast<int4*>(cx.out_width + o) = w;
             }
-        }
-    }
-    if constexpr (FAST && G::TMA_STORE) {
-        fence_proxy_async();
-        __syncthreads();
-        if (tid == 0) {
-            bulk_s2g(cx.out_snr + cx.n0, cx.sout, G::C * 4);
-            bulk_s2g(cx.out_width + cx.n0, cx.sout + G::C4, G::C * 4);
-            bulk_commit();
         }
     }
     // With no exchange level there is no barrier inside the step: add the one that
@@ -277,7 +245,7 @@ constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 
 template <int T, int R, int K>
 constexpr size_t tree_smem_bytes() {
     constexpr size_t C = 4 * T * R;
-    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + (Geo<T, R, K>::TMA_STORE ? 2 * C * 4 : 0) + kStages * 8;
+    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8;
 }
 
 template <int T, int R, int K>
@@ -290,8 +258,7 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     float4* const pp = reinterpret_cast<float4*>(smem_raw);
     float* const stages = reinterpret_cast<float*>(smem_raw + 2 * C * 4);
     float4* const halo = reinterpret_cast<float4*>(stages + kStages * (C + 8));
-    float4* const sout = halo + 2 * T;
-    uint64_t* const bars = reinterpret_cast<uint64_t*>(sout + (G::TMA_STORE ? 2 * G::C4 : 0));
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(halo + 2 * T);
 
     const int tid = threadIdx.x;
     const int d = blockIdx.x / p.segs_per_row;
@@ -307,7 +274,6 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
 
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
     ChunkCtx cx;
-    cx.sout = sout;
     cx.mu = p.mean[d];
     const float sg = p.sigma[d];
     cx.inv = 1.0f / sg;
@@ -398,10 +364,6 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
                 ++it;
             }
         });
-    }
-    // the staging buffer must outlive the last bulk stores
-    if constexpr (G::TMA_STORE) {
-        if (tid == 0) bulk_wait0();
     }
 }
 

@@ -68,14 +68,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
         "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
-__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem),
-                 "r"(smem_u32(src_smem)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -169,30 +161,15 @@ __device__ __forceinline__ void fold(float4& best, float4 before, float4 now, in
     }
 }
 
-// Shared-memory store of a float4: as one 128-bit store, or as two 64-bit stores.  The sums
-// are produced by packed FADD2 into register PAIRS; a 128-bit store needs an aligned QUAD
-// and costs up to four register moves when the allocator cannot place the pairs together.
-#ifndef SPD_TREE_STS64
-#define SPD_TREE_STS64 1
-#endif
-template <int SPLIT>
+// Shared-memory store of a float4, issued as two 64-bit halves in PTX.  The sums are produced
+// by packed FADD2 into register PAIRS; written as one 128-bit store the allocator spends up to
+// four register moves per store on forming an aligned QUAD.  ptxas re-merges the halves into
+// one STS.128 but no longer needs the moves (7 -> 2 moves per sample).
 __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
-    if constexpr (SPLIT) {
-        // inline PTX: as plain C++ the two halves are merged back into one 128-bit store
-        const uint32_t a = smem_u32(dst);
-        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
-        asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(a), "f"(v.z), "f"(v.w) : "memory");
-    } else {
-        *dst = v;
-    }
+    const uint32_t a = smem_u32(dst);
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
+    asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(a), "f"(v.z), "f"(v.w) : "memory");
 }
-
-#ifndef SPD_TREE_RADIX4
-#define SPD_TREE_RADIX4 0  // two exchange levels per barrier; measured 11.99 ms vs 11.41 ms (config 3)
-#endif
-#ifndef SPD_TREE_TMA_STORE
-#define SPD_TREE_TMA_STORE 0  // measured: 11.87 ms vs 11.41 ms with direct 128-bit stores (config 3)
-#endif
 
 // The chunk loop is unrolled over the delay FIFOs up to this factor: a FIFO no deeper than
 // the unroll gets a compile-time slot (no register moves), a deeper one is rotated by moves.
@@ -217,17 +194,11 @@ struct Geo {
     static constexpr int J = imax(0, LAST - LT - 2);
     static constexpr int ND = (1 << J) - 1;  // float4 of delay registers: sum of 2^j
     // Depth, in chunks, of the deepest delay FIFO = unroll factor of the chunk loop.
-    // Optional: unguarded chunks leave through a shared-memory staging buffer and two bulk
-    // stores (Y, W) instead of 128-bit global stores.  Off by default: the extra barrier and
-    // shared-memory stores cost more than the global stores they replace (DESIGN.md "Tuning
-    // log").  Needs an exchange level (its barrier orders the reuse of the staging buffer).
-    static constexpr bool TMA_STORE = SPD_TREE_TMA_STORE && LAST >= 4;
     static constexpr int TOPQ = J > 0 ? imax(1, (1 << (J - 1)) / R) : 1;
     static constexpr int U = TOPQ < tree_max_unroll(K) ? TOPQ : tree_max_unroll(K);
 };
 
 struct ChunkCtx {
-    float4* sout;  // staging of one chunk's Y (C floats) then W (C ints)
     float mu, inv;
     uint32_t tm;
     float* __restrict__ out_snr;

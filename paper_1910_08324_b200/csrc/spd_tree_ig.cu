@@ -80,7 +80,7 @@ __device__ __forceinline__ void ig_exchange_levels(float4 (&P)[R], float4 (&Ppre
         float4* const buf = pp + xsel * G::C4;
         xsel ^= 1;
 #pragma unroll
-        for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
+        for (int r = 0; r < R; ++r) st_shared4(buf + tid + T * r, P[r]);
         if (tid < d4) hw[hoff + tid] = P[0];
         __syncthreads();
 #pragma unroll
@@ -105,7 +105,7 @@ __device__ __forceinline__ void ig_exchange_levels(float4 (&P)[R], float4 (&Ppre
         float4* const buf = pp + xsel * G::C4;
         xsel ^= 1;
 #pragma unroll
-        for (int r = 0; r < R; ++r) st_shared4<SPD_TREE_STS64>(buf + tid + T * r, P[r]);
+        for (int r = 0; r < R; ++r) st_shared4(buf + tid + T * r, P[r]);
         if (tid < h4) hw[hoff + tid] = P[0];
         __syncthreads();
 #pragma unroll
@@ -326,7 +326,6 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(con
 
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
     ChunkCtx cx;
-    cx.sout = nullptr;
     cx.mu = p.mean[d];
     const float sg = p.sigma[d];
     cx.inv = 1.0f / sg;
