@@ -187,3 +187,56 @@ def test_full_size_config(spd, oracle_lib, cfg, width_kind):
             m = (cands["dm"] == p.dm) & (np.abs(cands["t"].astype(np.int64) - p.t0) <= 2 * p.width + 4)
             hit += bool(m.any())
         assert hit >= 0.95 * len(strong), f"config {cfg}: only {hit} of {len(strong)} strong pulses detected"
+
+
+@pytest.mark.parametrize("kind,param", [("POW2", 0), ("IGRID", 1)])
+def test_longest_row(spd, oracle_lib, kind, param):
+    """Maximum row length of the C ABI (n_t <= 2^31 - 1): one DM trial of 2^31 - 4 samples (8.6 GB),
+    widths up to 8192.  Windows at the row start, across the 2^30 and 2^31 - 2^28 marks, at segment
+    boundaries and at the very end are compared with the oracle; the whole row is checked for
+    Y >= SNR of width 1 and index range."""
+    dev = torch.device("cuda:0")
+    n_t = (1 << 31) - 4
+    free, _ = torch.cuda.mem_get_info(dev)
+    if free < 13 * n_t + (8 << 30):
+        pytest.skip("not enough device memory")
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(20260101)
+    plane = torch.empty((1, n_t), dtype=torch.float32, device=dev)
+    plane.normal_(generator=gen)
+    for t0, S in ((5, 3000), ((1 << 30) - 1500, 3000), (n_t - 40000, 6000), (n_t - 2500, 2500)):
+        plane[0, t0:t0 + S] += 12.0 / float(np.sqrt(S))
+    mean = torch.zeros(1, device=dev)
+    sigma = torch.ones(1, device=dev)
+    widths = spd.spd_width_set_generate(kind, param, 8192)
+    with spd.Plan(1, n_t, widths, 8192) as plan:
+        info = dict(plan.info)
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 6.0)
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, 6.0, 1 << 20)
+        torch.cuda.synchronize()
+        count, cands = spd.candidates_to_numpy(lst, n_found, 1 << 20)
+    mean_h, sigma_h = np.zeros(1), np.ones(1)
+    chunk, segs = info["chunk"], info["segments_per_row"]
+    chunks_per_row = (n_t + chunk - 1) // chunk
+    seg_chunks = (chunks_per_row + segs - 1) // segs
+    starts = [0, (1 << 30) - 2000, (1 << 31) - (1 << 28) - 700, n_t - 8192 - 1000, n_t - 1536]
+    starts += [s * seg_chunks * chunk - 700 for s in range(1, segs)][:3]
+    worst = 0.0
+    for t0 in starts:
+        st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, 8192, 0, t0, 1536, direct=True,
+                           what=f"longest row {kind}")
+        worst = max(worst, st.max_err_over_tol)
+    st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, 8192, 0, n_t - (1 << 18), 1 << 18,
+                       direct=False, what=f"longest row {kind} tail")
+    assert max(worst, st.max_err_over_tol) <= 1.0
+    # whole row, in pieces
+    piece = 1 << 28
+    for a in range(0, n_t, piece):
+        b = min(n_t, a + piece)
+        y, k = snr[0, a:b], idx[0, a:b]
+        assert bool(torch.isfinite(y).all()) and int(k.min()) >= 0 and int(k.max()) < len(widths)
+        assert bool((y >= plane[0, a:b] - 1e-4 * torch.clamp(plane[0, a:b].abs(), min=1.0)).all())
+    # the four injected pulses are in the candidate list
+    for t0 in (5, (1 << 30) - 1500, n_t - 40000, n_t - 2500):
+        assert bool(((cands["t"].astype(np.int64) - t0) ** 2 < 8192 ** 2).any()), t0
+    assert count == len(cands) or count > (1 << 20)
