@@ -572,14 +572,16 @@ def test_repeated_runs_are_bit_identical(spd, kind, param, max_width):
                 assert torch.equal(a, b), f"run {i} differs"
 
 
-def test_run_host_equals_device_run(spd):
-    """The end-to-end host entry point (several row blocks) returns exactly what spd_run does."""
+@pytest.mark.parametrize("kind,param,n_t", [("POW2", 0, 1 << 20), ("IGRID", 1, 1 << 20), ("IGRID", 2, (1 << 18) + 3)])
+def test_run_host_equals_device_run(spd, kind, param, n_t):
+    """The end-to-end host entry point (several row blocks) returns exactly what spd_run does
+    (both streaming trees and the any-width-set tile kernel)."""
     rng = np.random.default_rng(11)
-    n_dm, n_t = 6, 1 << 20
+    n_dm = 6
     x = rng.standard_normal((n_dm, n_t), dtype=np.float32)
     mu = rng.standard_normal(n_dm).astype(np.float32) * 0.01
     sg = (1.0 + 0.1 * rng.random(n_dm)).astype(np.float32)
-    widths = [1 << k for k in range(14)]
+    widths = spd.spd_width_set_generate(kind, param, 8192 if kind != "IGRID" or param == 1 else 512)
     got_snr, got_idx, _ = run_gpu(spd, x, mu, sg, widths)
     out_snr = np.empty((n_dm, n_t), dtype=np.float32)
     out_idx = np.empty((n_dm, n_t), dtype=np.int32)
