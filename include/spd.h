@@ -32,6 +32,12 @@
  * message for the calling thread's last error is in spd_last_error_string().
  * There is NO CPU fallback: on a machine without an sm_100 device every
  * compute entry point fails with SPD_ERR_UNSUPPORTED_DEVICE.
+ *
+ * Environment variables read at plan creation (test hooks, not tuning knobs):
+ *   SPD_SEGS_PER_ROW=n      streaming trees: n independent streams per DM row instead of the
+ *                           automatic choice (exercises the look-ahead replay of interior segments);
+ *   SPD_GENERIC_WORKSPACE=1 any-width-set path: use the device-workspace kernels even where the
+ *                           shared-memory tile kernel applies.
  */
 #ifndef SPD_B200_SPD_H_
 #define SPD_B200_SPD_H_
