@@ -148,6 +148,28 @@ def test_igrid_tree_flagged_candidates(spd, oracle_lib):
         assert np.array_equal(got["dm"], c_dm) and np.array_equal(got["t"], c_t)
 
 
+@pytest.mark.parametrize("seed", list(range(10)))
+def test_random_shapes_and_statistics(spd, oracle_lib, seed, monkeypatch):
+    """Seeded fuzz over plane shapes, depths, segmentation, width-set family and statistics: row lengths
+    that are not multiples of the chunk, rows shorter than a chunk or barely longer than max_width."""
+    rng = np.random.default_rng(9000 + seed)
+    family = ["POW2", "IGRID"][seed % 2]
+    K = int(rng.integers(5, 15))
+    M = 1 << (K - 1)
+    n_dm = int(rng.integers(1, 6))
+    n_t = 4 * int(rng.integers((M + 3) // 4, (M + 3) // 4 + 6000))
+    x = (rng.standard_normal((n_dm, n_t)) * rng.uniform(0.5, 4.0) + rng.uniform(-30, 30)).astype(np.float32)
+    for _ in range(3):
+        S = int(rng.integers(1, M + 1))
+        t0 = int(rng.integers(0, n_t - 1))
+        x[int(rng.integers(0, n_dm)), t0:t0 + S] += np.float32(rng.uniform(5, 15) / np.sqrt(S) * x.std())
+    mu, sg = oracle_lib.row_stats(x)
+    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(int(rng.integers(1, 5))))
+    widths = spd.spd_width_set_generate(family, 1 if family == "IGRID" else 0, M)
+    check(spd, oracle_lib, x, mu, sg, widths, f"fuzz seed={seed} {family} K={K} {n_dm}x{n_t}",
+          expect_path=spd.SPD_PATH_IGRID_TREE if family == "IGRID" else spd.SPD_PATH_DYADIC_TREE)
+
+
 @pytest.mark.parametrize("segs", [1, 2, 7])
 def test_dyadic_tree_segmentation_is_invisible(spd, oracle_lib, segs, monkeypatch):
     rng = np.random.default_rng(77)
