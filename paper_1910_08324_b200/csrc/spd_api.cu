@@ -314,7 +314,8 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
     if (is_tree_path(plan)) {
         info->launches_per_run = 1;
         info->threads_per_block = plan->tree.T;
-        info->blocks = static_cast<int32_t>(plan->n_dm * plan->tree.segs_per_row);
+        info->blocks = plan->tree.kind == 1 ? ws_grid_blocks(plan)
+                                            : static_cast<int32_t>(plan->n_dm * plan->tree.segs_per_row);
         info->chunk = plan->tree.chunk;
         info->segments_per_row = plan->tree.segs_per_row;
         info->smem_bytes = static_cast<int64_t>(plan->tree.smem_bytes);

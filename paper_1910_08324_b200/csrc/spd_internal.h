@@ -19,6 +19,7 @@ constexpr int kStages = 3;          // bulk-copy ring depth
 
 struct TreeConfig {
     int K = 0;            // number of widths: 2^0 .. 2^(K-1)
+    int kind = 0;         // 0: block per stream (spd_tree.cu), 1: warp per stream (spd_tree_ws.cu)
     int T = 0;            // threads per block
     int chunk = 0;        // 4 * T * R samples
     int warm_chunks = 0;  // look-ahead chunks an interior segment replays
@@ -84,6 +85,13 @@ int tree_configure_segments(spd_plan* plan);
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
              const float* sigma, float* out_snr, int32_t* out_width, float threshold,
              uint8_t* activity, cudaStream_t stream);
+
+// spd_tree_ws.cu: the dyadic tree with one warp per stream (tensor-memory delay lines)
+bool ws_applicable(int K);
+int ws_configure(spd_plan* plan);
+int ws_grid_blocks(const spd_plan* plan);
+int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream);
 
 // spd_tree_ig.cu: widths 2^k and 3 * 2^m (IGRID depth 1)
 int ig_applicable(const std::vector<int32_t>& widths, int64_t n_t);  // K (pow-2 levels) or 0

@@ -419,6 +419,8 @@ bool tree_applicable(const std::vector<int32_t>& widths, int64_t n_t) {
 int tree_configure(spd_plan* plan) {
     TreeConfig& cfg = plan->tree;
     cfg.K = static_cast<int>(plan->widths.size());
+    if (ws_applicable(cfg.K)) return ws_configure(plan);
+    cfg.kind = 0;
     cfg.T = tree_threads_for(cfg.K);
     cfg.chunk = 4 * cfg.T * tree_rows_for(cfg.K);
     cudaError_t e = cudaErrorInvalidValue;
@@ -466,6 +468,7 @@ int tree_configure_segments(spd_plan* plan) {
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
              float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
     const TreeConfig& cfg = plan->tree;
+    if (cfg.kind == 1) return ws_run(plan, n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     TreeParams prm;
     prm.plane = plane;
     prm.mean = mean;
@@ -475,6 +478,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     prm.activity = activity;
     prm.threshold = threshold;
     prm.n_t = plan->n_t;
+    prm.n_dm = n_dm;
     prm.chunks_per_row = cfg.chunks_per_row;
     prm.seg_chunks = cfg.seg_chunks;
     prm.segs_per_row = cfg.segs_per_row;

@@ -22,6 +22,7 @@ struct TreeParams {
     uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr
     float threshold;    // candidate threshold in SNR units (used only with activity)
     long long n_t;
+    long long n_dm;  // rows of this launch (warp-stream kernel: pieces may span rows)
     int chunks_per_row;
     int seg_chunks;
     int segs_per_row;

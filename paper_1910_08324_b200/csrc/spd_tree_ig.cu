@@ -476,6 +476,7 @@ int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     prm.activity = activity;
     prm.threshold = threshold;
     prm.n_t = plan->n_t;
+    prm.n_dm = n_dm;
     prm.chunks_per_row = cfg.chunks_per_row;
     prm.seg_chunks = cfg.seg_chunks;
     prm.segs_per_row = cfg.segs_per_row;

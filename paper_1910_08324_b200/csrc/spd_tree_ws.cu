@@ -1,0 +1,653 @@
+// Dyadic partial-sum tree, one WARP per stream, for
+// 8 <= K <= 14 widths {1, 2, ..., 2^(K-1)}.
+//
+// Same arithmetic as spd_tree.cu (eq. 2, 4, 5, 12 and the reuse of eq. 15/16:
+// P_{k+1}[n] = P_k[n] + P_k[n + 2^k]), different
+// decomposition.  In spd_tree.cu a block of 4 warps shares one stream, so every level whose
+// partner lies in another thread costs a shared-memory store, a block barrier and a load.
+// Here every warp streams its own segment of a DM row in reverse time and nothing is shared
+// between warps: no block barrier and no shared-memory exchange at all.
+//
+//   * A step is R = 8 "rows" of 128 samples; lane l owns the float4 4l..4l+3 of every row.
+//   * Widths 2, 4, 8: in the lane's registers from three raw float4 (as spd_tree.cu).
+//   * Partner 8, 16, 32, 64 samples later = 2, 4, 8, 16 lanes later: warp shuffles; the lanes
+//     that run off the row take the shuffled value of the NEXT row (same lane set, one row
+//     later), the last row takes it from the previous step's first row (4 float4 kept).
+//   * Partner 128 * 2^j samples later = the same lane, 2^j rows later: a register of this step
+//     (j < 3), of the previous step (7 float4 kept), or - 1, 2, 4 steps back - a FIFO.
+//   * The FIFOs (7 x 8 float4 per lane for K = 14: the 28 KB of delay state that forces
+//     spd_tree.cu to spread a stream over 128 threads) live in TENSOR MEMORY: each warp owns
+//     32 lanes x 224 columns, written with tcgen05.st and read with tcgen05.ld (32x32b.x32:
+//     one instruction moves the 8 float4 of a level), slot = step mod depth as a run-time
+//     column offset - no unrolling over FIFO phases, no register rotation.  TMEM is used as
+//     plain per-lane scratch; there is no MMA anywhere (streaming reduction, not a contraction).
+//   * Raw samples arrive by 1-D cp.async.bulk through a 3-stage mbarrier ring PER WARP.
+//   * SNR scale, width tag, 3-input max, threshold flag, guarded tail steps: as spd_tree.cu.
+//
+// One block of 8 warps per SM (2 warps per lane quarter of TMEM, 2 x 224 <= 512 columns).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <algorithm>
+#include <cstdlib>
+
+#include "spd_tree_common.cuh"
+
+namespace spd {
+namespace {
+
+constexpr int kWsWarps = 8;                 // streams per block
+#ifndef SPD_WS_ROWS
+#define SPD_WS_ROWS 4
+#endif
+constexpr int kWsRows = SPD_WS_ROWS;        // rows of 128 samples per step (4 or 8)
+static_assert(kWsRows == 4 || kWsRows == 8, "rows per step");
+constexpr int kWsStep = 128 * kWsRows;      // samples per step
+constexpr int kWsStage = kWsStep + 8;       // floats per stage: the step + two float4 of look-ahead
+constexpr int kWsMinK = 8, kWsMaxK = 14;
+#ifndef SPD_WS_STAGES
+#define SPD_WS_STAGES 4
+#endif
+constexpr int kWsStages = SPD_WS_STAGES;    // bulk-copy ring depth per warp
+
+template <int K>
+struct WsGeo {
+    static constexpr int LAST = K - 1;
+    // row levels j = 0 .. J-1: partner 2^j rows later, level 7+j -> level 8+j
+    static constexpr int J = imax(0, LAST - 7);
+    // partner inside this or the previous step (2^j <= kNearMax rows): registers
+    static constexpr int JNMAX = kWsRows == 8 ? 3 : 3;  // R = 8: 1, 2, 4 rows; R = 4: 1, 2, 4 (= one step)
+    static constexpr int JN = J < JNMAX ? J : JNMAX;
+    static constexpr int NEAR = (1 << JN) - 1;  // float4 kept from the previous step
+    static constexpr int JF = J - JN;           // FIFO levels i < JF: partner Q0 * 2^i steps back
+    static constexpr int Q0 = (1 << JNMAX) / kWsRows;  // steps back of the first FIFO level
+    static constexpr int COLS = 4 * kWsRows * Q0 * ((1 << JF) - 1);  // TMEM columns per warp
+};
+
+// ---- tensor memory as per-lane scratch ---------------------------------------------------
+__device__ __forceinline__ void tmem_alloc512(uint32_t* slot) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(slot))
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc512(uint32_t base) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// 8 float4 per lane <- 32 consecutive columns of the warp's lanes; complete on return.
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float4 (&v)[8]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        v[i] = make_float4(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1]), __uint_as_float(r[4 * i + 2]),
+                           __uint_as_float(r[4 * i + 3]));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float4 (&v)[8]) {
+    uint32_t r[32];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        r[4 * i] = __float_as_uint(v[i].x);
+        r[4 * i + 1] = __float_as_uint(v[i].y);
+        r[4 * i + 2] = __float_as_uint(v[i].z);
+        r[4 * i + 3] = __float_as_uint(v[i].w);
+    }
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float4 (&v)[4]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+        v[i] = make_float4(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1]), __uint_as_float(r[4 * i + 2]),
+                           __uint_as_float(r[4 * i + 3]));
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const float4 (&v)[4]) {
+    uint32_t r[16];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        r[4 * i] = __float_as_uint(v[i].x);
+        r[4 * i + 1] = __float_as_uint(v[i].y);
+        r[4 * i + 2] = __float_as_uint(v[i].z);
+        r[4 * i + 3] = __float_as_uint(v[i].w);
+    }
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+// One level's rows of a step (kWsRows float4 per lane) <-> 4 * kWsRows columns.
+__device__ __forceinline__ void tmem_ld_rows(uint32_t taddr, float4 (&v)[kWsRows]) {
+    if constexpr (kWsRows == 8) {
+        tmem_ld32(taddr, reinterpret_cast<float4(&)[8]>(v));
+    } else {
+        tmem_ld16(taddr, reinterpret_cast<float4(&)[4]>(v));
+    }
+}
+__device__ __forceinline__ void tmem_st_rows(uint32_t taddr, const float4 (&v)[kWsRows]) {
+    if constexpr (kWsRows == 8) {
+        tmem_st32(taddr, reinterpret_cast<const float4(&)[8]>(v));
+    } else {
+        tmem_st16(taddr, reinterpret_cast<const float4(&)[4]>(v));
+    }
+}
+
+__device__ __forceinline__ float4 shfl4(float4 v, int src) {
+    return make_float4(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src),
+                       __shfl_sync(0xffffffffu, v.z, src), __shfl_sync(0xffffffffu, v.w, src));
+}
+
+// Lane levels k = 3 .. 6: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner 2^k / 4 lanes later; the
+// lanes that run off a row continue in the next row, the last row in the first row of the
+// previous (later-in-time) step, kept in hs[k - 3].
+// SPD_WS_XCHG = 1: through a warp-private shared-memory buffer (one 128-bit store and load per
+// float4 and level, ordered by __syncwarp: two instructions where shuffles take eight; the
+// L1 data pipe has the room, the issue slots do not).  Two buffers alternate between levels.
+// SPD_WS_XCHG = 0: warp shuffles of a per-lane pre-selected source row.
+#ifndef SPD_WS_XCHG
+#define SPD_WS_XCHG 1
+#endif
+constexpr int kWsXBuf = (kWsRows + 1) * 32;  // float4 per exchange buffer: R rows + the kept row
+
+// Step modes: 0 = guarded (row tail: windows checked against the end of the row, output if
+// cx.do_out), 1 = interior step with output, 2 = interior look-ahead step (sums only).
+template <int MODE>
+__device__ __forceinline__ bool wants_out(const ChunkCtx& cx) {
+    if constexpr (MODE == 1) {
+        return true;
+    } else if constexpr (MODE == 2) {
+        return false;
+    } else {
+        return cx.do_out;
+    }
+}
+
+template <int K, int MODE, int k>
+__device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
+                                            const int (&lim)[kWsRows], float4 (&hs)[4], float4* __restrict__ xb,
+                                            int lane, const ChunkCtx& cx) {
+    constexpr int R = kWsRows;
+    if constexpr (k <= 6 && k + 1 <= WsGeo<K>::LAST) {
+        constexpr int d4 = (1 << k) / 4;
+        float4 partner[R];
+#if SPD_WS_XCHG
+        float4* const buf = xb + (k & 1) * kWsXBuf + lane;
+#pragma unroll
+        for (int r = 0; r < R; ++r) st_shared4(buf + 32 * r, P[r]);
+        st_shared4(buf + 32 * R, hs[k - 3]);
+        __syncwarp();
+#pragma unroll
+        for (int r = 0; r < R; ++r) partner[r] = buf[32 * r + d4];
+#else
+        const int src = (lane + d4) & 31;
+        const bool low = lane < d4;  // this lane's value is wanted by a lane of the row before
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 nxt = r + 1 < R ? P[r + 1] : hs[k - 3];
+            const float4 w = make_float4(low ? nxt.x : P[r].x, low ? nxt.y : P[r].y, low ? nxt.z : P[r].z,
+                                         low ? nxt.w : P[r].w);
+            partner[r] = shfl4(w, src);
+        }
+#endif
+        hs[k - 3] = P[0];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 now = add4(P[r], partner[r]);
+            if (wants_out<MODE>(cx)) fold<k + 1, K, (MODE != 0)>(best[r], P[r], now, lim[r], cx.tm);
+            P[r] = now;
+        }
+        lane_levels<K, MODE, k + 1>(P, best, lim, hs, xb, lane, cx);
+    }
+}
+
+// Row levels j < JN: partner 2^j rows later, in this step or among the first rows of the
+// previous step (nr[2^j - 1 .. 2^(j+1) - 2]).
+template <int K, int MODE, int j>
+__device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
+                                            const int (&lim)[kWsRows], float4 (&nr)[WsGeo<K>::NEAR + 1],
+                                            const ChunkCtx& cx) {
+    constexpr int R = kWsRows;
+    if constexpr (j < WsGeo<K>::JN) {
+        constexpr int D = 1 << j;
+        constexpr int off = D - 1;
+        constexpr int lvl = 8 + j;  // level produced
+        float4 now[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) now[r] = add4(P[r], r + D < R ? P[r + D] : nr[off + r + D - R]);
+#pragma unroll
+        for (int i = 0; i < D; ++i) nr[off + i] = P[i];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (wants_out<MODE>(cx)) fold<lvl, K, (MODE != 0)>(best[r], P[r], now[r], lim[r], cx.tm);
+            P[r] = now[r];
+        }
+        near_levels<K, MODE, j + 1>(P, best, lim, nr, cx);
+    }
+}
+
+// FIFO levels i < JF: partner 2^i steps back, same lane, same row: tensor memory.
+template <int K, int MODE, int i>
+__device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
+                                            const int (&lim)[kWsRows], uint32_t tbase, int it,
+                                            const ChunkCtx& cx) {
+    constexpr int R = kWsRows;
+    if constexpr (i < WsGeo<K>::JF) {
+        constexpr int Q = WsGeo<K>::Q0 << i;     // FIFO depth in steps
+        constexpr int lvl = 8 + WsGeo<K>::JN + i;  // level produced
+        constexpr int first = WsGeo<K>::Q0 * ((1 << i) - 1);  // slots of the levels below
+        const uint32_t taddr = tbase + 4u * R * static_cast<uint32_t>(first + (it & (Q - 1)));
+        float4 old[R];
+        tmem_ld_rows(taddr, old);
+        tmem_st_rows(taddr, P);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 now = add4(P[r], old[r]);
+            if (wants_out<MODE>(cx)) fold<lvl, K, (MODE != 0)>(best[r], P[r], now, lim[r], cx.tm);
+            P[r] = now;
+        }
+        fifo_levels<K, MODE, i + 1>(P, best, lim, tbase, it, cx);
+    }
+}
+
+// One step of one warp: the kWsStage floats at st4 -> Y, W of its kWsStep samples.
+template <int K, int MODE>
+__device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 (&hs)[4],
+                                         float4 (&nr)[WsGeo<K>::NEAR + 1], float4* __restrict__ xb, uint32_t tbase,
+                                         int it, int lane, const ChunkCtx& cx) {
+    constexpr int R = kWsRows;
+    const float mu = cx.mu;
+    const uint32_t tm = cx.tm;
+    float4 P[R], best[R];
+    int lim[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if constexpr (MODE != 0) {
+            lim[r] = 1 << 30;
+        } else {
+            const long long left = cx.n_t - (cx.n0 + 4ll * (lane + 32 * r));
+            lim[r] = left > (1ll << 30) ? (1 << 30) : (left < 0 ? 0 : static_cast<int>(left));
+        }
+        // widths 1, 2, 4, 8 from three raw float4 (eq. 2 on mean-removed samples)
+        const float4 a = norm4(st4[lane + 32 * r], mu);
+        const float4 b = norm4(st4[lane + 32 * r + 1], mu);
+        const float4 c = norm4(st4[lane + 32 * r + 2], mu);
+        const float s01 = a.x + a.y, s12 = a.y + a.z, s23 = a.z + a.w, s34 = a.w + b.x;
+        const float s45 = b.x + b.y, s56 = b.y + b.z, s67 = b.z + b.w, s78 = b.w + c.x;
+        const float s89 = c.x + c.y, s9a = c.y + c.z;
+        const float4 p1 = make_float4(s01, s12, s23, s34);
+        const float4 p2 = make_float4(s01 + s23, s12 + s34, s23 + s45, s34 + s56);
+        const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
+                                      (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
+        if (wants_out<MODE>(cx)) {
+            best[r] = max4(keyx<0, (MODE != 0)>(a, lim[r], tm), keyx<1, (MODE != 0)>(p1, lim[r], tm), keyx<2, (MODE != 0)>(p2, lim[r], tm));
+            fold<3, K, (MODE != 0)>(best[r], p2, p3, lim[r], tm);
+        }
+        P[r] = p3;
+    }
+    lane_levels<K, MODE, 3>(P, best, lim, hs, xb, lane, cx);
+    near_levels<K, MODE, 0>(P, best, lim, nr, cx);
+    fifo_levels<K, MODE, 0>(P, best, lim, tbase, it, cx);
+    if constexpr (WsGeo<K>::JF > 0) tmem_wait_st();
+
+    float top = __int_as_float(0xff800000);
+    if (wants_out<MODE>(cx)) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (MODE != 0 || lim[r] > 0) {
+                const float4 kq = best[r];
+                top = fmax3(top, fmax3(kq.x, kq.y, kq.z), kq.w);
+                const float4 y = scale4(make_float4(__uint_as_float(__float_as_uint(kq.x) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.y) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.z) & tm),
+                                                    __uint_as_float(__float_as_uint(kq.w) & tm)),
+                                        cx.inv);
+                const int4 w = make_int4(static_cast<int>(~__float_as_uint(kq.x) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.y) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.z) & kCodeMask),
+                                         static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
+                const long long o = cx.n0 + 4ll * (lane + 32 * r);
+                *reinterpret_cast<float4*>(cx.out_snr + o) = y;
+                *reinterpret_cast<int4*>(cx.out_width + o) = w;
+            }
+        }
+    }
+    return top;
+}
+
+constexpr size_t kWsStagesBytes = static_cast<size_t>(kWsWarps) * kWsStages * kWsStage * 4;
+constexpr size_t kWsXBytes = SPD_WS_XCHG ? static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16 : 0;
+constexpr size_t ws_smem_bytes() { return kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8 + 16; }
+
+template <int K>
+__global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const TreeParams p, const int n_pieces) {
+    using G = WsGeo<K>;
+    constexpr int S = kWsStep;
+    constexpr int M = 1 << (K - 1);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float* const stages = reinterpret_cast<float*>(smem_raw) + warp * kWsStages * kWsStage;
+    float4* const xb = reinterpret_cast<float4*>(smem_raw + kWsStagesBytes) + warp * 2 * kWsXBuf;
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(smem_raw + kWsStagesBytes + kWsXBytes) + warp * kWsStages;
+    uint32_t* const tslot =
+        reinterpret_cast<uint32_t*>(smem_raw + kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8);
+
+    if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < kWsStages; ++i) mbar_init(&bars[i], 1);
+        fence_mbar_init();
+    }
+    uint32_t tbase = 0;
+    if constexpr (G::COLS > 0) {
+        if (warp == 0) tmem_alloc512(tslot);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        // this warp's lane quarter, and its half of the columns
+        tbase = *tslot + (static_cast<uint32_t>(warp & 3) << 21) + static_cast<uint32_t>(warp >> 2) * 256u;
+    } else {
+        __syncthreads();
+    }
+
+    const long long n_t = p.n_t;
+    // step c runs unguarded iff (c + 1) * S + max(M, 8) <= n_t
+    const int c_fast_end = n_t >= M ? static_cast<int>((n_t - M) / S) : 0;
+    ChunkCtx cx;
+    cx.tm = p.tag_mask;
+    cx.n_t = n_t;
+    cx.tid = lane;
+    int stage = 0;
+    uint32_t phase = 0;
+    constexpr uint32_t kBytes = kWsStage * 4;
+
+    // A piece is a run of p.seg_chunks steps.  segs_per_row > 0: pieces are the segments of the
+    // rows (piece = row * segs_per_row + segment).  segs_per_row == 0: pieces partition the
+    // plane's steps in row-major order and may span several rows; every row part inside a
+    // piece is one stream (only a part that stops short of its row's end replays look-ahead).
+    const long long cpr = p.chunks_per_row;
+    for (int piece = blockIdx.x * kWsWarps + warp; piece < n_pieces; piece += gridDim.x * kWsWarps) {
+        long long lin_lo, lin_hi;  // steps [lin_lo, lin_hi) of the plane, row-major
+        if (p.segs_per_row > 0) {
+            const int d0 = piece / p.segs_per_row;
+            const int s0 = piece - d0 * p.segs_per_row;
+            lin_lo = d0 * cpr + static_cast<long long>(s0) * p.seg_chunks;
+            lin_hi = min(lin_lo + p.seg_chunks, (d0 + 1) * cpr);
+        } else {
+            lin_lo = static_cast<long long>(piece) * p.seg_chunks;
+            lin_hi = min(lin_lo + p.seg_chunks, cpr * p.n_dm);
+        }
+      while (lin_hi > lin_lo) {
+        const int d = static_cast<int>((lin_hi - 1) / cpr);
+        const long long row_lo = d * cpr;
+        const int c_hi = static_cast<int>(lin_hi - row_lo);
+        const int c_lo = static_cast<int>(max(lin_lo, row_lo) - row_lo);
+        lin_hi = row_lo + c_lo;
+        const int c_top = min(c_hi + p.warm_chunks, p.chunks_per_row);
+        // steps [c_lo, ring_top) are interior: bulk-copy ring; those >= c_hi are look-ahead only
+        const int ring_top = max(c_lo, min(c_top, c_fast_end));
+
+        const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
+        cx.mu = p.mean[d];
+        const float sg = p.sigma[d];
+        cx.inv = 1.0f / sg;
+        cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
+        cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
+        uint8_t* const act = p.activity ? p.activity + static_cast<long long>(d) * p.chunks_per_row : nullptr;
+        float thr_key = __int_as_float(0x7f800000);
+        if (act) {
+            const float t = p.threshold * sg;
+            thr_key = t - fabsf(t) * 2e-6f;
+        }
+
+        float4 hs[4], nr[G::NEAR + 1];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) hs[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < G::NEAR + 1; ++i) nr[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if constexpr (G::COLS > 0) {
+            float4 zero[kWsRows];
+#pragma unroll
+            for (int i = 0; i < kWsRows; ++i) zero[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int col = 0; col < G::COLS; col += 4 * kWsRows) tmem_st_rows(tbase + col, zero);
+            tmem_wait_st();
+        }
+        int it = 0;
+
+        // ---- guarded steps: the row tail (windows may cross the end of the row) ------------
+        float* const gbuf = stages + stage * kWsStage;
+        for (int c = c_top - 1; c >= ring_top; --c, ++it) {
+            const long long n0 = static_cast<long long>(c) * S;
+            // n0 and n_t are multiples of 4: a float4 lies entirely inside or outside the row
+            const float4* const row4 = reinterpret_cast<const float4*>(row + n0);
+            const float4 fill = make_float4(cx.mu, cx.mu, cx.mu, cx.mu);
+#pragma unroll
+            for (int j = 0; j < (kWsStage / 4 + 31) / 32; ++j) {
+                const int i = lane + 32 * j;
+                if (i < kWsStage / 4)
+                    reinterpret_cast<float4*>(gbuf)[i] = n0 + 4ll * i < n_t ? __ldg(row4 + i) : fill;
+            }
+            __syncwarp();
+            cx.n0 = n0;
+            cx.do_out = c < c_hi;
+            const float top = ws_step<K, 0>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
+            if (act && cx.do_out && top >= thr_key) act[c] = 1;
+            __syncwarp();
+        }
+
+        // ---- interior steps: this warp's bulk-copy ring ------------------------------------
+        const int n_ring = ring_top - c_lo;
+        if (n_ring <= 0) continue;  // next row part of the piece
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+            int sx = stage;
+#pragma unroll
+            for (int j = 0; j < kWsStages - 1; ++j) {
+                if (j < n_ring) {
+                    mbar_arrive_expect_tx(&bars[sx], kBytes);
+                    bulk_g2s(stages + sx * kWsStage, row + static_cast<long long>(ring_top - 1 - j) * S, kBytes,
+                             &bars[sx]);
+                }
+                sx = sx + 1 == kWsStages ? 0 : sx + 1;
+            }
+        }
+        // refill the stage read one step ago with the step kWsStages - 1 ahead, wait for this one
+        auto ring_next = [&](int f) {
+            __syncwarp();  // every lane has finished reading the stage that is refilled now
+            if (lane == 0) {
+                const int nx = f + kWsStages - 1;
+                if (nx < n_ring) {
+                    const int sx = stage == 0 ? kWsStages - 1 : stage - 1;  // (stage + kWsStages - 1) % kWsStages
+                    mbar_arrive_expect_tx(&bars[sx], kBytes);
+                    bulk_g2s(stages + sx * kWsStage, row + static_cast<long long>(ring_top - 1 - nx) * S, kBytes,
+                             &bars[sx]);
+                }
+            }
+            mbar_wait(&bars[stage], phase);
+        };
+        auto ring_done = [&]() {
+            if (++stage == kWsStages) {
+                stage = 0;
+                phase ^= 1;
+            }
+        };
+        const int n_warm = max(0, ring_top - c_hi);  // look-ahead steps first: sums only
+        int f = 0;
+        for (; f < n_warm; ++f, ++it) {
+            ring_next(f);
+            cx.n0 = static_cast<long long>(ring_top - 1 - f) * S;
+            ws_step<K, 2>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
+            ring_done();
+        }
+        for (; f < n_ring; ++f, ++it) {
+            ring_next(f);
+            const int c = ring_top - 1 - f;
+            cx.n0 = static_cast<long long>(c) * S;
+            const float top = ws_step<K, 1>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
+                                            tbase, it, lane, cx);
+            if (act && top >= thr_key) act[c] = 1;
+            ring_done();
+        }
+      }
+    }
+
+    if constexpr (G::COLS > 0) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0) tmem_dealloc512(*tslot);
+    }
+}
+
+#define SPD_WS_CASES(OP) OP(8) OP(9) OP(10) OP(11) OP(12) OP(13) OP(14)
+
+}  // namespace
+
+// Warp-stream kernel for this plan?  Default: yes for kWsMinK <= K <= kWsMaxK.  Test hook:
+// SPD_TREE_KERNEL=block keeps the block-per-stream kernel of spd_tree.cu, =warp forces this one
+// where it applies.
+bool ws_applicable(int K) {
+    if (K < kWsMinK || K > kWsMaxK) return false;
+    if (const char* env = std::getenv("SPD_TREE_KERNEL")) {
+        if (env[0] == 'b') return false;
+    }
+    return true;
+}
+
+int ws_configure(spd_plan* plan) {
+    TreeConfig& cfg = plan->tree;
+    cfg.kind = 1;
+    cfg.T = 32 * kWsWarps;
+    cfg.chunk = kWsStep;
+    cfg.blocks_per_sm = 1;
+    cfg.smem_bytes = ws_smem_bytes();
+    cudaError_t e = cudaErrorInvalidValue;
+#define SPD_PREP(KK)                                                                                          \
+    if (cfg.K == KK)                                                                                          \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
+                                 static_cast<int>(cfg.smem_bytes));
+    SPD_WS_CASES(SPD_PREP)
+#undef SPD_PREP
+    if (e != cudaSuccess) return cuda_fail(e, "configuring the warp-stream tree kernel");
+
+    const int64_t S = kWsStep;
+    const int64_t M = int64_t(1) << (cfg.K - 1);
+    cfg.chunks_per_row = static_cast<int>((plan->n_t + S - 1) / S);
+    cfg.warm_chunks = static_cast<int>((M - 1 + S - 1) / S);
+    // Work split.  Default: the steps of the plane, in row-major order, are cut into one piece
+    // per resident warp (sm_count * 8), so every warp does the same number of steps and only
+    // the one row part per piece that stops short of its row's end replays look-ahead.
+    // Test hook SPD_SEGS_PER_ROW = s: every row cut into s equal segments instead.
+    cfg.segs_per_row = 0;
+    cfg.seg_chunks = 0;  // per launch (depends on the rows of the launch): ws_pieces()
+    if (const char* env = std::getenv("SPD_SEGS_PER_ROW")) {
+        int64_t segs = std::max<int64_t>(1, std::atoll(env));
+        segs = std::min<int64_t>(segs, cfg.chunks_per_row);
+        cfg.seg_chunks = static_cast<int>((cfg.chunks_per_row + segs - 1) / segs);
+        cfg.segs_per_row = static_cast<int>((cfg.chunks_per_row + cfg.seg_chunks - 1) / cfg.seg_chunks);
+        if (plan->n_dm * cfg.segs_per_row > 0x7fffffffll) {
+            set_error("too many streams");
+            return SPD_ERR_INVALID_ARG;
+        }
+    }
+    return SPD_OK;
+}
+
+// Pieces of a launch over n_dm rows: steps per piece and number of pieces.
+static void ws_pieces(const spd_plan* plan, int64_t n_dm, int* piece_chunks, int64_t* n_pieces) {
+    const TreeConfig& cfg = plan->tree;
+    if (cfg.segs_per_row > 0) {
+        *piece_chunks = cfg.seg_chunks;
+        *n_pieces = n_dm * cfg.segs_per_row;
+        return;
+    }
+    const int64_t total = n_dm * cfg.chunks_per_row;
+    const int64_t slots = int64_t(plan->sm_count) * kWsWarps;
+    // a piece no shorter than a few look-aheads, so that replaying one stays cheap
+    const int64_t min_len = std::max<int64_t>(8, 4 * int64_t(cfg.warm_chunks));
+    const int64_t want = std::max<int64_t>(1, std::min<int64_t>(slots, total / min_len));
+    const int64_t len = std::min<int64_t>((total + want - 1) / want, 0x3fffffff);
+    *piece_chunks = static_cast<int>(len);
+    *n_pieces = (total + len - 1) / len;
+}
+
+int ws_grid_blocks(const spd_plan* plan) {
+    int pc = 0;
+    int64_t np = 0;
+    ws_pieces(plan, plan->n_dm, &pc, &np);
+    return static_cast<int>(std::max<int64_t>(1, std::min<int64_t>(plan->sm_count, (np + kWsWarps - 1) / kWsWarps)));
+}
+
+int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
+    const TreeConfig& cfg = plan->tree;
+    TreeParams prm;
+    prm.plane = plane;
+    prm.mean = mean;
+    prm.sigma = sigma;
+    prm.out_snr = out_snr;
+    prm.out_width = out_width;
+    prm.activity = activity;
+    prm.threshold = threshold;
+    int piece_chunks = 0;
+    int64_t n_pieces = 0;
+    ws_pieces(plan, n_dm, &piece_chunks, &n_pieces);
+    if (n_pieces > 0x7fffffffll) {
+        set_error("too many pieces");
+        return SPD_ERR_INVALID_ARG;
+    }
+    prm.n_t = plan->n_t;
+    prm.n_dm = n_dm;
+    prm.chunks_per_row = cfg.chunks_per_row;
+    prm.seg_chunks = piece_chunks;
+    prm.segs_per_row = cfg.segs_per_row;
+    prm.warm_chunks = cfg.warm_chunks;
+    prm.tag_mask = ~kCodeMask;
+    if (activity) {
+        const size_t bytes = (static_cast<size_t>(n_dm) * cfg.chunks_per_row + 127) / 128 * 128;
+        const cudaError_t em = cudaMemsetAsync(activity, 0, bytes, stream);
+        if (em != cudaSuccess) return cuda_fail(em, "clearing the activity map");
+    }
+    const int64_t blocks = std::min<int64_t>(plan->sm_count, (n_pieces + kWsWarps - 1) / kWsWarps);
+    const dim3 grid(static_cast<unsigned>(std::max<int64_t>(1, blocks)));
+    cudaError_t e = cudaErrorInvalidValue;
+#define SPD_LAUNCH(KK)                                                                                      \
+    if (cfg.K == KK) {                                                                                      \
+        spd_tree_ws_kernel<KK><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+        e = cudaGetLastError();                                                                             \
+    }
+    SPD_WS_CASES(SPD_LAUNCH)
+#undef SPD_LAUNCH
+    if (e != cudaSuccess) return cuda_fail(e, "launching the warp-stream tree kernel");
+    return SPD_OK;
+}
+
+}  // namespace spd
