@@ -360,8 +360,8 @@ def run_b200(args):
     k_ms = sum(run_ms) / len(run_ms)
     achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
     roofline = {
-        "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_kernel", spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel"}.get(
-            info["path"], "generic_tile_kernel"),
+        "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_ws_kernel" if info["tree_kernel"] == 2 else "spd_tree_kernel",
+                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel"}.get(info["path"], "generic_tile_kernel"),
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),
         "algorithmic_bytes_per_launch": BYTES_PER_SAMPLE * n, "bytes_per_sample": BYTES_PER_SAMPLE,
@@ -378,7 +378,7 @@ def run_b200(args):
             "path": {spd.SPD_PATH_DYADIC_TREE: "dyadic_tree", spd.SPD_PATH_IGRID_TREE: "igrid_tree"}.get(
                 info["path"], "generic"),
             "blocks": info["blocks"], "threads_per_block": info["threads_per_block"],
-            "segments_per_row": info["segments_per_row"], "chunk": info["chunk"], "smem_bytes": info["smem_bytes"],
+            "segments_per_row": info["segments_per_row"], "piece_chunks": info["piece_chunks"], "chunk": info["chunk"], "smem_bytes": info["smem_bytes"],
             "candidate_threshold": thr, "candidates_found": n_cand}),
         "roofline": roofline,
         "clocks": clocks,

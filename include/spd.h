@@ -100,6 +100,11 @@ typedef struct spd_plan_info {
     int64_t activity_bytes;     /* size of the activity map of spd_run_flagged (multiple of 128) */
     int32_t activity_block;     /* time samples of one row covered by one byte of that map */
     int32_t activity_per_row;   /* bytes of that map per DM row */
+    int32_t tree_kernel;        /* dyadic tree: 1 = one block per stream, 2 = one warp per stream (tensor-memory
+                                   delay lines, widths 2^k with 8 <= K <= 14); else 0 */
+    int32_t piece_chunks;       /* warp-per-stream kernel: steps per piece when the plane's steps are cut, in
+                                   row-major order, into one piece per resident warp (pieces may span rows;
+                                   segments_per_row is then 0); else 0 */
 } spd_plan_info;
 
 /*

@@ -58,7 +58,9 @@ class spd_plan_info(ctypes.Structure):
                 ("chunk", ctypes.c_int32), ("segments_per_row", ctypes.c_int32),
                 ("smem_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64),
                 ("activity_bytes", ctypes.c_int64), ("activity_block", ctypes.c_int32),
-                ("activity_per_row", ctypes.c_int32)]
+                ("activity_per_row", ctypes.c_int32),
+                ("tree_kernel", ctypes.c_int32),
+                ("piece_chunks", ctypes.c_int32)]
 
 
 _lib: Optional[ctypes.CDLL] = None

@@ -319,6 +319,8 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         info->chunk = plan->tree.chunk;
         info->segments_per_row = plan->tree.segs_per_row;
         info->smem_bytes = static_cast<int64_t>(plan->tree.smem_bytes);
+        if (plan->path == SPD_PATH_DYADIC_TREE) info->tree_kernel = plan->tree.kind == 1 ? 2 : 1;
+        if (plan->tree.kind == 1 && plan->tree.segs_per_row == 0) info->piece_chunks = ws_piece_chunks(plan);
     } else {
         if (plan->generic_tile > 0) {
             info->launches_per_run = 1;

@@ -180,7 +180,8 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
 }  // namespace
 
 int64_t activity_block(const spd_plan* plan) {
-    return is_tree_path(plan) ? plan->tree.chunk : 4096;
+    if (!is_tree_path(plan)) return 4096;
+    return plan->tree.act_block > 0 ? plan->tree.act_block : plan->tree.chunk;
 }
 int64_t activity_per_row(const spd_plan* plan) {
     const int64_t b = activity_block(plan);

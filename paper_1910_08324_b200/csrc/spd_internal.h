@@ -22,6 +22,7 @@ struct TreeConfig {
     int kind = 0;         // 0: block per stream (spd_tree.cu), 1: warp per stream (spd_tree_ws.cu)
     int T = 0;            // threads per block
     int chunk = 0;        // 4 * T * R samples
+    int act_block = 0;    // samples per activity-map byte (0: = chunk)
     int warm_chunks = 0;  // look-ahead chunks an interior segment replays
     int segs_per_row = 1;
     int seg_chunks = 0;   // chunks per segment
@@ -90,6 +91,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
 bool ws_applicable(int K);
 int ws_configure(spd_plan* plan);
 int ws_grid_blocks(const spd_plan* plan);
+int ws_piece_chunks(const spd_plan* plan);
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
            float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream);
 

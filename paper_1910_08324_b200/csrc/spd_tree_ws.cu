@@ -45,6 +45,9 @@ static_assert(kWsRows == 4 || kWsRows == 8, "rows per step");
 constexpr int kWsStep = 128 * kWsRows;      // samples per step
 constexpr int kWsStage = kWsStep + 8;       // floats per stage: the step + two float4 of look-ahead
 constexpr int kWsMinK = 8, kWsMaxK = 14;
+// Activity map: one byte per kWsActSteps steps (2048 samples, the block kernel's granularity:
+// finer flags only lengthen the candidate kernel's scan of the map).
+constexpr int kWsActSteps = 2048 / kWsStep;
 #ifndef SPD_WS_STAGES
 #define SPD_WS_STAGES 4
 #endif
@@ -420,7 +423,9 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
         cx.inv = 1.0f / sg;
         cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
         cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
-        uint8_t* const act = p.activity ? p.activity + static_cast<long long>(d) * p.chunks_per_row : nullptr;
+        uint8_t* const act =
+            p.activity ? p.activity + static_cast<long long>(d) * ((p.chunks_per_row + kWsActSteps - 1) / kWsActSteps)
+                       : nullptr;
         float thr_key = __int_as_float(0x7f800000);
         if (act) {
             const float t = p.threshold * sg;
@@ -459,7 +464,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             cx.n0 = n0;
             cx.do_out = c < c_hi;
             const float top = ws_step<K, 0>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
-            if (act && cx.do_out && top >= thr_key) act[c] = 1;
+            if (act && cx.do_out && top >= thr_key) act[c / kWsActSteps] = 1;
             __syncwarp();
         }
 
@@ -514,7 +519,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             cx.n0 = static_cast<long long>(c) * S;
             const float top = ws_step<K, 1>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
                                             tbase, it, lane, cx);
-            if (act && top >= thr_key) act[c] = 1;
+            if (act && top >= thr_key) act[c / kWsActSteps] = 1;
             ring_done();
         }
       }
@@ -547,6 +552,7 @@ int ws_configure(spd_plan* plan) {
     cfg.kind = 1;
     cfg.T = 32 * kWsWarps;
     cfg.chunk = kWsStep;
+    cfg.act_block = kWsStep * kWsActSteps;
     cfg.blocks_per_sm = 1;
     cfg.smem_bytes = ws_smem_bytes();
     cudaError_t e = cudaErrorInvalidValue;
@@ -599,6 +605,13 @@ static void ws_pieces(const spd_plan* plan, int64_t n_dm, int* piece_chunks, int
     *n_pieces = (total + len - 1) / len;
 }
 
+int ws_piece_chunks(const spd_plan* plan) {
+    int pc = 0;
+    int64_t np = 0;
+    ws_pieces(plan, plan->n_dm, &pc, &np);
+    return pc;
+}
+
 int ws_grid_blocks(const spd_plan* plan) {
     int pc = 0;
     int64_t np = 0;
@@ -632,7 +645,7 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     prm.warm_chunks = cfg.warm_chunks;
     prm.tag_mask = ~kCodeMask;
     if (activity) {
-        const size_t bytes = (static_cast<size_t>(n_dm) * cfg.chunks_per_row + 127) / 128 * 128;
+        const size_t bytes = (static_cast<size_t>(n_dm) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
         const cudaError_t em = cudaMemsetAsync(activity, 0, bytes, stream);
         if (em != cudaSuccess) return cuda_fail(em, "clearing the activity map");
     }

@@ -53,6 +53,14 @@ def _window_list(w, info, pulses, rng, n_random):
     for s in range(1, segs)[:3]:
         b = s * seg_chunks * chunk
         out.append((int(rng.integers(0, n_dm)), b - direct_span // 2, direct_span, "segment-boundary"))
+    # warp-per-stream kernel: the plane's steps are cut into pieces in row-major order
+    piece = info.get("piece_chunks", 0)
+    if piece > 0:
+        n_pieces = (n_dm * chunks_per_row + piece - 1) // piece
+        for pi in sorted({1, n_pieces // 3, n_pieces // 2, n_pieces - 1}):
+            if 0 < pi < n_pieces:
+                d, c = divmod(pi * piece, chunks_per_row)
+                out.append((d, max(0, c * chunk - direct_span // 2), direct_span, "piece-boundary"))
     for _ in range(3):
         b = int(rng.integers(1, chunks_per_row)) * chunk
         out.append((int(rng.integers(0, n_dm)), b - direct_span // 2, direct_span, "chunk-boundary"))
@@ -216,11 +224,15 @@ def test_longest_row(spd, oracle_lib, kind, param):
         torch.cuda.synchronize()
         count, cands = spd.candidates_to_numpy(lst, n_found, 1 << 20)
     mean_h, sigma_h = np.zeros(1), np.ones(1)
-    chunk, segs = info["chunk"], info["segments_per_row"]
+    chunk, segs = info["chunk"], max(info["segments_per_row"], 1)
     chunks_per_row = (n_t + chunk - 1) // chunk
     seg_chunks = (chunks_per_row + segs - 1) // segs
     starts = [0, (1 << 30) - 2000, (1 << 31) - (1 << 28) - 700, n_t - 8192 - 1000, n_t - 1536]
     starts += [s * seg_chunks * chunk - 700 for s in range(1, segs)][:3]
+    if info.get("piece_chunks", 0) > 0:  # one row: pieces are stretches of this row
+        n_pieces = (chunks_per_row + info["piece_chunks"] - 1) // info["piece_chunks"]
+        starts += [pi * info["piece_chunks"] * chunk - 700 for pi in sorted({1, n_pieces // 2, n_pieces - 1})
+                   if 0 < pi < n_pieces]
     worst = 0.0
     for t0 in starts:
         st = _check_window(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths, 8192, 0, t0, 1536, direct=True,
