@@ -33,9 +33,11 @@
  * There is NO CPU fallback: on a machine without an sm_100 device every
  * compute entry point fails with SPD_ERR_UNSUPPORTED_DEVICE.
  *
- * Environment variables read at plan creation (test hooks, not tuning knobs):
+ * Environment variables read at plan creation (three test hooks, not tuning knobs):
  *   SPD_SEGS_PER_ROW=n      streaming trees: n independent streams per DM row instead of the
  *                           automatic choice (exercises the look-ahead replay of interior segments);
+ *   SPD_TREE_KERNEL=block   widths {2^k}: keep the block-per-stream kernel where the warp-per-stream
+ *                           kernel (9 <= K <= 14 widths, tensor-memory delay lines) would be chosen;
  *   SPD_GENERIC_WORKSPACE=1 any-width-set path: use the device-workspace kernels even where the
  *                           shared-memory tile kernel applies.
  */

@@ -1,30 +1,38 @@
 // Dyadic partial-sum tree, one WARP per stream, for
-// 8 <= K <= 14 widths {1, 2, ..., 2^(K-1)}.
+// 9 <= K <= 14 widths {1, 2, ..., 2^(K-1)}.
 //
 // Same arithmetic as spd_tree.cu (eq. 2, 4, 5, 12 and the reuse of eq. 15/16:
 // P_{k+1}[n] = P_k[n] + P_k[n + 2^k]), different
 // decomposition.  In spd_tree.cu a block of 4 warps shares one stream, so every level whose
-// partner lies in another thread costs a shared-memory store, a block barrier and a load.
-// Here every warp streams its own segment of a DM row in reverse time and nothing is shared
-// between warps: no block barrier and no shared-memory exchange at all.
+// partner lies in another thread costs a block barrier.  Here every warp streams its own piece
+// of the plane in reverse time and nothing is shared between warps: no block barrier at all.
 //
-//   * A step is R = 8 "rows" of 128 samples; lane l owns the float4 4l..4l+3 of every row.
+//   * A step is R = 4 "rows" of 128 samples; lane l owns the float4 4l..4l+3 of every row.
 //   * Widths 2, 4, 8: in the lane's registers from three raw float4 (as spd_tree.cu).
-//   * Partner 8, 16, 32, 64 samples later = 2, 4, 8, 16 lanes later: warp shuffles; the lanes
-//     that run off the row take the shuffled value of the NEXT row (same lane set, one row
-//     later), the last row takes it from the previous step's first row (4 float4 kept).
-//   * Partner 128 * 2^j samples later = the same lane, 2^j rows later: a register of this step
-//     (j < 3), of the previous step (7 float4 kept), or - 1, 2, 4 steps back - a FIFO.
-//   * The FIFOs (7 x 8 float4 per lane for K = 14: the 28 KB of delay state that forces
+//   * Partner 8, 16, 32, 64 samples later = 2, 4, 8, 16 lanes later ("lane levels"): through a
+//     warp-private shared-memory buffer ordered by __syncwarp (one 128-bit store and load per
+//     float4; shuffles would take eight instructions, and the issue slots are what binds).
+//     A lane that runs off its row continues in the next row, which is adjacent in the buffer;
+//     the last row continues in the first row of the previous step (4 float4 kept, stored
+//     behind the rows).
+//   * Partner 128 * 2^j samples later = the same lane, 2^j rows later ("row levels"): a
+//     register of this step or of the previous step (7 float4 kept), or - 2, 4, 8 steps back -
+//     a FIFO.
+//   * The FIFOs (14 x 4 float4 per lane for K = 14: the 28 KB of delay state that forces
 //     spd_tree.cu to spread a stream over 128 threads) live in TENSOR MEMORY: each warp owns
-//     32 lanes x 224 columns, written with tcgen05.st and read with tcgen05.ld (32x32b.x32:
-//     one instruction moves the 8 float4 of a level), slot = step mod depth as a run-time
+//     32 lanes x 224 columns, written with tcgen05.st and read with tcgen05.ld (32x32b.x16:
+//     one instruction moves the 4 float4 of a level), slot = step mod depth as a run-time
 //     column offset - no unrolling over FIFO phases, no register rotation.  TMEM is used as
 //     plain per-lane scratch; there is no MMA anywhere (streaming reduction, not a contraction).
-//   * Raw samples arrive by 1-D cp.async.bulk through a 3-stage mbarrier ring PER WARP.
-//   * SNR scale, width tag, 3-input max, threshold flag, guarded tail steps: as spd_tree.cu.
+//   * Raw samples arrive by 1-D cp.async.bulk through a 4-stage mbarrier ring PER WARP.
+//   * SNR scale, width tag, 3-input max, threshold flag, guarded tail steps: as spd_tree.cu;
+//     look-ahead steps of a piece that starts inside a row compute the sums only.
+//   * Work split: the steps of the plane, in row-major order, are cut into one piece per
+//     resident warp (148 SMs x 8), so all warps finish together and a piece replays look-ahead
+//     once (for the one row part that stops short of its row's end).
 //
 // One block of 8 warps per SM (2 warps per lane quarter of TMEM, 2 x 224 <= 512 columns).
+// Measured on config 3: 10.7 ms against 11.4 ms of spd_tree.cu.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
