@@ -14,5 +14,6 @@ from .core import (  # noqa: F401
     row_stats_clipped,
     snr_of_width,
     spd_direct,
+    spd_grid,
     spd_prefix,
 )

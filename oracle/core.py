@@ -41,6 +41,8 @@ def _load() -> ctypes.CDLL:
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_spd_direct.restype = None
         lib.oracle_spd_direct.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
+        lib.oracle_spd_grid.restype = None
+        lib.oracle_spd_grid.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
         lib.oracle_spd_prefix.restype = None
         lib.oracle_spd_prefix.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _vp, _vp, _vp]
         lib.oracle_snr_of_width.restype = None
@@ -95,6 +97,28 @@ def spd_direct(x, mean, sigma, widths, t0: int = 0, t1: Optional[int] = None
     _load().oracle_spd_direct(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
                               w.ctypes.data, int(w.size), t0, t1,
                               snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
+
+
+def spd_grid(x, mean, sigma, widths, seps, t0: int = 0, t1: Optional[int] = None
+             ) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Direct summation with a boxcar separation per width (ascending widths, seps[k] >= 1):
+    width k is evaluated only where n % seps[k] == 0.  Returns (snr, width_idx, second)."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    t1 = n_t if t1 is None else int(t1)
+    t0 = int(t0)
+    assert 0 <= t0 <= t1 <= n_t
+    w = np.ascontiguousarray([int(v) for v in widths], dtype=np.int32)
+    sp = np.ascontiguousarray([int(v) for v in seps], dtype=np.int32)
+    assert w.size > 0 and w.size == sp.size and w[0] >= 1 and np.all(np.diff(w) > 0) and np.all(sp >= 1)
+    mu, sg = _stats(mean, n_dm), _stats(sigma, n_dm)
+    snr = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    idx = np.empty((n_dm, t1 - t0), dtype=np.int32)
+    sec = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    _load().oracle_spd_grid(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
+                            w.ctypes.data, sp.ctypes.data, int(w.size), t0, t1,
+                            snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
     return snr, idx, sec
 
 

@@ -27,6 +27,8 @@
  *                        C[n] of (x - mu) and X'_L[n] = C[n+L] - C[n]; a faster
  *                        route used on full planes, itself pinned to
  *                        oracle_spd_direct in tests (<= 1e-9).
+ *   oracle_spd_grid    : oracle_spd_direct with a boxcar separation per width (the
+ *                        paper's decimated grids, merged into one plane; reading A16).
  *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
  *   oracle_row_stats   : per-row mean and population standard deviation (reading A6).
  *   oracle_row_stats_clipped: mean / sigma with point-wise outlier rejection
@@ -77,6 +79,52 @@ void oracle_spd_direct(const float* x, int64_t n_dm, int64_t n_t,
             for (int32_t k = 0; k < n_w; ++k) {
                 const int64_t L = widths[k];
                 if (n + L > n_t) break;                       /* valid windows only (A3) */
+                double X = 0.0;
+                for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
+                const double snr = (X - (double)L * mean[d]) / (sqrt((double)L) * sigma[d]); /* eq. (4),(5) */
+                if (snr > best) {                              /* strict '>' (A4) */
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * span + (n - t0);
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+    }
+}
+
+/* Per-width boxcar separation (the paper's lossy grids): width k is
+ * evaluated only at the samples n that are multiples of its separation L_s[k]
+ * ("boxcar filters of width L=6,8,10,12 are calculated at every second point", PAPER.md:201;
+ * BoxDIT iteration i works at every D^(i)-th point, Alg. 1; DIT width 2^i at
+ * every 2^i-th point, Alg. 3; IGRID with P layers at 2^i / P).
+ * Reading A16: one merged full-resolution plane, Y[n] = max over the widths whose grid
+ * contains n (eq. 12 restricted to them), -inf / -1 where none does; everything else
+ * (eq. 2, 4, 5, valid windows only, strict '>' in ascending width order) as oracle_spd_direct.
+ * Pins (tests/test_oracle_pins.py): pulses slid over all shifts recover exactly the
+ * worst / best responses of eq. (27)-(31) and (24); the constant-offset
+ * closed form reproduces the example grid of PAPER.md:201; separations all 1 = oracle_spd_direct. */
+void oracle_spd_grid(const float* x, int64_t n_dm, int64_t n_t,
+                     const double* mean, const double* sigma,
+                     const int32_t* widths, const int32_t* seps, int32_t n_w,
+                     int64_t t0, int64_t t1,
+                     double* out_snr, int32_t* out_width, double* out_second) {
+    const int64_t span = t1 - t0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 256)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        for (int64_t n = t0; n < t1; ++n) {
+            const float* row = x + d * n_t;
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = 0; k < n_w; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;                       /* valid windows only (A3) */
+                if (n % (int64_t)seps[k] != 0) continue;      /* n is not on this width's grid */
                 double X = 0.0;
                 for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
                 const double snr = (X - (double)L * mean[d]) / (sqrt((double)L) * sigma[d]); /* eq. (4),(5) */

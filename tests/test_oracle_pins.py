@@ -401,3 +401,82 @@ def test_candidates_rule_edges_and_capacity(oracle_lib):
     assert list(zip(c_dm.tolist(), c_t.tolist())) == [(0, 0), (0, 3), (0, 7), (1, 7)]
     count2, c_dm2, *_ = oracle_lib.find_candidates(y, wid, 6.0, capacity=2)
     assert count2 == 4 and len(c_dm2) == 2
+
+
+# --- f2: per-width boxcar separation (the paper's decimated grids), oracle_spd_grid -----
+
+def _slid_pulses(S, n_shifts, n_t, t_first, snr_t=16.0):
+    """One noise-free row per shift of a width-S pulse (the paper's measurement method,
+    PAPER.md:492-494; C = 16, PAPER.md:553)."""
+    x = np.zeros((n_shifts, n_t), dtype=np.float32)
+    for s in range(n_shifts):
+        x[s] = _single_pulse_row(n_t, t_first + s, S, snr_t)
+    return x
+
+
+@pytest.mark.parametrize("L,Ls", [(5, 3), (8, 8), (8, 4), (8, 2), (16, 16), (12, 4), (7, 7), (9, 2)])
+def test_grid_single_width_recovers_eq30_and_eq23(oracle_lib, L, Ls):
+    """Boxcars of one width L at every Ls-th sample: over all pulse shifts the best response
+    per row has minimum eq. (30) and maximum eq. (23)."""
+    for S in list(range(1, 3 * L + 2 * Ls, 2)) + [L, L + Ls]:
+        n_t = 6 * (L + Ls) + 4 * S
+        t_first = (2 * (L + Ls) + Ls - 1) // Ls * Ls          # a grid point, far from both ends
+        x = _slid_pulses(S, Ls, n_t, t_first)
+        snr, idx, _ = oracle_lib.spd_grid(x, 0.0, 1.0, [L], [Ls])
+        per_shift = snr.max(axis=1) / 16.0
+        assert per_shift.min() == pytest.approx(F.rsnr_min_single(S, L, Ls), abs=1e-6), (S, L, Ls)
+        assert per_shift.max() == pytest.approx(F.rsnr_max_single(S, L), abs=1e-6), (S, L, Ls)
+        off_grid = np.arange(n_t) % Ls != 0
+        assert np.all(np.isneginf(snr[:, off_grid])) and np.all(idx[:, off_grid] == -1)
+
+
+@pytest.mark.parametrize("name", ["DIT", "BOXDIT4", "BOXDIT8", "IGRID1x4"])
+def test_grid_width_sets_lie_between_eq31_and_eq24(oracle_lib, name):
+    """The bound test of PAPER.md:152, 512 on the paper's grids: measured worst response >=
+    eq. (31), best == eq. (24); and both equal the shift scan written out in formulas.py."""
+    widths, sep = {"DIT": (F.widths_pow2(64), lambda L: L),
+                   "BOXDIT4": (F.widths_boxdit(4, 60), F.boxdit_separation(4)),
+                   "BOXDIT8": (F.widths_boxdit(8, 56), F.boxdit_separation(8)),
+                   "IGRID1x4": (F.widths_igrid(1, 64), F.igrid_separation(4))}[name]
+    seps = [sep(L) for L in widths]
+    period = max(seps)                                        # separations are powers of two
+    for S in (1, 2, 3, 5, 7, 9, 12, 17, 20, 31, 33, 45, 64, 70):
+        n_t = 4 * 64 + 2 * period + 2 * S
+        t_first = 2 * period
+        x = _slid_pulses(S, period, n_t, t_first)
+        snr, _, _ = oracle_lib.spd_grid(x, 0.0, 1.0, widths, seps)
+        per_shift = snr.max(axis=1) / 16.0
+        lo, hi, mean = F.brute_force_response(S, widths, sep)
+        assert per_shift.min() == pytest.approx(lo, abs=1e-6) and per_shift.max() == pytest.approx(hi, abs=1e-6)
+        assert per_shift.mean() == pytest.approx(mean, abs=1e-6)
+        assert per_shift.min() >= F.rsnr_min(S, widths, sep) - 1e-6
+        assert per_shift.max() == pytest.approx(F.rsnr_max(S, widths), abs=1e-6)
+
+
+def test_grid_paper_example_positions(oracle_lib):
+    """with L_max = 4, widths 1..4 are calculated at every point, 6, 8, 10, 12 at
+    every second point (and 16, 20, 24, 28 at every fourth).  On a constant offset
+    SNR_L = a sqrt(L) / sigma grows with L, so the winner is the largest width whose grid
+    contains n and whose window fits."""
+    n_t, mu, sg, a = 131, 0.5, 2.0, 1.5
+    widths = F.widths_boxdit(4, 28)
+    assert widths == [1, 2, 3, 4, 6, 8, 10, 12, 16, 20, 24, 28]
+    sepf = F.boxdit_separation(4)
+    seps = [sepf(L) for L in widths]
+    assert seps == [1, 1, 1, 1, 2, 2, 2, 2, 4, 4, 4, 4]
+    x = np.full(n_t, mu + a, dtype=np.float32)
+    snr, idx, _ = oracle_lib.spd_grid(x, mu, sg, widths, seps)
+    for n in range(n_t):
+        ok = [k for k, (L, s) in enumerate(zip(widths, seps)) if n % s == 0 and n + L <= n_t]
+        assert idx[0][n] == ok[-1]
+        assert snr[0][n] == pytest.approx(a * math.sqrt(widths[ok[-1]]) / sg, rel=1e-12)
+    assert idx[0][1] == 3 and idx[0][2] == 7 and idx[0][4] == 11 and idx[0][6] == 7
+
+
+def test_grid_with_unit_separations_is_direct(oracle_lib):
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal((3, 300)).astype(np.float32)
+    widths = F.widths_igrid(1, 64)
+    a = oracle_lib.spd_direct(x, 0.1, 1.3, widths)
+    b = oracle_lib.spd_grid(x, 0.1, 1.3, widths, [1] * len(widths))
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
