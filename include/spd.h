@@ -69,6 +69,15 @@ typedef enum spd_width_kind {
     SPD_WIDTHS_GEOMETRIC = 4  /* round(r^j), r = param / 1000 (> 1); this project's addition */
 } spd_width_kind;
 
+/* Boxcar-separation kinds of spd_separation_generate (the paper's decimated grids). */
+typedef enum spd_grid_kind {
+    SPD_GRID_EVERY_SAMPLE = 0, /* L_s = 1 for every width */
+    SPD_GRID_DIT = 1,          /* Alg. 3: width 2^i at every 2^i-th sample */
+    SPD_GRID_BOXDIT = 2,       /* Alg. 1, D = 2: the widths of iteration i (eq. 14, param = L_max)
+                                  at every 2^i-th sample ("6,8,10,12 at every second point") */
+    SPD_GRID_IGRID = 3         /* param = P layers: the widths of step 2^i at every (2^i / P)-th sample */
+} spd_grid_kind;
+
 /* Plan creation flags (spd_plan_create_ex). */
 #define SPD_FLAG_FORCE_GENERIC 0x1u /* use the any-width-set kernels even where a streaming tree applies */
 
@@ -76,6 +85,7 @@ typedef enum spd_width_kind {
 #define SPD_PATH_DYADIC_TREE 1 /* streaming partial-sum tree, widths {1,2,4,...,2^(K-1)} */
 #define SPD_PATH_IGRID_TREE 3  /* the same streaming tree for widths {2^k} U {3 * 2^m} (IGRID depth 1, eq. 18) */
 #define SPD_PATH_GENERIC 2     /* any width set: per-row running partial sums, staged per tile in shared memory */
+#define SPD_PATH_GRID 4        /* any width set with a boxcar separation per width (spd_plan_create_grid) */
 
 typedef struct spd_plan spd_plan; /* opaque */
 
@@ -141,6 +151,30 @@ int spd_plan_create(spd_plan** out, int64_t n_dm, int64_t n_t,
 int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t,
                        const int32_t* width_set, int32_t n_widths, int32_t max_width,
                        uint32_t flags);
+
+/*
+ * spd_separation_generate - boxcar separation L_s of each width of a set, by the paper's schedules.
+ *   widths : HOST array of n_widths widths (>= 1); out: HOST array of n_widths int32.
+ * Returns SPD_ERR_INVALID_ARG for an unknown kind, a bad param, or (SPD_GRID_DIT) a width
+ * that is not a power of two.
+ */
+int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, int32_t n_widths, int32_t* out);
+
+/*
+ * spd_plan_create_grid - a plan whose width k is evaluated only at the time samples that are
+ * multiples of separations[k] (the paper's lossy grids - "wider pulses ...
+ * at every D^(i) point"; sensitivity eq. (27)-(31)).
+ *   width_set   : HOST, n_widths widths, STRICTLY ascending, each in [1, max_width];
+ *   separations : HOST, n_widths powers of two that do not decrease with the width.
+ * spd_run / spd_run_flagged / spd_run_host on such a plan write one merged full-resolution
+ * plane: out_snr[d,n] = max over the widths whose grid contains n (and whose window fits,
+ * reading A3), out_width the index of that width; -inf / -1 where no width's grid contains n
+ * (only if separations[0] > 1).  Limits: max_width <= 45057, n_widths <= 1024.
+ * spd_plan_info.path is SPD_PATH_GRID.  Errors as spd_plan_create plus the conditions above.
+ */
+int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t,
+                         const int32_t* width_set, const int32_t* separations, int32_t n_widths,
+                         int32_t max_width);
 
 /* Frees the plan and everything it owns.  NULL is allowed. */
 void spd_plan_destroy(spd_plan* plan);

@@ -25,7 +25,9 @@ SPD_ERR_CUDA = -4
 SPD_WIDTHS_ALL, SPD_WIDTHS_POW2, SPD_WIDTHS_BOXDIT, SPD_WIDTHS_IGRID, SPD_WIDTHS_GEOMETRIC = range(5)
 WIDTH_KINDS = {"ALL": 0, "POW2": 1, "BOXDIT": 2, "IGRID": 3, "GEOMETRIC": 4}
 SPD_FLAG_FORCE_GENERIC = 0x1
-SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC, SPD_PATH_IGRID_TREE = 1, 2, 3
+SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC, SPD_PATH_IGRID_TREE, SPD_PATH_GRID = 1, 2, 3, 4
+SPD_GRID_EVERY_SAMPLE, SPD_GRID_DIT, SPD_GRID_BOXDIT, SPD_GRID_IGRID = range(4)
+GRID_KINDS = {"EVERY_SAMPLE": 0, "DIT": 1, "BOXDIT": 2, "IGRID": 3}
 
 # every symbol include/spd.h declares
 EXPORTS = (
@@ -33,6 +35,7 @@ EXPORTS = (
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
     "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
     "spd_run_host", "spd_last_error_string", "spd_version",
+    "spd_separation_generate", "spd_plan_create_grid",
 )
 
 
@@ -90,6 +93,10 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_plan_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _i32, _i32]
     lib.spd_plan_create_ex.restype = ctypes.c_int
     lib.spd_plan_create_ex.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _i32, _i32, ctypes.c_uint32]
+    lib.spd_plan_create_grid.restype = ctypes.c_int
+    lib.spd_plan_create_grid.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _i32, _i32]
+    lib.spd_separation_generate.restype = ctypes.c_int
+    lib.spd_separation_generate.argtypes = [_i32, _i32, _vp, _i32, _vp]
     lib.spd_plan_destroy.restype = None
     lib.spd_plan_destroy.argtypes = [_vp]
     lib.spd_plan_get_widths.restype = ctypes.c_int
@@ -148,6 +155,30 @@ def spd_plan_create(n_dm: int, n_t: int, width_set: Sequence[int], max_width: in
         st = lib.spd_plan_create(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, int(w.size),
                                  int(max_width))
     _check(st)
+    return int(handle.value)
+
+
+def spd_separation_generate(kind, param: int, widths: Sequence[int]) -> np.ndarray:
+    """Boxcar separation of every width; ``kind`` is an SPD_GRID_* value or its name."""
+    lib = load()
+    k = GRID_KINDS[kind.upper()] if isinstance(kind, str) else int(kind)
+    w = np.ascontiguousarray(np.asarray(widths, dtype=np.int32).reshape(-1))
+    out = np.empty(w.size, dtype=np.int32)
+    _check(lib.spd_separation_generate(k, int(param), w.ctypes.data, int(w.size), out.ctypes.data))
+    return out
+
+
+def spd_plan_create_grid(n_dm: int, n_t: int, width_set: Sequence[int], separations: Sequence[int],
+                         max_width: int) -> int:
+    """Plan with a boxcar separation per width; returns the opaque handle."""
+    lib = load()
+    w = np.ascontiguousarray(np.asarray(width_set, dtype=np.int32).reshape(-1))
+    sp = np.ascontiguousarray(np.asarray(separations, dtype=np.int32).reshape(-1))
+    if w.size != sp.size:
+        raise ValueError("width_set and separations differ in length")
+    handle = _vp(0)
+    _check(lib.spd_plan_create_grid(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, sp.ctypes.data,
+                                    int(w.size), int(max_width)))
     return int(handle.value)
 
 
@@ -322,9 +353,13 @@ class Plan:
     """Owns one ``spd_plan``; convenience wrapper over the functions above."""
 
     def __init__(self, n_dm: int, n_t: int, width_set: Sequence[int], max_width: Optional[int] = None,
-                 flags: int = 0):
+                 flags: int = 0, separations: Optional[Sequence[int]] = None):
         w = np.asarray(width_set, dtype=np.int32)
-        self.handle = spd_plan_create(n_dm, n_t, w, int(w.max()) if max_width is None else max_width, flags)
+        mw = int(w.max()) if max_width is None else max_width
+        if separations is None:
+            self.handle = spd_plan_create(n_dm, n_t, w, mw, flags)
+        else:
+            self.handle = spd_plan_create_grid(n_dm, n_t, w, separations, mw)
         self.info = spd_plan_get_info(self.handle)
         self.widths = spd_plan_get_widths(self.handle)
         self.n_dm, self.n_t = int(n_dm), int(n_t)

@@ -213,8 +213,79 @@ int spd_plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* wi
     return spd_plan_create_ex(out, n_dm, n_t, width_set, n_widths, max_width, 0u);
 }
 
+static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
+                       const int32_t* separations, int32_t n_widths, int32_t max_width, uint32_t flags);
+
 int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set, int32_t n_widths,
                        int32_t max_width, uint32_t flags) {
+    return plan_create(out, n_dm, n_t, width_set, nullptr, n_widths, max_width, flags);
+}
+
+int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
+                         const int32_t* separations, int32_t n_widths, int32_t max_width) {
+    if (!separations) {
+        set_error("spd_plan_create_grid: separations is NULL");
+        if (out) *out = nullptr;
+        return SPD_ERR_INVALID_ARG;
+    }
+    return plan_create(out, n_dm, n_t, width_set, separations, n_widths, max_width, 0u);
+}
+
+int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, int32_t n_widths, int32_t* out) {
+    if (!widths || !out || n_widths < 1) {
+        set_error("spd_separation_generate: NULL argument or no widths");
+        return SPD_ERR_INVALID_ARG;
+    }
+    for (int32_t k = 0; k < n_widths; ++k) {
+        const int64_t L = widths[k];
+        if (L < 1) {
+            set_error("spd_separation_generate: width %lld < 1", (long long)L);
+            return SPD_ERR_INVALID_ARG;
+        }
+        int64_t oct = 1;  // largest power of two <= L
+        while (oct * 2 <= L) oct *= 2;
+        int64_t sep = 1;
+        switch (kind) {
+            case SPD_GRID_EVERY_SAMPLE:
+                break;
+            case SPD_GRID_DIT:  // Alg. 3: width 2^i at every 2^i-th sample
+                if (oct != L) {
+                    set_error("SPD_GRID_DIT needs power-of-two widths (got %lld)", (long long)L);
+                    return SPD_ERR_INVALID_ARG;
+                }
+                sep = L;
+                break;
+            case SPD_GRID_BOXDIT: {  // Alg. 1 with D = 2: iteration i holds widths (2^i - 1) L_max + 2^i m (eq. 14)
+                if (param < 1) {
+                    set_error("SPD_GRID_BOXDIT needs param = L_max >= 1");
+                    return SPD_ERR_INVALID_ARG;
+                }
+                int64_t base = 0, step = 1;
+                while (L > base + step * param) {
+                    base += step * param;
+                    step *= 2;
+                }
+                sep = step;
+                break;
+            }
+            case SPD_GRID_IGRID:  // P layers: L_s = 2^i / P for the widths of step 2^i
+                if (param < 1 || (param & (param - 1))) {
+                    set_error("SPD_GRID_IGRID needs param = number of layers, a power of two");
+                    return SPD_ERR_INVALID_ARG;
+                }
+                sep = std::max<int64_t>(1, oct / param);
+                break;
+            default:
+                set_error("unknown separation kind %d", kind);
+                return SPD_ERR_INVALID_ARG;
+        }
+        out[k] = static_cast<int32_t>(sep);
+    }
+    return SPD_OK;
+}
+
+static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
+                       const int32_t* separations, int32_t n_widths, int32_t max_width, uint32_t flags) {
     if (!out) {
         set_error("spd_plan_create: out is NULL");
         return SPD_ERR_INVALID_ARG;
@@ -233,6 +304,33 @@ int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
         return SPD_ERR_INVALID_ARG;
     }
     std::vector<int32_t> w(width_set, width_set + n_widths);
+    std::vector<int32_t> seps;
+    GridGroups groups = {};
+    if (separations) {
+        // widths strictly ascending; separations powers of two that do not decrease with the width
+        // (the paper's grids: an iteration's widths share D^(i), later iterations are coarser)
+        seps.assign(separations, separations + n_widths);
+        for (int32_t k = 0; k < n_widths; ++k) {
+            const int32_t sp = seps[k];
+            if (sp < 1 || (sp & (sp - 1)) || (k > 0 && (w[k] <= w[k - 1] || sp < seps[k - 1]))) {
+                set_error("spd_plan_create_grid: widths must ascend strictly, separations must be powers of two "
+                          "that do not decrease (entry %d: width %d, separation %d)", k, w[k], sp);
+                return SPD_ERR_INVALID_ARG;
+            }
+            if (k == 0 || sp != seps[k - 1]) {
+                if (groups.n == kGridGroupsMax) {
+                    set_error("spd_plan_create_grid: more than %d distinct separations", kGridGroupsMax);
+                    return SPD_ERR_INVALID_ARG;
+                }
+                int sh = 0;
+                while ((1 << sh) < sp) ++sh;
+                groups.shift[groups.n] = sh;
+                groups.kb[groups.n] = k;
+                ++groups.n;
+            }
+            groups.ke[groups.n - 1] = k + 1;
+        }
+    }
     std::sort(w.begin(), w.end());
     w.erase(std::unique(w.begin(), w.end()), w.end());
     if (w.front() < 1 || w.back() > max_width) {
@@ -259,8 +357,13 @@ int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     plan->max_width = max_width;
     plan->device = device;
     plan->sm_count = sm_count;
+    plan->separations = seps;
+    plan->grid = groups;
     int ig_levels = 0;
-    if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
+    if (separations) {
+        plan->path = SPD_PATH_GRID;
+        rc = generic_configure(plan);
+    } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
         plan->path = SPD_PATH_DYADIC_TREE;
         rc = tree_configure(plan);
     } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && (ig_levels = ig_applicable(w, n_t)) > 0) {

@@ -167,34 +167,13 @@ constexpr int kSub = 64;                 // samples per float32 sub-block
 constexpr int kTileSpanMax = 48 * 1024;  // floats of shared memory for tile + look-ahead
 constexpr int kTileWidthsMax = 1024;     // width table kept in shared memory up to this many widths
 
-__global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
-    const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
-    const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, long long n_t, int tile,
-    int span, long long tiles_per_row, float* __restrict__ out_snr, int32_t* __restrict__ out_width) {
-    extern __shared__ __align__(16) unsigned char gsm[];
-    const int n_sub = span / kSub;  // span is a multiple of kSub
-    double* const B = reinterpret_cast<double*>(gsm);                        // [n_sub + 1] running sum of sub-block totals
-    float* const c = reinterpret_cast<float*>(gsm + (n_sub + 2) / 2 * 16);  // [span + 1] exclusive sum inside a sub-block
-    int32_t* const sw = reinterpret_cast<int32_t*>(c + (span + 4) / 4 * 4);   // [kTileWidthsMax] widths
-    float* const ss = reinterpret_cast<float*>(sw + kTileWidthsMax);          // [kTileWidthsMax] 1 / (sqrt(L) sigma)
-    const long long d = blockIdx.x / tiles_per_row;
-    const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
-    const float* __restrict__ row = plane + d * n_t;
-    const float mu = mean[d];
-    const float inv = 1.0f / sigma[d];
-    const long long avail = n_t - t0;  // samples of the row from t0 on
+// Phases 1 and 2 of a tile: the two-level running sum of (x - mu) over `span` samples from t0:
+// c[i] = float32 exclusive sum inside the 64-sample sub-block of i, B[j] = double running sum
+// of the sub-block totals, so that C[i] = B[i / kSub] + c[i].  Ends with a block barrier.
+__device__ __forceinline__ void build_running_sum(const float* __restrict__ row, long long t0, long long avail,
+                                                  float mu, int n_sub, int span, double* __restrict__ B,
+                                                  float* __restrict__ c) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const bool table_in_smem = n_w <= kTileWidthsMax;
-    if (table_in_smem) {
-        for (int k = threadIdx.x; k < n_w; k += kTileThreads) {
-            sw[k] = __ldg(widths + k);
-            ss[k] = __ldg(wscale + k) * inv;
-        }
-    }
-    const int32_t* __restrict__ wp = table_in_smem ? sw : widths;
-    const float* __restrict__ sp = table_in_smem ? ss : wscale;
-    const float post = table_in_smem ? 1.0f : inv;  // 1/sigma already folded into ss
-
     // phase 1: sub-block sums; samples beyond the row count as x = mu (never used by a valid window)
     for (int sb = warp; sb < n_sub; sb += kTileThreads / 32) {
         const int i = sb * kSub + 2 * lane;
@@ -240,6 +219,37 @@ __global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
         }
     }
     __syncthreads();
+}
+
+__global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
+    const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
+    const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, long long n_t, int tile,
+    int span, long long tiles_per_row, float* __restrict__ out_snr, int32_t* __restrict__ out_width) {
+    extern __shared__ __align__(16) unsigned char gsm[];
+    const int n_sub = span / kSub;  // span is a multiple of kSub
+    double* const B = reinterpret_cast<double*>(gsm);                        // [n_sub + 1] running sum of sub-block totals
+    float* const c = reinterpret_cast<float*>(gsm + (n_sub + 2) / 2 * 16);  // [span + 1] exclusive sum inside a sub-block
+    int32_t* const sw = reinterpret_cast<int32_t*>(c + (span + 4) / 4 * 4);   // [kTileWidthsMax] widths
+    float* const ss = reinterpret_cast<float*>(sw + kTileWidthsMax);          // [kTileWidthsMax] 1 / (sqrt(L) sigma)
+    const long long d = blockIdx.x / tiles_per_row;
+    const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
+    const float* __restrict__ row = plane + d * n_t;
+    const float mu = mean[d];
+    const float inv = 1.0f / sigma[d];
+    const long long avail = n_t - t0;  // samples of the row from t0 on
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool table_in_smem = n_w <= kTileWidthsMax;
+    if (table_in_smem) {
+        for (int k = threadIdx.x; k < n_w; k += kTileThreads) {
+            sw[k] = __ldg(widths + k);
+            ss[k] = __ldg(wscale + k) * inv;
+        }
+    }
+    const int32_t* __restrict__ wp = table_in_smem ? sw : widths;
+    const float* __restrict__ sp = table_in_smem ? ss : wscale;
+    const float post = table_in_smem ? 1.0f : inv;  // 1/sigma already folded into ss
+
+    build_running_sum(row, t0, avail, mu, n_sub, span, B, c);
     // phase 3: every width of every sample of the tile.  C[i] = B[i / kSub] + c[i].
     const int n_out = static_cast<int>(min(static_cast<long long>(tile), avail));
     const int max_w = __ldg(widths + n_w - 1);
@@ -280,6 +290,86 @@ __global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
     }
 }
 
+// ---- per-width boxcar separation (the paper's decimated grids) ----
+// Width k is evaluated only at samples that are multiples of its separation L_s[k] = 2^shift
+// (BoxDIT iteration i: every D^(i)-th point, Alg. 1; DIT: width 2^i every 2^i,
+// Alg. 3; IGRID with P layers: 2^i / P); one merged plane
+// Y[n] = max over the widths whose grid contains n (reading A16).  Widths ascend and their
+// separations do not decrease, so the widths form groups of equal separation (the paper's
+// iterations).  The tile's running sum is built as in generic_tile_kernel; then the groups are
+// visited in turn, one thread per grid point of the group (equal work per thread: a group's
+// widths), the running best of a sample living in the output planes between groups.
+__global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
+    const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
+    const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, const GridGroups groups,
+    long long n_t, int tile, int span, long long tiles_per_row, float* __restrict__ out_snr,
+    int32_t* __restrict__ out_width) {
+    extern __shared__ __align__(16) unsigned char gsm[];
+    const int n_sub = span / kSub;
+    double* const B = reinterpret_cast<double*>(gsm);
+    float* const c = reinterpret_cast<float*>(gsm + (n_sub + 2) / 2 * 16);
+    int32_t* const sw = reinterpret_cast<int32_t*>(c + (span + 4) / 4 * 4);
+    float* const ss = reinterpret_cast<float*>(sw + kTileWidthsMax);
+    const long long d = blockIdx.x / tiles_per_row;
+    const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
+    const float* __restrict__ row = plane + d * n_t;
+    const float mu = mean[d];
+    const float inv = 1.0f / sigma[d];
+    const long long avail = n_t - t0;
+    for (int k = threadIdx.x; k < n_w; k += kTileThreads) {  // n_w <= kTileWidthsMax (checked at plan creation)
+        sw[k] = __ldg(widths + k);
+        ss[k] = __ldg(wscale + k) * inv;
+    }
+    build_running_sum(row, t0, avail, mu, n_sub, span, B, c);
+
+    const int n_out = static_cast<int>(min(static_cast<long long>(tile), avail));
+    float* const ysnr = out_snr + d * n_t + t0;
+    int32_t* const yidx = out_width + d * n_t + t0;
+    // samples on no grid at all keep -inf / -1; the first group overwrites the ones on its grid
+    const int first_shift = groups.shift[0];
+    if (first_shift > 0) {
+        for (int i = threadIdx.x; i < n_out; i += kTileThreads) {
+            if ((t0 + i) & ((1ll << first_shift) - 1)) {
+                ysnr[i] = __int_as_float(0xff800000);
+                yidx[i] = -1;
+            }
+        }
+    }
+    for (int g = 0; g < groups.n; ++g) {
+        const int sh = groups.shift[g];
+        const int kb = groups.kb[g], ke = groups.ke[g];
+        const long long step = 1ll << sh;
+        const int i0 = static_cast<int>((step - (t0 & (step - 1))) & (step - 1));  // first grid point of the tile
+        const int count = i0 < n_out ? static_cast<int>((n_out - i0 + step - 1) >> sh) : 0;
+        for (int item = threadIdx.x; item < count; item += kTileThreads) {
+            const int i = i0 + (item << sh);
+            const long long room = avail - i;
+            const float c0 = c[i];
+            const double b0 = B[i / kSub];
+            float best = __int_as_float(0xff800000);
+            int idx = -1;
+            if (g > 0) {  // written by an earlier group of this block (same thread block: visible after the barrier)
+                best = ysnr[i];
+                idx = yidx[i];
+            }
+            for (int k = kb; k < ke; ++k) {
+                const int L = sw[k];
+                if (L > room) break;  // valid windows only (reading A3); widths ascend
+                const int e = i + L;
+                const float x = static_cast<float>(B[e / kSub] - b0) + (c[e] - c0);
+                const float snr = x * ss[k];  // eq. (4) with eq. (5)
+                if (snr > best) {             // strict '>' in ascending width order
+                    best = snr;
+                    idx = k;
+                }
+            }
+            ysnr[i] = best;
+            yidx[i] = idx;
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
 
 int generic_configure(spd_plan* plan) {
@@ -304,7 +394,14 @@ int generic_configure(spd_plan* plan) {
     // ---- tile kernel: no workspace -------------------------------------------------------
     const int64_t M = plan->max_width;
     plan->generic_tile = 0;
-    if (M - 1 + 4096 <= kTileSpanMax && !std::getenv("SPD_GENERIC_WORKSPACE")) {
+    const bool is_grid = !plan->separations.empty();
+    if (is_grid && (M - 1 + 4096 > kTileSpanMax || n_w > kTileWidthsMax)) {
+        set_error("a plan with boxcar separations needs max_width <= %d and at most %d widths",
+                  kTileSpanMax - 4095, kTileWidthsMax);
+        generic_release(plan);
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (M - 1 + 4096 <= kTileSpanMax && (is_grid || !std::getenv("SPD_GENERIC_WORKSPACE"))) {
         const int64_t tile_max = (kTileSpanMax - (M - 1)) / kSub * kSub;
         // enough tiles to fill the machine, but none so short that its look-ahead dominates
         const int64_t tiles_wanted = std::max<int64_t>(1, (2 * plan->sm_count + plan->n_dm - 1) / plan->n_dm);
@@ -322,8 +419,10 @@ int generic_configure(spd_plan* plan) {
             generic_release(plan);
             return SPD_ERR_INVALID_ARG;
         }
-        e = cudaFuncSetAttribute(generic_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 static_cast<int>(plan->generic_smem));
+        e = is_grid ? cudaFuncSetAttribute(grid_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           static_cast<int>(plan->generic_smem))
+                    : cudaFuncSetAttribute(generic_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           static_cast<int>(plan->generic_smem));
         if (e != cudaSuccess) {
             generic_release(plan);
             return cuda_fail(e, "configuring the any-width-set tile kernel");
@@ -367,6 +466,15 @@ void generic_release(spd_plan* plan) {
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                 float* out_snr, int32_t* out_width, cudaStream_t stream) {
     const long long n_t = plan->n_t;
+    if (!plan->separations.empty()) {
+        grid_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads, plan->generic_smem,
+                           stream>>>(plane, mean, sigma, plan->d_widths, plan->d_wscale,
+                                     static_cast<int>(plan->widths.size()), plan->grid, n_t, plan->generic_tile,
+                                     plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "launching the boxcar-separation tile kernel");
+        return SPD_OK;
+    }
     if (plan->generic_tile > 0) {
         generic_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads,
                               plan->generic_smem, stream>>>(

@@ -31,6 +31,15 @@ struct TreeConfig {
     size_t smem_bytes = 0;
 };
 
+// Per-width boxcar separation (spd_plan_create_grid): consecutive widths of equal separation.
+constexpr int kGridGroupsMax = 32;
+struct GridGroups {
+    int n;
+    int shift[kGridGroupsMax];  // log2 of the group's separation
+    int kb[kGridGroupsMax];     // first width of the group
+    int ke[kGridGroupsMax];     // one past its last width
+};
+
 struct HostStaging {
     bool ready = false;
     int64_t rows_per_block = 0;
@@ -59,6 +68,8 @@ struct spd_plan {
     double* d_prefix = nullptr;    // [n_dm][n_t + 1] running sums of (x - mu)
     double* d_blocksum = nullptr;  // [n_dm][blocks_per_row]
     int64_t generic_blocks_per_row = 0;
+    std::vector<int32_t> separations;  // empty, or one power of two per width (grid plans)
+    spd::GridGroups grid = {};
     int generic_tile = 0;  // > 0: tile kernel (time samples per block); 0: workspace kernels
     int generic_span = 0;  // tile + look-ahead, multiple of 64
     size_t generic_smem = 0;

@@ -63,6 +63,28 @@ def test_width_set_generators_match_paper_examples(spd, paper_pins):
         assert list(spd.spd_width_set_generate(kind, param, mw)) == formulas.width_set(kind, param, mw)
 
 
+def test_separation_generator_matches_formula_module_and_paper_example(spd):
+    """Host logic of spd_separation_generate (no device needed): PAPER.md:201 (L_max = 4: widths
+    1..4 at every point, 6..12 at every second point), Alg. 3 (width 2^i every 2^i), P layers."""
+    from oracle import formulas as F
+    w = spd.spd_width_set_generate("BOXDIT", 4, 28)
+    assert list(spd.spd_separation_generate("BOXDIT", 4, w)) == [1, 1, 1, 1, 2, 2, 2, 2, 4, 4, 4, 4]
+    for l_max in (8, 16, 32):
+        w = spd.spd_width_set_generate("BOXDIT", l_max, 8192)
+        sep = F.boxdit_separation(l_max)
+        assert list(spd.spd_separation_generate("BOXDIT", l_max, w)) == [sep(int(L)) for L in w]
+    w = spd.spd_width_set_generate("POW2", 0, 8192)
+    assert list(spd.spd_separation_generate("DIT", 0, w)) == list(w)
+    for depth, layers in ((1, 4), (2, 8), (3, 16)):
+        w = spd.spd_width_set_generate("IGRID", depth, 8192)
+        sep = F.igrid_separation(layers)
+        assert list(spd.spd_separation_generate("IGRID", layers, w)) == [sep(int(L)) for L in w]
+    assert list(spd.spd_separation_generate("EVERY_SAMPLE", 0, [1, 5, 9])) == [1, 1, 1]
+    for bad in (("DIT", 0, [3]), ("BOXDIT", 0, [1]), ("IGRID", 3, [4]), (9, 0, [1])):
+        with pytest.raises(spd.SpdError):
+            spd.spd_separation_generate(*bad)
+
+
 def test_width_set_generator_errors(spd):
     for kind, param, mw in [(99, 0, 8), ("BOXDIT", 0, 8), ("GEOMETRIC", 1000, 8), ("POW2", 0, 0), ("IGRID", -1, 8)]:
         with pytest.raises(spd.SpdError) as e:

@@ -643,3 +643,116 @@ def test_invalid_arguments_fail_loudly(spd):
     with pytest.raises(spd.SpdError):
         spd.spd_width_set_generate(99, 0, 8)
     assert "unknown" in spd.spd_last_error_string()
+
+
+# --- row f2: per-width boxcar separation (the paper's decimated grids), spd_plan_create_grid ----
+
+def run_gpu_grid(spd, x, mu, sg, widths, seps, max_width=None):
+    n_dm, n_t = x.shape
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(dev)
+    mean = torch.from_numpy(np.broadcast_to(np.asarray(mu, dtype=np.float32), (n_dm,)).copy()).to(dev)
+    sigma = torch.from_numpy(np.broadcast_to(np.asarray(sg, dtype=np.float32), (n_dm,)).copy()).to(dev)
+    with spd.Plan(n_dm, n_t, widths, max_width, separations=seps) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GRID
+        snr, idx = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+        return snr.cpu().numpy(), idx.cpu().numpy(), dict(plan.info)
+
+
+GRIDS = [("BOXDIT", 8, "BOXDIT", 8), ("BOXDIT", 16, "BOXDIT", 16), ("BOXDIT", 32, "BOXDIT", 32),
+         ("POW2", 0, "DIT", 0), ("IGRID", 1, "IGRID", 4), ("IGRID", 2, "IGRID", 8), ("IGRID", 3, "IGRID", 16)]
+
+
+@pytest.mark.parametrize("wkind,wparam,gkind,gparam", GRIDS)
+def test_grid_plans_match_oracle(spd, oracle_lib, wkind, wparam, gkind, gparam):
+    """The paper's BoxDIT / DIT / IGRID grids on noise + pulses: several
+    tiles, a ragged row length, pulses of widths between grid widths; the generators agree with
+    the formula module; a chosen width is always one whose grid contains the sample."""
+    from oracle import formulas as F
+    M = 600
+    widths = spd.spd_width_set_generate(wkind, wparam, M)
+    seps = spd.spd_separation_generate(gkind, gparam, widths)
+    sepf = {"BOXDIT": F.boxdit_separation(gparam) if gkind == "BOXDIT" else None, "DIT": (lambda L: L),
+            "IGRID": F.igrid_separation(gparam) if gkind == "IGRID" else None}[gkind]
+    assert [int(s) for s in seps] == [sepf(int(L)) for L in widths]
+    rng = np.random.default_rng(4242 + int(widths.size))
+    n_t = 11 * 1024 + 317
+    x = rng.standard_normal((3, n_t)).astype(np.float32)
+    for d, (t0, S) in enumerate([(1000, 23), (5003, 150), (n_t - 300, 290)]):
+        x[d, t0:t0 + S] += np.float32(14.0 / np.sqrt(S))
+    mu, sg = 0.25, 1.5
+    got_snr, got_idx, info = run_gpu_grid(spd, x + np.float32(mu), mu, sg, widths, seps, M)
+    mu64 = np.full(3, np.float32(mu), dtype=np.float64)
+    sg64 = np.full(3, np.float32(sg), dtype=np.float64)
+    xs = (x + np.float32(mu)).astype(np.float32)
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_grid(xs, mu64, sg64, widths, seps)
+    parity.assert_parity(oracle_lib, xs, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                         what=f"grid {gkind}:{gparam}")
+    n = np.arange(n_t)[None, :]
+    on = got_idx >= 0
+    assert np.all((n % np.asarray(seps)[np.where(on, got_idx, 0)] == 0) | ~on)
+
+
+@pytest.mark.parametrize("wkind,wparam,gkind,gparam", [("BOXDIT", 8, "BOXDIT", 8), ("IGRID", 1, "IGRID", 4),
+                                                       ("POW2", 0, "DIT", 0)])
+def test_grid_sliding_pulses_recover_the_paper_bounds(spd, wkind, wparam, gkind, gparam):
+    """a pulse slid over every shift; the best response per shift lies
+    between eq. (31) and eq. (24), its maximum equals eq. (24) and its minimum / mean equal the
+    shift scan of the formula module (itself pinned to the paper's printed losses)."""
+    from oracle import formulas as F
+    M = 120
+    widths = spd.spd_width_set_generate(wkind, wparam, M)
+    seps = spd.spd_separation_generate(gkind, gparam, widths)
+    sepd = {int(L): int(s) for L, s in zip(widths, seps)}
+    period = int(max(seps))
+    for S in (3, 9, 20, 33, 47, 100):
+        n_t = 4 * M + 2 * period + 2 * S
+        x = np.zeros((period, n_t), dtype=np.float32)
+        for s in range(period):
+            x[s, 2 * period + s: 2 * period + s + S] = np.float32(16.0 / np.sqrt(S))
+        got_snr, _, _ = run_gpu_grid(spd, x, 0.0, 1.0, widths, seps, M)
+        per_shift = got_snr.max(axis=1).astype(np.float64) / 16.0
+        lo, hi, mean = F.brute_force_response(S, [int(L) for L in widths], sepd)
+        assert abs(per_shift.min() - lo) < 1e-4 and abs(per_shift.max() - hi) < 1e-4
+        assert abs(per_shift.mean() - mean) < 1e-4
+        assert per_shift.min() >= F.rsnr_min(S, [int(L) for L in widths], sepd) - 1e-4
+        assert abs(per_shift.max() - F.rsnr_max(S, [int(L) for L in widths])) < 1e-4
+
+
+def test_grid_first_separation_above_one_and_flagged_candidates(spd, oracle_lib):
+    """Samples on no width's grid are -inf / -1; the flagged run and the candidate stage work on a grid plan."""
+    rng = np.random.default_rng(99)
+    n_t = 5000
+    x = rng.standard_normal((2, n_t)).astype(np.float32)
+    x[1, 2048:2048 + 64] += np.float32(2.0)
+    widths, seps = [4, 8, 16, 64], [2, 2, 4, 16]
+    got_snr, got_idx, _ = run_gpu_grid(spd, x, 0.0, 1.0, widths, seps, 64)
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_grid(x, 0.0, 1.0, widths, seps)
+    parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec, what="grid sep>1")
+    assert np.all(got_idx[:, 1::2] == -1) and np.all(np.isneginf(got_snr[:, 1::2]))
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(2, device=dev), torch.ones(2, device=dev)
+    with spd.Plan(2, n_t, widths, 64, separations=seps) as plan:
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 8.0)
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, 8.0, 4096)
+        torch.cuda.synchronize()
+        count, cands = spd.candidates_to_numpy(lst, n_found, 4096)
+    assert np.array_equal(snr.cpu().numpy(), got_snr)
+    ref_count = oracle_lib.find_candidates(got_snr, got_idx, 8.0)[0]
+    assert count == ref_count and count >= 1
+    assert np.any((cands["dm"] == 1) & (np.abs(cands["t"].astype(np.int64) - 2048) <= 64))
+
+
+def test_grid_invalid_arguments(spd):
+    with pytest.raises(spd.SpdError):
+        spd.Plan(1, 1000, [1, 2, 4], 4, separations=[1, 3, 4])       # not a power of two
+    with pytest.raises(spd.SpdError):
+        spd.Plan(1, 1000, [1, 2, 4], 4, separations=[2, 1, 4])       # decreasing
+    with pytest.raises(spd.SpdError):
+        spd.Plan(1, 1000, [1, 4, 2], 4, separations=[1, 1, 1])       # widths not ascending
+    with pytest.raises(spd.SpdError):
+        spd.Plan(1, 100000, [1, 60000], 60000, separations=[1, 1])   # max_width beyond the tile kernel
+    with pytest.raises(spd.SpdError):
+        spd.spd_separation_generate("DIT", 0, [1, 2, 3])
