@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--n-dm", type=int, default=0, help="override the number of DM trials (debugging)")
     ap.add_argument("--width-set", default="", help="override the workload's width set, e.g. IGRID:1 "
                     "(widths 2^k and 3*2^m, the paper's IG(1) set) - not the BASELINE configuration")
+    ap.add_argument("--grid", default="", help="boxcar separation per width (SURVEY.md sec. 8(f2)): BOXDIT:<L_max>, "
+                    "DIT or IGRID:<layers>; the width set is then evaluated on the paper's decimated grid")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -93,6 +95,8 @@ def workload_config(w, widths, extra=None):
     }
     if extra:
         cfg.update(extra)
+    if cfg.get("grid"):
+        cfg["width_set"] = cfg["width_set"].replace("every sample", "on the grid below")
     return cfg
 
 
@@ -121,9 +125,11 @@ def oracle_sample_plan(w, widths, target_s):
     return x, rows, span, cores
 
 
-def time_oracle(w, widths, target_s, steps=1, warmup=0):
+def time_oracle(w, widths, target_s, steps=1, warmup=0, seps=None):
     import numpy as np
     import oracle
+    if seps is not None:
+        return time_oracle_grid(w, widths, seps, target_s, steps, warmup)
     x, rows, span, cores = oracle_sample_plan(w, widths, target_s / max(1, steps + warmup))
     times = []
     for i in range(warmup + steps):
@@ -143,6 +149,45 @@ def time_oracle(w, widths, target_s, steps=1, warmup=0):
             "prefix_value": prefix, "ms_per_step": 1e3 * sum(times) / len(times), "samples_per_step": n}
 
 
+def time_oracle_grid(w, widths, seps, target_s, steps, warmup):
+    """cpu_baseline / reference arm of a --grid run: oracle_spd_grid on a bounded sample."""
+    import oracle
+    from workloads import make_plane_numpy
+    oracle.build()
+    cores = oracle.num_threads()
+    n_t = min(w.n_t, 1 << 18)
+    rows = max(1, min(w.n_dm, cores))
+    x, _ = make_plane_numpy(w.scaled(rows, n_t, max(1, min(w.n_pulses, rows))))
+    cal = 4096
+    t = time.perf_counter()
+    oracle.spd_grid(x, 0.0, 1.0, widths, seps, 0, cal)
+    rate = rows * cal / max(time.perf_counter() - t, 1e-4)
+    span = int(min(n_t - w.max_width, max(cal, rate * target_s / max(1, steps + warmup) / rows))) // 4096 * 4096
+    times = []
+    for i in range(warmup + steps):
+        t = time.perf_counter()
+        oracle.spd_grid(x, 0.0, 1.0, widths, seps, 0, span)
+        if i >= warmup:
+            times.append(time.perf_counter() - t)
+    n = rows * span
+    return {"value": n * len(times) / sum(times), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"oracle_spd_grid (double, direct summation on the grid, OpenMP) on the first {span} samples of "
+                      f"{rows} rows of the same recipe ({n} samples per step)",
+            "ms_per_step": 1e3 * sum(times) / len(times), "samples_per_step": n}
+
+
+def grid_separations(args, widths):
+    """Separations of --grid from the oracle's formula module (CPU legs only)."""
+    if not args.grid:
+        return None
+    from oracle import formulas
+    kind, _, param = args.grid.partition(":")
+    kind, param = kind.upper(), int(param or 0)
+    sep = {"BOXDIT": lambda: formulas.boxdit_separation(param), "DIT": lambda: (lambda L: L),
+           "IGRID": lambda: formulas.igrid_separation(param)}[kind]()
+    return [sep(int(L)) for L in widths]
+
+
 def oracle_widths(w):
     from oracle import formulas
     return formulas.width_set(w.width_kind, w.width_param, w.max_width)
@@ -157,13 +202,15 @@ def run_reference(args):
     w = apply_overrides(get_workload(args.workload), args)
     widths = oracle_widths(w)
     # bounded: the whole --steps/--warmup run is sized to about 4 * cpu_seconds
-    res = time_oracle(w, widths, 4.0 * args.cpu_seconds, steps=args.steps, warmup=args.warmup)
+    res = time_oracle(w, widths, 4.0 * args.cpu_seconds, steps=args.steps, warmup=args.warmup,
+                      seps=grid_separations(args, widths))
     line = {
         "impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT,
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(w, widths, {"sample_per_step": res["sample"]}),
+        "config": workload_config(w, widths, {"sample_per_step": res["sample"],
+                                              **({"grid": args.grid} if args.grid else {})}),
         "cpu_baseline": {"value": res["value"], "unit": UNIT, "cores": res["cores"], "kind": "oracle",
                          "sample": res["sample"]},
         "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -278,7 +325,11 @@ def run_b200(args):
     out_width = torch.empty((w.n_dm, w.n_t), dtype=torch.int32, device=dev)
     thr = w.candidate_threshold if w.candidate_threshold is not None else 6.0
     cap = 1 << 22
-    plan = spd.Plan(w.n_dm, w.n_t, widths, w.max_width)
+    seps = None
+    if args.grid:
+        gkind, _, gparam = args.grid.partition(":")
+        seps = spd.spd_separation_generate(gkind, int(gparam or 0), widths)
+    plan = spd.Plan(w.n_dm, w.n_t, widths, w.max_width, separations=seps)
     info = plan.info
     # Per-DM mu, sigma: supplied (0, 1) by the config, or measured (reading A6) by spd_row_stats.
     # The step before the hot path: timed on its own, outside the step.
@@ -361,7 +412,8 @@ def run_b200(args):
     achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_ws_kernel" if info["tree_kernel"] == 2 else "spd_tree_kernel",
-                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel"}.get(info["path"], "generic_tile_kernel"),
+                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel", spd.SPD_PATH_GRID: "grid_tile_kernel"}.get(
+                       info["path"], "generic_tile_kernel"),
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),
         "algorithmic_bytes_per_launch": BYTES_PER_SAMPLE * n, "bytes_per_sample": BYTES_PER_SAMPLE,
@@ -374,6 +426,8 @@ def run_b200(args):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": workload_config(w, widths, {
+            **({"grid": args.grid + " (a boxcar separation per width: widths of later iterations only at "
+                                    "every 2^i-th sample; one merged plane)"} if args.grid else {}),
             "parallelism": f"dm-rows x{world} (independent DM trials per GPU, no collective)",
             "path": {spd.SPD_PATH_DYADIC_TREE: "dyadic_tree", spd.SPD_PATH_IGRID_TREE: "igrid_tree"}.get(
                 info["path"], "generic"),
@@ -403,8 +457,8 @@ def run_b200(args):
 
     # ---- CPU oracle on the same box (rank 0, N=1 only) ----------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        res = time_oracle(w, oracle_widths(w), args.cpu_seconds)
-        line["cpu_baseline"] = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample", "prefix_value")}
+        res = time_oracle(w, oracle_widths(w), args.cpu_seconds, seps=grid_separations(args, oracle_widths(w)))
+        line["cpu_baseline"] = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample", "prefix_value") if k in res}
     else:
         line["cpu_baseline"] = None
 
@@ -455,7 +509,11 @@ def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
     h_width = torch.empty((rows, w.n_t), dtype=torch.int32, pin_memory=True)
     torch.cuda.synchronize()
     times = []
-    with spd.Plan(rows, w.n_t, widths, w.max_width) as plan:
+    seps = None
+    if args.grid:
+        gkind, _, gparam = args.grid.partition(":")
+        seps = spd.spd_separation_generate(gkind, int(gparam or 0), widths)
+    with spd.Plan(rows, w.n_t, widths, w.max_width, separations=seps) as plan:
         for i in range(1 + max(1, args.e2e_steps)):
             if distributed:
                 torch.distributed.barrier()

@@ -252,3 +252,53 @@ def test_longest_row(spd, oracle_lib, kind, param):
     for t0 in (5, (1 << 30) - 1500, n_t - 40000, n_t - 2500):
         assert bool(((cands["t"].astype(np.int64) - t0) ** 2 < 8192 ** 2).any()), t0
     assert count == len(cands) or count > (1 << 20)
+
+
+@pytest.mark.parametrize("wkind,wparam,gkind,gparam", [("BOXDIT", 8, "BOXDIT", 8), ("IGRID", 1, "IGRID", 4)])
+def test_full_size_config3_on_the_paper_grids(spd, oracle_lib, wkind, wparam, gkind, gparam):
+    """Row f2 at BASELINE's config-3 size, in the configuration `bench.py --grid` times: sampled
+    windows (injected pulses, row starts and tails, tile boundaries, random) against
+    oracle_spd_grid, and whole-plane properties that hold at any size."""
+    from dataclasses import replace
+    from workloads import get_workload, make_plane_torch
+    w = replace(get_workload(3), width_kind=wkind, width_param=wparam)
+    dev = torch.device("cuda:0")
+    free, _ = torch.cuda.mem_get_info(dev)
+    if free < 13 * w.n_samples + (6 << 30):
+        pytest.skip("not enough device memory")
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    seps = spd.spd_separation_generate(gkind, gparam, widths)
+    plane, pulses = make_plane_torch(w, dev)
+    mean, sigma = torch.zeros(w.n_dm, device=dev), torch.ones(w.n_dm, device=dev)
+    with spd.Plan(w.n_dm, w.n_t, widths, w.max_width, separations=seps) as plan:
+        info = dict(plan.info)
+        assert info["path"] == spd.SPD_PATH_GRID
+        snr, idx = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    tile, M, n_t = info["chunk"], w.max_width, w.n_t
+    rng = np.random.default_rng(w.seed + 23)
+    span = 768
+    wins = [(p.dm, max(0, p.t0 - span // 2)) for p in pulses[:: max(1, len(pulses) // 10)]]
+    wins += [(0, 0), (w.n_dm - 1, n_t - span), (7, n_t - M - span // 2)]
+    wins += [(int(rng.integers(0, w.n_dm)), int(rng.integers(1, n_t // tile)) * tile - span // 2) for _ in range(3)]
+    wins += [(int(rng.integers(0, w.n_dm)), int(rng.integers(0, n_t - span))) for _ in range(4)]
+    worst = 0.0
+    for row, t0 in wins:
+        t0 = t0 // 8192 * 8192 if t0 % 2 else t0          # keep a few windows on coarse grid points
+        t1 = min(n_t, t0 + span)
+        # the row up to t1 + M: every window of a sample < t1 ends inside it, or at the row's real end
+        seg = plane[row, : min(n_t, t1 + M)].cpu().numpy()[None, :]
+        ref_snr, ref_idx, ref_sec = oracle_lib.spd_grid(seg, 0.0, 1.0, widths, seps, t0, t1)
+        st = parity.assert_parity(oracle_lib, seg, 0.0, 1.0, widths, snr[row, t0:t1].cpu().numpy()[None, :],
+                                  idx[row, t0:t1].cpu().numpy()[None, :], ref_snr, ref_idx, ref_sec, t0=t0,
+                                  what=f"grid {gkind}:{gparam} row {row} t0 {t0}")
+        worst = max(worst, st.max_err_over_tol)
+    assert worst <= 1.0
+    # whole plane: finite, indices in range, width 1 is on every sample's grid, chosen widths on their grid
+    sp = torch.from_numpy(np.asarray(seps)).to(dev)
+    n = torch.arange(n_t, device=dev)
+    for r0 in range(0, w.n_dm, 64):
+        y, k = snr[r0:r0 + 64], idx[r0:r0 + 64]
+        assert bool(torch.isfinite(y).all()) and int(k.min()) >= 0 and int(k.max()) < len(widths)
+        assert bool((y >= plane[r0:r0 + 64] - 1e-4 * torch.clamp(plane[r0:r0 + 64].abs(), min=1.0)).all())
+        assert bool((n[None, :] % sp[k.long()] == 0).all())
