@@ -473,8 +473,8 @@ def run_b200(args):
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per sample of the dominant kernel from
 # the committed `ncu --set full` capture (taken on 1024 of the workload's DM trials: the kernel
 # streams rows independently, so traffic scales with the sample count); None where not captured.
-# profiles/r01d_tree_ws_kernel_full.md: 4.334169 + 8.536965 GB for 2^30 samples of the config-3 recipe.
-NCU_DRAM_BYTES_PER_SAMPLE = {3: (4.334169e9 + 8.536965e9) / float(1 << 30)}
+# profiles/r01d_tree_ws_kernel_full.md: 4.335046 + 8.536421 GB for 2^30 samples of the config-3 recipe.
+NCU_DRAM_BYTES_PER_SAMPLE = {3: (4.335046e9 + 8.536421e9) / float(1 << 30)}
 
 
 def ncu_traffic_bytes(w):
