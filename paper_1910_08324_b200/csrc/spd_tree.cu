@@ -101,6 +101,19 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
             // (the chunk loop is unrolled over the deepest FIFO); guarded steps keep the
             // FIFO in canonical order (slot 0 oldest) by moving registers.
             constexpr int Q = D / R;
+            if constexpr (tree_tmem(K)) {
+                // FIFO in tensor memory (K >= 15: the delay registers would otherwise cost 124 /
+                // 252 registers per thread): slot = step mod depth as a run-time column offset,
+                // one tcgen05.ld + tcgen05.st of R float4 per level.  Slots of the shallower FIFOs
+                // come first: Q - 1 of them.
+                static_assert(R == 4, "tensor-memory FIFOs move 4 float4 per level");
+                const uint32_t taddr = cx.tbase + 4u * R * static_cast<uint32_t>((Q - 1) + (cx.it & (Q - 1)));
+                float4 old[R];
+                tmem_ld16(taddr, old);
+                tmem_st16(taddr, P);
+#pragma unroll
+                for (int r = 0; r < R; ++r) now[r] = add4(P[r], old[r]);
+            } else {
             constexpr bool kSlotted = FAST && G::U >= Q;  // slot known at compile time
             constexpr int slot = kSlotted ? (PH % Q) : 0;
 #pragma unroll
@@ -116,6 +129,7 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
                 }
 #pragma unroll
                 for (int r = 0; r < R; ++r) dl[off + (Q - 1) * R + r] = P[r];
+            }
             }
         }
 #pragma unroll
@@ -217,6 +231,7 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
             }
         }
     }
+    if constexpr (tree_tmem(K)) tmem_wait_st();
     // With no exchange level there is no barrier inside the step: add the one that
     // orders this step's stage reads before the next refill of the stage.
     if constexpr (G::LAST < 4) __syncthreads();
@@ -238,14 +253,27 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
 #ifndef SPD_TREE_BPS
 #define SPD_TREE_BPS 3
 #endif
-constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? 128 : 512); }
-constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : (K == 15 ? 4 : 2); }
-constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 15 ? 2 : 1); }
+constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : 128; }
+constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : 4; }
+#ifndef SPD_TREE_BPS15
+#define SPD_TREE_BPS15 4
+#endif
+constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 15 ? SPD_TREE_BPS15 : 2); }
+// Tensor-memory columns a block allocates for its FIFOs (K >= 15): 4 R columns per FIFO slot,
+// 2^JF - 1 slots, rounded up to a power of two.
+template <int T, int R, int K>
+constexpr int tree_tmem_cols() {
+    using G = Geo<T, R, K>;
+    constexpr int LR = ilog2(R);
+    constexpr int JF = G::J > LR ? G::J - LR : 0;
+    constexpr int need = 4 * R * ((1 << JF) - 1);
+    return need <= 32 ? 32 : need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
+}
 
 template <int T, int R, int K>
 constexpr size_t tree_smem_bytes() {
     constexpr size_t C = 4 * T * R;
-    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8;
+    return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8 + 16;
 }
 
 template <int T, int R, int K>
@@ -259,6 +287,8 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     float* const stages = reinterpret_cast<float*>(smem_raw + 2 * C * 4);
     float4* const halo = reinterpret_cast<float4*>(stages + kStages * (C + 8));
     uint64_t* const bars = reinterpret_cast<uint64_t*>(halo + 2 * T);
+    uint32_t* const tslot = reinterpret_cast<uint32_t*>(bars + kStages);
+    constexpr int kTmemCols = tree_tmem_cols<T, R, K>();
 
     const int tid = threadIdx.x;
     const int d = blockIdx.x / p.segs_per_row;
@@ -301,7 +331,22 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
 #pragma unroll
     for (int i = 0; i < G::ND + 1; ++i) dl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     int xsel = 0, hsel = 0;
-    __syncthreads();
+    cx.tbase = 0;
+    cx.it = 0;
+    if constexpr (tree_tmem(K)) {
+        if (tid < 32) tmem_alloc<kTmemCols>(tslot);
+        tmem_fence_before_sync();
+        __syncthreads();
+        tmem_fence_after_sync();
+        cx.tbase = *tslot + (static_cast<uint32_t>((tid >> 5) & 3) << 21);  // this warp's lane quarter
+        const float4 zero[4] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f),
+                                make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
+#pragma unroll
+        for (int col = 0; col < kTmemCols; col += 16) tmem_st16(cx.tbase + col, zero);
+        tmem_wait_st();
+    } else {
+        __syncthreads();
+    }
 
     // ---- guarded steps: warm-up chunks of an interior segment, then the row tail -----
     for (int c = c_top - 1; c >= first_fast; --c) {
@@ -316,12 +361,13 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
         const float top = tree_chunk<T, R, K, false, 0>(reinterpret_cast<const float4*>(stages), pp, halo, xsel,
                                                         hsel, dl, cx);
         if (act && cx.do_out && top >= thr_key) act[c] = 1;
+        ++cx.it;
         __syncthreads();
     }
 
     // ---- unguarded steps: bulk-copy ring ----------------------------------------------
     const int n_fast = first_fast - c_lo;
-    if (n_fast <= 0) return;
+    if (n_fast > 0) {
     fence_proxy_async();
     __syncthreads();
     constexpr uint32_t kBytes = (C + 8) * 4;
@@ -340,7 +386,8 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     cx.do_out = true;
     int it = 0;
     while (it < n_fast) {
-        static_phases<0, G::U>([&](auto ph) {
+        // tensor-memory FIFOs take their slot at run time: two steps per trip only to overlap them
+        static_phases<0, (tree_tmem(K) ? 2 : G::U)>([&](auto ph) {
             if (it < n_fast) {
                 if (tid == 0) {
                     const int nx = it + kStages - 1;
@@ -362,8 +409,15 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
                     phase ^= 1;
                 }
                 ++it;
+                ++cx.it;
             }
         });
+    }
+    }
+    if constexpr (tree_tmem(K)) {
+        tmem_fence_before_sync();
+        __syncthreads();
+        if (tid < 32) tmem_dealloc<kTmemCols>(*tslot);
     }
 }
 
@@ -383,6 +437,19 @@ cudaError_t prepare_tree(TreeConfig& cfg) {
     int nb = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, R, K>, T, cfg.smem_bytes);
     if (e != cudaSuccess) return e;
+    if constexpr (tree_tmem(K)) {
+        // no more resident blocks than tensor memory has columns for (a block that cannot
+        // allocate would spin): pad the shared-memory request until the occupancy fits
+        const int max_blocks = 512 / tree_tmem_cols<T, R, K>();
+        while (nb > max_blocks && cfg.smem_bytes < (200u << 10)) {
+            cfg.smem_bytes += 4096;
+            e = cudaFuncSetAttribute(spd_tree_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     static_cast<int>(cfg.smem_bytes));
+            if (e != cudaSuccess) return e;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, R, K>, T, cfg.smem_bytes);
+            if (e != cudaSuccess) return e;
+        }
+    }
     cfg.blocks_per_sm = nb;
     return cudaSuccess;
 }

@@ -79,87 +79,6 @@ struct WsGeo {
     static constexpr int COLS = 4 * kWsRows * Q0 * ((1 << JF) - 1);  // TMEM columns per warp
 };
 
-// ---- tensor memory as per-lane scratch ---------------------------------------------------
-__device__ __forceinline__ void tmem_alloc512(uint32_t* slot) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(slot))
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc512(uint32_t base) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
-}
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-
-// 8 float4 per lane <- 32 consecutive columns of the warp's lanes; complete on return.
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float4 (&v)[8]) {
-    uint32_t r[32];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
-        "tcgen05.wait::ld.sync.aligned;"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr)
-        : "memory");
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-        v[i] = make_float4(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1]), __uint_as_float(r[4 * i + 2]),
-                           __uint_as_float(r[4 * i + 3]));
-}
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float4 (&v)[8]) {
-    uint32_t r[32];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        r[4 * i] = __float_as_uint(v[i].x);
-        r[4 * i + 1] = __float_as_uint(v[i].y);
-        r[4 * i + 2] = __float_as_uint(v[i].z);
-        r[4 * i + 3] = __float_as_uint(v[i].w);
-    }
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
-        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
-        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
-
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float4 (&v)[4]) {
-    uint32_t r[16];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
-        "tcgen05.wait::ld.sync.aligned;"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-        v[i] = make_float4(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1]), __uint_as_float(r[4 * i + 2]),
-                           __uint_as_float(r[4 * i + 3]));
-}
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const float4 (&v)[4]) {
-    uint32_t r[16];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        r[4 * i] = __float_as_uint(v[i].x);
-        r[4 * i + 1] = __float_as_uint(v[i].y);
-        r[4 * i + 2] = __float_as_uint(v[i].z);
-        r[4 * i + 3] = __float_as_uint(v[i].w);
-    }
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-        : "memory");
-}
 // One level's rows of a step (kWsRows float4 per lane) <-> 4 * kWsRows columns.
 __device__ __forceinline__ void tmem_ld_rows(uint32_t taddr, float4 (&v)[kWsRows]) {
     if constexpr (kWsRows == 8) {
@@ -380,10 +299,10 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
     }
     uint32_t tbase = 0;
     if constexpr (G::COLS > 0) {
-        if (warp == 0) tmem_alloc512(tslot);
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        if (warp == 0) tmem_alloc<512>(tslot);
+        tmem_fence_before_sync();
         __syncthreads();
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tmem_fence_after_sync();
         // this warp's lane quarter, and its half of the columns
         tbase = *tslot + (static_cast<uint32_t>(warp & 3) << 21) + static_cast<uint32_t>(warp >> 2) * 256u;
     } else {
@@ -540,9 +459,9 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
     }
 
     if constexpr (G::COLS > 0) {
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        tmem_fence_before_sync();
         __syncthreads();
-        if (warp == 0) tmem_dealloc512(*tslot);
+        if (warp == 0) tmem_dealloc<512>(*tslot);
     }
 }
 
