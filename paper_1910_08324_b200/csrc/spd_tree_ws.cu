@@ -70,8 +70,8 @@ struct WsGeo {
     static constexpr int LAST = K - 1;
     // row levels j = 0 .. J-1: partner 2^j rows later, level 7+j -> level 8+j
     static constexpr int J = imax(0, LAST - 7);
-    // partner inside this or the previous step (2^j <= kNearMax rows): registers
-    static constexpr int JNMAX = kWsRows == 8 ? 3 : 3;  // R = 8: 1, 2, 4 rows; R = 4: 1, 2, 4 (= one step)
+    // partner 1, 2 or 4 rows later: inside this step or the previous one (R = 4: 4 rows = one step back): registers
+    static constexpr int JNMAX = 3;
     static constexpr int JN = J < JNMAX ? J : JNMAX;
     static constexpr int NEAR = (1 << JN) - 1;  // float4 kept from the previous step
     static constexpr int JF = J - JN;           // FIFO levels i < JF: partner Q0 * 2^i steps back
@@ -95,10 +95,6 @@ __device__ __forceinline__ void tmem_st_rows(uint32_t taddr, const float4 (&v)[k
     }
 }
 
-__device__ __forceinline__ float4 shfl4(float4 v, int src) {
-    return make_float4(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src),
-                       __shfl_sync(0xffffffffu, v.z, src), __shfl_sync(0xffffffffu, v.w, src));
-}
 
 // Lane levels k = 3 .. 6: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner 2^k / 4 lanes later; the
 // lanes that run off a row continue in the next row, the last row in the first row of the
@@ -111,6 +107,12 @@ __device__ __forceinline__ float4 shfl4(float4 v, int src) {
 #define SPD_WS_XCHG 1
 #endif
 constexpr int kWsXBuf = (kWsRows + 1) * 32;  // float4 per exchange buffer: R rows + the kept row
+#if !SPD_WS_XCHG
+__device__ __forceinline__ float4 shfl4(float4 v, int src) {
+    return make_float4(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src),
+                       __shfl_sync(0xffffffffu, v.z, src), __shfl_sync(0xffffffffu, v.w, src));
+}
+#endif
 
 // Step modes: 0 = guarded (row tail: windows checked against the end of the row, output if
 // cx.do_out), 1 = interior step with output, 2 = interior look-ahead step (sums only).
