@@ -756,3 +756,45 @@ def test_grid_invalid_arguments(spd):
         spd.Plan(1, 100000, [1, 60000], 60000, separations=[1, 1])   # max_width beyond the tile kernel
     with pytest.raises(spd.SpdError):
         spd.spd_separation_generate("DIT", 0, [1, 2, 3])
+
+
+# --- the two dyadic-tree kernels: warp-per-stream pieces spanning rows, and the A/B hook -------------
+
+@pytest.mark.parametrize("K", [9, 10, 11, 12, 13, 14])
+def test_warp_stream_kernel_pieces_span_rows(spd, oracle_lib, K):
+    """Default work split of the warp-per-stream kernel: the plane's steps cut in row-major order into
+    pieces that start and stop inside rows (each interior stop replays look-ahead), many short rows with a
+    ragged tail, pulses across row ends.  Checked on every sample against the oracle."""
+    M = 1 << (K - 1)
+    n_dm = 37 if K <= 12 else 11
+    n_t = max(512 * 23 + 4 * 5, 3 * M + 512 + 4 * 3)
+    rng = np.random.default_rng(500 + K)
+    x = rng.standard_normal((n_dm, n_t)).astype(np.float32)
+    x[1, n_t // 2: n_t // 2 + M // 2] += np.float32(12.0 / np.sqrt(M // 2))
+    x[n_dm - 1, n_t - M // 3:] += np.float32(0.9)
+    x[0, :7] += np.float32(4.0)
+    got_snr, got_idx, info = run_gpu(spd, x, 0.0, 1.0, [1 << k for k in range(K)])
+    assert info["tree_kernel"] == 2 and info["piece_chunks"] > 0 and info["segments_per_row"] == 0
+    chunks_per_row = (n_t + info["chunk"] - 1) // info["chunk"]
+    assert info["piece_chunks"] % chunks_per_row != 0, "pieces were meant to stop inside rows"
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_prefix(x, 0.0, 1.0, [1 << k for k in range(K)])
+    parity.assert_parity(oracle_lib, x, 0.0, 1.0, [1 << k for k in range(K)], got_snr, got_idx, ref_snr, ref_idx,
+                         ref_sec, what=f"warp-stream K={K}")
+
+
+@pytest.mark.parametrize("K", [9, 14])
+def test_block_and_warp_kernels_agree(spd, oracle_lib, K, monkeypatch):
+    """SPD_TREE_KERNEL=block keeps the block-per-stream kernel: both kernels pass parity on the same plane, and
+    their SNR planes differ by no more than the tag perturbation (31 ulp)."""
+    rng = np.random.default_rng(77 + K)
+    n_t = 512 * 40 + 12
+    x = rng.standard_normal((4, n_t)).astype(np.float32)
+    widths = [1 << k for k in range(K)]
+    a_snr, a_idx, a_info = run_gpu(spd, x, 0.0, 1.0, widths)
+    monkeypatch.setenv("SPD_TREE_KERNEL", "block")
+    b_snr, b_idx, b_info = run_gpu(spd, x, 0.0, 1.0, widths)
+    assert a_info["tree_kernel"] == 2 and b_info["tree_kernel"] == 1
+    ref = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    for snr, idx, name in ((a_snr, a_idx, "warp"), (b_snr, b_idx, "block")):
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, snr, idx, *ref, what=f"{name} K={K}")
+    assert np.all(np.abs(a_snr - b_snr) <= 64 * np.spacing(np.abs(b_snr)) + 1e-30)
