@@ -174,25 +174,41 @@ __device__ __forceinline__ void build_running_sum(const float* __restrict__ row,
                                                   float mu, int n_sub, int span, double* __restrict__ B,
                                                   float* __restrict__ c) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // phase 1: sub-block sums; samples beyond the row count as x = mu (never used by a valid window)
-    for (int sb = warp; sb < n_sub; sb += kTileThreads / 32) {
-        const int i = sb * kSub + 2 * lane;
-        const float x0 = i < avail ? __ldg(row + t0 + i) - mu : 0.f;
-        const float x1 = i + 1 < avail ? __ldg(row + t0 + i + 1) - mu : 0.f;
-        const float s = x0 + x1;
-        float incl = s;
+    // phase 1: sub-block sums; samples beyond the row count as x = mu (never used by a valid window).
+    // A warp takes every 32nd sub-block; the loads of kAhead of them are issued before the first
+    // is scanned, so that a tile pays a few memory latencies instead of one per sub-block.
+    constexpr int kAhead = 4;
+    constexpr int kWarps = kTileThreads / 32;
+    for (int sb0 = warp; sb0 < n_sub; sb0 += kAhead * kWarps) {
+        float2 raw[kAhead];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const float u = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += u;
+        for (int u = 0; u < kAhead; ++u) {
+            const int i = (sb0 + u * kWarps) * kSub + 2 * lane;
+            raw[u].x = (sb0 + u * kWarps < n_sub && i < avail) ? __ldg(row + t0 + i) : mu;
+            raw[u].y = (sb0 + u * kWarps < n_sub && i + 1 < avail) ? __ldg(row + t0 + i + 1) : mu;
         }
-        c[i] = incl - s;
-        c[i + 1] = incl - s + x0;
-        // sub-block total in double (pairwise over the lanes)
-        double tot = static_cast<double>(x0) + static_cast<double>(x1);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-        if (lane == 0) B[sb + 1] = tot;
+        for (int u = 0; u < kAhead; ++u) {
+            const int sb = sb0 + u * kWarps;
+            if (sb >= n_sub) break;
+            const int i = sb * kSub + 2 * lane;
+            const float x0 = raw[u].x - mu;
+            const float x1 = raw[u].y - mu;
+            const float s = x0 + x1;
+            float incl = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const float v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            c[i] = incl - s;
+            c[i + 1] = incl - s + x0;
+            // sub-block total in double (pairwise over the lanes)
+            double tot = static_cast<double>(x0) + static_cast<double>(x1);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+            if (lane == 0) B[sb + 1] = tot;
+        }
     }
     __syncthreads();
     // phase 2: running sum of the totals (one warp, consecutive runs per lane)
@@ -298,7 +314,7 @@ __global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
 // separations do not decrease, so the widths form groups of equal separation (the paper's
 // iterations).  The tile's running sum is built as in generic_tile_kernel; then the groups are
 // visited in turn, one thread per grid point of the group (equal work per thread: a group's
-// widths), the running best of a sample living in the output planes between groups.
+// widths), the running best of every sample of the tile living in shared memory between groups.
 __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
     const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
     const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, const GridGroups groups,
@@ -323,18 +339,14 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
     build_running_sum(row, t0, avail, mu, n_sub, span, B, c);
 
     const int n_out = static_cast<int>(min(static_cast<long long>(tile), avail));
-    float* const ysnr = out_snr + d * n_t + t0;
-    int32_t* const yidx = out_width + d * n_t + t0;
-    // samples on no grid at all keep -inf / -1; the first group overwrites the ones on its grid
-    const int first_shift = groups.shift[0];
-    if (first_shift > 0) {
-        for (int i = threadIdx.x; i < n_out; i += kTileThreads) {
-            if ((t0 + i) & ((1ll << first_shift) - 1)) {
-                ysnr[i] = __int_as_float(0xff800000);
-                yidx[i] = -1;
-            }
-        }
+    // running best of every sample of the tile, in shared memory between the groups
+    float* const sbest = ss + kTileWidthsMax;                     // [tile]
+    int32_t* const sidx = reinterpret_cast<int32_t*>(sbest + tile);  // [tile]
+    for (int i = threadIdx.x; i < n_out; i += kTileThreads) {
+        sbest[i] = __int_as_float(0xff800000);  // samples on no grid at all keep -inf / -1
+        sidx[i] = -1;
     }
+    __syncthreads();
     for (int g = 0; g < groups.n; ++g) {
         const int sh = groups.shift[g];
         const int kb = groups.kb[g], ke = groups.ke[g];
@@ -346,12 +358,8 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
             const long long room = avail - i;
             const float c0 = c[i];
             const double b0 = B[i / kSub];
-            float best = __int_as_float(0xff800000);
-            int idx = -1;
-            if (g > 0) {  // written by an earlier group of this block (same thread block: visible after the barrier)
-                best = ysnr[i];
-                idx = yidx[i];
-            }
+            float best = sbest[i];
+            int idx = sidx[i];
             for (int k = kb; k < ke; ++k) {
                 const int L = sw[k];
                 if (L > room) break;  // valid windows only (reading A3); widths ascend
@@ -363,10 +371,16 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
                     idx = k;
                 }
             }
-            ysnr[i] = best;
-            yidx[i] = idx;
+            sbest[i] = best;
+            sidx[i] = idx;
         }
         __syncthreads();
+    }
+    float* const ysnr = out_snr + d * n_t + t0;
+    int32_t* const yidx = out_width + d * n_t + t0;
+    for (int i = threadIdx.x; i < n_out; i += kTileThreads) {
+        ysnr[i] = sbest[i];
+        yidx[i] = sidx[i];
     }
 }
 
@@ -402,7 +416,9 @@ int generic_configure(spd_plan* plan) {
         return SPD_ERR_INVALID_ARG;
     }
     if (M - 1 + 4096 <= kTileSpanMax && (is_grid || !std::getenv("SPD_GENERIC_WORKSPACE"))) {
-        const int64_t tile_max = (kTileSpanMax - (M - 1)) / kSub * kSub;
+        // a grid plan also keeps 8 bytes of running best per sample of the tile in shared memory
+        const int64_t tile_max = is_grid ? std::max<int64_t>(1024, ((200 << 10) - 4 * M) / 12 / 1024 * 1024)
+                                         : (kTileSpanMax - (M - 1)) / kSub * kSub;
         // enough tiles to fill the machine, but none so short that its look-ahead dominates
         const int64_t tiles_wanted = std::max<int64_t>(1, (2 * plan->sm_count + plan->n_dm - 1) / plan->n_dm);
         int64_t tile = ((plan->n_t + tiles_wanted - 1) / tiles_wanted + 1023) / 1024 * 1024;
@@ -412,7 +428,8 @@ int generic_configure(spd_plan* plan) {
         const int64_t n_sub = span / kSub;
         plan->generic_tile = static_cast<int>(tile);
         plan->generic_span = static_cast<int>(span);
-        plan->generic_smem = static_cast<size_t>((n_sub + 2) / 2 * 16 + (span + 4) / 4 * 16 + kTileWidthsMax * 8);
+        plan->generic_smem = static_cast<size_t>((n_sub + 2) / 2 * 16 + (span + 4) / 4 * 16 + kTileWidthsMax * 8) +
+                             (is_grid ? static_cast<size_t>(tile) * 8 : 0);
         plan->generic_tiles_per_row = (plan->n_t + tile - 1) / tile;
         if (plan->n_dm * plan->generic_tiles_per_row > 0x7fffffffll) {
             set_error("plane too large for the generic path's 1-D grid");
