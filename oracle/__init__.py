@@ -14,6 +14,8 @@ from .core import (  # noqa: F401
     row_stats_clipped,
     snr_of_width,
     spd_direct,
+    spd_direct_sw,
+    width_sigma,
     spd_grid,
     spd_prefix,
 )

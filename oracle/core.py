@@ -43,6 +43,10 @@ def _load() -> ctypes.CDLL:
         lib.oracle_spd_direct.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
         lib.oracle_spd_grid.restype = None
         lib.oracle_spd_grid.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
+        lib.oracle_width_sigma.restype = None
+        lib.oracle_width_sigma.argtypes = [_vp, _i64, _i64, _vp, _i32, _vp]
+        lib.oracle_spd_direct_sw.restype = None
+        lib.oracle_spd_direct_sw.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
         lib.oracle_spd_prefix.restype = None
         lib.oracle_spd_prefix.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _vp, _vp, _vp]
         lib.oracle_snr_of_width.restype = None
@@ -119,6 +123,36 @@ def spd_grid(x, mean, sigma, widths, seps, t0: int = 0, t1: Optional[int] = None
     _load().oracle_spd_grid(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
                             w.ctypes.data, sp.ctypes.data, int(w.size), t0, t1,
                             snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
+
+
+def width_sigma(x, widths) -> np.ndarray:
+    """Standard deviation per width from power-of-two decimations, interpolated (reading A17):
+    float64 [n_dm, n_widths] for the ascending, de-duplicated width set."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    w = _widths(widths)
+    out = np.empty((n_dm, w.size), dtype=np.float64)
+    _load().oracle_width_sigma(x.ctypes.data, n_dm, n_t, w.ctypes.data, int(w.size), out.ctypes.data)
+    return out
+
+
+def spd_direct_sw(x, mean, sigma_w, widths, t0: int = 0, t1: Optional[int] = None
+                  ) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Direct summation with a standard deviation per (row, width): sigma_w is [n_dm, n_widths]."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    t1 = n_t if t1 is None else int(t1)
+    t0 = int(t0)
+    w = _widths(widths)
+    mu = _stats(mean, n_dm)
+    sw = np.ascontiguousarray(sigma_w, dtype=np.float64).reshape(n_dm, w.size)
+    snr = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    idx = np.empty((n_dm, t1 - t0), dtype=np.int32)
+    sec = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    _load().oracle_spd_direct_sw(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sw.ctypes.data,
+                                 w.ctypes.data, int(w.size), t0, t1,
+                                 snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
     return snr, idx, sec
 
 

@@ -29,6 +29,8 @@
  *                        oracle_spd_direct in tests (<= 1e-9).
  *   oracle_spd_grid    : oracle_spd_direct with a boxcar separation per width (the
  *                        paper's decimated grids, merged into one plane; reading A16).
+ *   oracle_width_sigma : standard deviation per width from power-of-two decimations,
+ *                        interpolated (reading A17); oracle_spd_direct_sw uses it.
  *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
  *   oracle_row_stats   : per-row mean and population standard deviation (reading A6).
  *   oracle_row_stats_clipped: mean / sigma with point-wise outlier rejection
@@ -129,6 +131,96 @@ void oracle_spd_grid(const float* x, int64_t n_dm, int64_t n_t,
                 for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
                 const double snr = (X - (double)L * mean[d]) / (sqrt((double)L) * sigma[d]); /* eq. (4),(5) */
                 if (snr > best) {                              /* strict '>' (A4) */
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * span + (n - t0);
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+    }
+}
+
+/* Standard deviation per boxcar width on real (non-white) data, PAPER.md:728:
+ * "we calculate values of the standard deviation only for time-series which are decimations of the
+ * input time-series in time, i.e. ... only for boxcar filters of width that are equal to a powers of
+ * two.  We then interpolate values of standard deviation for all intermediate boxcar widths."
+ * Reading A17: level j = the series of sums of 2^j consecutive samples, x^j[m] = sum_{i<2^j} x[2^j m + i],
+ * m < floor(n_t / 2^j) (eq. 13 with D = 2, without its shift); sigma_j = its population
+ * standard deviation; for 2^j <= L < 2^(j+1) sigma_L is linear in L between sigma_j and sigma_(j+1);
+ * above the last level with at least two elements it follows eq. (5)'s sqrt(L) from that level.
+ * out_sigma_w is [n_dm][n_w].  Pins: numpy on hand-decimated rows, eq. (5) on white noise, the
+ * textbook variance of block sums of an AR(1) process, exact interpolation midpoints. */
+void oracle_width_sigma(const float* x, int64_t n_dm, int64_t n_t,
+                        const int32_t* widths, int32_t n_w, double* out_sigma_w) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float* row = x + d * n_t;
+        double sig[40];
+        int n_lev = 0;
+        for (int j = 0; j < 40; ++j) {
+            const int64_t blk = (int64_t)1 << j;
+            const int64_t cnt = n_t / blk;
+            if (cnt < 2) break;
+            double s1 = 0.0;
+            for (int64_t m = 0; m < cnt; ++m) {
+                double v = 0.0;
+                for (int64_t i = 0; i < blk; ++i) v += (double)row[m * blk + i];
+                s1 += v;
+            }
+            const double mean = s1 / (double)cnt;
+            double s2 = 0.0;
+            for (int64_t m = 0; m < cnt; ++m) {
+                double v = 0.0;
+                for (int64_t i = 0; i < blk; ++i) v += (double)row[m * blk + i];
+                s2 += (v - mean) * (v - mean);
+            }
+            sig[j] = sqrt(s2 / (double)cnt);
+            n_lev = j + 1;
+        }
+        for (int32_t k = 0; k < n_w; ++k) {
+            const int64_t L = widths[k];
+            int j = 0;
+            while (((int64_t)2 << j) <= L) ++j;               /* 2^j <= L < 2^(j+1) */
+            double s;
+            if (j + 1 < n_lev) {
+                const double lo = (double)((int64_t)1 << j);
+                s = sig[j] + (sig[j + 1] - sig[j]) * ((double)L - lo) / lo;
+            } else {
+                const int jj = n_lev - 1;
+                s = sig[jj] * sqrt((double)L / (double)((int64_t)1 << jj));
+            }
+            out_sigma_w[d * n_w + k] = s;
+        }
+    }
+}
+
+/* oracle_spd_direct with a measured standard deviation per width:
+ * SNR_L[n] = (X_L[n] - L mu_d) / sigma_{d,L}   (eq. 4, with mu(X_L) = L mu of eq. 5). */
+void oracle_spd_direct_sw(const float* x, int64_t n_dm, int64_t n_t,
+                          const double* mean, const double* sigma_w,
+                          const int32_t* widths, int32_t n_w,
+                          int64_t t0, int64_t t1,
+                          double* out_snr, int32_t* out_width, double* out_second) {
+    const int64_t span = t1 - t0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 256)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        for (int64_t n = t0; n < t1; ++n) {
+            const float* row = x + d * n_t;
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = 0; k < n_w; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;
+                double X = 0.0;
+                for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];
+                const double snr = (X - (double)L * mean[d]) / sigma_w[d * n_w + k];
+                if (snr > best) {
                     second = best;
                     best = snr;
                     idx = k;

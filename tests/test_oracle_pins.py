@@ -480,3 +480,76 @@ def test_grid_with_unit_separations_is_direct(oracle_lib):
     a = oracle_lib.spd_direct(x, 0.1, 1.3, widths)
     b = oracle_lib.spd_grid(x, 0.1, 1.3, widths, [1] * len(widths))
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+# --- f1 (second half): standard deviation per width from decimations --------
+
+def test_width_sigma_is_numpy_on_hand_decimated_rows(oracle_lib):
+    """Powers of two: numpy std of reshape(-1, 2^j).sum(1); a tiny row by hand; intermediate widths
+    linear between the neighbouring powers of two; above the last level sqrt(L) from it (eq. 5)."""
+    x = np.arange(1, 9, dtype=np.float32)[None, :]                 # 1..8
+    sw = oracle_lib.width_sigma(x, [1, 2, 3, 4, 6, 8])
+    s1 = np.std(np.arange(1, 9))                                   # 2.2913
+    s2 = np.std([3, 7, 11, 15])                                    # sqrt(20)
+    s4 = np.std([10, 26])                                          # 8
+    assert sw[0, 0] == pytest.approx(s1) and sw[0, 1] == pytest.approx(math.sqrt(20.0))
+    assert sw[0, 3] == pytest.approx(8.0)
+    assert sw[0, 2] == pytest.approx(0.5 * (s2 + s4))              # L = 3: midway between 2 and 4
+    assert sw[0, 4] == pytest.approx(s4 * math.sqrt(6 / 4))        # no level 8 (one element): sqrt law from 4
+    assert sw[0, 5] == pytest.approx(s4 * math.sqrt(8 / 4))
+    rng = np.random.default_rng(3)
+    y = (rng.standard_normal((2, 4096 + 37)) * 2.5 + 7).astype(np.float32)
+    widths = [1, 2, 4, 5, 8, 16, 24, 64, 100, 256]
+    sw = oracle_lib.width_sigma(y, widths)
+    for d in range(2):
+        lev = {}
+        for j in range(10):
+            b = 1 << j
+            m = y.shape[1] // b
+            lev[b] = np.std(y[d, :m * b].astype(np.float64).reshape(m, b).sum(axis=1))
+        for k, L in enumerate(widths):
+            lo = 1 << (int(L).bit_length() - 1)
+            want = lev[lo] + (lev[2 * lo] - lev[lo]) * (L - lo) / lo
+            assert sw[d, k] == pytest.approx(want, rel=1e-12)
+
+
+def test_width_sigma_white_noise_follows_eq5_and_ar1_follows_the_textbook(oracle_lib):
+    """eq. (5): sigma_L = sqrt(L) sigma on white noise.  On an AR(1) series
+    x[n] = rho x[n-1] + e[n] the variance of a sum of L samples is
+    s^2 [L (1+rho)/(1-rho) - 2 rho (1 - rho^L)/(1-rho)^2] (textbook), i.e. NOT sqrt(L): the case the
+    paper's measured sigma is for (Fig. 24)."""
+    rng = np.random.default_rng(11)
+    n = 1 << 20
+    w = rng.standard_normal(n)
+    widths = [1, 2, 4, 8, 16, 32, 64]
+    sw = oracle_lib.width_sigma(w.astype(np.float32)[None, :], widths)[0]
+    for L, s in zip(widths, sw):
+        assert s == pytest.approx(math.sqrt(L), rel=4.0 * math.sqrt(L / (2.0 * n)) + 1e-3)
+    rho = 0.6
+    x = np.empty(n)
+    x[0] = w[0] / math.sqrt(1 - rho * rho)
+    for i in range(1, n):
+        x[i] = rho * x[i - 1] + w[i]
+    s2 = 1.0 / (1 - rho * rho)
+    sw = oracle_lib.width_sigma(x.astype(np.float32)[None, :], widths)[0]
+    for L, s in zip(widths, sw):
+        var = s2 * (L * (1 + rho) / (1 - rho) - 2 * rho * (1 - rho ** L) / (1 - rho) ** 2)
+        assert s == pytest.approx(math.sqrt(var), rel=0.02), L
+    assert sw[-1] > 1.5 * math.sqrt(64) * math.sqrt(s2) * 0.9      # far from the white-noise law
+
+
+def test_direct_with_white_noise_sigma_table_is_direct(oracle_lib):
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal((2, 400)).astype(np.float32)
+    widths = [1, 2, 3, 8, 20]
+    sg = np.array([1.5, 0.7])
+    table = sg[:, None] * np.sqrt(np.asarray(widths, dtype=np.float64))[None, :]
+    a = oracle_lib.spd_direct(x, [0.1, -0.2], sg, widths)
+    b = oracle_lib.spd_direct_sw(x, [0.1, -0.2], table, widths)
+    assert np.allclose(a[0], b[0], rtol=1e-13, atol=1e-13) and np.array_equal(a[1], b[1])
+    # halving one width's sigma doubles that width's SNR only
+    table2 = table.copy()
+    table2[:, 3] *= 0.5
+    only8 = oracle_lib.spd_direct_sw(x, [0.1, -0.2], table2[:, 3:4], [8])
+    ref8 = oracle_lib.spd_direct(x, [0.1, -0.2], sg, [8])
+    assert np.allclose(only8[0][:, :392], 2.0 * ref8[0][:, :392], rtol=1e-13)
