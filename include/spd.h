@@ -262,6 +262,30 @@ int spd_row_stats(const spd_plan* plan, const float* plane, float clip_sigma, in
                   float* mean, float* sigma, void* cuda_stream);
 
 /*
+ * spd_width_sigma - standard deviation per boxcar width measured on the plane (SURVEY.md sec. 8(f1),
+ * "we calculate the standard deviation only for boxcar filters of width that are equal to
+ * a powers of two.  We then interpolate ... for all intermediate boxcar widths"; reading A17).
+ *   plane   : DEVICE [n_dm][n_t] float32.
+ *   mean    : DEVICE [n_dm] float32, the per-row mean (e.g. from spd_row_stats); used as the shift of
+ *             the variance sums only.
+ *   sigma_w : DEVICE [n_dm][n_widths] float32, written: sigma of the sums of 2^j consecutive samples
+ *             (population standard deviation over the floor(n_t / 2^j) aligned groups) at widths
+ *             2^j, linear in the width in between, sqrt(width) beyond the last level with two groups.
+ * Asynchronous on cuda_stream; uses a plan-owned workspace (one call per plan at a time).
+ */
+int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w,
+                    void* cuda_stream);
+
+/*
+ * spd_run_sigma_w - spd_run with SNR_L = (X_L - L mean) / sigma_w[d][L's index] (eq. 4, PAPER.md:69,
+ * with the measured sigma(X_L) of spd_width_sigma in place of eq. 5's sqrt(L) sigma).
+ * Only for SPD_PATH_GENERIC (shared-memory tile kernel) and SPD_PATH_GRID plans; a streaming-tree plan
+ * returns SPD_ERR_INVALID_ARG (create it with SPD_FLAG_FORCE_GENERIC).  Other arguments as spd_run.
+ */
+int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,
+                    float* out_snr, int32_t* out_width, void* cuda_stream);
+
+/*
  * spd_run_host - the same hot path on HOST buffers (end-to-end entry point):
  * copies row blocks of the plane to the device, runs the kernels and copies
  * Y and W back, overlapping copies and kernels on internal streams.

@@ -9,7 +9,7 @@ from ._build import LIB_PATH, build
 from .binding import (  # noqa: F401
     CANDIDATE_DTYPE, EXPORTS, Plan, SpdError,
     SPD_FLAG_FORCE_GENERIC, SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC, SPD_PATH_IGRID_TREE, SPD_PATH_GRID,
-    spd_separation_generate, spd_plan_create_grid,
+    spd_separation_generate, spd_plan_create_grid, spd_width_sigma, spd_run_sigma_w,
     candidates_to_numpy, load, spd_destroy, spd_find_candidates, spd_last_error_string,
     spd_plan_create, spd_plan_destroy, spd_plan_get_info, spd_plan_get_widths, spd_run,
     spd_run_flagged, spd_find_candidates_flagged, spd_row_stats,
@@ -19,7 +19,7 @@ from .binding import (  # noqa: F401
 __all__ = [
     "LIB_PATH", "build", "load", "Plan", "SpdError", "EXPORTS", "CANDIDATE_DTYPE",
     "SPD_FLAG_FORCE_GENERIC", "SPD_PATH_DYADIC_TREE", "SPD_PATH_GENERIC", "SPD_PATH_IGRID_TREE", "SPD_PATH_GRID",
-    "spd_separation_generate", "spd_plan_create_grid",
+    "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
     "spd_width_set_generate", "spd_plan_create", "spd_plan_destroy", "spd_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
     "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",

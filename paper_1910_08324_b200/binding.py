@@ -35,7 +35,7 @@ EXPORTS = (
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
     "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
     "spd_run_host", "spd_last_error_string", "spd_version",
-    "spd_separation_generate", "spd_plan_create_grid",
+    "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
 )
 
 
@@ -97,6 +97,10 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_plan_create_grid.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _i32, _i32]
     lib.spd_separation_generate.restype = ctypes.c_int
     lib.spd_separation_generate.argtypes = [_i32, _i32, _vp, _i32, _vp]
+    lib.spd_width_sigma.restype = ctypes.c_int
+    lib.spd_width_sigma.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.spd_run_sigma_w.restype = ctypes.c_int
+    lib.spd_run_sigma_w.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.spd_plan_destroy.restype = None
     lib.spd_plan_destroy.argtypes = [_vp]
     lib.spd_plan_get_widths.restype = ctypes.c_int
@@ -310,6 +314,32 @@ def spd_row_stats(plan: int, plane, clip_sigma: float = 0.0, n_reject_passes: in
     return mean, sigma
 
 
+def spd_width_sigma(plan: int, plane, mean, sigma_w=None, stream=None):
+    """Standard deviation per (DM row, width) from power-of-two decimations of ``plane``; returns the
+    float32 [n_dm, n_widths] device tensor."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    if sigma_w is None:
+        sigma_w = torch.empty((info["n_dm"], info["n_widths"]), dtype=torch.float32, device=plane.device)
+    _check(load().spd_width_sigma(
+        _vp(plan), _dev_ptr(plane, torch.float32, n, "plane"), _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
+        _dev_ptr(sigma_w, torch.float32, info["n_dm"] * info["n_widths"], "sigma_w"), _vp(_stream_handle(stream))))
+    return sigma_w
+
+
+def spd_run_sigma_w(plan: int, plane, mean, sigma_w, out_snr, out_width, stream=None) -> None:
+    """spd_run with a measured standard deviation per (row, width) instead of sqrt(width) * sigma."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    _check(load().spd_run_sigma_w(
+        _vp(plan), _dev_ptr(plane, torch.float32, n, "plane"), _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
+        _dev_ptr(sigma_w, torch.float32, info["n_dm"] * info["n_widths"], "sigma_w"),
+        _dev_ptr(out_snr, torch.float32, n, "out_snr"), _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _vp(_stream_handle(stream))))
+
+
 def candidates_to_numpy(lst, n_found, capacity: int) -> Tuple[int, np.ndarray]:
     """Synchronising helper: (count, structured array of the stored candidates sorted by (dm, t))."""
     count = int(n_found.item())
@@ -396,6 +426,18 @@ class Plan:
     def row_stats(self, plane, clip_sigma: float = 0.0, n_reject_passes: int = 0, mean=None, sigma=None,
                   stream=None):
         return spd_row_stats(self.handle, plane, clip_sigma, n_reject_passes, mean, sigma, stream)
+
+    def width_sigma(self, plane, mean, sigma_w=None, stream=None):
+        return spd_width_sigma(self.handle, plane, mean, sigma_w, stream)
+
+    def run_sigma_w(self, plane, mean, sigma_w, out_snr=None, out_width=None, stream=None):
+        import torch
+        if out_snr is None:
+            out_snr = torch.empty((self.n_dm, self.n_t), dtype=torch.float32, device=plane.device)
+        if out_width is None:
+            out_width = torch.empty((self.n_dm, self.n_t), dtype=torch.int32, device=plane.device)
+        spd_run_sigma_w(self.handle, plane, mean, sigma_w, out_snr, out_width, stream)
+        return out_snr, out_width
 
     def run_host(self, plane, mean, sigma, out_snr, out_width):
         spd_run_host(self.handle, plane, mean, sigma, out_snr, out_width)

@@ -375,9 +375,11 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
         rc = generic_configure(plan);
     }
     if (rc == SPD_OK) rc = stats_configure(plan);
+    if (rc == SPD_OK) rc = wsig_configure(plan);
     if (rc != SPD_OK) {
         generic_release(plan);
         stats_release(plan);
+        wsig_release(plan);
         delete plan;
         return rc;
     }
@@ -390,6 +392,7 @@ void spd_plan_destroy(spd_plan* plan) {
     release_host_staging(plan);
     generic_release(plan);
     stats_release(plan);
+    wsig_release(plan);
     delete plan;
 }
 
@@ -455,6 +458,29 @@ int spd_run(const spd_plan* plan, const float* plane, const float* mean, const f
         return SPD_ERR_INVALID_ARG;
     }
     return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma_w) {
+        set_error("spd_width_sigma: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return wsig_run(plan, plane, mean, sigma_w, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,
+                    float* out_snr, int32_t* out_width, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma_w || !out_snr || !out_width) {
+        set_error("spd_run_sigma_w: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (is_tree_path(plan)) {
+        set_error("spd_run_sigma_w: the streaming-tree kernels scale by sqrt(width) at compile time; create the plan "
+                  "with SPD_FLAG_FORCE_GENERIC (or with spd_plan_create_grid) to use a measured sigma per width");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return generic_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width,
+                       static_cast<cudaStream_t>(cuda_stream), sigma_w);
 }
 
 int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width, float threshold,

@@ -240,7 +240,8 @@ __device__ __forceinline__ void build_running_sum(const float* __restrict__ row,
 __global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
     const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
     const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, long long n_t, int tile,
-    int span, long long tiles_per_row, float* __restrict__ out_snr, int32_t* __restrict__ out_width) {
+    int span, long long tiles_per_row, float* __restrict__ out_snr, int32_t* __restrict__ out_width,
+    const float* __restrict__ sigma_w) {
     extern __shared__ __align__(16) unsigned char gsm[];
     const int n_sub = span / kSub;  // span is a multiple of kSub
     double* const B = reinterpret_cast<double*>(gsm);                        // [n_sub + 1] running sum of sub-block totals
@@ -251,14 +252,15 @@ __global__ void __launch_bounds__(kTileThreads) generic_tile_kernel(
     const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
     const float* __restrict__ row = plane + d * n_t;
     const float mu = mean[d];
-    const float inv = 1.0f / sigma[d];
+    // sigma_w: measured standard deviation per (row, width) instead of eq. (5)'s sqrt(L) sigma
+    // (PAPER.md:728); only with the width table in shared memory (checked by the caller)
+    const float inv = sigma_w ? 1.0f : 1.0f / sigma[d];
     const long long avail = n_t - t0;  // samples of the row from t0 on
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const bool table_in_smem = n_w <= kTileWidthsMax;
     if (table_in_smem) {
         for (int k = threadIdx.x; k < n_w; k += kTileThreads) {
             sw[k] = __ldg(widths + k);
-            ss[k] = __ldg(wscale + k) * inv;
+            ss[k] = sigma_w ? 1.0f / __ldg(sigma_w + d * n_w + k) : __ldg(wscale + k) * inv;
         }
     }
     const int32_t* __restrict__ wp = table_in_smem ? sw : widths;
@@ -319,7 +321,7 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
     const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
     const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, const GridGroups groups,
     long long n_t, int tile, int span, long long tiles_per_row, float* __restrict__ out_snr,
-    int32_t* __restrict__ out_width) {
+    int32_t* __restrict__ out_width, const float* __restrict__ sigma_w) {
     extern __shared__ __align__(16) unsigned char gsm[];
     const int n_sub = span / kSub;
     double* const B = reinterpret_cast<double*>(gsm);
@@ -330,11 +332,11 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
     const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
     const float* __restrict__ row = plane + d * n_t;
     const float mu = mean[d];
-    const float inv = 1.0f / sigma[d];
+    const float inv = sigma_w ? 1.0f : 1.0f / sigma[d];
     const long long avail = n_t - t0;
     for (int k = threadIdx.x; k < n_w; k += kTileThreads) {  // n_w <= kTileWidthsMax (checked at plan creation)
         sw[k] = __ldg(widths + k);
-        ss[k] = __ldg(wscale + k) * inv;
+        ss[k] = sigma_w ? 1.0f / __ldg(sigma_w + d * n_w + k) : __ldg(wscale + k) * inv;
     }
     build_running_sum(row, t0, avail, mu, n_sub, span, B, c);
 
@@ -481,13 +483,18 @@ void generic_release(spd_plan* plan) {
 }
 
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-                float* out_snr, int32_t* out_width, cudaStream_t stream) {
+                float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w) {
     const long long n_t = plan->n_t;
+    if (sigma_w && (plan->generic_tile <= 0 || static_cast<int>(plan->widths.size()) > kTileWidthsMax)) {
+        set_error("a standard deviation per width needs the shared-memory tile kernel (max_width <= %d, at most %d "
+                  "widths)", kTileSpanMax - 4095, kTileWidthsMax);
+        return SPD_ERR_INVALID_ARG;
+    }
     if (!plan->separations.empty()) {
         grid_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads, plan->generic_smem,
                            stream>>>(plane, mean, sigma, plan->d_widths, plan->d_wscale,
                                      static_cast<int>(plan->widths.size()), plan->grid, n_t, plan->generic_tile,
-                                     plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width);
+                                     plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width, sigma_w);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "launching the boxcar-separation tile kernel");
         return SPD_OK;
@@ -496,7 +503,7 @@ int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const fl
         generic_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads,
                               plan->generic_smem, stream>>>(
             plane, mean, sigma, plan->d_widths, plan->d_wscale, static_cast<int>(plan->widths.size()), n_t,
-            plan->generic_tile, plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width);
+            plan->generic_tile, plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width, sigma_w);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "launching the any-width-set tile kernel");
         return SPD_OK;

@@ -79,6 +79,11 @@ struct spd_plan {
     void* d_stats = nullptr;  // [n_dm][stats_parts] partial moments
     int stats_parts = 0;
     int64_t stats_part = 0;   // samples per part
+    // spd_width_sigma
+    void* d_wsig_partial = nullptr;  // [n_dm][parts][14] level sums
+    void* d_wsig_totals = nullptr;   // [n_dm][super-blocks] totals of 8192 samples
+    void* d_wsig_widths = nullptr;   // [n_widths] the plan's widths
+    int wsig_parts = 0, wsig_sb_per_part = 0, wsig_sb_per_row = 0, wsig_levels = 0;
     // spd_run_host
     spd::HostStaging host;
 };
@@ -120,14 +125,22 @@ inline bool is_tree_path(const spd_plan* plan) {
 // spd_generic.cu
 int generic_configure(spd_plan* plan);
 void generic_release(spd_plan* plan);
+// sigma_w: nullptr (eq. 5: sqrt(L) sigma[d]) or [n_dm][n_widths] measured standard deviations
+// (tile kernels only); then `sigma` is not read.
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
-                const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream);
+                const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream,
+                const float* sigma_w = nullptr);
 
 // spd_stats.cu
 int stats_configure(spd_plan* plan);
 void stats_release(spd_plan* plan);
 int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float* mean,
               float* sigma, cudaStream_t stream);
+
+// spd_width_sigma.cu: standard deviation per width from power-of-two decimations
+int wsig_configure(spd_plan* plan);
+void wsig_release(spd_plan* plan);
+int wsig_run(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w, cudaStream_t stream);
 
 // spd_candidates.cu
 // activity: nullptr (visit every sample) or the map written by spd_run_flagged, one byte

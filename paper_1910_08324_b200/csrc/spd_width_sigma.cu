@@ -1,0 +1,244 @@
+// Standard deviation per boxcar width, measured on the data (second half).
+//
+// PAPER.md:728 (sec. 4.6.2): "we calculate values of the standard deviation only for time-series
+// which are decimations of the input time-series in time, i.e. we calculate the standard deviation
+// only for boxcar filters of width that are equal to a powers of two.  We then interpolate values of
+// standard deviation for all intermediate boxcar widths."  It replaces eq. (5)'s white-noise
+// sigma(X_L) = sqrt(L) sigma on real data (Fig. 24).
+//
+// Reading (A17): level j is the series of sums of 2^j consecutive samples,
+// x^j[m] = sum_{i < 2^j} x[2^j m + i], m < floor(n_t / 2^j) (eq. 13 with D = 2, without its shift);
+// sigma_j is its population standard deviation; for 2^j <= L < 2^(j+1) sigma_L is linear in L
+// between sigma_j and sigma_(j+1); above the last level with two elements, sqrt(L) from that level.
+//
+// width_moments_kernel: a block walks "super-blocks" of 8192 samples of one row; a super-block is
+// staged in shared memory and halved thirteen times in place (level j+1 = sums of pairs of level j,
+// float32: these are the decimations themselves), and at every level each thread adds its elements
+// to shifted double-precision sums S1 = sum(v - 2^j mu), S2 = sum(v - 2^j mu)^2.  Block-reduced in a
+// fixed order -> one partial per (row, part, level); the super-block totals are kept for the levels
+// above 8192.  width_sigma_finish_kernel (one block per row) merges the partials in order, builds
+// the levels above 8192 from the totals, and interpolates the plan's widths.  Reads the plane once:
+// 4 B per sample, HBM-bound; results do not depend on scheduling.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <algorithm>
+
+#include "spd_internal.h"
+
+namespace spd {
+namespace {
+
+constexpr int kWsgThreads = 256;
+constexpr int kWsgLog = 13;
+constexpr int kWsgBlock = 1 << kWsgLog;  // samples per super-block
+constexpr int kWsgLevels = kWsgLog + 1;  // levels 0 .. 13 inside a super-block
+constexpr int kWsgMaxLevels = 32;
+
+struct LevelSums {
+    double n, s1, s2;
+};
+
+__device__ __forceinline__ double block_sum(double v, double* scratch) {
+    // fixed order: lanes by shuffle, then warps serially
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) scratch[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < kWsgThreads / 32; ++w) t += scratch[w];
+    return t;  // valid in thread 0
+}
+
+__global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float* __restrict__ plane,
+                                                                      const float* __restrict__ mean, long long n_t,
+                                                                      int sb_per_row, int sb_per_part, int parts,
+                                                                      LevelSums* __restrict__ partial,
+                                                                      double* __restrict__ totals) {
+    __shared__ float s[kWsgBlock];
+    __shared__ double scratch[kWsgThreads / 32];
+    const int d = blockIdx.x / parts;
+    const int part = blockIdx.x - d * parts;
+    const float* __restrict__ row = plane + static_cast<long long>(d) * n_t;
+    const double mu = static_cast<double>(mean[d]);
+    double s1[kWsgLevels], s2[kWsgLevels], cnt[kWsgLevels];
+#pragma unroll
+    for (int j = 0; j < kWsgLevels; ++j) s1[j] = s2[j] = cnt[j] = 0.0;
+    const int sb_lo = part * sb_per_part;
+    const int sb_hi = min(sb_lo + sb_per_part, sb_per_row);
+    for (int sb = sb_lo; sb < sb_hi; ++sb) {
+        const long long base = static_cast<long long>(sb) * kWsgBlock;
+        const long long avail = n_t - base;  // samples of the row from here on (> 0)
+        __syncthreads();
+        for (int i = threadIdx.x; i < kWsgBlock; i += kWsgThreads) s[i] = i < avail ? __ldg(row + base + i) : 0.f;
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kWsgLevels; ++j) {
+            const int n_el = kWsgBlock >> j;
+            // element m of level j is a full group iff (m + 1) 2^j <= avail
+            const long long full = avail >> j;
+            const double shift = mu * static_cast<double>(1 << j);
+            for (int m = threadIdx.x; m < n_el; m += kWsgThreads) {
+                if (m < full) {
+                    const double v = static_cast<double>(s[m]) - shift;
+                    s1[j] += v;
+                    s2[j] += v * v;
+                    cnt[j] += 1.0;
+                }
+            }
+            if (j + 1 < kWsgLevels) {
+                __syncthreads();
+                float nxt[(kWsgBlock / 2 + kWsgThreads - 1) / kWsgThreads];
+                int q = 0;
+                for (int m = threadIdx.x; m < n_el / 2; m += kWsgThreads) nxt[q++] = s[2 * m] + s[2 * m + 1];
+                __syncthreads();
+                q = 0;
+                for (int m = threadIdx.x; m < n_el / 2; m += kWsgThreads) s[m] = nxt[q++];
+                __syncthreads();
+            }
+        }
+        // total of a complete super-block, for the levels above it
+        if (threadIdx.x == 0)
+            totals[static_cast<long long>(d) * sb_per_row + sb] = static_cast<double>(s[0]);
+    }
+    LevelSums* out = partial + (static_cast<long long>(d) * parts + part) * kWsgLevels;
+#pragma unroll
+    for (int j = 0; j < kWsgLevels; ++j) {
+        const double a = block_sum(s1[j], scratch);
+        const double b = block_sum(s2[j], scratch);
+        const double c = block_sum(cnt[j], scratch);
+        if (threadIdx.x == 0) {
+            out[j].n = c;
+            out[j].s1 = a;
+            out[j].s2 = b;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(64) width_sigma_finish_kernel(const LevelSums* __restrict__ partial,
+                                                                const double* __restrict__ totals,
+                                                                const float* __restrict__ mean, long long n_t,
+                                                                int sb_per_row, int parts, int n_levels,
+                                                                const int32_t* __restrict__ widths, int n_w,
+                                                                float* __restrict__ sigma_w) {
+    __shared__ double sig[kWsgMaxLevels];
+    __shared__ int n_valid;
+    const int d = blockIdx.x;
+    const int j = threadIdx.x;
+    if (j < n_levels) {
+        double sd = -1.0;  // < 0: level has fewer than two elements
+        if (j < kWsgLevels) {
+            double n = 0.0, a = 0.0, b = 0.0;
+            const LevelSums* p = partial + static_cast<long long>(d) * parts * kWsgLevels + j;
+            for (int q = 0; q < parts; ++q) {
+                n += p[q * kWsgLevels].n;
+                a += p[q * kWsgLevels].s1;
+                b += p[q * kWsgLevels].s2;
+            }
+            if (n >= 2.0) sd = sqrt(fmax(0.0, (b - a * a / n) / n));
+        } else {
+            // groups of 2^(j - 13) complete super-blocks
+            const long long g = 1ll << (j - kWsgLog);
+            const long long n_groups = (n_t >> j);
+            const double shift = static_cast<double>(mean[d]) * static_cast<double>(1ll << j);
+            const double* t = totals + static_cast<long long>(d) * sb_per_row;
+            double a = 0.0, b = 0.0;
+            for (long long m = 0; m < n_groups; ++m) {
+                double v = 0.0;
+                for (long long i = 0; i < g; ++i) v += t[m * g + i];
+                v -= shift;
+                a += v;
+                b += v * v;
+            }
+            const double n = static_cast<double>(n_groups);
+            if (n_groups >= 2) sd = sqrt(fmax(0.0, (b - a * a / n) / n));
+        }
+        sig[j] = sd;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int nv = 0;
+        while (nv < n_levels && sig[nv] >= 0.0) ++nv;
+        n_valid = nv;  // >= 1 whenever n_t >= 2
+    }
+    __syncthreads();
+    const int nv = n_valid;
+    for (int k = threadIdx.x; k < n_w; k += blockDim.x) {
+        const long long L = widths[k];
+        int jj = 0;
+        while ((2ll << jj) <= L) ++jj;  // 2^jj <= L < 2^(jj+1)
+        double sd;
+        if (nv == 0) {
+            sd = 0.0;
+        } else if (jj + 1 < nv) {
+            const double lo = static_cast<double>(1ll << jj);
+            sd = sig[jj] + (sig[jj + 1] - sig[jj]) * (static_cast<double>(L) - lo) / lo;
+        } else {
+            const int top = nv - 1;
+            sd = sig[top] * sqrt(static_cast<double>(L) / static_cast<double>(1ll << top));
+        }
+        sigma_w[static_cast<long long>(d) * n_w + k] = static_cast<float>(sd);
+    }
+}
+
+}  // namespace
+
+int wsig_configure(spd_plan* plan) {
+    const int64_t sb_per_row = (plan->n_t + kWsgBlock - 1) / kWsgBlock;
+    // parts: enough blocks to fill the machine
+    const int64_t want = std::max<int64_t>(1, (8 * int64_t(plan->sm_count) + plan->n_dm - 1) / plan->n_dm);
+    const int64_t parts = std::max<int64_t>(1, std::min<int64_t>(sb_per_row, want));
+    plan->wsig_sb_per_part = static_cast<int>((sb_per_row + parts - 1) / parts);
+    plan->wsig_parts = static_cast<int>((sb_per_row + plan->wsig_sb_per_part - 1) / plan->wsig_sb_per_part);
+    plan->wsig_sb_per_row = static_cast<int>(sb_per_row);
+    int levels = 0;
+    while ((int64_t(1) << levels) <= plan->max_width) ++levels;  // floor(log2(max_width)) + 1
+    plan->wsig_levels = std::min(levels + 1, kWsgMaxLevels);       // one above, for the interpolation
+    if (plan->n_dm * int64_t(plan->wsig_parts) > 0x7fffffffll) {
+        set_error("plane too large for the width-sigma grid");
+        return SPD_ERR_INVALID_ARG;
+    }
+    const size_t pb = sizeof(LevelSums) * static_cast<size_t>(plan->n_dm) * plan->wsig_parts * kWsgLevels;
+    const size_t tb = sizeof(double) * static_cast<size_t>(plan->n_dm) * sb_per_row;
+    const size_t wb = sizeof(int32_t) * plan->widths.size();
+    cudaError_t e;
+    if ((e = cudaMalloc(&plan->d_wsig_partial, pb)) != cudaSuccess ||
+        (e = cudaMalloc(&plan->d_wsig_totals, tb)) != cudaSuccess ||
+        (e = cudaMalloc(&plan->d_wsig_widths, wb)) != cudaSuccess ||
+        (e = cudaMemcpy(plan->d_wsig_widths, plan->widths.data(), wb, cudaMemcpyHostToDevice)) != cudaSuccess) {
+        set_error("device allocation of the width-sigma workspace failed: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        wsig_release(plan);
+        return SPD_ERR_ALLOC;
+    }
+    plan->workspace_bytes += static_cast<int64_t>(pb + tb + wb);
+    return SPD_OK;
+}
+
+void wsig_release(spd_plan* plan) {
+    cudaFree(plan->d_wsig_partial);
+    cudaFree(plan->d_wsig_totals);
+    cudaFree(plan->d_wsig_widths);
+    plan->d_wsig_partial = nullptr;
+    plan->d_wsig_totals = nullptr;
+    plan->d_wsig_widths = nullptr;
+}
+
+int wsig_run(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w, cudaStream_t stream) {
+    LevelSums* partial = static_cast<LevelSums*>(plan->d_wsig_partial);
+    double* totals = static_cast<double*>(plan->d_wsig_totals);
+    width_moments_kernel<<<static_cast<unsigned>(plan->n_dm * plan->wsig_parts), kWsgThreads, 0, stream>>>(
+        plane, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_sb_per_part, plan->wsig_parts, partial, totals);
+    width_sigma_finish_kernel<<<static_cast<unsigned>(plan->n_dm), 64, 0, stream>>>(
+        partial, totals, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_parts, plan->wsig_levels,
+        static_cast<const int32_t*>(plan->d_wsig_widths), static_cast<int>(plan->widths.size()), sigma_w);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "launching the width-sigma kernels");
+    return SPD_OK;
+}
+
+}  // namespace spd

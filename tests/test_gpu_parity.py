@@ -798,3 +798,73 @@ def test_block_and_warp_kernels_agree(spd, oracle_lib, K, monkeypatch):
     for snr, idx, name in ((a_snr, a_idx, "warp"), (b_snr, b_idx, "block")):
         parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, snr, idx, *ref, what=f"{name} K={K}")
     assert np.all(np.abs(a_snr - b_snr) <= 64 * np.spacing(np.abs(b_snr)) + 1e-30)
+
+
+# --- row f1, second half: standard deviation per width from decimations ----------
+
+@pytest.mark.parametrize("n_dm,n_t,kind,param,M", [(3, 8192 * 5 + 1234, "IGRID", 1, 256), (2, 300001, "POW2", 0, 32768),
+                                                   (5, 4100, "ALL", 0, 48), (1, 8192 * 19, "BOXDIT", 8, 8184),
+                                                   (2, 700, "POW2", 0, 512)])
+def test_width_sigma_matches_oracle(spd, oracle_lib, n_dm, n_t, kind, param, M):
+    """White and red (random-walk-like) rows, ragged lengths, levels above the 8192-sample super-block,
+    rows too short for the upper levels (sqrt law from the last measured level)."""
+    rng = np.random.default_rng(n_t)
+    x = rng.standard_normal((n_dm, n_t))
+    x[0] = np.convolve(x[0], np.ones(9) / 3.0, mode="same") + 5.0          # correlated: sigma_L is not sqrt(L)
+    x = x.astype(np.float32)
+    widths = spd.spd_width_set_generate(kind, param, min(M, n_t))
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, int(widths.max()), flags=spd.SPD_FLAG_FORCE_GENERIC) as plan:
+        mean, _ = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        sw2 = plan.width_sigma(plane, mean)
+        torch.cuda.synchronize()
+    ref = oracle_lib.width_sigma(x, widths)
+    got = sw.cpu().numpy().astype(np.float64)
+    assert np.allclose(got, ref, rtol=2e-5, atol=0), np.abs(got / ref - 1).max()
+    assert torch.equal(sw, sw2)                                            # fixed-order reduction
+    if n_t >= 8192 * 4:
+        white = ref[1 if n_dm > 1 else 0] if n_dm > 1 else None
+        if white is not None:
+            L = np.asarray(widths, dtype=np.float64)
+            assert np.allclose(white[L <= 64], np.sqrt(L[L <= 64]), rtol=0.05)   # eq. (5) on the white row
+        assert ref[0][-1] > 0 and not np.allclose(ref[0], ref[0][0] * np.sqrt(np.asarray(widths) / widths[0]), rtol=0.05)
+
+
+def test_run_with_measured_sigma_per_width(spd, oracle_lib):
+    """spd_run_sigma_w on the any-width-set and the grid path against direct summation with the same table;
+    a streaming-tree plan refuses."""
+    rng = np.random.default_rng(31)
+    n_dm, n_t = 3, 20000
+    x = rng.standard_normal((n_dm, n_t))
+    x[1] = np.convolve(x[1], np.ones(5) / 2.0, mode="same")
+    x[2, 9000:9040] += 1.5
+    x = (x + 2.0).astype(np.float32)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    widths = spd.spd_width_set_generate("IGRID", 1, 128)
+    with spd.Plan(n_dm, n_t, widths, 128, flags=spd.SPD_FLAG_FORCE_GENERIC) as plan:
+        mean, _ = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    ref = oracle_lib.spd_direct_sw(x, mu64, sw64, widths)
+    got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+    tol = parity.snr_tolerance(ref[0])
+    assert np.all(np.abs(got_snr - ref[0]) <= tol)
+    decisive = (ref[0] - ref[2]) > tol
+    assert np.array_equal(got_idx[decisive], ref[1][decisive])
+    # grid plan with the same table
+    seps = spd.spd_separation_generate("IGRID", 4, widths)
+    with spd.Plan(n_dm, n_t, widths, 128, separations=seps) as plan:
+        snr_g, idx_g = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    on = (np.arange(n_t)[None, :] % np.asarray(seps)[np.clip(ref[1], 0, None)]) == 0
+    assert np.all(np.abs(snr_g.cpu().numpy() - ref[0])[on & decisive & (ref[1] == idx_g.cpu().numpy())] <= tol[on & decisive & (ref[1] == idx_g.cpu().numpy())])
+    assert np.all(snr_g.cpu().numpy() <= got_snr + tol)                    # a grid evaluates a subset of the windows
+    with spd.Plan(n_dm, n_t, [1, 2, 4, 8], 8) as plan:
+        with pytest.raises(spd.SpdError):
+            plan.run_sigma_w(plane, mean, sw[:, :4].contiguous())
