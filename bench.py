@@ -344,6 +344,14 @@ def run_b200(args):
     e1.record(torch.cuda.current_stream())
     torch.cuda.synchronize()
     stats_ms = e0.elapsed_time(e1)
+    # sigma per width from power-of-two decimations (row f1): one more read of the plane
+    sw = plan.width_sigma(plane, s_mean)
+    e0.record(torch.cuda.current_stream())
+    plan.width_sigma(plane, s_mean, sw)
+    e1.record(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    wsig_ms = e0.elapsed_time(e1)
+    del sw
     activity = torch.empty(info["activity_bytes"], dtype=torch.uint8, device=dev)
     cand_list = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
     cand_count = torch.zeros(1, dtype=torch.int64, device=dev)
@@ -442,6 +450,9 @@ def run_b200(args):
         "n_dm_real_time": value * w.sampling_time_s,
         "row_stats": {"what": "spd_row_stats, 3 passes (plain + 2 rejection passes at 2 sigma), not part of the step",
                       "ms": stats_ms, "gbs": 3 * 4 * n / (stats_ms * 1e-3) / 1e9, "bytes_per_sample_per_pass": 4},
+        "width_sigma": {"what": "spd_width_sigma: sigma per width from power-of-two decimations, interpolated; "
+                                "one pass, not part of the step",
+                        "ms": wsig_ms, "gbs": 4 * n / (wsig_ms * 1e-3) / 1e9, "bytes_per_sample": 4},
     }
     if flush is not None:
         line["config"]["l2_flush_ms_per_step_excluded"] = flush_ms / args.steps

@@ -11,14 +11,14 @@
 // sigma_j is its population standard deviation; for 2^j <= L < 2^(j+1) sigma_L is linear in L
 // between sigma_j and sigma_(j+1); above the last level with two elements, sqrt(L) from that level.
 //
-// width_moments_kernel: a block walks "super-blocks" of 8192 samples of one row; a super-block is
-// staged in shared memory and halved thirteen times in place (level j+1 = sums of pairs of level j,
-// float32: these are the decimations themselves), and at every level each thread adds its elements
-// to shifted double-precision sums S1 = sum(v - 2^j mu), S2 = sum(v - 2^j mu)^2.  Block-reduced in a
-// fixed order -> one partial per (row, part, level); the super-block totals are kept for the levels
-// above 8192.  width_sigma_finish_kernel (one block per row) merges the partials in order, builds
-// the levels above 8192 from the totals, and interpolates the plan's widths.  Reads the plane once:
-// 4 B per sample, HBM-bound; results do not depend on scheduling.
+// width_moments_kernel: a block walks "super-blocks" of 8192 samples of one row; the decimations
+// are formed by repeated pairwise sums in float32 - levels 0..5 in a thread's registers (32
+// consecutive samples each), 5..8 in the registers of one warp, 8..13 across its lanes by shuffles -
+// and every level adds its elements to shifted sums S1 = sum(v - 2^j mu), S2 = sum(v - 2^j mu)^2 kept
+// in double.  Block-reduced in a fixed order -> one partial per (row, part, level); the super-block
+// totals are kept for the levels above 8192.  width_sigma_finish_kernel (one block per row) merges the
+// partials in order, builds the levels above 8192 from the totals, and interpolates the plan's
+// widths.  Reads the plane once: 4 B per sample, HBM-bound; results do not depend on scheduling.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -37,7 +37,7 @@ constexpr int kWsgLevels = kWsgLog + 1;  // levels 0 .. 13 inside a super-block
 constexpr int kWsgMaxLevels = 32;
 
 struct LevelSums {
-    double n, s1, s2;
+    double s1, s2;
 };
 
 __device__ __forceinline__ double block_sum(double v, double* scratch) {
@@ -54,65 +54,117 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
     return t;  // valid in thread 0
 }
 
+// Adds the n values v[0..n) of level j (sums of 2^j samples, first sample at `first` of the
+// super-block) to the level's shifted sums; only groups that end inside the row count.
+template <int N>
+__device__ __forceinline__ void level_add(const float (&v)[N], int j, long long first, long long avail, float shift,
+                                          double& s1, double& s2) {
+    float a = 0.f, b = 0.f;
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        if (first + (static_cast<long long>(i + 1) << j) <= avail) {
+            const float u = v[i] - shift;
+            a += u;
+            b = fmaf(u, u, b);
+        }
+    }
+    s1 += static_cast<double>(a);
+    s2 += static_cast<double>(b);
+}
+
+// One block walks super-blocks of 8192 samples.  Thread t owns the 32 consecutive samples
+// 32 t .. 32 t + 31: levels 0..5 in its registers; the 256 level-5 sums go through shared memory to
+// warp 0, whose lane l owns 8 of them: levels 5..8 in registers, levels 8..13 across lanes by
+// shuffles.  One block barrier per super-block (two buffers).  Sums of a few values are formed in
+// float32 (they ARE the decimated series), the running S1 / S2 of each level in double.
 __global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float* __restrict__ plane,
                                                                       const float* __restrict__ mean, long long n_t,
                                                                       int sb_per_row, int sb_per_part, int parts,
                                                                       LevelSums* __restrict__ partial,
                                                                       double* __restrict__ totals) {
-    __shared__ float s[kWsgBlock];
+    __shared__ float v5[2][kWsgThreads];
     __shared__ double scratch[kWsgThreads / 32];
     const int d = blockIdx.x / parts;
     const int part = blockIdx.x - d * parts;
+    const int tid = threadIdx.x, lane = tid & 31;
     const float* __restrict__ row = plane + static_cast<long long>(d) * n_t;
-    const double mu = static_cast<double>(mean[d]);
-    double s1[kWsgLevels], s2[kWsgLevels], cnt[kWsgLevels];
+    const float mu = mean[d];
+    double s1[kWsgLevels], s2[kWsgLevels];
 #pragma unroll
-    for (int j = 0; j < kWsgLevels; ++j) s1[j] = s2[j] = cnt[j] = 0.0;
+    for (int j = 0; j < kWsgLevels; ++j) s1[j] = s2[j] = 0.0;
     const int sb_lo = part * sb_per_part;
     const int sb_hi = min(sb_lo + sb_per_part, sb_per_row);
-    for (int sb = sb_lo; sb < sb_hi; ++sb) {
+    int buf = 0;
+    for (int sb = sb_lo; sb < sb_hi; ++sb, buf ^= 1) {
         const long long base = static_cast<long long>(sb) * kWsgBlock;
         const long long avail = n_t - base;  // samples of the row from here on (> 0)
-        __syncthreads();
-        for (int i = threadIdx.x; i < kWsgBlock; i += kWsgThreads) s[i] = i < avail ? __ldg(row + base + i) : 0.f;
-        __syncthreads();
+        const long long mine = 32ll * tid;
+        float x[32];
+        if (mine + 32 <= avail && ((reinterpret_cast<uintptr_t>(row + base) & 15u) == 0)) {
+            const float4* p4 = reinterpret_cast<const float4*>(row + base + mine);
 #pragma unroll
-        for (int j = 0; j < kWsgLevels; ++j) {
-            const int n_el = kWsgBlock >> j;
-            // element m of level j is a full group iff (m + 1) 2^j <= avail
-            const long long full = avail >> j;
-            const double shift = mu * static_cast<double>(1 << j);
-            for (int m = threadIdx.x; m < n_el; m += kWsgThreads) {
-                if (m < full) {
-                    const double v = static_cast<double>(s[m]) - shift;
-                    s1[j] += v;
-                    s2[j] += v * v;
-                    cnt[j] += 1.0;
-                }
+            for (int q = 0; q < 8; ++q) {
+                const float4 f = __ldg(p4 + q);
+                x[4 * q] = f.x;
+                x[4 * q + 1] = f.y;
+                x[4 * q + 2] = f.z;
+                x[4 * q + 3] = f.w;
             }
-            if (j + 1 < kWsgLevels) {
-                __syncthreads();
-                float nxt[(kWsgBlock / 2 + kWsgThreads - 1) / kWsgThreads];
-                int q = 0;
-                for (int m = threadIdx.x; m < n_el / 2; m += kWsgThreads) nxt[q++] = s[2 * m] + s[2 * m + 1];
-                __syncthreads();
-                q = 0;
-                for (int m = threadIdx.x; m < n_el / 2; m += kWsgThreads) s[m] = nxt[q++];
-                __syncthreads();
-            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) x[i] = mine + i < avail ? __ldg(row + base + mine + i) : 0.f;
         }
-        // total of a complete super-block, for the levels above it
-        if (threadIdx.x == 0)
-            totals[static_cast<long long>(d) * sb_per_row + sb] = static_cast<double>(s[0]);
+        // levels 0..5 in registers (level j + 1 = sums of pairs of level j)
+        level_add(x, 0, mine, avail, mu, s1[0], s2[0]);
+        float y16[16], y8[8], y4[4], y2[2], y1[1];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) y16[i] = x[2 * i] + x[2 * i + 1];
+        level_add(y16, 1, mine, avail, 2.f * mu, s1[1], s2[1]);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) y8[i] = y16[2 * i] + y16[2 * i + 1];
+        level_add(y8, 2, mine, avail, 4.f * mu, s1[2], s2[2]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) y4[i] = y8[2 * i] + y8[2 * i + 1];
+        level_add(y4, 3, mine, avail, 8.f * mu, s1[3], s2[3]);
+#pragma unroll
+        for (int i = 0; i < 2; ++i) y2[i] = y4[2 * i] + y4[2 * i + 1];
+        level_add(y2, 4, mine, avail, 16.f * mu, s1[4], s2[4]);
+        y1[0] = y2[0] + y2[1];
+        v5[buf][tid] = y1[0];
+        __syncthreads();  // the other buffer is free again: its readers passed this barrier one trip ago
+        if (tid < 32) {
+            // lane l: level-5 sums 8 l .. 8 l + 7 of the super-block (first sample 256 l)
+            const long long first = 256ll * lane;
+            float z8[8], z4[4], z2[2], z1[1];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) z8[i] = v5[buf][8 * lane + i];
+            level_add(z8, 5, first, avail, 32.f * mu, s1[5], s2[5]);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) z4[i] = z8[2 * i] + z8[2 * i + 1];
+            level_add(z4, 6, first, avail, 64.f * mu, s1[6], s2[6]);
+#pragma unroll
+            for (int i = 0; i < 2; ++i) z2[i] = z4[2 * i] + z4[2 * i + 1];
+            level_add(z2, 7, first, avail, 128.f * mu, s1[7], s2[7]);
+            z1[0] = z2[0] + z2[1];
+            // levels 8..13 across lanes: after step q the lanes that are multiples of 2^q hold level 8 + q
+            float v = z1[0];
+#pragma unroll
+            for (int q = 0; q <= 5; ++q) {
+                if ((lane & ((1 << q) - 1)) == 0) {
+                    const float one[1] = {v};
+                    level_add(one, 8 + q, first, avail, static_cast<float>(256 << q) * mu, s1[8 + q], s2[8 + q]);
+                }
+                if (q < 5) v += __shfl_down_sync(0xffffffffu, v, 1 << q);
+            }
+            if (lane == 0) totals[static_cast<long long>(d) * sb_per_row + sb] = static_cast<double>(v);
+        }
     }
     LevelSums* out = partial + (static_cast<long long>(d) * parts + part) * kWsgLevels;
 #pragma unroll
     for (int j = 0; j < kWsgLevels; ++j) {
         const double a = block_sum(s1[j], scratch);
         const double b = block_sum(s2[j], scratch);
-        const double c = block_sum(cnt[j], scratch);
-        if (threadIdx.x == 0) {
-            out[j].n = c;
+        if (tid == 0) {
             out[j].s1 = a;
             out[j].s2 = b;
         }
@@ -132,13 +184,13 @@ __global__ void __launch_bounds__(64) width_sigma_finish_kernel(const LevelSums*
     if (j < n_levels) {
         double sd = -1.0;  // < 0: level has fewer than two elements
         if (j < kWsgLevels) {
-            double n = 0.0, a = 0.0, b = 0.0;
+            double a = 0.0, b = 0.0;
             const LevelSums* p = partial + static_cast<long long>(d) * parts * kWsgLevels + j;
             for (int q = 0; q < parts; ++q) {
-                n += p[q * kWsgLevels].n;
                 a += p[q * kWsgLevels].s1;
                 b += p[q * kWsgLevels].s2;
             }
+            const double n = static_cast<double>(n_t >> j);  // every full group of the row was counted once
             if (n >= 2.0) sd = sqrt(fmax(0.0, (b - a * a / n) / n));
         } else {
             // groups of 2^(j - 13) complete super-blocks
