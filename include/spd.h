@@ -279,8 +279,9 @@ int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean,
 /*
  * spd_run_sigma_w - spd_run with SNR_L = (X_L - L mean) / sigma_w[d][L's index] (eq. 4, PAPER.md:69,
  * with the measured sigma(X_L) of spd_width_sigma in place of eq. 5's sqrt(L) sigma).
- * Only for SPD_PATH_GENERIC (shared-memory tile kernel) and SPD_PATH_GRID plans; a streaming-tree plan
- * returns SPD_ERR_INVALID_ARG (create it with SPD_FLAG_FORCE_GENERIC).  Other arguments as spd_run.
+ * For SPD_PATH_DYADIC_TREE plans on the warp-per-stream kernel (9 to 14 widths 2^k: spd_plan_info.tree_kernel
+ * == 2), SPD_PATH_GENERIC plans (shared-memory tile kernel) and SPD_PATH_GRID plans; the other streaming-tree
+ * plans return SPD_ERR_INVALID_ARG (create them with SPD_FLAG_FORCE_GENERIC).  Other arguments as spd_run.
  */
 int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,
                     float* out_snr, int32_t* out_width, void* cuda_stream);

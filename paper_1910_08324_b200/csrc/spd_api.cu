@@ -474,9 +474,13 @@ int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean,
         set_error("spd_run_sigma_w: NULL argument");
         return SPD_ERR_INVALID_ARG;
     }
+    if (plan->path == SPD_PATH_DYADIC_TREE && plan->tree.kind == 1)  // warp-per-stream kernel: run-time scale per level
+        return ws_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width, 0.0f, nullptr,
+                      static_cast<cudaStream_t>(cuda_stream), sigma_w);
     if (is_tree_path(plan)) {
-        set_error("spd_run_sigma_w: the streaming-tree kernels scale by sqrt(width) at compile time; create the plan "
-                  "with SPD_FLAG_FORCE_GENERIC (or with spd_plan_create_grid) to use a measured sigma per width");
+        set_error("spd_run_sigma_w: this plan's streaming-tree kernel scales by sqrt(width) at compile time; create "
+                  "the plan with SPD_FLAG_FORCE_GENERIC (or with spd_plan_create_grid) to use a measured sigma per "
+                  "width");
         return SPD_ERR_INVALID_ARG;
     }
     return generic_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width,

@@ -108,8 +108,10 @@ bool ws_applicable(int K);
 int ws_configure(spd_plan* plan);
 int ws_grid_blocks(const spd_plan* plan);
 int ws_piece_chunks(const spd_plan* plan);
+// sigma_w: nullptr (eq. 5), or [n_dm][K] measured standard deviations per width (then sigma is not read)
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream);
+           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+           const float* sigma_w = nullptr);
 
 // spd_tree_ig.cu: widths 2^k and 3 * 2^m (IGRID depth 1)
 int ig_applicable(const std::vector<int32_t>& widths, int64_t n_t);  // K (pow-2 levels) or 0

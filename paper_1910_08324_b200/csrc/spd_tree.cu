@@ -540,6 +540,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     prm.plane = plane;
     prm.mean = mean;
     prm.sigma = sigma;
+    prm.sigma_w = nullptr;
     prm.out_snr = out_snr;
     prm.out_width = out_width;
     prm.activity = activity;

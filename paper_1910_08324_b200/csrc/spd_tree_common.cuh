@@ -19,6 +19,7 @@ struct TreeParams {
     const float* sigma;
     float* out_snr;
     int32_t* out_width;
+    const float* sigma_w;  // nullptr, or [n_dm][K] measured standard deviation per width (warp-stream kernel)
     uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr
     float threshold;    // candidate threshold in SNR units (used only with activity)
     long long n_t;
@@ -257,6 +258,34 @@ __device__ __forceinline__ void fold(float4& best, float4 before, float4 now, in
     }
 }
 
+// Run-time scale per level (a measured standard deviation per width, instead of
+// eq. (5)'s 2^(-k/2) / sigma): ls[k] = 1 / sigma_{d, 2^k}, the same tag and max.
+template <int k, bool FAST>
+__device__ __forceinline__ float4 keyx_rt(float4 p, int lim, uint32_t tm, float s) {
+    const float4 v = scale4(p, s);
+    float4 q = make_float4(pack1<k>(v.x, tm), pack1<k>(v.y, tm), pack1<k>(v.z, tm), pack1<k>(v.w, tm));
+    if constexpr (!FAST) {
+        const int w = 1 << k;
+        const float ninf = __int_as_float(0xff800000);
+        if (w > lim) q.x = ninf;
+        if (w > lim - 1) q.y = ninf;
+        if (w > lim - 2) q.z = ninf;
+        if (w > lim - 3) q.w = ninf;
+    }
+    return q;
+}
+template <int j, int K, bool FAST>
+__device__ __forceinline__ void fold_rt(float4& best, float4 before, float4 now, int lim, uint32_t tm,
+                                        const float (&ls)[16]) {
+    if constexpr (j >= 3) {
+        if constexpr ((j & 1) == 0) {
+            best = max4(best, keyx_rt<j - 1, FAST>(before, lim, tm, ls[j - 1]), keyx_rt<j, FAST>(now, lim, tm, ls[j]));
+        } else if constexpr (j == K - 1) {
+            best = max4(best, keyx_rt<j, FAST>(now, lim, tm, ls[j]));
+        }
+    }
+}
+
 // Shared-memory store of a float4, issued as two 64-bit halves in PTX.  The sums are produced
 // by packed FADD2 into register PAIRS; written as one 128-bit store the allocator spends up to
 // four register moves per store on forming an aligned QUAD.  ptxas re-merges the halves into
@@ -304,6 +333,7 @@ struct ChunkCtx {
     long long n0, n_t;
     bool do_out;
     int tid;
+    float ls[16];    // run-time scale per level (kernels instantiated for a sigma per width)
     uint32_t tbase;  // tensor-memory base of this thread's delay FIFOs (kernels that keep them there)
     int it;          // steps done on this stream (FIFO slot = it mod depth)
 };

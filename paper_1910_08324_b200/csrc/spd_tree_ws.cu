@@ -114,6 +114,16 @@ __device__ __forceinline__ float4 shfl4(float4 v, int src) {
 }
 #endif
 
+// eq. (5)'s compile-time scale 2^(-k/2) (1 / sigma applied at the store), or a measured sigma per width.
+template <int j, int K, bool FAST, bool SW>
+__device__ __forceinline__ void fold_sw(float4& best, float4 before, float4 now, int lim, const ChunkCtx& cx) {
+    if constexpr (SW) {
+        fold_rt<j, K, FAST>(best, before, now, lim, cx.tm, cx.ls);
+    } else {
+        fold<j, K, FAST>(best, before, now, lim, cx.tm);
+    }
+}
+
 // Step modes: 0 = guarded (row tail: windows checked against the end of the row, output if
 // cx.do_out), 1 = interior step with output, 2 = interior look-ahead step (sums only).
 template <int MODE>
@@ -127,7 +137,7 @@ __device__ __forceinline__ bool wants_out(const ChunkCtx& cx) {
     }
 }
 
-template <int K, int MODE, int k>
+template <int K, int MODE, bool SW, int k>
 __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], float4 (&hs)[4], float4* __restrict__ xb,
                                             int lane, const ChunkCtx& cx) {
@@ -158,16 +168,16 @@ __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], partner[r]);
-            if (wants_out<MODE>(cx)) fold<k + 1, K, (MODE != 0)>(best[r], P[r], now, lim[r], cx.tm);
+            if (wants_out<MODE>(cx)) fold_sw<k + 1, K, (MODE != 0), SW>(best[r], P[r], now, lim[r], cx);
             P[r] = now;
         }
-        lane_levels<K, MODE, k + 1>(P, best, lim, hs, xb, lane, cx);
+        lane_levels<K, MODE, SW, k + 1>(P, best, lim, hs, xb, lane, cx);
     }
 }
 
 // Row levels j < JN: partner 2^j rows later, in this step or among the first rows of the
 // previous step (nr[2^j - 1 .. 2^(j+1) - 2]).
-template <int K, int MODE, int j>
+template <int K, int MODE, bool SW, int j>
 __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], float4 (&nr)[WsGeo<K>::NEAR + 1],
                                             const ChunkCtx& cx) {
@@ -183,15 +193,15 @@ __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)
         for (int i = 0; i < D; ++i) nr[off + i] = P[i];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (wants_out<MODE>(cx)) fold<lvl, K, (MODE != 0)>(best[r], P[r], now[r], lim[r], cx.tm);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW>(best[r], P[r], now[r], lim[r], cx);
             P[r] = now[r];
         }
-        near_levels<K, MODE, j + 1>(P, best, lim, nr, cx);
+        near_levels<K, MODE, SW, j + 1>(P, best, lim, nr, cx);
     }
 }
 
 // FIFO levels i < JF: partner 2^i steps back, same lane, same row: tensor memory.
-template <int K, int MODE, int i>
+template <int K, int MODE, bool SW, int i>
 __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], uint32_t tbase, int it,
                                             const ChunkCtx& cx) {
@@ -207,15 +217,15 @@ __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], old[r]);
-            if (wants_out<MODE>(cx)) fold<lvl, K, (MODE != 0)>(best[r], P[r], now, lim[r], cx.tm);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW>(best[r], P[r], now, lim[r], cx);
             P[r] = now;
         }
-        fifo_levels<K, MODE, i + 1>(P, best, lim, tbase, it, cx);
+        fifo_levels<K, MODE, SW, i + 1>(P, best, lim, tbase, it, cx);
     }
 }
 
 // One step of one warp: the kWsStage floats at st4 -> Y, W of its kWsStep samples.
-template <int K, int MODE>
+template <int K, int MODE, bool SW>
 __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 (&hs)[4],
                                          float4 (&nr)[WsGeo<K>::NEAR + 1], float4* __restrict__ xb, uint32_t tbase,
                                          int it, int lane, const ChunkCtx& cx) {
@@ -244,14 +254,20 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
         const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
                                       (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
         if (wants_out<MODE>(cx)) {
-            best[r] = max4(keyx<0, (MODE != 0)>(a, lim[r], tm), keyx<1, (MODE != 0)>(p1, lim[r], tm), keyx<2, (MODE != 0)>(p2, lim[r], tm));
-            fold<3, K, (MODE != 0)>(best[r], p2, p3, lim[r], tm);
+            constexpr bool F = MODE != 0;
+            if constexpr (SW) {
+                best[r] = max4(keyx_rt<0, F>(a, lim[r], tm, cx.ls[0]), keyx_rt<1, F>(p1, lim[r], tm, cx.ls[1]),
+                               keyx_rt<2, F>(p2, lim[r], tm, cx.ls[2]));
+            } else {
+                best[r] = max4(keyx<0, F>(a, lim[r], tm), keyx<1, F>(p1, lim[r], tm), keyx<2, F>(p2, lim[r], tm));
+            }
+            fold_sw<3, K, F, SW>(best[r], p2, p3, lim[r], cx);
         }
         P[r] = p3;
     }
-    lane_levels<K, MODE, 3>(P, best, lim, hs, xb, lane, cx);
-    near_levels<K, MODE, 0>(P, best, lim, nr, cx);
-    fifo_levels<K, MODE, 0>(P, best, lim, tbase, it, cx);
+    lane_levels<K, MODE, SW, 3>(P, best, lim, hs, xb, lane, cx);
+    near_levels<K, MODE, SW, 0>(P, best, lim, nr, cx);
+    fifo_levels<K, MODE, SW, 0>(P, best, lim, tbase, it, cx);
     if constexpr (WsGeo<K>::JF > 0) tmem_wait_st();
 
     float top = __int_as_float(0xff800000);
@@ -281,7 +297,7 @@ constexpr size_t kWsStagesBytes = static_cast<size_t>(kWsWarps) * kWsStages * kW
 constexpr size_t kWsXBytes = SPD_WS_XCHG ? static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16 : 0;
 constexpr size_t ws_smem_bytes() { return kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8 + 16; }
 
-template <int K>
+template <int K, bool SW>
 __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const TreeParams p, const int n_pieces) {
     using G = WsGeo<K>;
     constexpr int S = kWsStep;
@@ -350,8 +366,15 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
 
         const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
         cx.mu = p.mean[d];
-        const float sg = p.sigma[d];
+        const float sg = SW ? 1.0f : p.sigma[d];
         cx.inv = 1.0f / sg;
+        if constexpr (SW) {
+            // keys are SNRs already: 1 / sigma_{d, 2^k} per level, nothing left for the store
+            const float* __restrict__ swr = p.sigma_w + static_cast<long long>(d) * K;
+#pragma unroll
+            for (int k = 0; k < K; ++k) cx.ls[k] = 1.0f / __ldg(swr + k);
+            cx.inv = 1.0f;
+        }
         cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
         cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
         uint8_t* const act =
@@ -359,7 +382,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
                        : nullptr;
         float thr_key = __int_as_float(0x7f800000);
         if (act) {
-            const float t = p.threshold * sg;
+            const float t = SW ? p.threshold : p.threshold * sg;
             thr_key = t - fabsf(t) * 2e-6f;
         }
 
@@ -394,7 +417,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             __syncwarp();
             cx.n0 = n0;
             cx.do_out = c < c_hi;
-            const float top = ws_step<K, 0>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
+            const float top = ws_step<K, 0, SW>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
             if (act && cx.do_out && top >= thr_key) act[c / kWsActSteps] = 1;
             __syncwarp();
         }
@@ -441,7 +464,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
         for (; f < n_warm; ++f, ++it) {
             ring_next(f);
             cx.n0 = static_cast<long long>(ring_top - 1 - f) * S;
-            ws_step<K, 2>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
+            ws_step<K, 2, SW>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
             ring_done();
         }
         // Two steps per loop trip: the values kept from one step to the next (hs, nr: 11 float4)
@@ -452,7 +475,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             ring_next(f);
             const int c = ring_top - 1 - f;
             cx.n0 = static_cast<long long>(c) * S;
-            const float top = ws_step<K, 1>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
+            const float top = ws_step<K, 1, SW>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
                                             tbase, it, lane, cx);
             if (act && top >= thr_key) act[c / kWsActSteps] = 1;
             ring_done();
@@ -493,7 +516,10 @@ int ws_configure(spd_plan* plan) {
     cudaError_t e = cudaErrorInvalidValue;
 #define SPD_PREP(KK)                                                                                          \
     if (cfg.K == KK)                                                                                          \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                                 static_cast<int>(cfg.smem_bytes));                                           \
+    if (cfg.K == KK && e == cudaSuccess)                                                                      \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
                                  static_cast<int>(cfg.smem_bytes));
     SPD_WS_CASES(SPD_PREP)
 #undef SPD_PREP
@@ -555,12 +581,14 @@ int ws_grid_blocks(const spd_plan* plan) {
 }
 
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
+           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+           const float* sigma_w) {
     const TreeConfig& cfg = plan->tree;
     TreeParams prm;
     prm.plane = plane;
     prm.mean = mean;
     prm.sigma = sigma;
+    prm.sigma_w = sigma_w;
     prm.out_snr = out_snr;
     prm.out_width = out_width;
     prm.activity = activity;
@@ -589,7 +617,10 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     cudaError_t e = cudaErrorInvalidValue;
 #define SPD_LAUNCH(KK)                                                                                      \
     if (cfg.K == KK) {                                                                                      \
-        spd_tree_ws_kernel<KK><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+        if (sigma_w)                                                                                        \
+            spd_tree_ws_kernel<KK, true><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+        else                                                                                                \
+            spd_tree_ws_kernel<KK, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
         e = cudaGetLastError();                                                                             \
     }
     SPD_WS_CASES(SPD_LAUNCH)

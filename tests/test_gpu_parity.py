@@ -868,3 +868,39 @@ def test_run_with_measured_sigma_per_width(spd, oracle_lib):
     with spd.Plan(n_dm, n_t, [1, 2, 4, 8], 8) as plan:
         with pytest.raises(spd.SpdError):
             plan.run_sigma_w(plane, mean, sw[:, :4].contiguous())
+
+
+@pytest.mark.parametrize("K", [9, 12, 14])
+def test_warp_stream_kernel_with_measured_sigma_per_width(spd, oracle_lib, K):
+    """spd_run_sigma_w on the tuned dyadic path: the warp-per-stream kernel takes 1 / sigma_{d, 2^k} per level
+    at run time.  White, correlated and offset rows; parity with direct summation using the same table;
+    with the table sqrt(L) sigma it reproduces spd_run to the last few ulp."""
+    M = 1 << (K - 1)
+    rng = np.random.default_rng(900 + K)
+    n_dm, n_t = 4, max(512 * 21 + 8, 3 * M + 516)
+    x = rng.standard_normal((n_dm, n_t))
+    x[1] = np.convolve(x[1], np.ones(7) / 2.5, mode="same")
+    x[2, n_t // 2: n_t // 2 + M // 4] += 10.0 / np.sqrt(M // 4)
+    x = (x + np.array([0.0, 3.0, -1.0, 0.5])[:, None]).astype(np.float32)
+    widths = [1 << k for k in range(K)]
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, M) as plan:
+        assert plan.info["tree_kernel"] == 2
+        mean, sigma = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        white = (sigma[:, None] * torch.sqrt(torch.tensor(widths, dtype=torch.float32, device=dev))[None, :]).contiguous()
+        snr_w, idx_w = plan.run_sigma_w(plane, mean, white)
+        snr_0, idx_0 = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    ref = oracle_lib.spd_direct_sw(x, mu64, sw.cpu().numpy().astype(np.float64), widths)
+    got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+    tol = parity.snr_tolerance(ref[0])
+    assert np.all(np.abs(got_snr - ref[0]) <= tol), float(np.max(np.abs(got_snr - ref[0]) / tol))
+    decisive = (ref[0] - ref[2]) > tol
+    assert np.array_equal(got_idx[decisive], ref[1][decisive])
+    a, b = snr_w.cpu().numpy(), snr_0.cpu().numpy()
+    assert np.all(np.abs(a - b) <= 1e-5 * np.maximum(1.0, np.abs(b)))
+    assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
