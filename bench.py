@@ -351,6 +351,18 @@ def run_b200(args):
     e1.record(torch.cuda.current_stream())
     torch.cuda.synchronize()
     wsig_ms = e0.elapsed_time(e1)
+    # the same pass with the measured sigma per width in place of eq. (5) (where the plan's kernels take it)
+    run_sw_ms = None
+    if info["tree_kernel"] == 2 or info["path"] in (spd.SPD_PATH_GENERIC, spd.SPD_PATH_GRID):
+        try:
+            plan.run_sigma_w(plane, s_mean, sw, out_snr, out_width)
+            e0.record(torch.cuda.current_stream())
+            plan.run_sigma_w(plane, s_mean, sw, out_snr, out_width)
+            e1.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            run_sw_ms = e0.elapsed_time(e1)
+        except spd.SpdError:
+            run_sw_ms = None
     del sw
     activity = torch.empty(info["activity_bytes"], dtype=torch.uint8, device=dev)
     cand_list = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
@@ -452,7 +464,8 @@ def run_b200(args):
                       "ms": stats_ms, "gbs": 3 * 4 * n / (stats_ms * 1e-3) / 1e9, "bytes_per_sample_per_pass": 4},
         "width_sigma": {"what": "spd_width_sigma: sigma per width from power-of-two decimations, interpolated; "
                                 "one pass, not part of the step",
-                        "ms": wsig_ms, "gbs": 4 * n / (wsig_ms * 1e-3) / 1e9, "bytes_per_sample": 4},
+                        "ms": wsig_ms, "gbs": 4 * n / (wsig_ms * 1e-3) / 1e9, "bytes_per_sample": 4,
+                        "run_sigma_w_ms": run_sw_ms},
     }
     if flush is not None:
         line["config"]["l2_flush_ms_per_step_excluded"] = flush_ms / args.steps
