@@ -302,3 +302,53 @@ def test_full_size_config3_on_the_paper_grids(spd, oracle_lib, wkind, wparam, gk
         assert bool(torch.isfinite(y).all()) and int(k.min()) >= 0 and int(k.max()) < len(widths)
         assert bool((y >= plane[r0:r0 + 64] - 1e-4 * torch.clamp(plane[r0:r0 + 64].abs(), min=1.0)).all())
         assert bool((n[None, :] % sp[k.long()] == 0).all())
+
+
+def test_full_size_config3_sigma_per_width(spd, oracle_lib):
+    """Row f1 at config 3's size, as `bench.py` runs it: spd_width_sigma on the whole plane checked against the
+    oracle on sampled rows, then spd_run_sigma_w (warp-per-stream kernel) against direct summation with the
+    same table on sampled windows, and eq. (5) as a property of the white-noise plane."""
+    from workloads import get_workload, make_plane_torch
+    w = get_workload(3)
+    dev = torch.device("cuda:0")
+    free, _ = torch.cuda.mem_get_info(dev)
+    if free < 13 * w.n_samples + (6 << 30):
+        pytest.skip("not enough device memory")
+    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+    plane, pulses = make_plane_torch(w, dev)
+    with spd.Plan(w.n_dm, w.n_t, widths, w.max_width) as plan:
+        assert plan.info["tree_kernel"] == 2
+        mean, sigma = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    sw_h = sw.cpu().numpy().astype(np.float64)
+    # the plane is white noise (+ a few pulses): sigma_L = sqrt(L) sigma to the sampling error of each level
+    L = np.asarray(widths, dtype=np.float64)
+    rel = sw_h / (sigma.cpu().numpy().astype(np.float64)[:, None] * np.sqrt(L)[None, :]) - 1.0
+    quiet = np.ones(w.n_dm, dtype=bool)
+    quiet[[p.dm for p in pulses]] = False     # an injected pulse is an outlier of the level near its width
+    assert quiet.sum() > w.n_dm // 2
+    assert np.all(np.abs(rel[quiet]) < 6.0 * np.sqrt(L / (2.0 * w.n_t))[None, :] + 0.02)
+    rng = np.random.default_rng(w.seed + 31)
+    rows = sorted({0, w.n_dm - 1, pulses[0].dm, int(rng.integers(0, w.n_dm))})
+    for r in rows:
+        ref = oracle_lib.width_sigma(plane[r].cpu().numpy()[None, :], widths)[0]
+        assert np.allclose(sw_h[r], ref, rtol=2e-5, atol=0), (r, np.abs(sw_h[r] / ref - 1).max())
+    mean_h = mean.cpu().numpy().astype(np.float64)
+    M, n_t, span = w.max_width, w.n_t, 1024
+    wins = [(p.dm, max(0, p.t0 - span // 2)) for p in pulses[:: max(1, len(pulses) // 6)]]
+    wins += [(0, 0), (w.n_dm - 1, n_t - span), (5, n_t - M - span // 2), (int(rng.integers(0, w.n_dm)), int(rng.integers(0, n_t - span)))]
+    for row, t0 in wins:
+        t1 = min(n_t, t0 + span)
+        lo, hi = t0, min(n_t, t1 + M)
+        seg = plane[row, lo:hi].cpu().numpy()[None, :]
+        if hi < n_t:   # not the row's end: every window of a sample < t1 must count as fitting
+            seg = np.concatenate([seg, np.zeros((1, 1), np.float32)], axis=1)
+        ref_snr, ref_idx, ref_sec = oracle_lib.spd_direct_sw(seg, mean_h[row], sw_h[row][None, :], widths, 0, t1 - t0)
+        got_snr = snr[row, t0:t1].cpu().numpy()[None, :]
+        got_idx = idx[row, t0:t1].cpu().numpy()[None, :]
+        tol = parity.snr_tolerance(ref_snr)
+        assert np.all(np.abs(got_snr - ref_snr) <= tol), (row, t0)
+        decisive = (ref_snr - ref_sec) > tol
+        assert np.array_equal(got_idx[decisive], ref_idx[decisive]), (row, t0)
