@@ -188,7 +188,9 @@ void oracle_width_sigma(const float* x, int64_t n_dm, int64_t n_t,
             int j = 0;
             while (((int64_t)2 << j) <= L) ++j;               /* 2^j <= L < 2^(j+1) */
             double s;
-            if (j + 1 < n_lev) {
+            if (n_lev == 0) {
+                s = 0.0;                                      /* a one-sample row has no deviation */
+            } else if (j + 1 < n_lev) {
                 const double lo = (double)((int64_t)1 << j);
                 s = sig[j] + (sig[j + 1] - sig[j]) * ((double)L - lo) / lo;
             } else {
