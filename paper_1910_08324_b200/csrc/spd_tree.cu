@@ -106,11 +106,16 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
                 // 252 registers per thread): slot = step mod depth as a run-time column offset,
                 // one tcgen05.ld + tcgen05.st of R float4 per level.  Slots of the shallower FIFOs
                 // come first: Q - 1 of them.
-                static_assert(R == 4, "tensor-memory FIFOs move 4 float4 per level");
+                static_assert(R == 4 || R == 2, "tensor-memory FIFOs move 2 or 4 float4 per level");
                 const uint32_t taddr = cx.tbase + 4u * R * static_cast<uint32_t>((Q - 1) + (cx.it & (Q - 1)));
                 float4 old[R];
-                tmem_ld16(taddr, old);
-                tmem_st16(taddr, P);
+                if constexpr (R == 4) {
+                    tmem_ld16(taddr, reinterpret_cast<float4(&)[4]>(old));
+                    tmem_st16(taddr, reinterpret_cast<const float4(&)[4]>(P));
+                } else {
+                    tmem_ld8(taddr, reinterpret_cast<float4(&)[2]>(old));
+                    tmem_st8(taddr, reinterpret_cast<const float4(&)[2]>(P));
+                }
 #pragma unroll
                 for (int r = 0; r < R; ++r) now[r] = add4(P[r], old[r]);
             } else {
@@ -253,8 +258,14 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
 #ifndef SPD_TREE_BPS
 #define SPD_TREE_BPS 3
 #endif
-constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : 128; }
-constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : 4; }
+#ifndef SPD_TREE_T16
+#define SPD_TREE_T16 128
+#endif
+#ifndef SPD_TREE_R16
+#define SPD_TREE_R16 4
+#endif
+constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? 128 : SPD_TREE_T16); }
+constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : (K == 15 ? 4 : SPD_TREE_R16); }
 #ifndef SPD_TREE_BPS15
 #define SPD_TREE_BPS15 4
 #endif
@@ -266,7 +277,8 @@ constexpr int tree_tmem_cols() {
     using G = Geo<T, R, K>;
     constexpr int LR = ilog2(R);
     constexpr int JF = G::J > LR ? G::J - LR : 0;
-    constexpr int need = 4 * R * ((1 << JF) - 1);
+    // warps w and w + 4 share a lane quarter: every set of 128 threads has its own columns
+    constexpr int need = (T / 128) * 4 * R * ((1 << JF) - 1);
     return need <= 32 ? 32 : need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
 }
 
@@ -338,11 +350,12 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
         tmem_fence_before_sync();
         __syncthreads();
         tmem_fence_after_sync();
-        cx.tbase = *tslot + (static_cast<uint32_t>((tid >> 5) & 3) << 21);  // this warp's lane quarter
-        const float4 zero[4] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f),
-                                make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
+        constexpr int kSetCols = kTmemCols / (T / 128);  // columns of one set of 128 threads
+        // this warp's lane quarter, and the columns of its set of 128 threads
+        cx.tbase = *tslot + (static_cast<uint32_t>((tid >> 5) & 3) << 21) + static_cast<uint32_t>(tid >> 7) * kSetCols;
+        const float4 zero[2] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
 #pragma unroll
-        for (int col = 0; col < kTmemCols; col += 16) tmem_st16(cx.tbase + col, zero);
+        for (int col = 0; col < kSetCols; col += 8) tmem_st8(cx.tbase + col, zero);
         tmem_wait_st();
     } else {
         __syncthreads();

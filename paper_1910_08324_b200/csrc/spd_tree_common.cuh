@@ -143,6 +143,26 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const float4 (&v)[8]) 
         : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float4 (&v)[2]) {
+    uint32_t r[8];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+        : "r"(taddr)
+        : "memory");
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+        v[i] = make_float4(__uint_as_float(r[4 * i]), __uint_as_float(r[4 * i + 1]), __uint_as_float(r[4 * i + 2]),
+                           __uint_as_float(r[4 * i + 3]));
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const float4 (&v)[2]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+                 "r"(__float_as_uint(v[0].x)), "r"(__float_as_uint(v[0].y)), "r"(__float_as_uint(v[0].z)),
+                 "r"(__float_as_uint(v[0].w)), "r"(__float_as_uint(v[1].x)), "r"(__float_as_uint(v[1].y)),
+                 "r"(__float_as_uint(v[1].z)), "r"(__float_as_uint(v[1].w))
+                 : "memory");
+}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float4 (&v)[4]) {
     uint32_t r[16];
     asm volatile(
