@@ -432,7 +432,8 @@ def run_b200(args):
     achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
     roofline = {
         "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_ws_kernel" if info["tree_kernel"] == 2 else "spd_tree_kernel",
-                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel", spd.SPD_PATH_GRID: "grid_tile_kernel"}.get(
+                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel",
+                   spd.SPD_PATH_GRID: "spd_tree_ws_kernel (grid)" if info["tree_kernel"] == 2 else "grid_tile_kernel"}.get(
                        info["path"], "generic_tile_kernel"),
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),

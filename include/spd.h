@@ -169,7 +169,9 @@ int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, 
  * spd_run / spd_run_flagged / spd_run_host on such a plan write one merged full-resolution
  * plane: out_snr[d,n] = max over the widths whose grid contains n (and whose window fits,
  * reading A3), out_width the index of that width; -inf / -1 where no width's grid contains n
- * (only if separations[0] > 1).  Limits: max_width <= 45057, n_widths <= 1024.
+ * (only if separations[0] > 1).  Limits: max_width <= 45057, n_widths <= 1024.  A set {1, 2, 4, ..., 2^(K-1)}
+ * with 9 <= K <= 14 runs on the warp-per-stream tree kernel (spd_plan_info.tree_kernel == 2), other sets on a
+ * shared-memory tile kernel.
  * spd_plan_info.path is SPD_PATH_GRID.  Errors as spd_plan_create plus the conditions above.
  */
 int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t,

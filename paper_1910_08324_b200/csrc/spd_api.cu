@@ -167,6 +167,8 @@ int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const flo
         return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
     if (plan->path == SPD_PATH_IGRID_TREE)
         return ig_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
+    if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1)
+        return ws_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
     return generic_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
 }
 
@@ -363,6 +365,12 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     if (separations) {
         plan->path = SPD_PATH_GRID;
         rc = generic_configure(plan);
+        // widths {2^k} on a grid: the warp-per-stream tree kernel with the keys of a level counted only on
+        // that level's grid (the any-width-set grid kernel stays configured for spd_run_sigma_w)
+        if (rc == SPD_OK && tree_applicable(w, n_t) && ws_applicable(static_cast<int>(w.size()))) {
+            plan->tree.K = static_cast<int>(w.size());
+            rc = ws_configure(plan);
+        }
     } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
         plan->path = SPD_PATH_DYADIC_TREE;
         rc = tree_configure(plan);
@@ -440,6 +448,7 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
             info->blocks = static_cast<int32_t>(plan->n_dm * ((plan->n_t + 255) / 256));
         }
     }
+    if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1) info->tree_kernel = 2;
     info->workspace_bytes = plan->workspace_bytes;
     info->activity_bytes = static_cast<int64_t>(activity_bytes(plan));
     info->activity_block = static_cast<int32_t>(activity_block(plan));
@@ -512,11 +521,13 @@ int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean,
         return tree_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     if (plan->path == SPD_PATH_IGRID_TREE)
         return ig_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1)
+        return ws_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     // any-width-set path: no fused test, every block stays active (padding included: the
     // candidate kernel bounds the flag index itself)
     const cudaError_t e = cudaMemsetAsync(activity, 1, activity_bytes(plan), stream);
     if (e != cudaSuccess) return cuda_fail(e, "filling the activity map");
-    return generic_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, stream);
+    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, stream);
 }
 
 int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const int32_t* out_width,

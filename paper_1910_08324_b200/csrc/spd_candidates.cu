@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(kCandThreads) find_candidates_flagged_kernel(
 }  // namespace
 
 int64_t activity_block(const spd_plan* plan) {
-    if (!is_tree_path(plan)) return 4096;
+    if (!runs_tree_kernel(plan)) return 4096;
     return plan->tree.act_block > 0 ? plan->tree.act_block : plan->tree.chunk;
 }
 int64_t activity_per_row(const spd_plan* plan) {
@@ -194,7 +194,7 @@ int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* ou
     if (e != cudaSuccess) return cuda_fail(e, "clearing the candidate counter");
     // the any-width-set path marks everything: visiting every sample with the dense kernel is
     // the same work with more parallelism
-    if (activity && is_tree_path(plan)) {
+    if (activity && runs_tree_kernel(plan)) {
         const long long per_row = activity_per_row(plan);
         const long long n_flags = plan->n_dm * per_row;
         const long long steps = (n_flags + 31) / 32;

@@ -123,6 +123,11 @@ int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
 inline bool is_tree_path(const spd_plan* plan) {
     return plan->path == SPD_PATH_DYADIC_TREE || plan->path == SPD_PATH_IGRID_TREE;
 }
+// A streaming-tree kernel runs this plan (fused threshold test, activity map per tree.act_block / chunk):
+// the tree paths, and a grid plan over widths 2^k (warp-per-stream kernel with per-level grids).
+inline bool runs_tree_kernel(const spd_plan* plan) {
+    return is_tree_path(plan) || (plan->path == SPD_PATH_GRID && plan->tree.kind == 1);
+}
 
 // spd_generic.cu
 int generic_configure(spd_plan* plan);

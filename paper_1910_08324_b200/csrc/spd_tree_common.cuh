@@ -19,6 +19,7 @@ struct TreeParams {
     const float* sigma;
     float* out_snr;
     int32_t* out_width;
+    uint32_t gmask[16];    // grid plans: separation of level k minus one (a power of two minus one); else unused
     const float* sigma_w;  // nullptr, or [n_dm][K] measured standard deviation per width (warp-stream kernel)
     uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr
     float threshold;    // candidate threshold in SNR units (used only with activity)
@@ -353,6 +354,7 @@ struct ChunkCtx {
     long long n0, n_t;
     bool do_out;
     int tid;
+    uint32_t gmask[16];  // boxcar separation per level minus one (kernels instantiated for a grid plan)
     float ls[16];    // run-time scale per level (kernels instantiated for a sigma per width)
     uint32_t tbase;  // tensor-memory base of this thread's delay FIFOs (kernels that keep them there)
     int it;          // steps done on this stream (FIFO slot = it mod depth)

@@ -472,6 +472,7 @@ int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     prm.mean = mean;
     prm.sigma = sigma;
     prm.sigma_w = nullptr;
+    for (int k = 0; k < 16; ++k) prm.gmask[k] = 0u;
     prm.out_snr = out_snr;
     prm.out_width = out_width;
     prm.activity = activity;

@@ -114,13 +114,48 @@ __device__ __forceinline__ float4 shfl4(float4 v, int src) {
 }
 #endif
 
-// eq. (5)'s compile-time scale 2^(-k/2) (1 / sigma applied at the store), or a measured sigma per width.
-template <int j, int K, bool FAST, bool SW>
-__device__ __forceinline__ void fold_sw(float4& best, float4 before, float4 now, int lim, const ChunkCtx& cx) {
+// Keys of level k: eq. (5)'s compile-time scale 2^(-k/2) (1 / sigma applied at the store), or a measured
+// sigma per width (SW).
+template <int k, bool FAST, bool SW>
+__device__ __forceinline__ float4 key_sw(float4 p, int lim, const ChunkCtx& cx) {
     if constexpr (SW) {
-        fold_rt<j, K, FAST>(best, before, now, lim, cx.tm, cx.ls);
+        return keyx_rt<k, FAST>(p, lim, cx.tm, cx.ls[k]);
     } else {
-        fold<j, K, FAST>(best, before, now, lim, cx.tm);
+        return keyx<k, FAST>(p, lim, cx.tm);
+    }
+}
+// Grid plans (row f2, reading A16): level k counts only at samples that are multiples of its separation
+// gmask[k] + 1 (a power of two).  nb = index of the float4's first sample (a multiple of 4), so of the
+// four samples x is on the grid iff nb & gmask == 0, z iff the separation is 1 or 2, y and w iff it is 1.
+template <int k>
+__device__ __forceinline__ float4 grid_mask(float4 q, uint32_t nb, const ChunkCtx& cx) {
+    const uint32_t m = cx.gmask[k];
+    const float ninf = __int_as_float(0xff800000);
+    if ((nb & m) != 0u) q.x = ninf;
+    if (m != 0u) {
+        q.y = ninf;
+        q.w = ninf;
+    }
+    if (m > 1u) q.z = ninf;
+    return q;
+}
+template <int j, int K, bool FAST, bool SW, bool GR>
+__device__ __forceinline__ void fold_sw(float4& best, float4 before, float4 now, int lim, uint32_t nb,
+                                        const ChunkCtx& cx) {
+    if constexpr (j >= 3) {
+        if constexpr ((j & 1) == 0) {
+            float4 a = key_sw<j - 1, FAST, SW>(before, lim, cx);
+            float4 b = key_sw<j, FAST, SW>(now, lim, cx);
+            if constexpr (GR) {
+                a = grid_mask<j - 1>(a, nb, cx);
+                b = grid_mask<j>(b, nb, cx);
+            }
+            best = max4(best, a, b);
+        } else if constexpr (j == K - 1) {
+            float4 b = key_sw<j, FAST, SW>(now, lim, cx);
+            if constexpr (GR) b = grid_mask<j>(b, nb, cx);
+            best = max4(best, b);
+        }
     }
 }
 
@@ -137,9 +172,10 @@ __device__ __forceinline__ bool wants_out(const ChunkCtx& cx) {
     }
 }
 
-template <int K, int MODE, bool SW, int k>
+template <int K, int MODE, bool SW, bool GR, int k>
 __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
-                                            const int (&lim)[kWsRows], float4 (&hs)[4], float4* __restrict__ xb,
+                                            const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows], float4 (&hs)[4],
+                                            float4* __restrict__ xb,
                                             int lane, const ChunkCtx& cx) {
     constexpr int R = kWsRows;
     if constexpr (k <= 6 && k + 1 <= WsGeo<K>::LAST) {
@@ -168,19 +204,19 @@ __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], partner[r]);
-            if (wants_out<MODE>(cx)) fold_sw<k + 1, K, (MODE != 0), SW>(best[r], P[r], now, lim[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<k + 1, K, (MODE != 0), SW, GR>(best[r], P[r], now, lim[r], nb[r], cx);
             P[r] = now;
         }
-        lane_levels<K, MODE, SW, k + 1>(P, best, lim, hs, xb, lane, cx);
+        lane_levels<K, MODE, SW, GR, k + 1>(P, best, lim, nb, hs, xb, lane, cx);
     }
 }
 
 // Row levels j < JN: partner 2^j rows later, in this step or among the first rows of the
 // previous step (nr[2^j - 1 .. 2^(j+1) - 2]).
-template <int K, int MODE, bool SW, int j>
+template <int K, int MODE, bool SW, bool GR, int j>
 __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
-                                            const int (&lim)[kWsRows], float4 (&nr)[WsGeo<K>::NEAR + 1],
-                                            const ChunkCtx& cx) {
+                                            const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows],
+                                            float4 (&nr)[WsGeo<K>::NEAR + 1], const ChunkCtx& cx) {
     constexpr int R = kWsRows;
     if constexpr (j < WsGeo<K>::JN) {
         constexpr int D = 1 << j;
@@ -193,18 +229,18 @@ __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)
         for (int i = 0; i < D; ++i) nr[off + i] = P[i];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW>(best[r], P[r], now[r], lim[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, GR>(best[r], P[r], now[r], lim[r], nb[r], cx);
             P[r] = now[r];
         }
-        near_levels<K, MODE, SW, j + 1>(P, best, lim, nr, cx);
+        near_levels<K, MODE, SW, GR, j + 1>(P, best, lim, nb, nr, cx);
     }
 }
 
 // FIFO levels i < JF: partner 2^i steps back, same lane, same row: tensor memory.
-template <int K, int MODE, bool SW, int i>
+template <int K, int MODE, bool SW, bool GR, int i>
 __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
-                                            const int (&lim)[kWsRows], uint32_t tbase, int it,
-                                            const ChunkCtx& cx) {
+                                            const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows], uint32_t tbase,
+                                            int it, const ChunkCtx& cx) {
     constexpr int R = kWsRows;
     if constexpr (i < WsGeo<K>::JF) {
         constexpr int Q = WsGeo<K>::Q0 << i;     // FIFO depth in steps
@@ -217,15 +253,15 @@ __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], old[r]);
-            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW>(best[r], P[r], now, lim[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, GR>(best[r], P[r], now, lim[r], nb[r], cx);
             P[r] = now;
         }
-        fifo_levels<K, MODE, SW, i + 1>(P, best, lim, tbase, it, cx);
+        fifo_levels<K, MODE, SW, GR, i + 1>(P, best, lim, nb, tbase, it, cx);
     }
 }
 
 // One step of one warp: the kWsStage floats at st4 -> Y, W of its kWsStep samples.
-template <int K, int MODE, bool SW>
+template <int K, int MODE, bool SW, bool GR>
 __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 (&hs)[4],
                                          float4 (&nr)[WsGeo<K>::NEAR + 1], float4* __restrict__ xb, uint32_t tbase,
                                          int it, int lane, const ChunkCtx& cx) {
@@ -234,8 +270,10 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
     const uint32_t tm = cx.tm;
     float4 P[R], best[R];
     int lim[R];
+    uint32_t nb[R];  // index of each float4's first sample (low 32 bits; grid plans only)
 #pragma unroll
     for (int r = 0; r < R; ++r) {
+        nb[r] = static_cast<uint32_t>(cx.n0) + 4u * static_cast<uint32_t>(lane + 32 * r);
         if constexpr (MODE != 0) {
             lim[r] = 1 << 30;
         } else {
@@ -255,19 +293,21 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
                                       (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
         if (wants_out<MODE>(cx)) {
             constexpr bool F = MODE != 0;
-            if constexpr (SW) {
-                best[r] = max4(keyx_rt<0, F>(a, lim[r], tm, cx.ls[0]), keyx_rt<1, F>(p1, lim[r], tm, cx.ls[1]),
-                               keyx_rt<2, F>(p2, lim[r], tm, cx.ls[2]));
-            } else {
-                best[r] = max4(keyx<0, F>(a, lim[r], tm), keyx<1, F>(p1, lim[r], tm), keyx<2, F>(p2, lim[r], tm));
+            float4 k0 = key_sw<0, F, SW>(a, lim[r], cx), k1 = key_sw<1, F, SW>(p1, lim[r], cx),
+                   k2 = key_sw<2, F, SW>(p2, lim[r], cx);
+            if constexpr (GR) {
+                k0 = grid_mask<0>(k0, nb[r], cx);
+                k1 = grid_mask<1>(k1, nb[r], cx);
+                k2 = grid_mask<2>(k2, nb[r], cx);
             }
-            fold_sw<3, K, F, SW>(best[r], p2, p3, lim[r], cx);
+            best[r] = max4(k0, k1, k2);
+            fold_sw<3, K, F, SW, GR>(best[r], p2, p3, lim[r], nb[r], cx);
         }
         P[r] = p3;
     }
-    lane_levels<K, MODE, SW, 3>(P, best, lim, hs, xb, lane, cx);
-    near_levels<K, MODE, SW, 0>(P, best, lim, nr, cx);
-    fifo_levels<K, MODE, SW, 0>(P, best, lim, tbase, it, cx);
+    lane_levels<K, MODE, SW, GR, 3>(P, best, lim, nb, hs, xb, lane, cx);
+    near_levels<K, MODE, SW, GR, 0>(P, best, lim, nb, nr, cx);
+    fifo_levels<K, MODE, SW, GR, 0>(P, best, lim, nb, tbase, it, cx);
     if constexpr (WsGeo<K>::JF > 0) tmem_wait_st();
 
     float top = __int_as_float(0xff800000);
@@ -284,9 +324,17 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
                                          static_cast<int>(~__float_as_uint(kq.y) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.z) & kCodeMask),
                                          static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
+                int4 wv = w;
+                if constexpr (GR) {  // on no width's grid: -inf / -1 (reading A16)
+                    const float ninf = __int_as_float(0xff800000);
+                    if (kq.x == ninf) wv.x = -1;
+                    if (kq.y == ninf) wv.y = -1;
+                    if (kq.z == ninf) wv.z = -1;
+                    if (kq.w == ninf) wv.w = -1;
+                }
                 const long long o = cx.n0 + 4ll * (lane + 32 * r);
                 *reinterpret_cast<float4*>(cx.out_snr + o) = y;
-                *reinterpret_cast<int4*>(cx.out_width + o) = w;
+                *reinterpret_cast<int4*>(cx.out_width + o) = wv;
             }
         }
     }
@@ -297,7 +345,7 @@ constexpr size_t kWsStagesBytes = static_cast<size_t>(kWsWarps) * kWsStages * kW
 constexpr size_t kWsXBytes = SPD_WS_XCHG ? static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16 : 0;
 constexpr size_t ws_smem_bytes() { return kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8 + 16; }
 
-template <int K, bool SW>
+template <int K, bool SW, bool GR>
 __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const TreeParams p, const int n_pieces) {
     using G = WsGeo<K>;
     constexpr int S = kWsStep;
@@ -332,6 +380,10 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
     const int c_fast_end = n_t >= M ? static_cast<int>((n_t - M) / S) : 0;
     ChunkCtx cx;
     cx.tm = p.tag_mask;
+    if constexpr (GR) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) cx.gmask[k] = p.gmask[k];
+    }
     cx.n_t = n_t;
     cx.tid = lane;
     int stage = 0;
@@ -417,7 +469,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             __syncwarp();
             cx.n0 = n0;
             cx.do_out = c < c_hi;
-            const float top = ws_step<K, 0, SW>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
+            const float top = ws_step<K, 0, SW, GR>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
             if (act && cx.do_out && top >= thr_key) act[c / kWsActSteps] = 1;
             __syncwarp();
         }
@@ -464,18 +516,19 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
         for (; f < n_warm; ++f, ++it) {
             ring_next(f);
             cx.n0 = static_cast<long long>(ring_top - 1 - f) * S;
-            ws_step<K, 2, SW>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
+            ws_step<K, 2, SW, GR>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
             ring_done();
         }
         // Two steps per loop trip: the values kept from one step to the next (hs, nr: 11 float4)
         // alternate between two register sets instead of being moved, and the first levels of a
         // step overlap the last levels of the one before (10.70 -> 10.26 ms on config 3; x3: see DESIGN).
-#pragma unroll kWsUnroll
+        constexpr int kTrip = GR ? 1 : kWsUnroll;  // the grid body is larger: one step per trip
+#pragma unroll kTrip
         for (; f < n_ring; ++f, ++it) {
             ring_next(f);
             const int c = ring_top - 1 - f;
             cx.n0 = static_cast<long long>(c) * S;
-            const float top = ws_step<K, 1, SW>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
+            const float top = ws_step<K, 1, SW, GR>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
                                             tbase, it, lane, cx);
             if (act && top >= thr_key) act[c / kWsActSteps] = 1;
             ring_done();
@@ -516,10 +569,13 @@ int ws_configure(spd_plan* plan) {
     cudaError_t e = cudaErrorInvalidValue;
 #define SPD_PREP(KK)                                                                                          \
     if (cfg.K == KK)                                                                                          \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                  static_cast<int>(cfg.smem_bytes));                                           \
     if (cfg.K == KK && e == cudaSuccess)                                                                      \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                 static_cast<int>(cfg.smem_bytes));                                           \
+    if (cfg.K == KK && e == cudaSuccess)                                                                      \
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                  static_cast<int>(cfg.smem_bytes));
     SPD_WS_CASES(SPD_PREP)
 #undef SPD_PREP
@@ -607,6 +663,8 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     prm.segs_per_row = cfg.segs_per_row;
     prm.warm_chunks = cfg.warm_chunks;
     prm.tag_mask = ~kCodeMask;
+    for (int k = 0; k < 16; ++k)
+        prm.gmask[k] = k < static_cast<int>(plan->separations.size()) ? static_cast<uint32_t>(plan->separations[k] - 1) : 0u;
     if (activity) {
         const size_t bytes = (static_cast<size_t>(n_dm) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
         const cudaError_t em = cudaMemsetAsync(activity, 0, bytes, stream);
@@ -618,9 +676,11 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
 #define SPD_LAUNCH(KK)                                                                                      \
     if (cfg.K == KK) {                                                                                      \
         if (sigma_w)                                                                                        \
-            spd_tree_ws_kernel<KK, true><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+            spd_tree_ws_kernel<KK, true, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+        else if (!plan->separations.empty())                                                                \
+            spd_tree_ws_kernel<KK, false, true><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
         else                                                                                                \
-            spd_tree_ws_kernel<KK, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
+            spd_tree_ws_kernel<KK, false, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
         e = cudaGetLastError();                                                                             \
     }
     SPD_WS_CASES(SPD_LAUNCH)

@@ -904,3 +904,51 @@ def test_warp_stream_kernel_with_measured_sigma_per_width(spd, oracle_lib, K):
     a, b = snr_w.cpu().numpy(), snr_0.cpu().numpy()
     assert np.all(np.abs(a - b) <= 1e-5 * np.maximum(1.0, np.abs(b)))
     assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
+
+
+@pytest.mark.parametrize("K,gkind,gparam", [(14, "DIT", 0), (12, "IGRID", 4), (9, "IGRID", 16), (13, "EVERY_SAMPLE", 0)])
+def test_grid_plans_with_dyadic_widths_run_on_the_tree_kernel(spd, oracle_lib, K, gkind, gparam):
+    """Widths {2^k} on a grid (Alg. 3's DIT, or the same widths on P layers) take the
+    warp-per-stream tree kernel with each level counted only on its grid; against oracle_spd_grid on every
+    sample, pieces stopping inside rows, a ragged tail; off-grid samples never win."""
+    M = 1 << (K - 1)
+    widths = [1 << k for k in range(K)]
+    seps = spd.spd_separation_generate(gkind, gparam, widths)
+    rng = np.random.default_rng(600 + K)
+    n_dm, n_t = 5, max(512 * 19 + 12, 3 * M + 520)
+    x = rng.standard_normal((n_dm, n_t)).astype(np.float32)
+    x[1, 3 * 512 + 77: 3 * 512 + 77 + M // 2] += np.float32(11.0 / np.sqrt(M // 2))
+    x[4, n_t - M // 3:] += np.float32(0.8)
+    got_snr, got_idx, info = run_gpu_grid(spd, x, 0.0, 1.0, widths, seps, M)
+    assert info["tree_kernel"] == 2
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_grid(x, 0.0, 1.0, widths, seps)
+    parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                         what=f"grid tree K={K} {gkind}:{gparam}")
+    n = np.arange(n_t)[None, :]
+    assert np.all(n % np.asarray(seps)[got_idx] == 0)
+
+
+def test_grid_tree_plan_flagged_candidates(spd, oracle_lib):
+    """A grid plan over widths 2^k fuses the threshold test like the tree plans: flagged run = plain run,
+    flagged candidates = the rule on the plane."""
+    rng = np.random.default_rng(61)
+    K, n_dm, n_t = 11, 3, 512 * 40 + 16
+    widths = [1 << k for k in range(K)]
+    seps = spd.spd_separation_generate("DIT", 0, widths)
+    x = rng.standard_normal((n_dm, n_t)).astype(np.float32)
+    x[2, 7000:7000 + 256] += np.float32(0.9)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(n_dm, device=dev), torch.ones(n_dm, device=dev)
+    with spd.Plan(n_dm, n_t, widths, 1 << (K - 1), separations=seps) as plan:
+        assert plan.info["tree_kernel"] == 2 and plan.info["activity_block"] == 2048
+        snr0, idx0 = plan.run(plane, mean, sigma)
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 5.0)
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, 5.0, 1 << 14)
+        torch.cuda.synchronize()
+        count, cands = spd.candidates_to_numpy(lst, n_found, 1 << 14)
+    assert torch.equal(snr, snr0) and torch.equal(idx, idx0)
+    ref_count, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.cpu().numpy(), idx.cpu().numpy(), 5.0)
+    assert count == ref_count and count > 0
+    assert np.array_equal(cands["dm"], c_dm) and np.array_equal(cands["t"], c_t)
+    assert 0 < int(act.sum().item()) < act.numel()
