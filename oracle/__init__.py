@@ -8,6 +8,7 @@ A plain double-precision CPU statement of the SPD hot path written from
 from . import formulas  # noqa: F401
 from .core import (  # noqa: F401
     build,
+    cluster_candidates,
     find_candidates,
     num_threads,
     row_stats,
@@ -17,5 +18,6 @@ from .core import (  # noqa: F401
     spd_direct_sw,
     width_sigma,
     spd_grid,
+    spd_grid_sw,
     spd_prefix,
 )

@@ -54,7 +54,11 @@ def _load() -> ctypes.CDLL:
         lib.oracle_row_stats.restype = None
         lib.oracle_row_stats.argtypes = [_vp, _i64, _i64, _vp, _vp]
         lib.oracle_row_stats_clipped.restype = None
-        lib.oracle_row_stats_clipped.argtypes = [_vp, _i64, _i64, ctypes.c_float, _i32, _vp, _vp]
+        lib.oracle_row_stats_clipped.argtypes = [_vp, _i64, _i64, _f64, _i32, _f64, _f64, _vp, _vp, _vp, _vp]
+        lib.oracle_spd_grid_sw.restype = None
+        lib.oracle_spd_grid_sw.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
+        lib.oracle_cluster_candidates.restype = _i64
+        lib.oracle_cluster_candidates.argtypes = [_vp, _i64, _i64, _vp, _i32, _vp, _vp, _vp, _i64, _i32, _vp]
         lib.oracle_find_candidates.restype = _i64
         lib.oracle_find_candidates.argtypes = [_vp, _vp, _i64, _i64, ctypes.c_float, _i64, _vp, _vp, _vp, _vp]
         _lib = lib
@@ -191,16 +195,47 @@ def row_stats(x) -> Tuple[np.ndarray, np.ndarray]:
     return mu, sg
 
 
-def row_stats_clipped(x, clip: float, n_reject_passes: int) -> Tuple[np.ndarray, np.ndarray]:
-    """Per-row mean and population sigma after ``n_reject_passes`` rounds of point-wise outlier
-    rejection at ``clip`` sigmas (reading A14); float32-rounded values as float64."""
+def row_stats_clipped(x, clip: float, n_reject_passes: int, rel_tol: float = -1.0, border_eps: float = 0.0,
+                      details: bool = False):
+    """Per-row mean and population sigma with point-wise outlier rejection at ``clip`` sigmas
+    (reading A14), all in double: at most ``n_reject_passes`` rejection passes,
+    stopping early once a pass changes neither estimate by more than ``rel_tol`` * sigma
+    (``rel_tol`` < 0: never).  Returns (mean, sigma), or with ``details`` also the passes done per
+    row and the number of samples within ``border_eps`` * sigma of a rejection limit."""
     x = _plane(x)
     n_dm, n_t = x.shape
     mu = np.empty(n_dm, dtype=np.float64)
     sg = np.empty(n_dm, dtype=np.float64)
-    _load().oracle_row_stats_clipped(x.ctypes.data, n_dm, n_t, ctypes.c_float(clip), int(n_reject_passes),
-                                     mu.ctypes.data, sg.ctypes.data)
+    n_pass = np.empty(n_dm, dtype=np.int32)
+    n_border = np.empty(n_dm, dtype=np.int64)
+    _load().oracle_row_stats_clipped(x.ctypes.data, n_dm, n_t, float(clip), int(n_reject_passes),
+                                     float(rel_tol), float(border_eps), mu.ctypes.data, sg.ctypes.data,
+                                     n_pass.ctypes.data, n_border.ctypes.data)
+    if details:
+        return mu, sg, n_pass, n_border
     return mu, sg
+
+
+def spd_grid_sw(x, mean, sigma_w, widths, seps, t0: int = 0, t1: Optional[int] = None
+                ) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """``spd_grid`` with a standard deviation per (row, width): sigma_w is [n_dm, n_widths]."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    t1 = n_t if t1 is None else int(t1)
+    t0 = int(t0)
+    assert 0 <= t0 <= t1 <= n_t
+    w = np.ascontiguousarray([int(v) for v in widths], dtype=np.int32)
+    sp = np.ascontiguousarray([int(v) for v in seps], dtype=np.int32)
+    assert w.size > 0 and w.size == sp.size and w[0] >= 1 and np.all(np.diff(w) > 0) and np.all(sp >= 1)
+    mu = _stats(mean, n_dm)
+    sw = np.ascontiguousarray(sigma_w, dtype=np.float64).reshape(n_dm, w.size)
+    snr = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    idx = np.empty((n_dm, t1 - t0), dtype=np.int32)
+    sec = np.empty((n_dm, t1 - t0), dtype=np.float64)
+    _load().oracle_spd_grid_sw(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sw.ctypes.data,
+                               w.ctypes.data, sp.ctypes.data, int(w.size), t0, t1,
+                               snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
 
 
 def find_candidates(snr, width_idx, threshold: float, capacity: Optional[int] = None):
@@ -220,3 +255,20 @@ def find_candidates(snr, width_idx, threshold: float, capacity: Optional[int] = 
                                                c_snr.ctypes.data, c_w.ctypes.data))
     k = min(count, cap)
     return count, c_dm[:k], c_t[:k], c_snr[:k], c_w[:k]
+
+
+def cluster_candidates(snr, widths, c_dm, c_t, c_width, dm_radius: int) -> np.ndarray:
+    """Reading A18: 2-D (DM x time) peak rule over 1-D candidates of a float32 SNR plane.
+    ``c_width`` are indices into the ascending width set.  Returns the boolean keep mask."""
+    snr = _plane(snr)
+    n_dm, n_t = snr.shape
+    w = _widths(widths)
+    cd = np.ascontiguousarray(c_dm, dtype=np.int32)
+    ct = np.ascontiguousarray(c_t, dtype=np.int32)
+    cw = np.ascontiguousarray(c_width, dtype=np.int32)
+    assert cd.size == ct.size == cw.size
+    keep = np.zeros(cd.size, dtype=np.uint8)
+    _load().oracle_cluster_candidates(snr.ctypes.data, n_dm, n_t, w.ctypes.data, int(w.size),
+                                      cd.ctypes.data, ct.ctypes.data, cw.ctypes.data, int(cd.size),
+                                      int(dm_radius), keep.ctypes.data)
+    return keep.astype(bool)

@@ -33,9 +33,12 @@
  *                        interpolated (reading A17); oracle_spd_direct_sw uses it.
  *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
  *   oracle_row_stats   : per-row mean and population standard deviation (reading A6).
- *   oracle_row_stats_clipped: mean / sigma with point-wise outlier rejection
- *                        repeated a given number of times (reading A14).
+ *   oracle_spd_grid_sw : oracle_spd_grid with a measured standard deviation per width.
+ *   oracle_row_stats_clipped: mean / sigma with point-wise outlier rejection, a given number
+ *                        of passes or "until convergence" (reading A14),
+ *                        everything in double.
  *   oracle_find_candidates: threshold + 1-D local-peak rule (reading A9).
+ *   oracle_cluster_candidates: 2-D (DM x time) peak rule over the 1-D candidates (reading A18).
  *
  * Pins: tests/test_oracle_pins.py (closed form eq. 22 on single-pulse planes,
  * numpy.convolve for single widths, constant / ramp / impulse closed forms,
@@ -46,6 +49,10 @@
  * oracle_find_candidates: the rule is this project's reading A9 (the paper
  * names "peak-finding" only) - pinned by closed form on
  * isolated pulses; otherwise "parity unpinned by the paper".
+ * oracle_cluster_candidates: reading A18, this project's definition as well (same passages):
+ * pinned on hand-built planes (a pulse smeared over neighbouring DM rows gives one cluster at
+ * its peak; two pulses further apart than the window give two; exact ties keep the first in
+ * (dm, t) order) and against a brute-force window scan; "parity unpinned by the paper".
  */
 #include <math.h>
 #include <stdint.h>
@@ -238,6 +245,45 @@ void oracle_spd_direct_sw(const float* x, int64_t n_dm, int64_t n_t,
     }
 }
 
+/* oracle_spd_grid with a measured standard deviation per width (rows f1 + f2 together):
+ * SNR_L[n] = (X_L[n] - L mu_d) / sigma_{d,L} (eq. 4; sigma(X_L) measured and interpolated,
+ * PAPER.md:728) for the widths whose grid contains n (reading A16).  Pins: with sigma_w = sqrt(L) sigma
+ * it reproduces oracle_spd_grid bit for bit; with separations all 1 it reproduces oracle_spd_direct_sw. */
+void oracle_spd_grid_sw(const float* x, int64_t n_dm, int64_t n_t,
+                        const double* mean, const double* sigma_w,
+                        const int32_t* widths, const int32_t* seps, int32_t n_w,
+                        int64_t t0, int64_t t1,
+                        double* out_snr, int32_t* out_width, double* out_second) {
+    const int64_t span = t1 - t0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 256)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        for (int64_t n = t0; n < t1; ++n) {
+            const float* row = x + d * n_t;
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = 0; k < n_w; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;                       /* valid windows only (A3) */
+                if (n % (int64_t)seps[k] != 0) continue;      /* n is not on this width's grid (A16) */
+                double X = 0.0;
+                for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
+                const double snr = (X - (double)L * mean[d]) / sigma_w[d * n_w + k];  /* eq. (4) */
+                if (snr > best) {
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * span + (n - t0);
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+    }
+}
+
 /* Same quantities through a double-precision running sum of (x - mu). */
 void oracle_spd_prefix(const float* x, int64_t n_dm, int64_t n_t,
                        const double* mean, const double* sigma,
@@ -306,27 +352,38 @@ void oracle_row_stats(const float* x, int64_t n_dm, int64_t n_t, double* mean, d
     }
 }
 
-/* Mean and standard deviation with point-wise outlier rejection (PAPER.md:720-726,
- * sec. 4.6.2; reading A14).  Pass 0: mean and population sigma of all samples of the row.
- * Pass i = 1..n_reject_passes: "each point is compared with the current estimate of the mean
- * and standard deviation and rejected if it is significantly different (the threshold is
- * user defined)": keep x iff |x - mu| <= clip * sigma, with mu, sigma the float32-rounded
- * estimates of pass i-1 and the comparison in float32 (the precision the CUDA path takes
- * this decision in); mean and sigma of the kept samples by the plain two-pass definition in
- * double.  A pass that rejects every sample keeps the previous estimate.  Outputs are the
- * float32-rounded estimates widened to double. */
-void oracle_row_stats_clipped(const float* x, int64_t n_dm, int64_t n_t, float clip, int32_t n_reject_passes,
-                              double* mean, double* sigma) {
+/* Mean and standard deviation with point-wise outlier rejection (sec. 4.6.2:
+ * "Each point is compared with the current estimate of the mean and standard deviation and
+ * rejected if it is significantly different (the threshold is user defined).  This is repeated
+ * until convergence."; reading A14).  Everything in double:
+ *   pass 0: mean and population sigma of all samples of the row;
+ *   pass i >= 1: keep x iff |x - mu| <= clip * sigma with mu, sigma of pass i-1; mean and sigma
+ *           of the kept samples by the plain two-pass definition.
+ * Stops after max_reject_passes rejection passes or - "until convergence" - after the first
+ * pass that changes neither estimate by more than rel_tol * sigma(previous pass)
+ * (|mu_i - mu_(i-1)| and |sigma_i - sigma_(i-1)|; rel_tol < 0 never stops early, so that the
+ * pass count is the caller's).  A pass that rejects every sample keeps the previous estimate
+ * and stops.  n_passes[d] (may be NULL) receives the rejection passes done.
+ * n_border[d] (may be NULL) counts, over all passes, the samples within border_eps * sigma of
+ * the rejection limit: the samples whose side a single-precision implementation may decide
+ * differently (tests/ bound the CUDA path's deviation by it). */
+void oracle_row_stats_clipped(const float* x, int64_t n_dm, int64_t n_t, double clip,
+                              int32_t max_reject_passes, double rel_tol, double border_eps,
+                              double* mean, double* sigma, int32_t* n_passes, int64_t* n_border) {
 #pragma omp parallel for schedule(static)
     for (int64_t d = 0; d < n_dm; ++d) {
         const float* row = x + d * n_t;
-        float mu = 0.0f, sg = 0.0f;
-        for (int32_t pass = 0; pass <= n_reject_passes; ++pass) {
-            const float lim = clip * sg;
+        double mu = 0.0, sg = 0.0;
+        int32_t done = 0;
+        int64_t border = 0;
+        for (int32_t pass = 0; pass <= max_reject_passes; ++pass) {
+            const double lim = clip * sg;
             double s = 0.0;
             int64_t cnt = 0;
             for (int64_t n = 0; n < n_t; ++n) {
-                if (pass == 0 || fabsf(row[n] - mu) <= lim) {
+                const double dev = fabs((double)row[n] - mu);
+                if (pass > 0 && fabs(dev - lim) <= border_eps * sg) ++border;
+                if (pass == 0 || dev <= lim) {
                     s += (double)row[n];
                     ++cnt;
                 }
@@ -335,16 +392,22 @@ void oracle_row_stats_clipped(const float* x, int64_t n_dm, int64_t n_t, float c
             const double m = s / (double)cnt;
             double v = 0.0;
             for (int64_t n = 0; n < n_t; ++n) {
-                if (pass == 0 || fabsf(row[n] - mu) <= lim) {
+                if (pass == 0 || fabs((double)row[n] - mu) <= lim) {
                     const double e = (double)row[n] - m;
                     v += e * e;
                 }
             }
-            mu = (float)m;
-            sg = (float)sqrt(v / (double)cnt);
+            const double sg_new = sqrt(v / (double)cnt);
+            const int converged = pass > 0 && fabs(m - mu) <= rel_tol * sg && fabs(sg_new - sg) <= rel_tol * sg;
+            mu = m;
+            sg = sg_new;
+            if (pass > 0) done = pass;
+            if (converged) break;
         }
-        mean[d] = (double)mu;
-        sigma[d] = (double)sg;
+        mean[d] = mu;
+        sigma[d] = sg;
+        if (n_passes) n_passes[d] = done;
+        if (n_border) n_border[d] = border;
     }
 }
 
@@ -374,4 +437,45 @@ int64_t oracle_find_candidates(const float* snr, const int32_t* width, int64_t n
         }
     }
     return count;
+}
+
+/* 2-D (DM x time) peak rule over the 1-D candidates (the paper names the
+ * stage only: "lastly candidates are selected using a peak-finding algorithm").
+ * Reading A18 (this project's definition): a 1-D candidate (d, n) with best width L = widths[W[d,n]]
+ * is kept iff no sample of the window |d' - d| <= dm_radius, |n' - n| <= L (clipped to the plane)
+ * has a larger Y, and no sample of the window that comes EARLIER in (d, n) order has an equal Y
+ * (the first of an exact tie is the peak).  The half-width L ties the window to the width being
+ * tested, as a 3 x 3 neighbourhood on a plane decimated by the boxcar separation would.
+ * Inputs: the float32 planes and the candidate list (c_dm, c_t, c_width index into widths), any
+ * order; keep[i] receives 1 / 0.  Returns the number kept. */
+int64_t oracle_cluster_candidates(const float* snr, int64_t n_dm, int64_t n_t,
+                                  const int32_t* widths, int32_t n_w,
+                                  const int32_t* c_dm, const int32_t* c_t, const int32_t* c_width,
+                                  int64_t n_cand, int32_t dm_radius, uint8_t* keep) {
+    int64_t kept = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : kept)
+    for (int64_t i = 0; i < n_cand; ++i) {
+        const int64_t d = c_dm[i], n = c_t[i];
+        const int32_t wi = c_width[i];
+        const int64_t L = (wi >= 0 && wi < n_w) ? widths[wi] : 1;
+        const float v = snr[d * n_t + n];
+        const int64_t d_lo = d - dm_radius < 0 ? 0 : d - dm_radius;
+        const int64_t d_hi = d + dm_radius >= n_dm ? n_dm - 1 : d + dm_radius;
+        const int64_t n_lo = n - L < 0 ? 0 : n - L;
+        const int64_t n_hi = n + L >= n_t ? n_t - 1 : n + L;
+        int ok = 1;
+        for (int64_t dd = d_lo; dd <= d_hi && ok; ++dd) {
+            const float* y = snr + dd * n_t;
+            for (int64_t nn = n_lo; nn <= n_hi; ++nn) {
+                const float u = y[nn];
+                if (u > v || (u == v && (dd < d || (dd == d && nn < n)))) {
+                    ok = 0;
+                    break;
+                }
+            }
+        }
+        keep[i] = (uint8_t)ok;
+        kept += ok;
+    }
+    return kept;
 }

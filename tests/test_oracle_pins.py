@@ -116,8 +116,7 @@ def test_clipped_stats_zero_passes_is_plain_stats(oracle_lib):
     x = (rng.standard_normal((4, 5000)) * 1.7 - 0.4).astype(np.float32)
     mu0, sg0 = oracle_lib.row_stats(x)
     mu, sg = oracle_lib.row_stats_clipped(x, 2.0, 0)
-    assert np.array_equal(mu, mu0.astype(np.float32).astype(np.float64))
-    assert np.array_equal(sg, sg0.astype(np.float32).astype(np.float64))
+    assert np.array_equal(mu, mu0) and np.array_equal(sg, sg0)
 
 
 def test_clipped_stats_two_valued_row_with_outliers_exact(oracle_lib):
@@ -166,16 +165,59 @@ def test_clipped_stats_rejection_is_monotone_and_affine(oracle_lib):
     for a, b in zip(sgs, sgs[1:]):
         assert np.all(b <= a + 1e-12)              # rejecting outliers never raises sigma
     assert sgs[0][1] > 2.0 and abs(sgs[3][1] - sgs[3][0]) < 0.05  # the pulse is gone after a few passes
-    # power-of-two scaling and integer shift commute exactly with the float32 comparison
+    # scaling by a power of two is exact in float32 and in double: the kept sets are the same
     mu, sg = oracle_lib.row_stats_clipped(x, 2.5, 2)
     mu2, sg2 = oracle_lib.row_stats_clipped((x * np.float32(4.0)), 2.5, 2)
-    assert np.allclose(mu2, 4.0 * mu, rtol=0, atol=1e-6) and np.allclose(sg2, 4.0 * sg, rtol=1e-6)
+    assert np.array_equal(mu2, 4.0 * mu) and np.array_equal(sg2, 4.0 * sg)
 
 
 def test_clipped_stats_everything_rejected_keeps_estimate(oracle_lib):
     x = np.array([[0.0, 0.0, 10.0, 10.0]], dtype=np.float32)  # mean 5, sigma 5: clip 0.5 rejects all
     mu, sg = oracle_lib.row_stats_clipped(x, 0.5, 3)
     assert mu[0] == 5.0 and sg[0] == 5.0
+
+
+def test_clipped_stats_until_convergence(oracle_lib):
+    """PAPER.md:726 "This is repeated until convergence".  (a) The two-valued row with outliers: pass 1
+    removes exactly the outliers, pass 2 changes nothing, so the iteration stops after 2 rejection passes
+    whatever the pass limit; a row without outliers stops after 1.  (b) On N(0,1) data the fixed point of
+    sigma -> sigma_trunc(clip * sigma) is the root of s^2 = 1 - 2 t phi(t) / (2 Phi(t) - 1), t = clip * s
+    (variance of a normal truncated at +-t, textbook), found here by iterating the formula."""
+    n, k, V = 4000, 8, 50.0
+    row = np.tile(np.array([1.0, -1.0], dtype=np.float32), n // 2)
+    row_out = row.copy()
+    row_out[np.arange(k) * 401 + 7] = V
+    x = np.stack([row, row_out])
+    mu, sg, n_pass, _ = oracle_lib.row_stats_clipped(x, 3.0, 50, rel_tol=0.0, details=True)
+    assert list(n_pass) == [1, 2] and sg[0] == 1.0 and abs(sg[1] - 1.0) < 1e-5
+    mu5, sg5 = oracle_lib.row_stats_clipped(x, 3.0, 2)                 # the same two passes, counted by the caller
+    assert np.array_equal(mu, mu5) and np.array_equal(sg, sg5)
+    rng = np.random.default_rng(15)
+    y = rng.standard_normal((2, 1 << 20)).astype(np.float32)
+    clip = 2.0
+    mu, sg, n_pass, _ = oracle_lib.row_stats_clipped(y, clip, 200, rel_tol=1e-7, details=True)
+    s = 1.0
+    for _ in range(500):
+        t = clip * s
+        phi = math.exp(-0.5 * t * t) / math.sqrt(2.0 * math.pi)
+        Phi = 0.5 * (1.0 + math.erf(t / math.sqrt(2.0)))
+        s = math.sqrt(1.0 - 2.0 * t * phi / (2.0 * Phi - 1.0))
+    assert np.all(np.abs(sg - s) < 6e-3) and np.all(n_pass < 200) and np.all(n_pass > 5)
+    # a looser tolerance stops earlier and lands between the first pass and the fixed point
+    _, sg_loose, n_loose, _ = oracle_lib.row_stats_clipped(y, clip, 200, rel_tol=1e-2, details=True)
+    _, sg_one = oracle_lib.row_stats_clipped(y, clip, 1)
+    assert np.all(n_loose < n_pass) and np.all(sg_loose <= sg_one + 1e-12) and np.all(sg_loose >= sg - 1e-12)
+
+
+def test_clipped_stats_border_count(oracle_lib):
+    """n_border counts the samples within border_eps * sigma of the rejection limit, per pass: the row
+    (-1, +1) x 8 has mean 0, sigma 1; with clip 1 all sixteen samples sit exactly on the limit in every
+    pass (and are kept: '<='); with clip 2 none is within 1e-3."""
+    x = np.tile(np.array([-1.0, 1.0], dtype=np.float32), 8)[None, :]
+    mu, sg, n_pass, n_border = oracle_lib.row_stats_clipped(x, 1.0, 3, border_eps=1e-3, details=True)
+    assert mu[0] == 0.0 and sg[0] == 1.0 and n_pass[0] == 3 and n_border[0] == 3 * 16
+    _, _, _, n_border = oracle_lib.row_stats_clipped(x, 2.0, 3, border_eps=1e-3, details=True)
+    assert n_border[0] == 0
 
 
 # --- sec. 4.3: other pulse shapes (PAPER.md:529-581; reading A15) ---------------------
@@ -497,6 +539,9 @@ def test_width_sigma_is_numpy_on_hand_decimated_rows(oracle_lib):
     assert sw[0, 2] == pytest.approx(0.5 * (s2 + s4))              # L = 3: midway between 2 and 4
     assert sw[0, 4] == pytest.approx(s4 * math.sqrt(6 / 4))        # no level 8 (one element): sqrt law from 4
     assert sw[0, 5] == pytest.approx(s4 * math.sqrt(8 / 4))
+    # rows too short for any level with two elements: a single sample has no deviation (numpy agrees)
+    one = oracle_lib.width_sigma(np.array([[3.5]], dtype=np.float32), [1])
+    assert one[0, 0] == 0.0 == np.std(np.array([3.5]))
     rng = np.random.default_rng(3)
     y = (rng.standard_normal((2, 4096 + 37)) * 2.5 + 7).astype(np.float32)
     widths = [1, 2, 4, 5, 8, 16, 24, 64, 100, 256]
@@ -553,3 +598,115 @@ def test_direct_with_white_noise_sigma_table_is_direct(oracle_lib):
     only8 = oracle_lib.spd_direct_sw(x, [0.1, -0.2], table2[:, 3:4], [8])
     ref8 = oracle_lib.spd_direct(x, [0.1, -0.2], sg, [8])
     assert np.allclose(only8[0][:, :392], 2.0 * ref8[0][:, :392], rtol=1e-13)
+
+
+def test_grid_with_sigma_table_reduces_to_grid_and_to_direct_sw(oracle_lib):
+    """oracle_spd_grid_sw: the table sqrt(L) sigma reproduces oracle_spd_grid bit for bit (same expression
+    evaluated on the same doubles is not guaranteed, so: to 1e-13 and identical indices), separations all 1
+    reproduce oracle_spd_direct_sw exactly, and halving one width's sigma doubles that width's SNR on its
+    grid only."""
+    rng = np.random.default_rng(21)
+    x = rng.standard_normal((3, 500)).astype(np.float32)
+    x[1, 200:230] += 2.0
+    widths = [1, 2, 3, 4, 6, 8, 10, 12, 16, 24]
+    seps = [1, 1, 1, 1, 2, 2, 2, 2, 4, 4]
+    sg = np.array([1.5, 0.7, 1.0])
+    mu = [0.1, -0.2, 0.0]
+    table = sg[:, None] * np.sqrt(np.asarray(widths, dtype=np.float64))[None, :]
+    a = oracle_lib.spd_grid(x, mu, sg, widths, seps)
+    b = oracle_lib.spd_grid_sw(x, mu, table, widths, seps)
+    fin = np.isfinite(a[0])
+    assert np.array_equal(a[1], b[1]) and np.allclose(a[0][fin], b[0][fin], rtol=1e-13, atol=1e-13)
+    rough = rng.uniform(0.5, 2.0, size=table.shape) * table
+    c = oracle_lib.spd_direct_sw(x, mu, rough, widths)
+    d = oracle_lib.spd_grid_sw(x, mu, rough, widths, [1] * len(widths))
+    assert np.array_equal(c[0], d[0]) and np.array_equal(c[1], d[1]) and np.array_equal(c[2], d[2])
+    # a single width on a grid: SNR only at multiples of its separation, scaled by 1 / sigma_w
+    one = oracle_lib.spd_grid_sw(x, mu, 0.5 * table[:, 8:9], [16], [4])
+    ref = oracle_lib.spd_grid(x, mu, sg, [16], [4])
+    on = np.arange(500) % 4 == 0
+    valid = on & (np.arange(500) + 16 <= 500)
+    assert np.allclose(one[0][:, valid], 2.0 * ref[0][:, valid], rtol=1e-13)
+    assert np.all(np.isneginf(one[0][:, ~on])) and np.all(one[1][:, ~on] == -1)
+
+
+# --- f4: 2-D (DM x time) peaks over the 1-D candidates (reading A18; PAPER.md:708, 742) ----
+
+def _cluster_brute(snr, widths, c_dm, c_t, c_w, R):
+    """The rule of reading A18 written out with numpy windows."""
+    n_dm, n_t = snr.shape
+    keep = []
+    for d, n, wi in zip(c_dm, c_t, c_w):
+        L = int(widths[wi])
+        d0, d1 = max(0, d - R), min(n_dm - 1, d + R)
+        n0, n1 = max(0, n - L), min(n_t - 1, n + L)
+        win = snr[d0:d1 + 1, n0:n1 + 1]
+        v = snr[d, n]
+        ok = not np.any(win > v)
+        if ok:
+            dd, nn = np.nonzero(win == v)
+            first = min(zip(dd + d0, nn + n0))
+            ok = first == (d, n)
+        keep.append(ok)
+    return np.array(keep, dtype=bool)
+
+
+def test_cluster_one_pulse_smeared_over_dm_rows_is_one_cluster(oracle_lib):
+    """A pulse seen in five neighbouring DM rows with SNR falling away from the middle row, each row a
+    plateau with ripples: the 1-D rule (A9) reports several peaks per row, the 2-D rule (A18, dm_radius 1)
+    keeps exactly one - the highest sample of the middle row, with its width index."""
+    widths = [1, 2, 4, 8, 16, 32]
+    n_dm, n_t = 9, 600
+    snr = np.full((n_dm, n_t), 0.5, dtype=np.float32)
+    wid = np.zeros((n_dm, n_t), dtype=np.int32)
+    for d, amp in zip(range(2, 7), [7.0, 9.0, 12.0, 9.5, 6.5]):
+        t = np.arange(280, 321)
+        snr[d, t] = (amp - 0.02 * np.abs(t - 300) + 0.3 * ((t % 5) == 0)).astype(np.float32)
+        wid[d, t] = 5                                   # best width 32
+    cnt, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr, wid, 6.0)
+    assert cnt > 10                                     # ripples: many 1-D peaks
+    keep = oracle_lib.cluster_candidates(snr, widths, c_dm, c_t, c_w, 1)
+    assert keep.sum() == 1
+    i = int(np.nonzero(keep)[0][0])
+    assert (c_dm[i], c_t[i], c_w[i]) == (4, 300, 5) and c_snr[i] == np.float32(12.3)
+    assert np.array_equal(keep, _cluster_brute(snr, widths, c_dm, c_t, c_w, 1))
+
+
+def test_cluster_separation_ties_and_edges(oracle_lib):
+    """Two pulses further apart than the window are two clusters, closer than it one (the larger);
+    a pulse two rows away is separate at dm_radius 1 and merged at dm_radius 2; of two equal samples
+    inside each other's window the first in (dm, t) order is kept; windows are clipped at the edges."""
+    widths = [1, 2, 4, 8, 16]
+    n_dm, n_t = 6, 400
+
+    def run(points, R):
+        snr = np.zeros((n_dm, n_t), dtype=np.float32)
+        wid = np.zeros((n_dm, n_t), dtype=np.int32)
+        for d, t, v, wi in points:
+            snr[d, t] = v
+            wid[d, t] = wi
+        cnt, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr, wid, 5.0)
+        assert cnt == len(points)
+        keep = oracle_lib.cluster_candidates(snr, widths, c_dm, c_t, c_w, R)
+        assert np.array_equal(keep, _cluster_brute(snr, widths, c_dm, c_t, c_w, R))
+        return {(int(a), int(b)) for a, b, k in zip(c_dm, c_t, keep) if k}
+
+    assert run([(1, 100, 8.0, 3), (1, 109, 9.0, 3)], 1) == {(1, 100), (1, 109)}   # 9 > width 8: apart
+    assert run([(1, 100, 8.0, 3), (1, 108, 9.0, 3)], 1) == {(1, 108)}             # 8 <= 8: one cluster
+    assert run([(1, 100, 8.0, 0), (1, 108, 9.0, 4)], 1) == {(1, 100), (1, 108)}   # window = OWN width (1)
+    assert run([(1, 100, 8.0, 3), (3, 100, 9.0, 3)], 1) == {(1, 100), (3, 100)}
+    assert run([(1, 100, 8.0, 3), (3, 100, 9.0, 3)], 2) == {(3, 100)}
+    assert run([(2, 50, 7.0, 2), (2, 53, 7.0, 2), (1, 52, 7.0, 2)], 1) == {(1, 52)}  # ties: first in (dm, t)
+    assert run([(0, 0, 6.0, 4), (5, 399, 6.5, 4)], 3) == {(0, 0), (5, 399)}        # clipped windows
+
+
+def test_cluster_random_planes_match_window_scan(oracle_lib):
+    rng = np.random.default_rng(33)
+    widths = [1, 2, 3, 5, 8, 13, 21]
+    for R in (0, 1, 3):
+        snr = rng.standard_normal((12, 700)).astype(np.float32) * 2.0
+        snr = np.round(snr * 4) / 4                     # many exact ties
+        wid = rng.integers(0, len(widths), size=snr.shape).astype(np.int32)
+        cnt, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.astype(np.float32), wid, 2.0)
+        keep = oracle_lib.cluster_candidates(snr.astype(np.float32), widths, c_dm, c_t, c_w, R)
+        assert cnt > 50 and np.array_equal(keep, _cluster_brute(snr, widths, c_dm, c_t, c_w, R))
