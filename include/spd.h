@@ -32,14 +32,15 @@
  * message for the calling thread's last error is in spd_last_error_string().
  * There is NO CPU fallback: on a machine without an sm_100 device every
  * compute entry point fails with SPD_ERR_UNSUPPORTED_DEVICE.
+ * The library reads no environment variable: kernel choice and work split are plan flags
+ * (spd_plan_create_ex) and plan options (spd_plan_set_option).
  *
- * Environment variables read at plan creation (three test hooks, not tuning knobs):
- *   SPD_SEGS_PER_ROW=n      streaming trees: n independent streams per DM row instead of the
- *                           automatic choice (exercises the look-ahead replay of interior segments);
- *   SPD_TREE_KERNEL=block   widths {2^k}: keep the block-per-stream kernel where the warp-per-stream
- *                           kernel (9 <= K <= 14 widths, tensor-memory delay lines) would be chosen;
- *   SPD_GENERIC_WORKSPACE=1 any-width-set path: use the device-workspace kernels even where the
- *                           shared-memory tile kernel applies.
+ * Output-visible artefact of the streaming-tree kernels: the width index rides in the 5 low
+ * mantissa bits of the SNR while the maximum is taken, so out_snr differs from the exact float32
+ * product by up to 31 ulp (3.7e-6 relative, inside the 1e-4 tolerance of the method's parity
+ * rule).  The warp-per-stream kernel (spd_plan_info.tree_kernel == 2) stores those 5 bits as they
+ * are - the low mantissa bits of out_snr then equal 31 - out_width; the block-per-stream kernel
+ * (tree_kernel == 1) and the any-width-set kernels store them cleared / untouched.
  */
 #ifndef SPD_B200_SPD_H_
 #define SPD_B200_SPD_H_
@@ -50,7 +51,7 @@
 extern "C" {
 #endif
 
-#define SPD_VERSION 100
+#define SPD_VERSION 200
 
 typedef enum spd_status {
     SPD_OK = 0,
@@ -79,7 +80,22 @@ typedef enum spd_grid_kind {
 } spd_grid_kind;
 
 /* Plan creation flags (spd_plan_create_ex). */
-#define SPD_FLAG_FORCE_GENERIC 0x1u /* use the any-width-set kernels even where a streaming tree applies */
+#define SPD_FLAG_FORCE_GENERIC 0x1u     /* use the any-width-set kernels even where a streaming tree applies */
+#define SPD_FLAG_BLOCK_TREE 0x2u        /* widths {2^k}: keep the block-per-stream kernel where the warp-per-stream
+                                           kernel (9 <= K <= 14 widths, tensor-memory delay lines) would be chosen */
+#define SPD_FLAG_GENERIC_WORKSPACE 0x4u /* any-width-set path: use the device-workspace kernels even where the
+                                           shared-memory tile kernel applies */
+#define SPD_FLAG_WIDTH_U8 0x8u          /* out_width is uint8 [n_dm][n_t] instead of int32 (SURVEY.md sec. 8(f) row f4,
+                                           "compact width index": 9 B per sample instead of 12); 255 stands for -1.
+                                           SPD_PATH_DYADIC_TREE plans only (else SPD_ERR_INVALID_ARG) */
+
+/* Plan options (spd_plan_set_option). */
+#define SPD_OPT_SEGMENTS_PER_ROW 1 /* streaming trees: value >= 1 cuts every DM row into that many independent
+                                      streams (each replays its look-ahead once); value 0 restores the automatic
+                                      split (warp-per-stream kernel: one piece of the plane's steps per resident warp) */
+#define SPD_OPT_HOST_ROWS_PER_BLOCK 2 /* spd_run_host / spd_run_host_candidates: DM rows per staged row block
+                                         (value >= 1); value 0 restores the automatic choice (about 256 MiB of rows).
+                                         Frees the staging buffers; the next host call allocates them again */
 
 /* Which kernels a plan dispatches to (spd_plan_info.path). */
 #define SPD_PATH_DYADIC_TREE 1 /* streaming partial-sum tree, widths {1,2,4,...,2^(K-1)} */
@@ -117,6 +133,8 @@ typedef struct spd_plan_info {
     int32_t piece_chunks;       /* warp-per-stream kernel: steps per piece when the plane's steps are cut, in
                                    row-major order, into one piece per resident warp (pieces may span rows;
                                    segments_per_row is then 0); else 0 */
+    int32_t width_bytes;        /* bytes per element of out_width: 4, or 1 with SPD_FLAG_WIDTH_U8 */
+    uint32_t flags;             /* the SPD_FLAG_* bits the plan was created with */
 } spd_plan_info;
 
 /*
@@ -180,6 +198,15 @@ int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t,
 
 /* Frees the plan and everything it owns.  NULL is allowed. */
 void spd_plan_destroy(spd_plan* plan);
+/* The same under north_star's name (spd_plan_create / spd_run / spd_destroy). */
+void spd_destroy(spd_plan* plan);
+
+/*
+ * spd_plan_set_option - change one SPD_OPT_* setting of a plan; call it between runs (not while a
+ * run of this plan is being enqueued from another thread).  Returns SPD_ERR_INVALID_ARG for an
+ * unknown option, a value out of range, or an option that does not apply to the plan's path.
+ */
+int spd_plan_set_option(spd_plan* plan, int32_t option, int64_t value);
 
 /* Copies the plan's ascending width table to out[0..*n) (HOST); *n receives the count.
  * out may be NULL to query the count. */
@@ -194,7 +221,8 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info);
  *   mean, sigma: DEVICE, float32 [n_dm]; per-DM mu(x) and sigma(x) of eq. (5).
  *                sigma > 0 and finite inputs are preconditions (not checked).
  *   out_snr    : DEVICE, float32 [n_dm][n_t], fully overwritten with Y.
- *   out_width  : DEVICE, int32 [n_dm][n_t], fully overwritten with W.
+ *   out_width  : DEVICE, int32 [n_dm][n_t] (uint8 [n_dm][n_t] for a plan created with SPD_FLAG_WIDTH_U8),
+ *                fully overwritten with W.
  *   cuda_stream: a cudaStream_t (NULL = default stream).  The call only
  *                enqueues work; it never synchronises.
  * Buffers are owned by the caller and must not alias.  A SPD_PATH_DYADIC_TREE
@@ -203,7 +231,7 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info);
  * at a time.
  */
 int spd_run(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
-            float* out_snr, int32_t* out_width, void* cuda_stream);
+            float* out_snr, void* out_width, void* cuda_stream);
 
 /*
  * spd_find_candidates - threshold + 1-D peak stage (row a8; reading A9):
@@ -215,7 +243,7 @@ int spd_run(const spd_plan* plan, const float* plane, const float* mean, const f
  *               exceed capacity (overflow: only the first `capacity` appends are stored).
  * Asynchronous on cuda_stream.
  */
-int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+int spd_find_candidates(const spd_plan* plan, const float* out_snr, const void* out_width,
                         float threshold, spd_candidate* list, int64_t capacity,
                         int64_t* n_found, void* cuda_stream);
 
@@ -232,7 +260,7 @@ int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_
  * marks every block active.
  */
 int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
-                    float* out_snr, int32_t* out_width, float threshold, uint8_t* activity,
+                    float* out_snr, void* out_width, float threshold, uint8_t* activity,
                     void* cuda_stream);
 
 /*
@@ -241,7 +269,7 @@ int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean,
  * one).  Same rule, same outputs; samples of unmarked blocks are never candidates
  * because their Y is below the threshold.
  */
-int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const void* out_width,
                                 const uint8_t* activity, float threshold, spd_candidate* list,
                                 int64_t capacity, int64_t* n_found, void* cuda_stream);
 
@@ -281,12 +309,12 @@ int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean,
 /*
  * spd_run_sigma_w - spd_run with SNR_L = (X_L - L mean) / sigma_w[d][L's index] (eq. 4, PAPER.md:69,
  * with the measured sigma(X_L) of spd_width_sigma in place of eq. 5's sqrt(L) sigma).
- * For SPD_PATH_DYADIC_TREE plans on the warp-per-stream kernel (9 to 14 widths 2^k: spd_plan_info.tree_kernel
- * == 2), SPD_PATH_GENERIC plans (shared-memory tile kernel) and SPD_PATH_GRID plans; the other streaming-tree
- * plans return SPD_ERR_INVALID_ARG (create them with SPD_FLAG_FORCE_GENERIC).  Other arguments as spd_run.
+ * For every plan except SPD_PATH_GENERIC plans on the device-workspace kernels (max_width above about 45 000, or
+ * SPD_FLAG_GENERIC_WORKSPACE) and SPD_FLAG_WIDTH_U8 plans, which return SPD_ERR_INVALID_ARG.  Other arguments
+ * (alignment included) as spd_run.
  */
 int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,
-                    float* out_snr, int32_t* out_width, void* cuda_stream);
+                    float* out_snr, void* out_width, void* cuda_stream);
 
 /*
  * spd_run_host - the same hot path on HOST buffers (end-to-end entry point):
@@ -294,12 +322,63 @@ int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean,
  * Y and W back, overlapping copies and kernels on internal streams.
  *   plane, out_snr, out_width : HOST (pinned memory recommended), shapes as spd_run.
  *   mean, sigma               : HOST float32 [n_dm].
- * Blocks until the results are in out_snr / out_width.  Needs a
- * SPD_PATH_DYADIC_TREE or SPD_PATH_GENERIC plan; device staging buffers are
- * allocated on first use and kept in the plan (hence the non-const plan).
+ * Blocks until the results are in out_snr / out_width.  Any plan; device staging
+ * buffers are allocated on first use and kept in the plan (hence the non-const plan).
+ * On an error in the middle of the run the internal streams are drained before returning,
+ * so no copy into the caller's buffers is in flight afterwards.
  */
 int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const float* sigma,
-                 float* out_snr, int32_t* out_width);
+                 float* out_snr, void* out_width);
+
+/*
+ * spd_row_stats_converge - spd_row_stats "repeated until convergence": rejection
+ * passes go on, per DM row, until one changes neither the mean nor sigma by more than
+ * rel_tol * sigma(previous pass), or max_reject_passes are done (1 <= max_reject_passes <= 64,
+ * rel_tol >= 0).  The test runs on the device; a row that has converged is skipped by the later
+ * passes (its plane samples are not read again), so over-provisioning max_reject_passes costs
+ * kernel launches only.
+ *   n_passes : DEVICE int32 [n_dm] (may be NULL): rejection passes done for each row.
+ * Other arguments and conventions as spd_row_stats.
+ */
+int spd_row_stats_converge(const spd_plan* plan, const float* plane, float clip_sigma, int32_t max_reject_passes,
+                           float rel_tol, float* mean, float* sigma, int32_t* n_passes, void* cuda_stream);
+
+/*
+ * spd_cluster_candidates - 2-D (DM x time) peak stage over the 1-D candidates (SURVEY.md sec. 8(f)
+ * row f4; the paper names it only: "candidates are selected using a peak-finding algorithm",
+ * PAPER.md:708, 742).  Reading A18 (this project's definition): candidate (d, n) with best width
+ * L = widths[width_idx] is kept iff no sample of the window |d' - d| <= dm_radius, |n' - n| <= L
+ * (clipped to the plane) has a larger out_snr and none that comes earlier in (d, n) order has an
+ * equal one.
+ *   out_snr   : DEVICE plane written by spd_run*.
+ *   list_in   : DEVICE, the candidates of spd_find_candidates(_flagged); n_in : DEVICE int64, their
+ *               count as that call wrote it (values above capacity_in are clamped to it).
+ *   dm_radius : >= 0, half-height of the window in DM trials.
+ *   list_out  : DEVICE array of capacity_out spd_candidate (must not alias list_in); n_out : DEVICE
+ *               int64, receives the number kept (may exceed capacity_out: overflow as spd_find_candidates).
+ * Asynchronous on cuda_stream; order of list_out unspecified.
+ */
+int spd_cluster_candidates(const spd_plan* plan, const float* out_snr, const spd_candidate* list_in,
+                           const int64_t* n_in, int64_t capacity_in, int32_t dm_radius, spd_candidate* list_out,
+                           int64_t capacity_out, int64_t* n_out, void* cuda_stream);
+
+/*
+ * spd_run_host_candidates - end-to-end entry point that returns what a pipeline consumes: the
+ * candidate list.  Row blocks of the HOST plane go to the device, every block runs the hot path with
+ * the fused threshold test and the 1-D candidate stage (rows a1-a8), the 2-D peak stage runs over
+ * the whole list (row f4; skipped when dm_radius < 0), and only the list comes back.
+ *   plane, mean, sigma : HOST, as spd_run_host (pinned memory recommended).
+ *   list      : HOST array of `capacity` spd_candidate, in unspecified order; n_found : HOST int64,
+ *               the number found, which may exceed capacity (then only `capacity` are stored; with
+ *               the 2-D stage an overflow of the 1-D list makes the result incomplete - n_1d, if not
+ *               NULL, receives the 1-D count so that the caller can tell).
+ * Needs the whole plane's out_snr on the device when dm_radius >= 0 (windows cross row blocks):
+ * 4 B per sample of device memory, allocated on first use and kept; dm_radius < 0 needs two row
+ * blocks only.  Blocks until the list is in host memory.
+ */
+int spd_run_host_candidates(spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                            float threshold, int32_t dm_radius, spd_candidate* list, int64_t capacity,
+                            int64_t* n_found, int64_t* n_1d);
 
 /* Message describing the calling thread's most recent error ("" if none). */
 const char* spd_last_error_string(void);

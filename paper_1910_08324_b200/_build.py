@@ -14,8 +14,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-# SPD_B200_LIB points the binding at another build of the same library (kernel-tuning sweeps).
-LIB_PATH = os.environ.get("SPD_B200_LIB") or os.path.join(_HERE, "libspd_b200.so")
+LIB_PATH = os.path.join(_HERE, "libspd_b200.so")
 
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo", "--expt-relaxed-constexpr",
@@ -50,8 +49,6 @@ def nvcc_path() -> str:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every CUDA source for sm_100a into ``libspd_b200.so``; returns its path.
     The translation units are compiled in parallel (one nvcc per file), then linked."""
-    if os.environ.get("SPD_B200_LIB"):
-        return LIB_PATH  # an explicitly chosen build is used as it is
     if force or needs_build():
         from concurrent.futures import ThreadPoolExecutor
         nvcc = nvcc_path()

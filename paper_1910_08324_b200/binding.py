@@ -25,6 +25,11 @@ SPD_ERR_CUDA = -4
 SPD_WIDTHS_ALL, SPD_WIDTHS_POW2, SPD_WIDTHS_BOXDIT, SPD_WIDTHS_IGRID, SPD_WIDTHS_GEOMETRIC = range(5)
 WIDTH_KINDS = {"ALL": 0, "POW2": 1, "BOXDIT": 2, "IGRID": 3, "GEOMETRIC": 4}
 SPD_FLAG_FORCE_GENERIC = 0x1
+SPD_FLAG_BLOCK_TREE = 0x2
+SPD_FLAG_GENERIC_WORKSPACE = 0x4
+SPD_FLAG_WIDTH_U8 = 0x8
+SPD_OPT_SEGMENTS_PER_ROW = 1
+SPD_OPT_HOST_ROWS_PER_BLOCK = 2
 SPD_PATH_DYADIC_TREE, SPD_PATH_GENERIC, SPD_PATH_IGRID_TREE, SPD_PATH_GRID = 1, 2, 3, 4
 SPD_GRID_EVERY_SAMPLE, SPD_GRID_DIT, SPD_GRID_BOXDIT, SPD_GRID_IGRID = range(4)
 GRID_KINDS = {"EVERY_SAMPLE": 0, "DIT": 1, "BOXDIT": 2, "IGRID": 3}
@@ -36,6 +41,8 @@ EXPORTS = (
     "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
     "spd_run_host", "spd_last_error_string", "spd_version",
     "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
+    "spd_destroy", "spd_plan_set_option", "spd_row_stats_converge", "spd_cluster_candidates",
+    "spd_run_host_candidates",
 )
 
 
@@ -63,7 +70,9 @@ class spd_plan_info(ctypes.Structure):
                 ("activity_bytes", ctypes.c_int64), ("activity_block", ctypes.c_int32),
                 ("activity_per_row", ctypes.c_int32),
                 ("tree_kernel", ctypes.c_int32),
-                ("piece_chunks", ctypes.c_int32)]
+                ("piece_chunks", ctypes.c_int32),
+                ("width_bytes", ctypes.c_int32),
+                ("flags", ctypes.c_uint32)]
 
 
 _lib: Optional[ctypes.CDLL] = None
@@ -119,6 +128,17 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_row_stats.argtypes = [_vp, _vp, ctypes.c_float, _i32, _vp, _vp, _vp]
     lib.spd_run_host.restype = ctypes.c_int
     lib.spd_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+    lib.spd_destroy.restype = None
+    lib.spd_destroy.argtypes = [_vp]
+    lib.spd_plan_set_option.restype = ctypes.c_int
+    lib.spd_plan_set_option.argtypes = [_vp, _i32, _i64]
+    lib.spd_row_stats_converge.restype = ctypes.c_int
+    lib.spd_row_stats_converge.argtypes = [_vp, _vp, ctypes.c_float, _i32, ctypes.c_float, _vp, _vp, _vp, _vp]
+    lib.spd_cluster_candidates.restype = ctypes.c_int
+    lib.spd_cluster_candidates.argtypes = [_vp, _vp, _vp, _vp, _i64, _i32, _vp, _i64, _vp, _vp]
+    lib.spd_run_host_candidates.restype = ctypes.c_int
+    lib.spd_run_host_candidates.argtypes = [_vp, _vp, _vp, _vp, ctypes.c_float, _i32, _vp, _i64,
+                                            ctypes.POINTER(_i64), ctypes.POINTER(_i64)]
     _lib = lib
     return lib
 
@@ -191,7 +211,14 @@ def spd_plan_destroy(plan: int) -> None:
         load().spd_plan_destroy(_vp(plan))
 
 
-spd_destroy = spd_plan_destroy  # north_star's short name
+def spd_destroy(plan: int) -> None:
+    """north_star's name for spd_plan_destroy (the C symbol of the same name)."""
+    if plan:
+        load().spd_destroy(_vp(plan))
+
+
+def spd_plan_set_option(plan: int, option: int, value: int) -> None:
+    _check(load().spd_plan_set_option(_vp(plan), int(option), int(value)))
 
 
 def spd_plan_get_widths(plan: int) -> np.ndarray:
@@ -220,6 +247,11 @@ def _dev_ptr(t, dtype, numel: Optional[int], name: str) -> int:
     return t.data_ptr()
 
 
+def _width_dtype(info):
+    import torch
+    return torch.uint8 if info["width_bytes"] == 1 else torch.int32
+
+
 def _stream_handle(stream) -> int:
     import torch
     if stream is None:
@@ -240,7 +272,7 @@ def spd_run(plan: int, plane, mean, sigma, out_snr, out_width, stream=None) -> N
         _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
         _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
         _dev_ptr(out_snr, torch.float32, n, "out_snr"),
-        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _dev_ptr(out_width, _width_dtype(info), n, "out_width"),
         _vp(_stream_handle(stream))))
 
 
@@ -254,7 +286,7 @@ def spd_find_candidates(plan: int, out_snr, out_width, threshold: float, capacit
     n_found = torch.zeros(1, dtype=torch.int64, device=out_snr.device)
     _check(load().spd_find_candidates(
         _vp(plan), _dev_ptr(out_snr, torch.float32, n, "out_snr"),
-        _dev_ptr(out_width, torch.int32, n, "out_width"), ctypes.c_float(threshold),
+        _dev_ptr(out_width, _width_dtype(info), n, "out_width"), ctypes.c_float(threshold),
         _vp(lst.data_ptr()), int(capacity), _vp(n_found.data_ptr()), _vp(_stream_handle(stream))))
     return lst, n_found
 
@@ -272,7 +304,7 @@ def spd_run_flagged(plan: int, plane, mean, sigma, out_snr, out_width, threshold
         _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
         _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
         _dev_ptr(out_snr, torch.float32, n, "out_snr"),
-        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _dev_ptr(out_width, _width_dtype(info), n, "out_width"),
         ctypes.c_float(threshold),
         _dev_ptr(activity, torch.uint8, info["activity_bytes"], "activity"),
         _vp(_stream_handle(stream))))
@@ -291,7 +323,7 @@ def spd_find_candidates_flagged(plan: int, out_snr, out_width, activity, thresho
         n_found = torch.zeros(1, dtype=torch.int64, device=out_snr.device)
     _check(load().spd_find_candidates_flagged(
         _vp(plan), _dev_ptr(out_snr, torch.float32, n, "out_snr"),
-        _dev_ptr(out_width, torch.int32, n, "out_width"),
+        _dev_ptr(out_width, _width_dtype(info), n, "out_width"),
         _dev_ptr(activity, torch.uint8, info["activity_bytes"], "activity"), ctypes.c_float(threshold),
         _vp(lst.data_ptr()), int(capacity), _vp(n_found.data_ptr()), _vp(_stream_handle(stream))))
     return lst, n_found
@@ -312,6 +344,44 @@ def spd_row_stats(plan: int, plane, clip_sigma: float = 0.0, n_reject_passes: in
         _dev_ptr(mean, torch.float32, info["n_dm"], "mean"), _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
         _vp(_stream_handle(stream))))
     return mean, sigma
+
+
+def spd_row_stats_converge(plan: int, plane, clip_sigma: float, max_reject_passes: int, rel_tol: float,
+                           mean=None, sigma=None, n_passes=None, stream=None):
+    """spd_row_stats repeated until convergence on the device; returns (mean, sigma, n_passes)."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    if mean is None:
+        mean = torch.empty(info["n_dm"], dtype=torch.float32, device=plane.device)
+    if sigma is None:
+        sigma = torch.empty(info["n_dm"], dtype=torch.float32, device=plane.device)
+    if n_passes is None:
+        n_passes = torch.empty(info["n_dm"], dtype=torch.int32, device=plane.device)
+    _check(load().spd_row_stats_converge(
+        _vp(plan), _dev_ptr(plane, torch.float32, n, "plane"), ctypes.c_float(clip_sigma), int(max_reject_passes),
+        ctypes.c_float(rel_tol), _dev_ptr(mean, torch.float32, info["n_dm"], "mean"),
+        _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"), _dev_ptr(n_passes, torch.int32, info["n_dm"], "n_passes"),
+        _vp(_stream_handle(stream))))
+    return mean, sigma, n_passes
+
+
+def spd_cluster_candidates(plan: int, out_snr, lst, n_found, capacity_in: int, dm_radius: int, capacity_out: int,
+                           stream=None, lst_out=None, n_out=None):
+    """2-D (DM x time) peak stage over a candidate list; returns (list_out, n_out) as spd_find_candidates."""
+    import torch
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    if lst_out is None:
+        lst_out = torch.empty(max(int(capacity_out), 1) * ctypes.sizeof(spd_candidate), dtype=torch.uint8,
+                              device=out_snr.device)
+    if n_out is None:
+        n_out = torch.zeros(1, dtype=torch.int64, device=out_snr.device)
+    _check(load().spd_cluster_candidates(
+        _vp(plan), _dev_ptr(out_snr, torch.float32, n, "out_snr"), _vp(lst.data_ptr()), _vp(n_found.data_ptr()),
+        int(capacity_in), int(dm_radius), _vp(lst_out.data_ptr()), int(capacity_out), _vp(n_out.data_ptr()),
+        _vp(_stream_handle(stream))))
+    return lst_out, n_out
 
 
 def spd_width_sigma(plan: int, plane, mean, sigma_w=None, stream=None):
@@ -375,8 +445,33 @@ def spd_run_host(plan: int, plane, mean, sigma, out_snr, out_width) -> None:
     p1, _k1 = _host_ptr(mean, np.float32, info["n_dm"], "mean")
     p2, _k2 = _host_ptr(sigma, np.float32, info["n_dm"], "sigma")
     p3, _k3 = _host_ptr(out_snr, np.float32, n, "out_snr")
-    p4, _k4 = _host_ptr(out_width, np.int32, n, "out_width")
+    p4, _k4 = _host_ptr(out_width, np.uint8 if info["width_bytes"] == 1 else np.int32, n, "out_width")
     _check(load().spd_run_host(_vp(plan), _vp(p0), _vp(p1), _vp(p2), _vp(p3), _vp(p4)))
+
+
+def spd_run_host_candidates(plan: int, plane, mean, sigma, threshold: float, dm_radius: int, capacity: int,
+                            out_list=None):
+    """End-to-end call on HOST buffers that returns the candidate list (blocking).  ``out_list`` may be a
+    preallocated (pinned) uint8 buffer of capacity * 16 bytes.  Returns (n_found, n_1d, structured array of the
+    stored candidates sorted by (dm, t))."""
+    info = spd_plan_get_info(plan)
+    n = info["n_dm"] * info["n_t"]
+    p0, _k0 = _host_ptr(plane, np.float32, n, "plane")
+    p1, _k1 = _host_ptr(mean, np.float32, info["n_dm"], "mean")
+    p2, _k2 = _host_ptr(sigma, np.float32, info["n_dm"], "sigma")
+    nbytes = max(int(capacity), 1) * ctypes.sizeof(spd_candidate)
+    if out_list is None:
+        out_list = np.empty(nbytes, dtype=np.uint8)
+    p3, keep = _host_ptr(out_list, np.uint8, nbytes, "out_list")
+    n_found, n_1d = _i64(0), _i64(0)
+    _check(load().spd_run_host_candidates(_vp(plan), _vp(p0), _vp(p1), _vp(p2), ctypes.c_float(threshold),
+                                          int(dm_radius), _vp(p3), int(capacity), ctypes.byref(n_found),
+                                          ctypes.byref(n_1d)))
+    k = min(int(n_found.value), int(capacity))
+    raw = keep.numpy() if hasattr(keep, "numpy") else np.asarray(keep)
+    arr = raw[: k * ctypes.sizeof(spd_candidate)].view(CANDIDATE_DTYPE).copy()
+    arr.sort(order=["dm", "t"])
+    return int(n_found.value), int(n_1d.value), arr
 
 
 class Plan:
@@ -394,12 +489,20 @@ class Plan:
         self.widths = spd_plan_get_widths(self.handle)
         self.n_dm, self.n_t = int(n_dm), int(n_t)
 
+    def set_option(self, option: int, value: int):
+        spd_plan_set_option(self.handle, option, value)
+        self.info = spd_plan_get_info(self.handle)
+
+    def _new_width(self, device):
+        import torch
+        return torch.empty((self.n_dm, self.n_t), dtype=_width_dtype(self.info), device=device)
+
     def run(self, plane, mean, sigma, out_snr=None, out_width=None, stream=None):
         import torch
         if out_snr is None:
             out_snr = torch.empty((self.n_dm, self.n_t), dtype=torch.float32, device=plane.device)
         if out_width is None:
-            out_width = torch.empty((self.n_dm, self.n_t), dtype=torch.int32, device=plane.device)
+            out_width = self._new_width(plane.device)
         spd_run(self.handle, plane, mean, sigma, out_snr, out_width, stream)
         return out_snr, out_width
 
@@ -412,7 +515,7 @@ class Plan:
         if out_snr is None:
             out_snr = torch.empty((self.n_dm, self.n_t), dtype=torch.float32, device=plane.device)
         if out_width is None:
-            out_width = torch.empty((self.n_dm, self.n_t), dtype=torch.int32, device=plane.device)
+            out_width = self._new_width(plane.device)
         if activity is None:
             activity = torch.empty(self.info["activity_bytes"], dtype=torch.uint8, device=plane.device)
         spd_run_flagged(self.handle, plane, mean, sigma, out_snr, out_width, threshold, activity, stream)
@@ -426,6 +529,20 @@ class Plan:
     def row_stats(self, plane, clip_sigma: float = 0.0, n_reject_passes: int = 0, mean=None, sigma=None,
                   stream=None):
         return spd_row_stats(self.handle, plane, clip_sigma, n_reject_passes, mean, sigma, stream)
+
+    def row_stats_converge(self, plane, clip_sigma: float, max_reject_passes: int, rel_tol: float, mean=None,
+                           sigma=None, n_passes=None, stream=None):
+        return spd_row_stats_converge(self.handle, plane, clip_sigma, max_reject_passes, rel_tol, mean, sigma,
+                                      n_passes, stream)
+
+    def cluster_candidates(self, out_snr, lst, n_found, capacity_in: int, dm_radius: int, capacity_out: int,
+                           stream=None, lst_out=None, n_out=None):
+        return spd_cluster_candidates(self.handle, out_snr, lst, n_found, capacity_in, dm_radius, capacity_out,
+                                      stream, lst_out, n_out)
+
+    def run_host_candidates(self, plane, mean, sigma, threshold: float, dm_radius: int, capacity: int,
+                            out_list=None):
+        return spd_run_host_candidates(self.handle, plane, mean, sigma, threshold, dm_radius, capacity, out_list)
 
     def width_sigma(self, plane, mean, sigma_w=None, stream=None):
         return spd_width_sigma(self.handle, plane, mean, sigma_w, stream)

@@ -128,9 +128,21 @@ void release_host_staging(spd_plan* plan) {
         h.d_width[i] = nullptr;
         h.stream[i] = nullptr;
     }
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(h.d_act[i]);
+        h.d_act[i] = nullptr;
+    }
     cudaFree(h.d_mean);
     cudaFree(h.d_sigma);
-    h.d_mean = h.d_sigma = nullptr;
+    cudaFree(h.d_snr_full);
+    cudaFree(h.d_list);
+    cudaFree(h.d_list2);
+    cudaFree(h.d_counts);
+    if (h.h_counts) cudaFreeHost(h.h_counts);
+    h.d_mean = h.d_sigma = h.d_snr_full = nullptr;
+    h.d_list = h.d_list2 = nullptr;
+    h.d_counts = h.h_counts = nullptr;
+    h.list_cap = h.list2_cap = 0;
     h.ready = false;
 }
 
@@ -141,13 +153,14 @@ int prepare_host_staging(spd_plan* plan) {
     // streaming rate, small enough that two of them (double buffering) cost 1.5 GiB.
     const int64_t row_bytes = plan->n_t * 4;
     h.rows_per_block = std::max<int64_t>(1, std::min<int64_t>(plan->n_dm, (int64_t(256) << 20) / row_bytes));
+    if (plan->host_rows_option > 0) h.rows_per_block = std::min<int64_t>(plan->n_dm, plan->host_rows_option);
     const size_t elems = static_cast<size_t>(h.rows_per_block) * static_cast<size_t>(plan->n_t);
     cudaError_t e = cudaSuccess;
     for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
         if ((e = cudaStreamCreateWithFlags(&h.stream[i], cudaStreamNonBlocking)) != cudaSuccess) break;
         if ((e = cudaMalloc(&h.d_plane[i], elems * 4)) != cudaSuccess) break;
         if ((e = cudaMalloc(&h.d_snr[i], elems * 4)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&h.d_width[i], elems * 4)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&h.d_width[i], elems * plan->width_bytes)) != cudaSuccess) break;
     }
     if (e == cudaSuccess) e = cudaMalloc(&h.d_mean, sizeof(float) * plan->n_dm);
     if (e == cudaSuccess) e = cudaMalloc(&h.d_sigma, sizeof(float) * plan->n_dm);
@@ -161,20 +174,30 @@ int prepare_host_staging(spd_plan* plan) {
     return SPD_OK;
 }
 
+// Rows a1-a7 (+ the threshold test of a8 when activity != nullptr) over n_rows rows.
 int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const float* mean, const float* sigma,
-             float* out_snr, int32_t* out_width, cudaStream_t stream) {
+             float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
     if (plan->path == SPD_PATH_DYADIC_TREE)
-        return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
+        return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     if (plan->path == SPD_PATH_IGRID_TREE)
-        return ig_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
+        return ig_run(plan, n_rows, plane, mean, sigma, out_snr, static_cast<int32_t*>(out_width), threshold, activity,
+                      stream);
     if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1)
-        return ws_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr, stream);
-    return generic_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, stream);
+        return ws_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (activity) {
+        // any-width-set path: no fused test, every block stays active (padding included: the
+        // candidate kernel bounds the flag index itself)
+        const size_t bytes = (static_cast<size_t>(n_rows) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
+        const cudaError_t e = cudaMemsetAsync(activity, 1, bytes, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "filling the activity map");
+    }
+    return generic_run(plan, n_rows, plane, mean, sigma, out_snr, static_cast<int32_t*>(out_width), stream);
 }
 
-size_t activity_bytes(const spd_plan* plan) {
-    return (static_cast<size_t>(plan->n_dm) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
+size_t activity_bytes_rows(const spd_plan* plan, int64_t rows) {
+    return (static_cast<size_t>(rows) * static_cast<size_t>(activity_per_row(plan)) + 127) / 128 * 128;
 }
+size_t activity_bytes(const spd_plan* plan) { return activity_bytes_rows(plan, plan->n_dm); }
 
 bool misaligned16(const void* a, const void* b, const void* c) {
     return ((reinterpret_cast<uintptr_t>(a) | reinterpret_cast<uintptr_t>(b) | reinterpret_cast<uintptr_t>(c)) & 15u) != 0;
@@ -361,13 +384,21 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     plan->sm_count = sm_count;
     plan->separations = seps;
     plan->grid = groups;
+    plan->flags = flags;
+    plan->width_bytes = (flags & SPD_FLAG_WIDTH_U8) ? 1 : 4;
+    if ((flags & SPD_FLAG_WIDTH_U8) &&
+        (separations || (flags & SPD_FLAG_FORCE_GENERIC) || !tree_applicable(w, n_t))) {
+        set_error("SPD_FLAG_WIDTH_U8 needs a width set {1, 2, 4, ..., 2^(K-1)} on the streaming tree (n_t %% 4 == 0)");
+        delete plan;
+        return SPD_ERR_INVALID_ARG;
+    }
     int ig_levels = 0;
     if (separations) {
         plan->path = SPD_PATH_GRID;
         rc = generic_configure(plan);
         // widths {2^k} on a grid: the warp-per-stream tree kernel with the keys of a level counted only on
         // that level's grid (the any-width-set grid kernel stays configured for spd_run_sigma_w)
-        if (rc == SPD_OK && tree_applicable(w, n_t) && ws_applicable(static_cast<int>(w.size()))) {
+        if (rc == SPD_OK && tree_applicable(w, n_t) && ws_applicable(static_cast<int>(w.size()), 0u)) {
             plan->tree.K = static_cast<int>(w.size());
             rc = ws_configure(plan);
         }
@@ -404,6 +435,43 @@ void spd_plan_destroy(spd_plan* plan) {
     delete plan;
 }
 
+void spd_destroy(spd_plan* plan) { spd_plan_destroy(plan); }
+
+int spd_plan_set_option(spd_plan* plan, int32_t option, int64_t value) {
+    if (!plan) {
+        set_error("spd_plan_set_option: plan is NULL");
+        return SPD_ERR_INVALID_ARG;
+    }
+    switch (option) {
+        case SPD_OPT_SEGMENTS_PER_ROW: {
+            if (!runs_tree_kernel(plan) || value < 0 || value > 0x7fffffffll) {
+                set_error("SPD_OPT_SEGMENTS_PER_ROW needs a streaming-tree plan and a value >= 0 (got %lld)",
+                          static_cast<long long>(value));
+                return SPD_ERR_INVALID_ARG;
+            }
+            const int old = plan->segs_option;
+            plan->segs_option = static_cast<int>(value);
+            const int rc = plan->tree.kind == 1 ? ws_configure(plan) : tree_configure_segments(plan);
+            if (rc != SPD_OK) {
+                plan->segs_option = old;
+                if (plan->tree.kind == 1) ws_configure(plan); else tree_configure_segments(plan);
+            }
+            return rc;
+        }
+        case SPD_OPT_HOST_ROWS_PER_BLOCK:
+            if (value < 0) {
+                set_error("SPD_OPT_HOST_ROWS_PER_BLOCK needs a value >= 0");
+                return SPD_ERR_INVALID_ARG;
+            }
+            plan->host_rows_option = value;
+            release_host_staging(plan);
+            return SPD_OK;
+        default:
+            set_error("spd_plan_set_option: unknown option %d", option);
+            return SPD_ERR_INVALID_ARG;
+    }
+}
+
 int spd_plan_get_widths(const spd_plan* plan, int32_t* out, int32_t* n) {
     if (!plan || !n) {
         set_error("spd_plan_get_widths: NULL argument");
@@ -425,7 +493,9 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
     info->n_widths = static_cast<int32_t>(plan->widths.size());
     info->max_width = plan->max_width;
     info->path = plan->path;
-    if (is_tree_path(plan)) {
+    info->width_bytes = plan->width_bytes;
+    info->flags = plan->flags;
+    if (runs_tree_kernel(plan)) {
         info->launches_per_run = 1;
         info->threads_per_block = plan->tree.T;
         info->blocks = plan->tree.kind == 1 ? ws_grid_blocks(plan)
@@ -457,7 +527,7 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
 }
 
 int spd_run(const spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
-            int32_t* out_width, void* cuda_stream) {
+            void* out_width, void* cuda_stream) {
     if (!plan || !plane || !mean || !sigma || !out_snr || !out_width) {
         set_error("spd_run: NULL argument");
         return SPD_ERR_INVALID_ARG;
@@ -466,7 +536,8 @@ int spd_run(const spd_plan* plan, const float* plane, const float* mean, const f
         set_error("spd_run: plane, out_snr and out_width must be 16-byte aligned");
         return SPD_ERR_INVALID_ARG;
     }
-    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, static_cast<cudaStream_t>(cuda_stream));
+    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, 0.0f, nullptr,
+                    static_cast<cudaStream_t>(cuda_stream));
 }
 
 int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w, void* cuda_stream) {
@@ -478,36 +549,41 @@ int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean,
 }
 
 int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,
-                    float* out_snr, int32_t* out_width, void* cuda_stream) {
+                    float* out_snr, void* out_width, void* cuda_stream) {
     if (!plan || !plane || !mean || !sigma_w || !out_snr || !out_width) {
         set_error("spd_run_sigma_w: NULL argument");
         return SPD_ERR_INVALID_ARG;
     }
-    if (plan->path == SPD_PATH_DYADIC_TREE && plan->tree.kind == 1)  // warp-per-stream kernel: run-time scale per level
-        return ws_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width, 0.0f, nullptr,
-                      static_cast<cudaStream_t>(cuda_stream), sigma_w);
-    if (is_tree_path(plan)) {
-        set_error("spd_run_sigma_w: this plan's streaming-tree kernel scales by sqrt(width) at compile time; create "
-                  "the plan with SPD_FLAG_FORCE_GENERIC (or with spd_plan_create_grid) to use a measured sigma per "
-                  "width");
+    if (misaligned16(plane, out_snr, out_width)) {
+        set_error("spd_run_sigma_w: plane, out_snr and out_width must be 16-byte aligned");
         return SPD_ERR_INVALID_ARG;
     }
-    return generic_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width,
-                       static_cast<cudaStream_t>(cuda_stream), sigma_w);
+    if (plan->width_bytes != 4) {
+        set_error("spd_run_sigma_w: not available for SPD_FLAG_WIDTH_U8 plans");
+        return SPD_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (plan->path == SPD_PATH_DYADIC_TREE)  // run-time scale 1 / sigma_{d, 2^k} per level
+        return tree_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width, 0.0f, nullptr, stream, sigma_w);
+    if (plan->path == SPD_PATH_IGRID_TREE)
+        return ig_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, static_cast<int32_t*>(out_width), 0.0f, nullptr,
+                      stream, sigma_w);
+    return generic_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, static_cast<int32_t*>(out_width), stream,
+                       sigma_w);
 }
 
-int spd_find_candidates(const spd_plan* plan, const float* out_snr, const int32_t* out_width, float threshold,
+int spd_find_candidates(const spd_plan* plan, const float* out_snr, const void* out_width, float threshold,
                         spd_candidate* list, int64_t capacity, int64_t* n_found, void* cuda_stream) {
     if (!plan || !out_snr || !out_width || !n_found || capacity < 0 || (capacity > 0 && !list)) {
         set_error("spd_find_candidates: NULL argument or negative capacity");
         return SPD_ERR_INVALID_ARG;
     }
-    return candidates_run(plan, out_snr, out_width, nullptr, threshold, list, capacity, n_found,
+    return candidates_run(plan, plan->n_dm, 0, out_snr, out_width, nullptr, threshold, list, capacity, n_found, true,
                           static_cast<cudaStream_t>(cuda_stream));
 }
 
 int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
-                    int32_t* out_width, float threshold, uint8_t* activity, void* cuda_stream) {
+                    void* out_width, float threshold, uint8_t* activity, void* cuda_stream) {
     if (!plan || !plane || !mean || !sigma || !out_snr || !out_width || !activity) {
         set_error("spd_run_flagged: NULL argument");
         return SPD_ERR_INVALID_ARG;
@@ -516,21 +592,11 @@ int spd_run_flagged(const spd_plan* plan, const float* plane, const float* mean,
         set_error("spd_run_flagged: plane, out_snr, out_width and activity must be 16-byte aligned");
         return SPD_ERR_INVALID_ARG;
     }
-    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    if (plan->path == SPD_PATH_DYADIC_TREE)
-        return tree_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
-    if (plan->path == SPD_PATH_IGRID_TREE)
-        return ig_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
-    if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1)
-        return ws_run(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
-    // any-width-set path: no fused test, every block stays active (padding included: the
-    // candidate kernel bounds the flag index itself)
-    const cudaError_t e = cudaMemsetAsync(activity, 1, activity_bytes(plan), stream);
-    if (e != cudaSuccess) return cuda_fail(e, "filling the activity map");
-    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, stream);
+    return run_rows(plan, plan->n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity,
+                    static_cast<cudaStream_t>(cuda_stream));
 }
 
-int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
+int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, const void* out_width,
                                 const uint8_t* activity, float threshold, spd_candidate* list, int64_t capacity,
                                 int64_t* n_found, void* cuda_stream) {
     if (!plan || !out_snr || !out_width || !activity || !n_found || capacity < 0 || (capacity > 0 && !list)) {
@@ -541,7 +607,7 @@ int spd_find_candidates_flagged(const spd_plan* plan, const float* out_snr, cons
         set_error("spd_find_candidates_flagged: out_snr and activity must be 16-byte aligned");
         return SPD_ERR_INVALID_ARG;
     }
-    return candidates_run(plan, out_snr, out_width, activity, threshold, list, capacity, n_found,
+    return candidates_run(plan, plan->n_dm, 0, out_snr, out_width, activity, threshold, list, capacity, n_found, true,
                           static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -556,11 +622,39 @@ int spd_row_stats(const spd_plan* plan, const float* plane, float clip_sigma, in
                   n_reject_passes, static_cast<double>(clip_sigma));
         return SPD_ERR_INVALID_ARG;
     }
-    return stats_run(plan, plane, clip_sigma, n_reject_passes, mean, sigma, static_cast<cudaStream_t>(cuda_stream));
+    return stats_run(plan, plane, clip_sigma, n_reject_passes, -1.0f, mean, sigma, nullptr,
+                     static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_row_stats_converge(const spd_plan* plan, const float* plane, float clip_sigma, int32_t max_reject_passes,
+                           float rel_tol, float* mean, float* sigma, int32_t* n_passes, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma) {
+        set_error("spd_row_stats_converge: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (max_reject_passes < 1 || max_reject_passes > 64 || !(clip_sigma > 0.0f) || !(rel_tol >= 0.0f)) {
+        set_error("spd_row_stats_converge: need 1 <= max_reject_passes <= 64, clip_sigma > 0, rel_tol >= 0 "
+                  "(got %d, %g, %g)", max_reject_passes, static_cast<double>(clip_sigma), static_cast<double>(rel_tol));
+        return SPD_ERR_INVALID_ARG;
+    }
+    return stats_run(plan, plane, clip_sigma, max_reject_passes, rel_tol, mean, sigma, n_passes,
+                     static_cast<cudaStream_t>(cuda_stream));
+}
+
+int spd_cluster_candidates(const spd_plan* plan, const float* out_snr, const spd_candidate* list_in,
+                           const int64_t* n_in, int64_t capacity_in, int32_t dm_radius, spd_candidate* list_out,
+                           int64_t capacity_out, int64_t* n_out, void* cuda_stream) {
+    if (!plan || !out_snr || !n_in || !n_out || capacity_in < 0 || capacity_out < 0 || dm_radius < 0 ||
+        (capacity_in > 0 && !list_in) || (capacity_out > 0 && !list_out)) {
+        set_error("spd_cluster_candidates: NULL argument, negative capacity or negative dm_radius");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return cluster_run(plan, out_snr, list_in, n_in, capacity_in, dm_radius, list_out, capacity_out, n_out,
+                       static_cast<cudaStream_t>(cuda_stream));
 }
 
 int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const float* sigma, float* out_snr,
-                 int32_t* out_width) {
+                 void* out_width) {
     if (!plan || !plane || !mean || !sigma || !out_snr || !out_width) {
         set_error("spd_run_host: NULL argument");
         return SPD_ERR_INVALID_ARG;
@@ -576,27 +670,122 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
         (e = cudaStreamSynchronize(h.stream[0])) != cudaSuccess)
         return cuda_fail(e, "copying mean / sigma to the device");
     // The workspace variant of the any-width-set path shares one workspace: one stream.
-    const int n_streams = (is_tree_path(plan) || plan->generic_tile > 0) ? 2 : 1;
+    const int n_streams = (runs_tree_kernel(plan) || plan->generic_tile > 0) ? 2 : 1;
+    const size_t wb = static_cast<size_t>(plan->width_bytes);
     int64_t blk = 0;
-    for (int64_t r0 = 0; r0 < plan->n_dm; r0 += h.rows_per_block, ++blk) {
+    for (int64_t r0 = 0; r0 < plan->n_dm && rc == SPD_OK; r0 += h.rows_per_block, ++blk) {
+        const int64_t rows = std::min<int64_t>(h.rows_per_block, plan->n_dm - r0);
+        const int b = static_cast<int>(blk % 2);
+        cudaStream_t st = h.stream[blk % n_streams];  // buffer b was last used two blocks ago on this stream
+        const size_t off = static_cast<size_t>(r0) * static_cast<size_t>(plan->n_t);
+        const size_t elems = static_cast<size_t>(rows) * static_cast<size_t>(plan->n_t);
+        if ((e = cudaMemcpyAsync(h.d_plane[b], plane + off, elems * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+            rc = cuda_fail(e, "copying a row block to the device");
+            break;
+        }
+        rc = run_rows(plan, rows, h.d_plane[b], h.d_mean + r0, h.d_sigma + r0, h.d_snr[b], h.d_width[b], 0.0f, nullptr,
+                      st);
+        if (rc != SPD_OK) break;
+        if ((e = cudaMemcpyAsync(out_snr + off, h.d_snr[b], elems * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(static_cast<char*>(out_width) + off * wb, h.d_width[b], elems * wb,
+                                 cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+            rc = cuda_fail(e, "copying results to the host");
+    }
+    // drain both streams whatever happened: no copy into the caller's buffers stays in flight
+    for (int i = 0; i < 2; ++i)
+        if ((e = cudaStreamSynchronize(h.stream[i])) != cudaSuccess && rc == SPD_OK)
+            rc = cuda_fail(e, "waiting for the host run");
+    return rc;
+}
+
+int spd_run_host_candidates(spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                            float threshold, int32_t dm_radius, spd_candidate* list, int64_t capacity,
+                            int64_t* n_found, int64_t* n_1d) {
+    if (!plan || !plane || !mean || !sigma || !n_found || capacity < 0 || (capacity > 0 && !list)) {
+        set_error("spd_run_host_candidates: NULL argument or negative capacity");
+        return SPD_ERR_INVALID_ARG;
+    }
+    int rc = prepare_host_staging(plan);
+    if (rc != SPD_OK) return rc;
+    HostStaging& h = plan->host;
+    cudaError_t e = cudaSuccess;
+    const bool two_d = dm_radius >= 0;
+    // device lists: the 1-D list of all blocks (at least 2^22 entries: a pulse gives hundreds of 1-D peaks),
+    // the list after the 2-D stage (the caller's capacity)
+    const int64_t cap1 = std::max<int64_t>(capacity, int64_t(1) << 22);
+    const size_t act_bytes = activity_bytes_rows(plan, h.rows_per_block);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i)
+        if (!h.d_act[i]) e = cudaMalloc(&h.d_act[i], act_bytes);
+    if (e == cudaSuccess && !h.d_counts) e = cudaMalloc(&h.d_counts, 2 * sizeof(int64_t));
+    if (e == cudaSuccess && !h.h_counts) e = cudaMallocHost(&h.h_counts, 2 * sizeof(int64_t));
+    if (e == cudaSuccess && h.list_cap < cap1) {
+        cudaFree(h.d_list);
+        h.d_list = nullptr;
+        h.list_cap = 0;
+        if ((e = cudaMalloc(&h.d_list, sizeof(spd_candidate) * static_cast<size_t>(cap1))) == cudaSuccess) h.list_cap = cap1;
+    }
+    if (e == cudaSuccess && two_d && h.list2_cap < std::max<int64_t>(capacity, 1)) {
+        cudaFree(h.d_list2);
+        h.d_list2 = nullptr;
+        h.list2_cap = 0;
+        const int64_t c2 = std::max<int64_t>(capacity, 1);
+        if ((e = cudaMalloc(&h.d_list2, sizeof(spd_candidate) * static_cast<size_t>(c2))) == cudaSuccess) h.list2_cap = c2;
+    }
+    if (e == cudaSuccess && two_d && !h.d_snr_full)
+        e = cudaMalloc(&h.d_snr_full, sizeof(float) * static_cast<size_t>(plan->n_dm) * static_cast<size_t>(plan->n_t));
+    if (e != cudaSuccess) {
+        set_error("allocating the candidate staging buffers failed: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return SPD_ERR_ALLOC;
+    }
+    if ((e = cudaMemcpyAsync(h.d_mean, mean, sizeof(float) * plan->n_dm, cudaMemcpyHostToDevice, h.stream[0])) !=
+            cudaSuccess ||
+        (e = cudaMemcpyAsync(h.d_sigma, sigma, sizeof(float) * plan->n_dm, cudaMemcpyHostToDevice, h.stream[0])) !=
+            cudaSuccess ||
+        (e = cudaMemsetAsync(h.d_counts, 0, 2 * sizeof(int64_t), h.stream[0])) != cudaSuccess ||
+        (e = cudaStreamSynchronize(h.stream[0])) != cudaSuccess)
+        return cuda_fail(e, "copying mean / sigma to the device");
+    const int n_streams = (runs_tree_kernel(plan) || plan->generic_tile > 0) ? 2 : 1;
+    int64_t blk = 0;
+    for (int64_t r0 = 0; r0 < plan->n_dm && rc == SPD_OK; r0 += h.rows_per_block, ++blk) {
         const int64_t rows = std::min<int64_t>(h.rows_per_block, plan->n_dm - r0);
         const int b = static_cast<int>(blk % 2);
         cudaStream_t st = h.stream[blk % n_streams];
         const size_t off = static_cast<size_t>(r0) * static_cast<size_t>(plan->n_t);
-        const size_t bytes = static_cast<size_t>(rows) * static_cast<size_t>(plan->n_t) * 4;
-        if (n_streams == 1 && blk >= 2) {
-            // buffer b was last used two blocks ago on the same stream: stream order suffices
+        const size_t elems = static_cast<size_t>(rows) * static_cast<size_t>(plan->n_t);
+        if ((e = cudaMemcpyAsync(h.d_plane[b], plane + off, elems * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess) {
+            rc = cuda_fail(e, "copying a row block to the device");
+            break;
         }
-        if ((e = cudaMemcpyAsync(h.d_plane[b], plane + off, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-            return cuda_fail(e, "copying a row block to the device");
-        rc = run_rows(plan, rows, h.d_plane[b], h.d_mean + r0, h.d_sigma + r0, h.d_snr[b], h.d_width[b], st);
-        if (rc != SPD_OK) return rc;
-        if ((e = cudaMemcpyAsync(out_snr + off, h.d_snr[b], bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-            (e = cudaMemcpyAsync(out_width + off, h.d_width[b], bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-            return cuda_fail(e, "copying results to the host");
+        float* const snr = two_d ? h.d_snr_full + off : h.d_snr[b];
+        rc = run_rows(plan, rows, h.d_plane[b], h.d_mean + r0, h.d_sigma + r0, snr, h.d_width[b], threshold, h.d_act[b],
+                      st);
+        if (rc == SPD_OK)
+            rc = candidates_run(plan, rows, r0, snr, h.d_width[b], h.d_act[b], threshold, h.d_list, h.list_cap,
+                                h.d_counts, false, st);
     }
     for (int i = 0; i < 2; ++i)
-        if ((e = cudaStreamSynchronize(h.stream[i])) != cudaSuccess) return cuda_fail(e, "waiting for the host run");
+        if ((e = cudaStreamSynchronize(h.stream[i])) != cudaSuccess && rc == SPD_OK)
+            rc = cuda_fail(e, "waiting for the row blocks");
+    if (rc != SPD_OK) return rc;
+    cudaStream_t st = h.stream[0];
+    if (two_d) {
+        rc = cluster_run(plan, h.d_snr_full, h.d_list, h.d_counts, h.list_cap, dm_radius, h.d_list2, capacity,
+                         h.d_counts + 1, st);
+        if (rc != SPD_OK) return rc;
+    }
+    if ((e = cudaMemcpyAsync(h.h_counts, h.d_counts, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess)
+        return cuda_fail(e, "reading the candidate counts");
+    const int64_t found = two_d ? h.h_counts[1] : h.h_counts[0];
+    const int64_t stored = std::min<int64_t>(found, two_d ? capacity : std::min<int64_t>(capacity, h.list_cap));
+    if (stored > 0 &&
+        ((e = cudaMemcpyAsync(list, two_d ? h.d_list2 : h.d_list, sizeof(spd_candidate) * static_cast<size_t>(stored),
+                              cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+         (e = cudaStreamSynchronize(st)) != cudaSuccess))
+        return cuda_fail(e, "copying the candidate list to the host");
+    *n_found = found;
+    if (n_1d) *n_1d = h.h_counts[0];
     return SPD_OK;
 }
 

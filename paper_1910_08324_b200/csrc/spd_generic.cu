@@ -417,7 +417,7 @@ int generic_configure(spd_plan* plan) {
         generic_release(plan);
         return SPD_ERR_INVALID_ARG;
     }
-    if (M - 1 + 4096 <= kTileSpanMax && (is_grid || !std::getenv("SPD_GENERIC_WORKSPACE"))) {
+    if (M - 1 + 4096 <= kTileSpanMax && (is_grid || !(plan->flags & SPD_FLAG_GENERIC_WORKSPACE))) {
         // a grid plan also keeps 8 bytes of running best per sample of the tile in shared memory
         const int64_t tile_max = is_grid ? std::max<int64_t>(1024, ((200 << 10) - 4 * M) / 12 / 1024 * 1024)
                                          : (kTileSpanMax - (M - 1)) / kSub * kSub;

@@ -46,9 +46,17 @@ struct HostStaging {
     cudaStream_t stream[2] = {nullptr, nullptr};
     float* d_plane[2] = {nullptr, nullptr};
     float* d_snr[2] = {nullptr, nullptr};
-    int32_t* d_width[2] = {nullptr, nullptr};
+    void* d_width[2] = {nullptr, nullptr};
     float* d_mean = nullptr;
     float* d_sigma = nullptr;
+    // spd_run_host_candidates
+    uint8_t* d_act[2] = {nullptr, nullptr};  // activity map of one row block
+    float* d_snr_full = nullptr;             // whole-plane Y for the 2-D peak stage (allocated on first use)
+    spd_candidate* d_list = nullptr;         // 1-D candidates of all blocks
+    spd_candidate* d_list2 = nullptr;        // after the 2-D stage
+    int64_t list_cap = 0, list2_cap = 0;
+    int64_t* d_counts = nullptr;             // [0] 1-D count, [1] 2-D count
+    int64_t* h_counts = nullptr;             // pinned copy
 };
 
 }  // namespace spd
@@ -58,6 +66,10 @@ struct spd_plan {
     std::vector<int32_t> widths;
     int32_t max_width = 0;
     int32_t path = 0;
+    uint32_t flags = 0;      // SPD_FLAG_* of spd_plan_create_ex
+    int width_bytes = 4;     // out_width element size: 4, or 1 (SPD_FLAG_WIDTH_U8)
+    int segs_option = 0;     // SPD_OPT_SEGMENTS_PER_ROW (0 = automatic)
+    int64_t host_rows_option = 0;  // SPD_OPT_HOST_ROWS_PER_BLOCK (0 = automatic)
     int device = 0;
     int sm_count = 0;
     // dyadic tree
@@ -77,6 +89,7 @@ struct spd_plan {
     int64_t workspace_bytes = 0;
     // spd_row_stats
     void* d_stats = nullptr;  // [n_dm][stats_parts] partial moments
+    int32_t* d_stats_state = nullptr;  // [n_dm][2]: converged flag, rejection passes done
     int stats_parts = 0;
     int64_t stats_part = 0;   // samples per part
     // spd_width_sigma
@@ -99,18 +112,19 @@ int tree_configure(spd_plan* plan);
 int tree_configure_segments(spd_plan* plan);
 // activity: nullptr, or [n_dm][chunks_per_row] bytes (cleared here, set by the kernel for
 // every chunk whose best SNR reaches `threshold`).
+// sigma_w: nullptr (eq. 5), or [n_dm][K] measured standard deviations per width (then sigma is not read)
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
-             const float* sigma, float* out_snr, int32_t* out_width, float threshold,
-             uint8_t* activity, cudaStream_t stream);
+             const float* sigma, float* out_snr, void* out_width, float threshold,
+             uint8_t* activity, cudaStream_t stream, const float* sigma_w = nullptr);
 
 // spd_tree_ws.cu: the dyadic tree with one warp per stream (tensor-memory delay lines)
-bool ws_applicable(int K);
+bool ws_applicable(int K, uint32_t flags);
 int ws_configure(spd_plan* plan);
 int ws_grid_blocks(const spd_plan* plan);
 int ws_piece_chunks(const spd_plan* plan);
 // sigma_w: nullptr (eq. 5), or [n_dm][K] measured standard deviations per width (then sigma is not read)
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+           float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
            const float* sigma_w = nullptr);
 
 // spd_tree_ig.cu: widths 2^k and 3 * 2^m (IGRID depth 1)
@@ -118,7 +132,7 @@ int ig_applicable(const std::vector<int32_t>& widths, int64_t n_t);  // K (pow-2
 int ig_configure(spd_plan* plan);
 int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,
            const float* sigma, float* out_snr, int32_t* out_width, float threshold,
-           uint8_t* activity, cudaStream_t stream);
+           uint8_t* activity, cudaStream_t stream, const float* sigma_w = nullptr);
 
 inline bool is_tree_path(const spd_plan* plan) {
     return plan->path == SPD_PATH_DYADIC_TREE || plan->path == SPD_PATH_IGRID_TREE;
@@ -141,8 +155,10 @@ int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const fl
 // spd_stats.cu
 int stats_configure(spd_plan* plan);
 void stats_release(spd_plan* plan);
-int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float* mean,
-              float* sigma, cudaStream_t stream);
+// rel_tol < 0: exactly n_iter rejection passes; else stop a row once a pass changes neither estimate by
+// more than rel_tol * sigma (device-side test); n_passes: nullptr or [n_dm] rejection passes done.
+int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float rel_tol, float* mean,
+              float* sigma, int32_t* n_passes, cudaStream_t stream);
 
 // spd_width_sigma.cu: standard deviation per width from power-of-two decimations
 int wsig_configure(spd_plan* plan);
@@ -152,9 +168,15 @@ int wsig_run(const spd_plan* plan, const float* plane, const float* mean, float*
 // spd_candidates.cu
 // activity: nullptr (visit every sample) or the map written by spd_run_flagged, one byte
 // per `act_block` samples of each row (`act_per_row` bytes per row).
-int candidates_run(const spd_plan* plan, const float* out_snr, const int32_t* out_width,
-                   const uint8_t* activity, float threshold, spd_candidate* list, int64_t capacity,
-                   int64_t* n_found, cudaStream_t stream);
+// The planes hold n_rows rows whose first is DM trial dm_offset (candidates carry dm_offset + row);
+// clear: zero *n_found first (false: append to a list other launches are filling too).
+int candidates_run(const spd_plan* plan, int64_t n_rows, int64_t dm_offset, const float* out_snr,
+                   const void* out_width, const uint8_t* activity, float threshold, spd_candidate* list,
+                   int64_t capacity, int64_t* n_found, bool clear, cudaStream_t stream);
+// 2-D peak stage over a candidate list (reading A18); out_snr is the whole plane.
+int cluster_run(const spd_plan* plan, const float* out_snr, const spd_candidate* list_in, const int64_t* n_in,
+                int64_t capacity_in, int dm_radius, spd_candidate* list_out, int64_t capacity_out, int64_t* n_out,
+                cudaStream_t stream);
 
 // Activity-map geometry of a plan (both paths): samples per byte and bytes per row.
 int64_t activity_block(const spd_plan* plan);

@@ -8,8 +8,11 @@
 //
 // Reading (A14): pass 0 takes every sample; each further pass takes the samples with
 // |x - mu| <= clip * sigma of the previous pass (comparison in float32 on the float32 mu, sigma
-// the caller receives); sigma is the population standard deviation (ddof 0, as reading A6); the
-// caller fixes the number of rejection passes (the paper's convergence rule is not given).
+// the caller receives - the oracle decides in double and counts the border-line samples); sigma is
+// the population standard deviation (ddof 0, as reading A6).  The caller fixes the number of
+// rejection passes (spd_row_stats), or gives a limit and a tolerance (spd_row_stats_converge):
+// "until convergence" is then tested on the device, per row, on the double-precision estimates of
+// consecutive passes, and the blocks of a converged row return at once in the passes that follow.
 //
 // Partial statistics (n, mean, M2) are combined with the pairwise update of Chan, Golub &
 // LeVeque: delta = mean_b - mean_a, mean = mean_a + delta n_b / n,
@@ -32,6 +35,12 @@ constexpr int kStatThreads = 256;
 
 struct Moments {
     double n, mean, m2;
+};
+
+// Per-row state of the iteration (plan workspace): estimates of the last pass in double.
+struct RowState {
+    int32_t converged, passes;
+    double mu, sg;
 };
 
 __device__ __forceinline__ Moments merge(const Moments a, const Moments b) {
@@ -61,9 +70,11 @@ __global__ void __launch_bounds__(kStatThreads) row_moments_kernel(const float* 
                                                                    long long part, int parts, int clip_on,
                                                                    float clip, const float* __restrict__ mean,
                                                                    const float* __restrict__ sigma,
+                                                                   const RowState* __restrict__ state,
                                                                    Moments* __restrict__ out) {
     __shared__ Moments warp_m[kStatThreads / 32];
     const long long d = blockIdx.x / parts;
+    if (clip_on && state[d].converged) return;  // this row's iteration has stopped
     const int b = blockIdx.x - static_cast<int>(d) * parts;
     const float* __restrict__ row = plane + d * n_t;
     const long long lo = static_cast<long long>(b) * part;
@@ -121,17 +132,40 @@ __global__ void __launch_bounds__(kStatThreads) row_moments_kernel(const float* 
     }
 }
 
-// One thread per row: merge its parts in order, write float32 mean and population sigma.
-__global__ void row_moments_finish_kernel(const Moments* __restrict__ parts_m, int parts, long long n_dm,
-                                          float* __restrict__ mean, float* __restrict__ sigma) {
+// One thread per row: merge its parts in order, write float32 mean and population sigma, and decide
+// whether the row's iteration stops ("repeated until convergence").
+__global__ void row_moments_finish_kernel(const Moments* __restrict__ parts_m, int parts, long long n_dm, int pass,
+                                          float rel_tol, RowState* __restrict__ state, float* __restrict__ mean,
+                                          float* __restrict__ sigma, int32_t* __restrict__ n_passes) {
     const long long d = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (d >= n_dm) return;
+    RowState st = state[d];
+    if (pass == 0) {
+        st.converged = 0;
+        st.passes = 0;
+    } else if (st.converged) {
+        return;
+    }
     Moments t = parts_m[d * parts];
     for (int b = 1; b < parts; ++b) t = merge(t, parts_m[d * parts + b]);
-    // no sample survived the rejection: keep the previous estimate
-    if (t.n == 0.0) return;
-    mean[d] = static_cast<float>(t.mean);
-    sigma[d] = static_cast<float>(sqrt(t.m2 / t.n));
+    if (t.n == 0.0) {
+        // no sample survived the rejection: keep the previous estimate and stop
+        st.converged = 1;
+    } else {
+        const double mu = t.mean, sg = sqrt(t.m2 / t.n);
+        if (pass > 0) {
+            st.passes = pass;
+            if (rel_tol >= 0.0f && fabs(mu - st.mu) <= static_cast<double>(rel_tol) * st.sg &&
+                fabs(sg - st.sg) <= static_cast<double>(rel_tol) * st.sg)
+                st.converged = 1;
+        }
+        st.mu = mu;
+        st.sg = sg;
+        mean[d] = static_cast<float>(mu);
+        sigma[d] = static_cast<float>(sg);
+    }
+    state[d] = st;
+    if (n_passes) n_passes[d] = st.passes;
 }
 
 }  // namespace
@@ -158,17 +192,30 @@ int stats_configure(spd_plan* plan) {
         return SPD_ERR_ALLOC;
     }
     plan->workspace_bytes += static_cast<int64_t>(bytes);
+    const size_t sbytes = sizeof(RowState) * static_cast<size_t>(plan->n_dm);
+    void* st = nullptr;
+    const cudaError_t e2 = cudaMalloc(&st, sbytes);
+    if (e2 != cudaSuccess) {
+        set_error("device allocation of the statistics state (%zu bytes) failed: %s", sbytes, cudaGetErrorString(e2));
+        cudaGetLastError();
+        return SPD_ERR_ALLOC;
+    }
+    plan->d_stats_state = static_cast<int32_t*>(st);
+    plan->workspace_bytes += static_cast<int64_t>(sbytes);
     return SPD_OK;
 }
 
 void stats_release(spd_plan* plan) {
     cudaFree(plan->d_stats);
+    cudaFree(plan->d_stats_state);
     plan->d_stats = nullptr;
+    plan->d_stats_state = nullptr;
 }
 
-int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float* mean, float* sigma,
-              cudaStream_t stream) {
+int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, float rel_tol, float* mean,
+              float* sigma, int32_t* n_passes, cudaStream_t stream) {
     Moments* ws = static_cast<Moments*>(plan->d_stats);
+    RowState* state = reinterpret_cast<RowState*>(plan->d_stats_state);
     const int parts = plan->stats_parts;
     const unsigned grid = static_cast<unsigned>(plan->n_dm * parts);
     const bool vec = plan->n_t % 4 == 0 && (reinterpret_cast<uintptr_t>(plane) & 15u) == 0;
@@ -177,11 +224,12 @@ int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, 
         const int clip_on = pass > 0;
         if (vec)
             row_moments_kernel<true><<<grid, kStatThreads, 0, stream>>>(plane, plan->n_t, plan->stats_part, parts,
-                                                                        clip_on, clip, mean, sigma, ws);
+                                                                        clip_on, clip, mean, sigma, state, ws);
         else
             row_moments_kernel<false><<<grid, kStatThreads, 0, stream>>>(plane, plan->n_t, plan->stats_part, parts,
-                                                                         clip_on, clip, mean, sigma, ws);
-        row_moments_finish_kernel<<<fin_grid, 128, 0, stream>>>(ws, parts, plan->n_dm, mean, sigma);
+                                                                         clip_on, clip, mean, sigma, state, ws);
+        row_moments_finish_kernel<<<fin_grid, 128, 0, stream>>>(ws, parts, plan->n_dm, pass, rel_tol, state, mean,
+                                                                sigma, n_passes);
     }
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launching the statistics kernels");

@@ -42,17 +42,35 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "spd_tree_common.cuh"
 
 namespace spd {
 namespace {
 
+// Keys of level k and the fold of a level pair: eq. (5)'s compile-time scale 2^(-k/2) (1 / sigma applied at
+// the store), or - SW - a measured sigma per width: cx.ls[k] = 1 / sigma_{d, 2^k}.
+template <int k, bool FAST, bool SW>
+__device__ __forceinline__ float4 key_b(float4 p, int lim, const ChunkCtx& cx) {
+    if constexpr (SW) {
+        return keyx_rt<k, FAST>(p, lim, cx.tm, cx.ls[k]);
+    } else {
+        return keyx<k, FAST>(p, lim, cx.tm);
+    }
+}
+template <int j, int K, bool FAST, bool SW>
+__device__ __forceinline__ void fold_b(float4& best, float4 before, float4 now, int lim, const ChunkCtx& cx) {
+    if constexpr (SW) {
+        fold_rt<j, K, FAST>(best, before, now, lim, cx.tm, cx.ls);
+    } else {
+        fold<j, K, FAST>(best, before, now, lim, cx.tm);
+    }
+}
+
 // Exchange levels k = 3 .. LT+1: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner in another thread.
 // hoff: halo slots used by the levels below (d4 slots each: the row-0 values that the next
 // chunk's last row wraps into).
-template <int T, int R, int K, bool FAST, int k, int hoff>
+template <int T, int R, int K, bool FAST, bool SW, int k, int hoff>
 __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
                                                 float4* __restrict__ pp, float4* __restrict__ hr,
                                                 float4* __restrict__ hw, int& xsel, const ChunkCtx& cx) {
@@ -72,16 +90,16 @@ __device__ __forceinline__ void exchange_levels(float4 (&P)[R], float4 (&best)[R
             const float4* src = buf + (tid + T * r + d4);
             if (r == R - 1 && tid + d4 >= T) src = hr + (hoff + tid + d4 - T);
             const float4 now = add4(P[r], *src);
-            if (FAST || cx.do_out) fold<k + 1, K, FAST>(best[r], P[r], now, lim[r], cx.tm);
+            if (FAST || cx.do_out) fold_b<k + 1, K, FAST, SW>(best[r], P[r], now, lim[r], cx);
             P[r] = now;
         }
-        exchange_levels<T, R, K, FAST, k + 1, hoff + d4>(P, best, lim, pp, hr, hw, xsel, cx);
+        exchange_levels<T, R, K, FAST, SW, k + 1, hoff + d4>(P, best, lim, pp, hr, hw, xsel, cx);
     }
 }
 
 // In-register levels j = 0 .. J-1: partner 2^j rows later in the same thread.  Delay
 // registers of level j live at dl[2^j - 1 .. 2^(j+1) - 2].
-template <int T, int R, int K, bool FAST, int PH, int j>
+template <int T, int R, int K, bool FAST, bool SW, int PH, int j>
 __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
                                                 float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
     using G = Geo<T, R, K>;
@@ -139,17 +157,17 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (FAST || cx.do_out) fold<lvl, K, FAST>(best[r], P[r], now[r], lim[r], cx.tm);
+            if (FAST || cx.do_out) fold_b<lvl, K, FAST, SW>(best[r], P[r], now[r], lim[r], cx);
             P[r] = now[r];
         }
-        register_levels<T, R, K, FAST, PH, j + 1>(P, best, lim, dl, cx);
+        register_levels<T, R, K, FAST, SW, PH, j + 1>(P, best, lim, dl, cx);
     }
 }
 
 // One streaming step: the chunk staged at `st4` (C + 8 floats: the chunk and the first two
 // float4 of the following chunk) -> Y, W for its C samples.  Returns the largest tagged,
 // sigma-unscaled key of the chunk's samples owned by this thread (for the activity map).
-template <int T, int R, int K, bool FAST, int PH>
+template <int T, int R, int K, bool FAST, int PH, bool SW, bool U8>
 __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, float4* __restrict__ pp,
                                             float4* __restrict__ halo, int& xsel, int& hsel,
                                             float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
@@ -173,20 +191,21 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
         const float4 a = norm4(st4[tid + T * r], mu);
         if constexpr (K == 1) {
             P[r] = a;
-            if (FAST || cx.do_out) best[r] = keyx<0, FAST>(a, lim[r], tm);
+            if (FAST || cx.do_out) best[r] = key_b<0, FAST, SW>(a, lim[r], cx);
         } else {
             const float4 b = norm4(st4[tid + T * r + 1], mu);
             const float s01 = a.x + a.y, s12 = a.y + a.z, s23 = a.z + a.w, s34 = a.w + b.x;
             const float4 p1 = make_float4(s01, s12, s23, s34);
             if constexpr (K == 2) {
                 P[r] = p1;
-                if (FAST || cx.do_out) best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm));
+                if (FAST || cx.do_out)
+                    best[r] = max4(key_b<0, FAST, SW>(a, lim[r], cx), key_b<1, FAST, SW>(p1, lim[r], cx));
             } else {
                 const float s45 = b.x + b.y, s56 = b.y + b.z;
                 const float4 p2 = make_float4(s01 + s23, s12 + s34, s23 + s45, s34 + s56);
                 if (FAST || cx.do_out)
-                    best[r] = max4(keyx<0, FAST>(a, lim[r], tm), keyx<1, FAST>(p1, lim[r], tm),
-                                   keyx<2, FAST>(p2, lim[r], tm));
+                    best[r] = max4(key_b<0, FAST, SW>(a, lim[r], cx), key_b<1, FAST, SW>(p1, lim[r], cx),
+                                   key_b<2, FAST, SW>(p2, lim[r], cx));
                 if constexpr (K == 3) {
                     P[r] = p2;
                 } else {
@@ -195,9 +214,13 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
                     // exchange (the L1/shared data pipe is the binding unit).
                     const float4 c = norm4(st4[tid + T * r + 2], mu);
                     const float s67 = b.z + b.w, s78 = b.w + c.x, s89 = c.x + c.y, s9a = c.y + c.z;
-                    const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
-                                                  (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
-                    if (FAST || cx.do_out) fold<3, K, FAST>(best[r], p2, p3, lim[r], tm);
+                    // packed adds of aligned pairs, same association as (s01 + s23) + (s45 + s67) ...
+                    const float2 q2lo = __fadd2_rn(make_float2(s45, s56), make_float2(s67, s78));
+                    const float2 q2hi = __fadd2_rn(make_float2(s67, s78), make_float2(s89, s9a));
+                    const float2 p3lo = __fadd2_rn(make_float2(p2.x, p2.y), q2lo);
+                    const float2 p3hi = __fadd2_rn(make_float2(p2.z, p2.w), q2hi);
+                    const float4 p3 = make_float4(p3lo.x, p3lo.y, p3hi.x, p3hi.y);
+                    if (FAST || cx.do_out) fold_b<3, K, FAST, SW>(best[r], p2, p3, lim[r], cx);
                     P[r] = p3;
                 }
             }
@@ -208,10 +231,10 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
     float4* const hr = halo + hsel * T;        // written by the previous (later-in-time) chunk
     float4* const hw = halo + (hsel ^ 1) * T;  // read by the next chunk
     hsel ^= 1;
-    exchange_levels<T, R, K, FAST, 3, 0>(P, best, lim, pp, hr, hw, xsel, cx);
+    exchange_levels<T, R, K, FAST, SW, 3, 0>(P, best, lim, pp, hr, hw, xsel, cx);
 
     // ---- in-register levels: partner 1, 2, 4, ... rows later (same thread) -------------
-    register_levels<T, R, K, FAST, PH, 0>(P, best, lim, dl, cx);
+    register_levels<T, R, K, FAST, SW, PH, 0>(P, best, lim, dl, cx);
 
     // ---- unpack and store: Y = key (code bits cleared) / sigma, W = inverted code ---------------------------
     float top = __int_as_float(0xff800000);
@@ -232,7 +255,15 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
                                          static_cast<int>(~__float_as_uint(kq.w) & kCodeMask));
                 const long long o = cx.n0 + 4ll * (tid + T * r);
                 *reinterpret_cast<float4*>(cx.out_snr + o) = y;
-                *reinterpret_cast<int4*>(cx.out_width + o) = w;
+                if constexpr (U8) {
+                    // the four low bytes of the keys into one word (3 PRMT), inverted and masked at once
+                    const uint32_t t = __byte_perm(__float_as_uint(kq.x), __float_as_uint(kq.y), 0x0040);
+                    const uint32_t u = __byte_perm(__float_as_uint(kq.z), __float_as_uint(kq.w), 0x4000);
+                    const uint32_t packed = ~__byte_perm(t, u, 0x7610) & 0x1f1f1f1fu;
+                    *reinterpret_cast<uint32_t*>(reinterpret_cast<uint8_t*>(cx.out_width) + o) = packed;
+                } else {
+                    *reinterpret_cast<int4*>(cx.out_width + o) = w;
+                }
             }
         }
     }
@@ -288,7 +319,7 @@ constexpr size_t tree_smem_bytes() {
     return 2 * C * 4 + kStages * (C + 8) * 4 + 2 * T * 16 + kStages * 8 + 16;
 }
 
-template <int T, int R, int K>
+template <int T, int R, int K, bool SW, bool U8>
 __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(const TreeParams p) {
     using G = Geo<T, R, K>;
     constexpr int C = G::C;
@@ -317,11 +348,18 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
     ChunkCtx cx;
     cx.mu = p.mean[d];
-    const float sg = p.sigma[d];
+    const float sg = SW ? 1.0f : p.sigma[d];
     cx.inv = 1.0f / sg;
+    if constexpr (SW) {
+        // keys are SNRs already: 1 / sigma_{d, 2^k} per level, nothing left for the store
+        const float* __restrict__ swr = p.sigma_w + static_cast<long long>(d) * K;
+#pragma unroll
+        for (int k = 0; k < K; ++k) cx.ls[k] = 1.0f / __ldg(swr + k);
+    }
     cx.tm = p.tag_mask;
     cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
-    cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
+    // a uint8 plane advances by n_t bytes per row: n_t / 4 int32 (n_t % 4 == 0 on this path)
+    cx.out_width = p.out_width + static_cast<long long>(d) * (U8 ? n_t / 4 : n_t);
     cx.n_t = n_t;
     cx.tid = tid;
     // Activity threshold on the sigma-unscaled key: Y = key / sigma >= thr  <=  key >= thr * sigma
@@ -371,8 +409,8 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
         __syncthreads();
         cx.n0 = n0;
         cx.do_out = c < c_hi;
-        const float top = tree_chunk<T, R, K, false, 0>(reinterpret_cast<const float4*>(stages), pp, halo, xsel,
-                                                        hsel, dl, cx);
+        const float top = tree_chunk<T, R, K, false, 0, SW, U8>(reinterpret_cast<const float4*>(stages), pp, halo,
+                                                                xsel, hsel, dl, cx);
         if (act && cx.do_out && top >= thr_key) act[c] = 1;
         ++cx.it;
         __syncthreads();
@@ -414,7 +452,7 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
                 mbar_wait(&bars[stage], phase);
                 const int c = first_fast - 1 - it;
                 cx.n0 = static_cast<long long>(c) * C;
-                const float top = tree_chunk<T, R, K, true, decltype(ph)::value>(
+                const float top = tree_chunk<T, R, K, true, decltype(ph)::value, SW, U8>(
                     reinterpret_cast<const float4*>(stages + stage * (C + 8)), pp, halo, xsel, hsel, dl, cx);
                 if (act && top >= thr_key) act[c] = 1;
                 if (++stage == kStages) {
@@ -434,21 +472,38 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     }
 }
 
+// Variants: 0 = eq. (5) scale, int32 index; 1 = measured sigma per width (spd_run_sigma_w); 2 = uint8 index
+// (SPD_FLAG_WIDTH_U8).  1 and 2 are instantiated where this kernel is the plan's default (K <= 8, K >= 15).
+constexpr bool tree_has_variants(int K) { return K <= 8 || K >= 15; }
+
 template <int T, int R, int K>
-cudaError_t launch_tree(const TreeConfig& cfg, const TreeParams& prm, int64_t n_dm, cudaStream_t stream) {
+cudaError_t launch_tree(const TreeConfig& cfg, const TreeParams& prm, int64_t n_dm, int variant, cudaStream_t stream) {
     const dim3 grid(static_cast<unsigned>(n_dm * cfg.segs_per_row));
-    spd_tree_kernel<T, R, K><<<grid, T, cfg.smem_bytes, stream>>>(prm);
+    if (variant == 0) {
+        spd_tree_kernel<T, R, K, false, false><<<grid, T, cfg.smem_bytes, stream>>>(prm);
+    } else if constexpr (tree_has_variants(K)) {
+        if (variant == 1)
+            spd_tree_kernel<T, R, K, true, false><<<grid, T, cfg.smem_bytes, stream>>>(prm);
+        else
+            spd_tree_kernel<T, R, K, false, true><<<grid, T, cfg.smem_bytes, stream>>>(prm);
+    } else {
+        return cudaErrorNotSupported;
+    }
     return cudaGetLastError();
+}
+
+template <typename Kern>
+cudaError_t prepare_kernel(Kern kern, int T, size_t smem, int* nb) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(nb, kern, T, smem);
 }
 
 template <int T, int R, int K>
 cudaError_t prepare_tree(TreeConfig& cfg) {
     cfg.smem_bytes = tree_smem_bytes<T, R, K>();
-    cudaError_t e = cudaFuncSetAttribute(spd_tree_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(cfg.smem_bytes));
-    if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, R, K>, T, cfg.smem_bytes);
+    cudaError_t e = prepare_kernel(spd_tree_kernel<T, R, K, false, false>, T, cfg.smem_bytes, &nb);
     if (e != cudaSuccess) return e;
     if constexpr (tree_tmem(K)) {
         // no more resident blocks than tensor memory has columns for (a block that cannot
@@ -456,12 +511,15 @@ cudaError_t prepare_tree(TreeConfig& cfg) {
         const int max_blocks = 512 / tree_tmem_cols<T, R, K>();
         while (nb > max_blocks && cfg.smem_bytes < (200u << 10)) {
             cfg.smem_bytes += 4096;
-            e = cudaFuncSetAttribute(spd_tree_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     static_cast<int>(cfg.smem_bytes));
-            if (e != cudaSuccess) return e;
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_kernel<T, R, K>, T, cfg.smem_bytes);
+            e = prepare_kernel(spd_tree_kernel<T, R, K, false, false>, T, cfg.smem_bytes, &nb);
             if (e != cudaSuccess) return e;
         }
+    }
+    if constexpr (tree_has_variants(K)) {
+        // the variants use a few more registers: never more resident blocks than the plain kernel
+        int nv = 0;
+        if ((e = prepare_kernel(spd_tree_kernel<T, R, K, true, false>, T, cfg.smem_bytes, &nv)) != cudaSuccess) return e;
+        if ((e = prepare_kernel(spd_tree_kernel<T, R, K, false, true>, T, cfg.smem_bytes, &nv)) != cudaSuccess) return e;
     }
     cfg.blocks_per_sm = nb;
     return cudaSuccess;
@@ -499,7 +557,7 @@ bool tree_applicable(const std::vector<int32_t>& widths, int64_t n_t) {
 int tree_configure(spd_plan* plan) {
     TreeConfig& cfg = plan->tree;
     cfg.K = static_cast<int>(plan->widths.size());
-    if (ws_applicable(cfg.K)) return ws_configure(plan);
+    if (ws_applicable(cfg.K, plan->flags)) return ws_configure(plan);
     cfg.kind = 0;
     cfg.T = tree_threads_for(cfg.K);
     cfg.chunk = 4 * cfg.T * tree_rows_for(cfg.K);
@@ -529,8 +587,8 @@ int tree_configure_segments(spd_plan* plan) {
     const int64_t slots = int64_t(plan->sm_count) * cfg.blocks_per_sm;
     int64_t segs = 1;
     const int64_t min_seg_chunks = std::max<int64_t>(16 * cfg.warm_chunks, 8);
-    if (const char* env = std::getenv("SPD_SEGS_PER_ROW")) {
-        segs = std::max<int64_t>(1, std::atoll(env));
+    if (plan->segs_option > 0) {  // SPD_OPT_SEGMENTS_PER_ROW
+        segs = plan->segs_option;
     } else {
         while (plan->n_dm * segs < 8 * slots && (cfg.chunks_per_row + 2 * segs - 1) / (2 * segs) >= min_seg_chunks)
             segs *= 2;
@@ -546,17 +604,25 @@ int tree_configure_segments(spd_plan* plan) {
 }
 
 int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-             float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
+             float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+             const float* sigma_w) {
     const TreeConfig& cfg = plan->tree;
-    if (cfg.kind == 1) return ws_run(plan, n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (cfg.kind == 1)
+        return ws_run(plan, n_dm, plane, mean, sigma, out_snr, out_width, threshold, activity, stream, sigma_w);
+    const int variant = sigma_w ? 1 : (plan->width_bytes == 1 ? 2 : 0);
+    if (variant != 0 && !tree_has_variants(cfg.K)) {
+        set_error("the block-per-stream kernel forced by SPD_FLAG_BLOCK_TREE has no sigma-per-width / uint8 variant "
+                  "for %d widths", cfg.K);
+        return SPD_ERR_INVALID_ARG;
+    }
     TreeParams prm;
     prm.plane = plane;
     prm.mean = mean;
     prm.sigma = sigma;
-    prm.sigma_w = nullptr;
+    prm.sigma_w = sigma_w;
     for (int k = 0; k < 16; ++k) prm.gmask[k] = 0u;
     prm.out_snr = out_snr;
-    prm.out_width = out_width;
+    prm.out_width = static_cast<int32_t*>(out_width);
     prm.activity = activity;
     prm.threshold = threshold;
     prm.n_t = plan->n_t;
@@ -575,7 +641,7 @@ int tree_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float
     }
     e = cudaErrorInvalidValue;
 #define SPD_LAUNCH(KK) \
-    if (cfg.K == KK) e = launch_tree<tree_threads_for(KK), tree_rows_for(KK), KK>(cfg, prm, n_dm, stream);
+    if (cfg.K == KK) e = launch_tree<tree_threads_for(KK), tree_rows_for(KK), KK>(cfg, prm, n_dm, variant, stream);
     SPD_TREE_CASES(SPD_LAUNCH)
 #undef SPD_LAUNCH
     if (e != cudaSuccess) return cuda_fail(e, "launching the dyadic-tree kernel");

@@ -234,7 +234,7 @@ __device__ __forceinline__ float pack1(float v, uint32_t tm) {
 }
 template <int k>
 __device__ __forceinline__ float4 key4(float4 p, uint32_t tm) {
-    const float4 v = scale4(p, level_scale<k>());
+    const float4 v = k == 0 ? p : scale4(p, level_scale<k>());  // x * 1.0f is not folded by the compiler
     return make_float4(pack1<k>(v.x, tm), pack1<k>(v.y, tm), pack1<k>(v.z, tm), pack1<k>(v.w, tm));
 }
 // Guarded variant: element v of the float4 is valid iff 2^k <= lim - v (reading A3).

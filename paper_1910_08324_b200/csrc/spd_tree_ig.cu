@@ -22,7 +22,6 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "spd_tree_common.cuh"
 
@@ -465,8 +464,13 @@ int ig_configure(spd_plan* plan) {
 }
 
 int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
+           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+           const float* sigma_w) {
     const TreeConfig& cfg = plan->tree;
+    if (sigma_w) {
+        set_error("the IGRID-tree kernel scales by sqrt(width) at compile time");
+        return SPD_ERR_INVALID_ARG;
+    }
     TreeParams prm;
     prm.plane = plane;
     prm.mean = mean;

@@ -37,7 +37,6 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "spd_tree_common.cuh"
 
@@ -45,25 +44,15 @@ namespace spd {
 namespace {
 
 constexpr int kWsWarps = 8;                 // streams per block
-#ifndef SPD_WS_ROWS
-#define SPD_WS_ROWS 4
-#endif
-constexpr int kWsRows = SPD_WS_ROWS;        // rows of 128 samples per step (4 or 8)
-static_assert(kWsRows == 4 || kWsRows == 8, "rows per step");
+constexpr int kWsRows = 4;                  // rows of 128 samples per step (8: 32 KB loop body, slower - DESIGN.md 10b)
 constexpr int kWsStep = 128 * kWsRows;      // samples per step
 constexpr int kWsStage = kWsStep + 8;       // floats per stage: the step + two float4 of look-ahead
 constexpr int kWsMinK = 9, kWsMaxK = 14;  // K = 8: the block kernel is 2 % faster (measured)
 // Activity map: one byte per kWsActSteps steps (2048 samples, the block kernel's granularity:
 // finer flags only lengthen the candidate kernel's scan of the map).
 constexpr int kWsActSteps = 2048 / kWsStep;
-#ifndef SPD_WS_STAGES
-#define SPD_WS_STAGES 4
-#endif
-constexpr int kWsStages = SPD_WS_STAGES;    // bulk-copy ring depth per warp
-#ifndef SPD_WS_UNROLL
-#define SPD_WS_UNROLL 2
-#endif
-constexpr int kWsUnroll = SPD_WS_UNROLL;    // steps per trip of the main loop
+constexpr int kWsStages = 4;                // bulk-copy ring depth per warp (3 and 6 measure the same)
+constexpr int kWsUnroll = 2;                // steps per trip of the main loop (3: past the instruction cache)
 
 template <int K>
 struct WsGeo {
@@ -80,39 +69,18 @@ struct WsGeo {
 };
 
 // One level's rows of a step (kWsRows float4 per lane) <-> 4 * kWsRows columns.
-__device__ __forceinline__ void tmem_ld_rows(uint32_t taddr, float4 (&v)[kWsRows]) {
-    if constexpr (kWsRows == 8) {
-        tmem_ld32(taddr, reinterpret_cast<float4(&)[8]>(v));
-    } else {
-        tmem_ld16(taddr, reinterpret_cast<float4(&)[4]>(v));
-    }
-}
-__device__ __forceinline__ void tmem_st_rows(uint32_t taddr, const float4 (&v)[kWsRows]) {
-    if constexpr (kWsRows == 8) {
-        tmem_st32(taddr, reinterpret_cast<const float4(&)[8]>(v));
-    } else {
-        tmem_st16(taddr, reinterpret_cast<const float4(&)[4]>(v));
-    }
-}
+__device__ __forceinline__ void tmem_ld_rows(uint32_t taddr, float4 (&v)[kWsRows]) { tmem_ld16(taddr, v); }
+__device__ __forceinline__ void tmem_st_rows(uint32_t taddr, const float4 (&v)[kWsRows]) { tmem_st16(taddr, v); }
 
 
 // Lane levels k = 3 .. 6: P_{k+1}[n] = P_k[n] + P_k[n + 2^k], partner 2^k / 4 lanes later; the
 // lanes that run off a row continue in the next row, the last row in the first row of the
 // previous (later-in-time) step, kept in hs[k - 3].
-// SPD_WS_XCHG = 1: through a warp-private shared-memory buffer (one 128-bit store and load per
-// float4 and level, ordered by __syncwarp: two instructions where shuffles take eight; the
-// L1 data pipe has the room, the issue slots do not).  Two buffers alternate between levels.
-// SPD_WS_XCHG = 0: warp shuffles of a per-lane pre-selected source row.
-#ifndef SPD_WS_XCHG
-#define SPD_WS_XCHG 1
-#endif
+// The exchange goes through a warp-private shared-memory buffer (one 128-bit store and load per
+// float4 and level, ordered by __syncwarp: two instructions where shuffles take eight - measured
+// 11.37 against 11.86 ms; the L1 data pipe has the room, the issue slots do not).  Two buffers
+// alternate between levels.
 constexpr int kWsXBuf = (kWsRows + 1) * 32;  // float4 per exchange buffer: R rows + the kept row
-#if !SPD_WS_XCHG
-__device__ __forceinline__ float4 shfl4(float4 v, int src) {
-    return make_float4(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src),
-                       __shfl_sync(0xffffffffu, v.z, src), __shfl_sync(0xffffffffu, v.w, src));
-}
-#endif
 
 // Keys of level k: eq. (5)'s compile-time scale 2^(-k/2) (1 / sigma applied at the store), or a measured
 // sigma per width (SW).
@@ -181,7 +149,6 @@ __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)
     if constexpr (k <= 6 && k + 1 <= WsGeo<K>::LAST) {
         constexpr int d4 = (1 << k) / 4;
         float4 partner[R];
-#if SPD_WS_XCHG
         float4* const buf = xb + (k & 1) * kWsXBuf + lane;
 #pragma unroll
         for (int r = 0; r < R; ++r) st_shared4(buf + 32 * r, P[r]);
@@ -189,17 +156,6 @@ __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)
         __syncwarp();
 #pragma unroll
         for (int r = 0; r < R; ++r) partner[r] = buf[32 * r + d4];
-#else
-        const int src = (lane + d4) & 31;
-        const bool low = lane < d4;  // this lane's value is wanted by a lane of the row before
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 nxt = r + 1 < R ? P[r + 1] : hs[k - 3];
-            const float4 w = make_float4(low ? nxt.x : P[r].x, low ? nxt.y : P[r].y, low ? nxt.z : P[r].z,
-                                         low ? nxt.w : P[r].w);
-            partner[r] = shfl4(w, src);
-        }
-#endif
         hs[k - 3] = P[0];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -261,7 +217,7 @@ __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)
 }
 
 // One step of one warp: the kWsStage floats at st4 -> Y, W of its kWsStep samples.
-template <int K, int MODE, bool SW, bool GR>
+template <int K, int MODE, bool SW, bool GR, bool U8>
 __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 (&hs)[4],
                                          float4 (&nr)[WsGeo<K>::NEAR + 1], float4* __restrict__ xb, uint32_t tbase,
                                          int it, int lane, const ChunkCtx& cx) {
@@ -288,9 +244,15 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
         const float s45 = b.x + b.y, s56 = b.y + b.z, s67 = b.z + b.w, s78 = b.w + c.x;
         const float s89 = c.x + c.y, s9a = c.y + c.z;
         const float4 p1 = make_float4(s01, s12, s23, s34);
-        const float4 p2 = make_float4(s01 + s23, s12 + s34, s23 + s45, s34 + s56);
-        const float4 p3 = make_float4((s01 + s23) + (s45 + s67), (s12 + s34) + (s56 + s78),
-                                      (s23 + s45) + (s67 + s89), (s34 + s56) + (s78 + s9a));
+        // widths 4 and 8 as packed adds of aligned pairs of the width-2 sums: the same additions in
+        // the same association as (s01 + s23) + (s45 + s67) ..., 6 FADD2 for 12 FADD
+        const float2 u01 = make_float2(s01, s12), u23 = make_float2(s23, s34), u45 = make_float2(s45, s56),
+                     u67 = make_float2(s67, s78), u89 = make_float2(s89, s9a);
+        const float2 p2lo = __fadd2_rn(u01, u23), p2hi = __fadd2_rn(u23, u45);
+        const float2 q2lo = __fadd2_rn(u45, u67), q2hi = __fadd2_rn(u67, u89);
+        const float2 p3lo = __fadd2_rn(p2lo, q2lo), p3hi = __fadd2_rn(p2hi, q2hi);
+        const float4 p2 = make_float4(p2lo.x, p2lo.y, p2hi.x, p2hi.y);
+        const float4 p3 = make_float4(p3lo.x, p3lo.y, p3hi.x, p3hi.y);
         if (wants_out<MODE>(cx)) {
             constexpr bool F = MODE != 0;
             float4 k0 = key_sw<0, F, SW>(a, lim[r], cx), k1 = key_sw<1, F, SW>(p1, lim[r], cx),
@@ -334,7 +296,15 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
                 }
                 const long long o = cx.n0 + 4ll * (lane + 32 * r);
                 *reinterpret_cast<float4*>(cx.out_snr + o) = y;
-                *reinterpret_cast<int4*>(cx.out_width + o) = wv;
+                if constexpr (U8) {
+                    // the four low bytes of the keys into one word (3 PRMT), inverted and masked at once
+                    const uint32_t t = __byte_perm(__float_as_uint(kq.x), __float_as_uint(kq.y), 0x0040);
+                    const uint32_t u = __byte_perm(__float_as_uint(kq.z), __float_as_uint(kq.w), 0x4000);
+                    const uint32_t packed = ~__byte_perm(t, u, 0x7610) & 0x1f1f1f1fu;
+                    *reinterpret_cast<uint32_t*>(reinterpret_cast<uint8_t*>(cx.out_width) + o) = packed;
+                } else {
+                    *reinterpret_cast<int4*>(cx.out_width + o) = wv;
+                }
             }
         }
     }
@@ -342,10 +312,10 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
 }
 
 constexpr size_t kWsStagesBytes = static_cast<size_t>(kWsWarps) * kWsStages * kWsStage * 4;
-constexpr size_t kWsXBytes = SPD_WS_XCHG ? static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16 : 0;
+constexpr size_t kWsXBytes = static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16;
 constexpr size_t ws_smem_bytes() { return kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8 + 16; }
 
-template <int K, bool SW, bool GR>
+template <int K, bool SW, bool GR, bool U8>
 __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const TreeParams p, const int n_pieces) {
     using G = WsGeo<K>;
     constexpr int S = kWsStep;
@@ -428,7 +398,8 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             cx.inv = 1.0f;
         }
         cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
-        cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
+        // a uint8 plane advances by n_t bytes per row: n_t / 4 int32 (n_t % 4 == 0 on this path)
+        cx.out_width = p.out_width + static_cast<long long>(d) * (U8 ? n_t / 4 : n_t);
         uint8_t* const act =
             p.activity ? p.activity + static_cast<long long>(d) * ((p.chunks_per_row + kWsActSteps - 1) / kWsActSteps)
                        : nullptr;
@@ -469,7 +440,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             __syncwarp();
             cx.n0 = n0;
             cx.do_out = c < c_hi;
-            const float top = ws_step<K, 0, SW, GR>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
+            const float top = ws_step<K, 0, SW, GR, U8>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
             if (act && cx.do_out && top >= thr_key) act[c / kWsActSteps] = 1;
             __syncwarp();
         }
@@ -516,7 +487,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
         for (; f < n_warm; ++f, ++it) {
             ring_next(f);
             cx.n0 = static_cast<long long>(ring_top - 1 - f) * S;
-            ws_step<K, 2, SW, GR>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
+            ws_step<K, 2, SW, GR, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
             ring_done();
         }
         // Two steps per loop trip: the values kept from one step to the next (hs, nr: 11 float4)
@@ -528,7 +499,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             ring_next(f);
             const int c = ring_top - 1 - f;
             cx.n0 = static_cast<long long>(c) * S;
-            const float top = ws_step<K, 1, SW, GR>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
+            const float top = ws_step<K, 1, SW, GR, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
                                             tbase, it, lane, cx);
             if (act && top >= thr_key) act[c / kWsActSteps] = 1;
             ring_done();
@@ -547,15 +518,23 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
 
 }  // namespace
 
-// Warp-stream kernel for this plan?  Default: yes for kWsMinK <= K <= kWsMaxK.  Test hook:
-// SPD_TREE_KERNEL=block keeps the block-per-stream kernel of spd_tree.cu, =warp forces this one
-// where it applies.
-bool ws_applicable(int K) {
-    if (K < kWsMinK || K > kWsMaxK) return false;
-    if (const char* env = std::getenv("SPD_TREE_KERNEL")) {
-        if (env[0] == 'b') return false;
-    }
-    return true;
+// Warp-stream kernel for this plan?  Yes for kWsMinK <= K <= kWsMaxK unless the plan was created with
+// SPD_FLAG_BLOCK_TREE (A/B runs against the block-per-stream kernel of spd_tree.cu).
+bool ws_applicable(int K, uint32_t flags) {
+    return K >= kWsMinK && K <= kWsMaxK && !(flags & SPD_FLAG_BLOCK_TREE);
+}
+
+template <int K>
+static cudaError_t ws_prepare(int smem) {
+    cudaError_t e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, false, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return e;
 }
 
 int ws_configure(spd_plan* plan) {
@@ -567,16 +546,8 @@ int ws_configure(spd_plan* plan) {
     cfg.blocks_per_sm = 1;
     cfg.smem_bytes = ws_smem_bytes();
     cudaError_t e = cudaErrorInvalidValue;
-#define SPD_PREP(KK)                                                                                          \
-    if (cfg.K == KK)                                                                                          \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                 static_cast<int>(cfg.smem_bytes));                                           \
-    if (cfg.K == KK && e == cudaSuccess)                                                                      \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                 static_cast<int>(cfg.smem_bytes));                                           \
-    if (cfg.K == KK && e == cudaSuccess)                                                                      \
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<KK, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                 static_cast<int>(cfg.smem_bytes));
+#define SPD_PREP(KK) \
+    if (cfg.K == KK) e = ws_prepare<KK>(static_cast<int>(cfg.smem_bytes));
     SPD_WS_CASES(SPD_PREP)
 #undef SPD_PREP
     if (e != cudaSuccess) return cuda_fail(e, "configuring the warp-stream tree kernel");
@@ -588,12 +559,11 @@ int ws_configure(spd_plan* plan) {
     // Work split.  Default: the steps of the plane, in row-major order, are cut into one piece
     // per resident warp (sm_count * 8), so every warp does the same number of steps and only
     // the one row part per piece that stops short of its row's end replays look-ahead.
-    // Test hook SPD_SEGS_PER_ROW = s: every row cut into s equal segments instead.
+    // SPD_OPT_SEGMENTS_PER_ROW = s: every row cut into s equal segments instead.
     cfg.segs_per_row = 0;
     cfg.seg_chunks = 0;  // per launch (depends on the rows of the launch): ws_pieces()
-    if (const char* env = std::getenv("SPD_SEGS_PER_ROW")) {
-        int64_t segs = std::max<int64_t>(1, std::atoll(env));
-        segs = std::min<int64_t>(segs, cfg.chunks_per_row);
+    if (plan->segs_option > 0) {
+        const int64_t segs = std::min<int64_t>(plan->segs_option, cfg.chunks_per_row);
         cfg.seg_chunks = static_cast<int>((cfg.chunks_per_row + segs - 1) / segs);
         cfg.segs_per_row = static_cast<int>((cfg.chunks_per_row + cfg.seg_chunks - 1) / cfg.seg_chunks);
         if (plan->n_dm * cfg.segs_per_row > 0x7fffffffll) {
@@ -637,7 +607,7 @@ int ws_grid_blocks(const spd_plan* plan) {
 }
 
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-           float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+           float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
            const float* sigma_w) {
     const TreeConfig& cfg = plan->tree;
     TreeParams prm;
@@ -646,7 +616,7 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     prm.sigma = sigma;
     prm.sigma_w = sigma_w;
     prm.out_snr = out_snr;
-    prm.out_width = out_width;
+    prm.out_width = static_cast<int32_t*>(out_width);
     prm.activity = activity;
     prm.threshold = threshold;
     int piece_chunks = 0;
@@ -673,15 +643,24 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     const int64_t blocks = std::min<int64_t>(plan->sm_count, (n_pieces + kWsWarps - 1) / kWsWarps);
     const dim3 grid(static_cast<unsigned>(std::max<int64_t>(1, blocks)));
     cudaError_t e = cudaErrorInvalidValue;
-#define SPD_LAUNCH(KK)                                                                                      \
-    if (cfg.K == KK) {                                                                                      \
-        if (sigma_w)                                                                                        \
-            spd_tree_ws_kernel<KK, true, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
-        else if (!plan->separations.empty())                                                                \
-            spd_tree_ws_kernel<KK, false, true><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
-        else                                                                                                \
-            spd_tree_ws_kernel<KK, false, false><<<grid, 32 * kWsWarps, cfg.smem_bytes, stream>>>(prm, static_cast<int>(n_pieces)); \
-        e = cudaGetLastError();                                                                             \
+    const bool u8 = plan->width_bytes == 1;
+    if (u8 && (sigma_w || !plan->separations.empty())) {
+        set_error("a uint8 width plane (SPD_FLAG_WIDTH_U8) is written by spd_run / spd_run_flagged only");
+        return SPD_ERR_INVALID_ARG;
+    }
+    const int np = static_cast<int>(n_pieces);
+    const size_t sm = cfg.smem_bytes;
+#define SPD_LAUNCH(KK)                                                                              \
+    if (cfg.K == KK) {                                                                              \
+        if (sigma_w)                                                                                \
+            spd_tree_ws_kernel<KK, true, false, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
+        else if (!plan->separations.empty())                                                        \
+            spd_tree_ws_kernel<KK, false, true, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
+        else if (u8)                                                                                \
+            spd_tree_ws_kernel<KK, false, false, true><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
+        else                                                                                        \
+            spd_tree_ws_kernel<KK, false, false, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
+        e = cudaGetLastError();                                                                     \
     }
     SPD_WS_CASES(SPD_LAUNCH)
 #undef SPD_LAUNCH

@@ -32,7 +32,7 @@ def test_library_exports_every_declared_symbol(spd):
     lib = ctypes.CDLL(spd.LIB_PATH)
     for name in declared_functions():
         assert hasattr(lib, name), f"{name} is declared in include/spd.h but not exported"
-    assert spd.spd_version() == 100
+    assert spd.spd_version() == 200
 
 
 def test_library_is_built_for_sm_100a_only(spd):
@@ -113,6 +113,22 @@ def test_no_cpu_fallback_without_a_device(spd):
         spd.spd_plan_create(4, 1024, [1, 2, 4], 4)
     assert e.value.status == -2
     assert "no CPU fallback" in str(e.value) or "not supported" in str(e.value)
+
+
+def test_library_reads_no_environment_variable():
+    """Kernel choice and work split are plan flags / options (include/spd.h), not process-global state."""
+    pkg = os.path.join(ROOT, "paper_1910_08324_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".cu", ".h", ".cuh", ".cpp")):
+                assert "getenv" not in open(os.path.join(dirpath, f)).read(), f
+
+
+def test_spd_destroy_is_a_c_symbol_and_accepts_null(spd):
+    lib = spd.load()
+    lib.spd_destroy(None)
+    lib.spd_plan_destroy(None)
+    assert lib.spd_plan_set_option(None, 1, 2) == -1
 
 
 def test_product_never_imports_the_oracle():

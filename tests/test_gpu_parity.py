@@ -21,21 +21,27 @@ def spd():
     return spd
 
 
-def run_gpu(spd, x: np.ndarray, mu, sg, widths, max_width=None, flags=0):
-    """One spd_run through the binding; returns (snr f32, idx i32) numpy arrays and plan info."""
+def run_gpu(spd, x: np.ndarray, mu, sg, widths, max_width=None, flags=0, segs=0):
+    """One spd_run through the binding; returns (snr f32, idx i32) numpy arrays and plan info.
+    segs > 0: SPD_OPT_SEGMENTS_PER_ROW (every row cut into that many streams); 0: the default work split."""
     n_dm, n_t = x.shape
     dev = torch.device("cuda:0")
     plane = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(dev)
     mean = torch.from_numpy(np.broadcast_to(np.asarray(mu, dtype=np.float32), (n_dm,)).copy()).to(dev)
     sigma = torch.from_numpy(np.broadcast_to(np.asarray(sg, dtype=np.float32), (n_dm,)).copy()).to(dev)
     with spd.Plan(n_dm, n_t, widths, max_width, flags) as plan:
+        if segs:
+            plan.set_option(spd.SPD_OPT_SEGMENTS_PER_ROW, segs)
         snr, idx = plan.run(plane, mean, sigma)
         torch.cuda.synchronize()
-        return snr.cpu().numpy(), idx.cpu().numpy(), dict(plan.info)
+        return snr.cpu().numpy().astype(np.float32), idx.cpu().numpy().astype(np.int32), dict(plan.info)
 
 
-def check(spd, oracle, x, mu, sg, widths, what, direct=False, flags=0, expect_path=None):
-    got_snr, got_idx, info = run_gpu(spd, x, mu, sg, widths, flags=flags)
+def check(spd, oracle, x, mu, sg, widths, what, direct=False, flags=0, expect_path=None, segs=0,
+          direct_windows=()):
+    """Element-by-element parity of one run against oracle B (running sum) or, direct=True, oracle A (direct
+    summation); direct_windows = [(t0, t1), ...] adds oracle A on those sample ranges of every row."""
+    got_snr, got_idx, info = run_gpu(spd, x, mu, sg, widths, flags=flags, segs=segs)
     if expect_path is not None:
         assert info["path"] == expect_path, f"{what}: plan took path {info['path']}"
     # both sides see the float32-rounded mu / sigma the C ABI takes
@@ -43,8 +49,13 @@ def check(spd, oracle, x, mu, sg, widths, what, direct=False, flags=0, expect_pa
     sg64 = np.broadcast_to(np.asarray(sg, dtype=np.float32), (x.shape[0],)).astype(np.float64)
     fn = oracle.spd_direct if direct else oracle.spd_prefix
     ref_snr, ref_idx, ref_sec = fn(x, mu64, sg64, widths)
-    return parity.assert_parity(oracle, x, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
-                                what=what)
+    st = parity.assert_parity(oracle, x, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                              what=what)
+    for t0, t1 in direct_windows:
+        d_snr, d_idx, d_sec = oracle.spd_direct(x, mu64, sg64, widths, t0, t1)
+        parity.assert_parity(oracle, x, mu64, sg64, widths, got_snr[:, t0:t1], got_idx[:, t0:t1], d_snr, d_idx,
+                             d_sec, t0=t0, what=f"{what} direct [{t0}, {t1})")
+    return st
 
 
 def test_config1_tiny_lossless_full_plane(spd, oracle_lib):
@@ -66,11 +77,12 @@ def test_config1_plane_dyadic_set_direct_oracle(spd, oracle_lib):
     check(spd, oracle_lib, x, 0.0, 1.0, widths, "config1/pow2", direct=True, expect_path=spd.SPD_PATH_DYADIC_TREE)
 
 
+@pytest.mark.parametrize("segs", [0, 3])
 @pytest.mark.parametrize("K", list(range(1, 17)))
-def test_dyadic_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
+def test_dyadic_tree_every_depth_ragged(spd, oracle_lib, K, segs):
     """Every kernel instantiation (widths 1..2^(K-1)); n_t spans several chunks plus a ragged
-    tail that is not a multiple of the chunk; several segments per row so that interior
-    segments replay their look-ahead."""
+    tail that is not a multiple of the chunk; with the default work split (segs 0) and with several
+    segments per row, so that interior segments replay their look-ahead."""
     M = 1 << (K - 1)
     T = 128 if K <= 14 else (256 if K == 15 else 512)
     chunk = 16 * T
@@ -79,13 +91,14 @@ def test_dyadic_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
     x = rng.standard_normal((3, n_t), dtype=np.float32)
     x[1, n_t // 3: n_t // 3 + max(1, M // 2)] += np.float32(12.0 / np.sqrt(max(1, M // 2)))
     x[2, n_t - M // 2 - 3:] += np.float32(0.7)  # a pulse running off the end of the row
-    monkeypatch.setenv("SPD_SEGS_PER_ROW", "3")
     widths = [1 << k for k in range(K)]
-    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"tree K={K}", expect_path=spd.SPD_PATH_DYADIC_TREE)
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"tree K={K} segs={segs}", expect_path=spd.SPD_PATH_DYADIC_TREE,
+          segs=segs)
 
 
+@pytest.mark.parametrize("segs", [0, 3])
 @pytest.mark.parametrize("K", list(range(5, 17)))
-def test_igrid_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
+def test_igrid_tree_every_depth_ragged(spd, oracle_lib, K, segs):
     """Every instantiation of the IGRID depth-1 streaming tree (widths 2^k and 3 * 2^m up to 2^(K-1)):
     several chunks, ragged tail, several segments per row, pulses of non-power-of-two widths."""
     M = 1 << (K - 1)
@@ -96,22 +109,22 @@ def test_igrid_tree_every_depth_ragged(spd, oracle_lib, K, monkeypatch):
     S = max(1, 3 * M // 8)
     x[1, n_t // 3: n_t // 3 + S] += np.float32(12.0 / np.sqrt(S))
     x[2, n_t - M // 2 - 3:] += np.float32(0.7)  # a pulse running off the end of the row
-    monkeypatch.setenv("SPD_SEGS_PER_ROW", "3")
     widths = spd.spd_width_set_generate("IGRID", 1, M)
     assert len(widths) == 2 * K - 2
-    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"igrid tree K={K}", expect_path=spd.SPD_PATH_IGRID_TREE)
+    check(spd, oracle_lib, x, 0.0, 1.0, widths, f"igrid tree K={K} segs={segs}",
+          expect_path=spd.SPD_PATH_IGRID_TREE, segs=segs)
 
 
 @pytest.mark.parametrize("segs", [1, 2, 5])
-def test_igrid_tree_segmentation_and_statistics(spd, oracle_lib, segs, monkeypatch):
+def test_igrid_tree_segmentation_and_statistics(spd, oracle_lib, segs):
     rng = np.random.default_rng(78)
     n_t = 2048 * 19 + 4 * 3
     x = (rng.standard_normal((2, n_t)) * 3.1 - 17.0).astype(np.float32)
     x[0, 9000:9000 + 96] += np.float32(4.0)  # width 96 = 3 * 32 is in the set
     mu, sg = oracle_lib.row_stats(x)
-    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(segs))
     widths = spd.spd_width_set_generate("IGRID", 1, 4096)
-    check(spd, oracle_lib, x, mu, sg, widths, f"igrid tree segs={segs}", expect_path=spd.SPD_PATH_IGRID_TREE)
+    check(spd, oracle_lib, x, mu, sg, widths, f"igrid tree segs={segs}", expect_path=spd.SPD_PATH_IGRID_TREE,
+          segs=segs)
 
 
 def test_igrid_tree_exact_ties_and_plateau(spd, oracle_lib):
@@ -149,7 +162,7 @@ def test_igrid_tree_flagged_candidates(spd, oracle_lib):
 
 
 @pytest.mark.parametrize("seed", list(range(10)))
-def test_random_shapes_and_statistics(spd, oracle_lib, seed, monkeypatch):
+def test_random_shapes_and_statistics(spd, oracle_lib, seed):
     """Seeded fuzz over plane shapes, depths, segmentation, width-set family and statistics: row lengths
     that are not multiples of the chunk, rows shorter than a chunk or barely longer than max_width."""
     rng = np.random.default_rng(9000 + seed)
@@ -164,19 +177,18 @@ def test_random_shapes_and_statistics(spd, oracle_lib, seed, monkeypatch):
         t0 = int(rng.integers(0, n_t - 1))
         x[int(rng.integers(0, n_dm)), t0:t0 + S] += np.float32(rng.uniform(5, 15) / np.sqrt(S) * x.std())
     mu, sg = oracle_lib.row_stats(x)
-    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(int(rng.integers(1, 5))))
+    segs = int(rng.integers(0, 5))  # 0: the default work split
     widths = spd.spd_width_set_generate(family, 1 if family == "IGRID" else 0, M)
-    check(spd, oracle_lib, x, mu, sg, widths, f"fuzz seed={seed} {family} K={K} {n_dm}x{n_t}",
-          expect_path=spd.SPD_PATH_IGRID_TREE if family == "IGRID" else spd.SPD_PATH_DYADIC_TREE)
+    check(spd, oracle_lib, x, mu, sg, widths, f"fuzz seed={seed} {family} K={K} {n_dm}x{n_t} segs={segs}",
+          expect_path=spd.SPD_PATH_IGRID_TREE if family == "IGRID" else spd.SPD_PATH_DYADIC_TREE, segs=segs)
 
 
 @pytest.mark.parametrize("segs", [1, 2, 7])
-def test_dyadic_tree_segmentation_is_invisible(spd, oracle_lib, segs, monkeypatch):
+def test_dyadic_tree_segmentation_is_invisible(spd, oracle_lib, segs):
     rng = np.random.default_rng(77)
     n_t = 2048 * 23 + 4 * 3
     x = rng.standard_normal((2, n_t), dtype=np.float32)
-    monkeypatch.setenv("SPD_SEGS_PER_ROW", str(segs))
-    check(spd, oracle_lib, x, 0.0, 1.0, [1 << k for k in range(12)], f"tree segs={segs}")
+    check(spd, oracle_lib, x, 0.0, 1.0, [1 << k for k in range(12)], f"tree segs={segs}", segs=segs)
 
 
 def test_small_lossy_measured_statistics(spd, oracle_lib):
@@ -200,8 +212,9 @@ def test_generic_width_sets(spd, oracle_lib, kind, param, max_width):
     x = rng.standard_normal((5, 10007), dtype=np.float32)  # n_t odd: tree not applicable anyway
     x[2, 5000:5100] += np.float32(1.5)
     widths = spd.spd_width_set_generate(kind, param, max_width)
+    # oracle B on the whole plane, oracle A (direct summation) around the pulse and on the row tail
     check(spd, oracle_lib, x, 0.0, 1.0, widths, f"generic {kind}({param})<= {max_width}",
-          expect_path=spd.SPD_PATH_GENERIC)
+          expect_path=spd.SPD_PATH_GENERIC, direct_windows=[(4900, 5200), (10007 - 300, 10007)])
 
 
 def test_generic_tile_kernel_wide_sets_and_tile_boundaries(spd, oracle_lib):
@@ -216,25 +229,27 @@ def test_generic_tile_kernel_wide_sets_and_tile_boundaries(spd, oracle_lib):
     for kind, param, mw in [("IGRID", 1, 8192), ("BOXDIT", 16, 3000), ("GEOMETRIC", 1500, 20000)]:
         widths = spd.spd_width_set_generate(kind, param, mw)
         st = check(spd, oracle_lib, x, mu, sg, widths, f"tile {kind}({param})<= {mw}",
-                   expect_path=spd.SPD_PATH_GENERIC)
+                   expect_path=spd.SPD_PATH_GENERIC, direct_windows=[(62900, 63100), (n_t - 150, n_t)])
         assert st.max_err_over_tol < 0.5
 
 
-def test_generic_workspace_fallback(spd, oracle_lib, monkeypatch):
-    """The running-sum-in-device-memory kernels (used when max_width does not fit a shared-memory tile)."""
+def test_generic_workspace_fallback(spd, oracle_lib):
+    """The running-sum-in-device-memory kernels (used when max_width does not fit a shared-memory tile;
+    SPD_FLAG_GENERIC_WORKSPACE selects them on a small plane)."""
     rng = np.random.default_rng(32)
     x = rng.standard_normal((4, 30011), dtype=np.float32)
     x[3, 1000:1400] += np.float32(0.8)
     widths = spd.spd_width_set_generate("IGRID", 2, 1024)
-    monkeypatch.setenv("SPD_GENERIC_WORKSPACE", "1")
-    got_snr, got_idx, info = run_gpu(spd, x, 0.0, 1.0, widths)
+    got_snr, got_idx, info = run_gpu(spd, x, 0.0, 1.0, widths, flags=spd.SPD_FLAG_GENERIC_WORKSPACE)
     assert info["launches_per_run"] == 4 and info["workspace_bytes"] > 8 * 4 * 30011
-    monkeypatch.delenv("SPD_GENERIC_WORKSPACE")
     got_snr2, got_idx2, info2 = run_gpu(spd, x, 0.0, 1.0, widths)
     assert info2["launches_per_run"] == 1
     ref_snr, ref_idx, ref_sec = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    d_snr, d_idx, d_sec = oracle_lib.spd_direct(x, 0.0, 1.0, widths, 900, 1500)   # oracle A around the pulse
     for gs, gi, what in ((got_snr, got_idx, "workspace"), (got_snr2, got_idx2, "tile")):
         parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, gs, gi, ref_snr, ref_idx, ref_sec, what=what)
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, gs[:, 900:1500], gi[:, 900:1500], d_snr, d_idx, d_sec,
+                             t0=900, what=what + " direct")
 
 
 def test_width_set_generators_agree_with_formula_module(spd):
@@ -421,17 +436,14 @@ def _activity_truth(snr_h, block, per_row, thr):
     return (y.reshape(n_dm, per_row, block) >= thr).any(axis=2)
 
 
-@pytest.mark.parametrize("cfg,n_dm,n_t,thr,segs", [(3, 6, 262144 + 4 * 11, 6.0, None), (5, 4, 262144, 6.0, "3"),
-                                                     (2, 8, 65536, 4.5, None), (3, 3, 40000, 3.0, "2")])
-def test_flagged_run_equals_plain_run_and_dense_candidates(spd, oracle_lib, cfg, n_dm, n_t, thr, segs,
-                                                           monkeypatch):
+@pytest.mark.parametrize("cfg,n_dm,n_t,thr,segs", [(3, 6, 262144 + 4 * 11, 6.0, 0), (5, 4, 262144, 6.0, 3),
+                                                     (2, 8, 65536, 4.5, 0), (3, 3, 40000, 3.0, 2)])
+def test_flagged_run_equals_plain_run_and_dense_candidates(spd, oracle_lib, cfg, n_dm, n_t, thr, segs):
     """Row a8 fused: spd_run_flagged writes the same Y, W as spd_run; its activity map marks every block
     that holds a sample >= threshold (and may mark no block whose samples are all clearly below it);
     spd_find_candidates_flagged returns exactly the list of the visit-everything kernel, which equals
     the reading-A9 rule evaluated by the oracle on that plane."""
     from workloads import get_workload, make_plane_numpy
-    if segs:
-        monkeypatch.setenv("SPD_SEGS_PER_ROW", segs)
     w = get_workload(cfg).scaled(n_dm, n_t, 12)
     x, _ = make_plane_numpy(w)
     widths = spd.spd_width_set_generate(w.width_kind, w.width_param, min(w.max_width, 8192))
@@ -443,6 +455,9 @@ def test_flagged_run_equals_plain_run_and_dense_candidates(spd, oracle_lib, cfg,
     cap = 1 << 20
     with spd.Plan(n_dm, n_t, widths) as plan:
         assert plan.info["path"] == spd.SPD_PATH_DYADIC_TREE
+        if segs:
+            plan.set_option(spd.SPD_OPT_SEGMENTS_PER_ROW, segs)
+            assert plan.info["segments_per_row"] == segs
         snr0, idx0 = plan.run(plane, mean, sigma)
         snr, idx, act = plan.run_flagged(plane, mean, sigma, thr)
         assert torch.equal(snr0, snr) and torch.equal(idx0, idx)
@@ -514,26 +529,76 @@ def test_flagged_no_detections_and_all_detections(spd):
         assert int(n1.item()) == int(n_d.item()) > 0
 
 
-@pytest.mark.parametrize("n_dm,n_t", [(16, 65536), (5, 10007), (300, 4096 + 4), (2, 1 << 21)])
-@pytest.mark.parametrize("clip,passes", [(0.0, 0), (2.0, 1), (2.5, 4), (3.0, 8)])
-def test_row_stats_against_oracle(spd, oracle_lib, n_dm, n_t, clip, passes):
-    """Row f1: per-DM mean / sigma with point-wise outlier rejection (reading A14).
-    Tolerance 2e-6 * sigma: the kept set is decided in float32 on both sides; a sample within an ulp
-    of the rejection limit may fall on the other side when the previous pass's float32 estimate
-    differs in its last bit."""
-    rng = np.random.default_rng(n_dm * 31 + passes)
+def _stats_plane(n_dm, n_t, seed):
+    rng = np.random.default_rng(seed)
     x = (rng.standard_normal((n_dm, n_t)) * 2.5 + 11.0).astype(np.float32)
     x[0, n_t // 4: n_t // 4 + max(4, n_t // 50)] += np.float32(40.0)  # a strong wide pulse
     x[n_dm - 1, ::97] -= np.float32(25.0)                             # scattered outliers
+    return x
+
+
+def _assert_stats_close(got_mu, got_sg, ref_mu, ref_sg, n_border, n_t, clip):
+    """The oracle decides |x - mu| <= clip sigma in double on unrounded estimates, the kernel in float32 on the
+    float32 estimates it hands out.  Rows without a border-line sample (none within 1e-6 sigma of a limit in
+    any pass) must agree to 2e-6 sigma; every border-line sample may change sides and then moves the mean
+    by at most clip sigma / n_kept and sigma by about (clip^2 + 1) sigma / (2 n_kept)."""
+    base = 2e-6 * ref_sg + 1e-7 * np.abs(ref_mu)
+    per_flip = (clip * clip + 2.0) * ref_sg / (0.5 * n_t)
+    tol = base + n_border * per_flip
+    assert np.all(np.abs(got_mu - ref_mu) <= tol), float(np.max(np.abs(got_mu - ref_mu) / tol))
+    assert np.all(np.abs(got_sg - ref_sg) <= tol), float(np.max(np.abs(got_sg - ref_sg) / tol))
+    if n_t <= 100000:
+        assert np.mean(n_border == 0) > 0.5, "the tight comparison must cover most rows"
+
+
+@pytest.mark.parametrize("n_dm,n_t", [(16, 65536), (5, 10007), (300, 4096 + 4), (2, 1 << 21)])
+@pytest.mark.parametrize("clip,passes", [(0.0, 0), (2.0, 1), (2.5, 4), (3.0, 8)])
+def test_row_stats_against_oracle(spd, oracle_lib, n_dm, n_t, clip, passes):
+    """Row f1: per-DM mean / sigma with point-wise outlier rejection (reading A14) against
+    the double-precision oracle; see _assert_stats_close for the bound."""
+    x = _stats_plane(n_dm, n_t, n_dm * 31 + passes)
     dev = torch.device("cuda:0")
     widths = [1, 2, 4] if n_t % 4 == 0 else [1, 3]
     with spd.Plan(n_dm, n_t, widths) as plan:
         mean, sigma = plan.row_stats(torch.from_numpy(x).to(dev), clip, passes)
         got_mu, got_sg = mean.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
-    ref_mu, ref_sg = oracle_lib.row_stats_clipped(x, clip, passes)
-    tol = 2e-6 * ref_sg + 1e-7 * np.abs(ref_mu)
-    assert np.all(np.abs(got_mu - ref_mu) <= tol), float(np.max(np.abs(got_mu - ref_mu) / tol))
-    assert np.all(np.abs(got_sg - ref_sg) <= tol), float(np.max(np.abs(got_sg - ref_sg) / tol))
+    ref_mu, ref_sg, n_pass, n_border = oracle_lib.row_stats_clipped(x, clip, passes, border_eps=1e-6, details=True)
+    _assert_stats_close(got_mu, got_sg, ref_mu, ref_sg, n_border, n_t, clip)
+
+
+@pytest.mark.parametrize("n_dm,n_t,clip,rel_tol", [(24, 65536, 2.0, 1e-4), (7, 30001, 2.5, 1e-3), (64, 8192, 3.0, 0.0),
+                                                    (3, 1 << 20, 2.0, 1e-5)])
+def test_row_stats_until_convergence(spd, oracle_lib, n_dm, n_t, clip, rel_tol):
+    """spd_row_stats_converge ("repeated until convergence"): the device-side stop against the
+    oracle's, rule stated in double there.  Pass counts agree (a row whose last change is within 2e-6 of the
+    tolerance may stop one pass apart), estimates within the border-line bound, and a row that has stopped
+    is not touched by later passes (same result with a larger pass limit)."""
+    x = _stats_plane(n_dm, n_t, 4000 + n_dm)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    widths = [1, 2, 4] if n_t % 4 == 0 else [1, 3]
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        mean, sigma, n_p = plan.row_stats_converge(plane, clip, 40, rel_tol)
+        got_mu, got_sg = mean.cpu().numpy().astype(np.float64), sigma.cpu().numpy().astype(np.float64)
+        got_p = n_p.cpu().numpy()
+        mean2, sigma2, n_p2 = plan.row_stats_converge(plane, clip, 64, rel_tol)
+        assert torch.equal(mean, mean2) and torch.equal(sigma, sigma2) and torch.equal(n_p, n_p2)
+        # the caller's fixed count reproduces it where the counts agree
+        mean3, sigma3 = plan.row_stats(plane, clip, int(got_p.max()))
+        with pytest.raises(spd.SpdError):
+            plan.row_stats_converge(plane, clip, 0, rel_tol)       # needs at least one rejection pass
+        with pytest.raises(spd.SpdError):
+            plan.row_stats_converge(plane, clip, 8, -1.0)
+    ref_mu, ref_sg, ref_p, n_border = oracle_lib.row_stats_clipped(x, clip, 40, rel_tol=rel_tol, border_eps=1e-6,
+                                                                  details=True)
+    assert np.all(got_p >= 1) and np.all(got_p < 40), "the iteration must stop on its own"
+    same = got_p == ref_p
+    assert np.all(np.abs(got_p - ref_p) <= 1) and same.mean() > 0.8, (got_p, ref_p)
+    _assert_stats_close(got_mu[same], got_sg[same], ref_mu[same], ref_sg[same], n_border[same], n_t, clip)
+    # one pass apart: both sides are within the tolerance of the fixed point
+    assert np.all(np.abs(got_sg - ref_sg)[~same] <= (2.0 * rel_tol + 1e-5) * ref_sg[~same])
+    top = got_p == got_p.max()
+    assert np.array_equal(mean3.cpu().numpy()[top], mean.cpu().numpy()[top])
 
 
 def test_row_stats_feed_the_hot_path(spd, oracle_lib):
@@ -783,16 +848,15 @@ def test_warp_stream_kernel_pieces_span_rows(spd, oracle_lib, K):
 
 
 @pytest.mark.parametrize("K", [9, 14])
-def test_block_and_warp_kernels_agree(spd, oracle_lib, K, monkeypatch):
-    """SPD_TREE_KERNEL=block keeps the block-per-stream kernel: both kernels pass parity on the same plane, and
+def test_block_and_warp_kernels_agree(spd, oracle_lib, K):
+    """SPD_FLAG_BLOCK_TREE keeps the block-per-stream kernel: both kernels pass parity on the same plane, and
     their SNR planes differ by no more than the tag perturbation (31 ulp)."""
     rng = np.random.default_rng(77 + K)
     n_t = 512 * 40 + 12
     x = rng.standard_normal((4, n_t)).astype(np.float32)
     widths = [1 << k for k in range(K)]
     a_snr, a_idx, a_info = run_gpu(spd, x, 0.0, 1.0, widths)
-    monkeypatch.setenv("SPD_TREE_KERNEL", "block")
-    b_snr, b_idx, b_info = run_gpu(spd, x, 0.0, 1.0, widths)
+    b_snr, b_idx, b_info = run_gpu(spd, x, 0.0, 1.0, widths, flags=spd.SPD_FLAG_BLOCK_TREE)
     assert a_info["tree_kernel"] == 2 and b_info["tree_kernel"] == 1
     ref = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
     for snr, idx, name in ((a_snr, a_idx, "warp"), (b_snr, b_idx, "block")):
@@ -832,15 +896,19 @@ def test_width_sigma_matches_oracle(spd, oracle_lib, n_dm, n_t, kind, param, M):
         assert ref[0][-1] > 0 and not np.allclose(ref[0], ref[0][0] * np.sqrt(np.asarray(widths) / widths[0]), rtol=0.05)
 
 
-def test_run_with_measured_sigma_per_width(spd, oracle_lib):
-    """spd_run_sigma_w on the any-width-set and the grid path against direct summation with the same table;
-    a streaming-tree plan refuses."""
-    rng = np.random.default_rng(31)
-    n_dm, n_t = 3, 20000
+def _plane_for_sigma_w(n_dm, n_t, seed):
+    rng = np.random.default_rng(seed)
     x = rng.standard_normal((n_dm, n_t))
-    x[1] = np.convolve(x[1], np.ones(5) / 2.0, mode="same")
-    x[2, 9000:9040] += 1.5
-    x = (x + 2.0).astype(np.float32)
+    x[1] = np.convolve(x[1], np.ones(5) / 2.0, mode="same")      # correlated: sigma_L is not sqrt(L) sigma
+    x[2, n_t // 2: n_t // 2 + 40] += 1.5
+    return (x + 2.0).astype(np.float32)
+
+
+def test_run_with_measured_sigma_per_width(spd, oracle_lib):
+    """spd_run_sigma_w on the any-width-set path against direct summation with the same table (oracle A,
+    every sample); a uint8-index plan refuses; misaligned buffers are an error, not a fault."""
+    n_dm, n_t = 3, 20000
+    x = _plane_for_sigma_w(n_dm, n_t, 31)
     dev = torch.device("cuda:0")
     plane = torch.from_numpy(x).to(dev)
     widths = spd.spd_width_set_generate("IGRID", 1, 128)
@@ -849,25 +917,86 @@ def test_run_with_measured_sigma_per_width(spd, oracle_lib):
         sw = plan.width_sigma(plane, mean)
         snr, idx = plan.run_sigma_w(plane, mean, sw)
         torch.cuda.synchronize()
+        big = torch.empty(n_dm * n_t + 4, dtype=torch.float32, device=dev)
+        with pytest.raises(spd.SpdError) as e:   # an offset view: 4-byte aligned only
+            spd.binding._check(spd.load().spd_run_sigma_w(
+                plan.handle, plane.data_ptr(), mean.data_ptr(), sw.data_ptr(), big.data_ptr() + 4,
+                idx.data_ptr(), 0))
+        assert e.value.status == -1
     mu64 = mean.cpu().numpy().astype(np.float64)
     sw64 = sw.cpu().numpy().astype(np.float64)
     ref = oracle_lib.spd_direct_sw(x, mu64, sw64, widths)
-    got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
-    tol = parity.snr_tolerance(ref[0])
-    assert np.all(np.abs(got_snr - ref[0]) <= tol)
-    decisive = (ref[0] - ref[2]) > tol
-    assert np.array_equal(got_idx[decisive], ref[1][decisive])
-    # grid plan with the same table
-    seps = spd.spd_separation_generate("IGRID", 4, widths)
-    with spd.Plan(n_dm, n_t, widths, 128, separations=seps) as plan:
-        snr_g, idx_g = plan.run_sigma_w(plane, mean, sw)
-        torch.cuda.synchronize()
-    on = (np.arange(n_t)[None, :] % np.asarray(seps)[np.clip(ref[1], 0, None)]) == 0
-    assert np.all(np.abs(snr_g.cpu().numpy() - ref[0])[on & decisive & (ref[1] == idx_g.cpu().numpy())] <= tol[on & decisive & (ref[1] == idx_g.cpu().numpy())])
-    assert np.all(snr_g.cpu().numpy() <= got_snr + tol)                    # a grid evaluates a subset of the windows
-    with spd.Plan(n_dm, n_t, [1, 2, 4, 8], 8) as plan:
+    parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, None, snr.cpu().numpy(), idx.cpu().numpy(), *ref,
+                               what="sigma_w generic")
+    with spd.Plan(n_dm, n_t, [1, 2, 4, 8], 8, flags=spd.SPD_FLAG_WIDTH_U8) as plan:
         with pytest.raises(spd.SpdError):
             plan.run_sigma_w(plane, mean, sw[:, :4].contiguous())
+
+
+@pytest.mark.parametrize("wkind,wparam,M,gkind,gparam", [("BOXDIT", 8, 120, "BOXDIT", 8), ("IGRID", 1, 128, "IGRID", 4),
+                                                          ("POW2", 0, 256, "DIT", 0), ("POW2", 0, 4096, "IGRID", 4),
+                                                          ("IGRID", 2, 512, "EVERY_SAMPLE", 0)])
+def test_grid_plans_with_measured_sigma_per_width(spd, oracle_lib, wkind, wparam, M, gkind, gparam):
+    """spd_run_sigma_w on SPD_PATH_GRID plans (rows f1 + f2 together), every sample against
+    oracle_spd_grid_sw with the table the device measured: BoxDIT, IGRID and DIT grids, and a {2^k} set that
+    also has a tree plan (K = 13: spd_run takes the tree kernel, spd_run_sigma_w the grid tile kernel)."""
+    n_dm, n_t = 3, 12000 + 4 * 13
+    x = _plane_for_sigma_w(n_dm, n_t, 77 + M)
+    widths = spd.spd_width_set_generate(wkind, wparam, M)
+    seps = spd.spd_separation_generate(gkind, gparam, widths)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, M, separations=seps) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GRID
+        mean, _ = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    ref = oracle_lib.spd_grid_sw(x, mu64, sw64, widths, seps)
+    st = parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, seps, snr.cpu().numpy(), idx.cpu().numpy(),
+                                    *ref, what=f"sigma_w grid {wkind}/{gkind}")
+    assert st.n == n_dm * n_t
+
+
+@pytest.mark.parametrize("K", [3, 8, 15, 16])
+def test_block_kernel_with_measured_sigma_per_width(spd, oracle_lib, K):
+    """spd_run_sigma_w on the block-per-stream kernel (K <= 8 and configs 4 / 5: K = 16 / 15), PAPER.md:728:
+    parity with direct summation using the same table; the table sqrt(L) sigma reproduces spd_run."""
+    M = 1 << (K - 1)
+    n_dm, n_t = 3, max(2048 * 7 + 8, 2 * M + 2048 + 20)
+    x = _plane_for_sigma_w(n_dm, n_t, 500 + K)
+    x[0, n_t // 3: n_t // 3 + max(1, M // 2)] += np.float32(9.0 / np.sqrt(max(1, M // 2)))
+    widths = [1 << k for k in range(K)]
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, M) as plan:
+        assert plan.info["tree_kernel"] == 1
+        plan.set_option(spd.SPD_OPT_SEGMENTS_PER_ROW, 2)
+        mean, sigma = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        white = (sigma[:, None] * torch.sqrt(torch.tensor(widths, dtype=torch.float32, device=dev))[None, :]).contiguous()
+        snr_w, idx_w = plan.run_sigma_w(plane, mean, white)
+        snr_0, idx_0 = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    # oracle A on windows (direct summation of 2^15-sample boxcars over whole rows is minutes): the pulse,
+    # a segment boundary, the row tail
+    got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+    for t0, t1 in [(n_t // 3 - 300, n_t // 3 + 300), (n_t // 2 - 200, n_t // 2 + 200), (n_t - 500, n_t), (0, 300)]:
+        ref = oracle_lib.spd_direct_sw(x, mu64, sw64, widths, t0, t1)
+        tol = parity.snr_tolerance(ref[0])
+        fit = ref[1] >= 0
+        assert np.all(np.abs(got_snr[:, t0:t1] - ref[0])[fit] <= tol[fit]), (K, t0)
+        decisive = fit & ((ref[0] - ref[2]) > tol)
+        assert np.array_equal(got_idx[:, t0:t1][decisive], ref[1][decisive]), (K, t0)
+    a, b = snr_w.cpu().numpy(), snr_0.cpu().numpy()
+    fin = np.isfinite(b)
+    assert np.all(np.abs(a - b)[fin] <= 1e-5 * np.maximum(1.0, np.abs(b[fin])))
+    assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
 
 
 @pytest.mark.parametrize("K", [9, 12, 14])
