@@ -48,6 +48,10 @@ def parse_args():
                     "(widths 2^k and 3*2^m, the paper's IG(1) set) - not the BASELINE configuration")
     ap.add_argument("--grid", default="", help="boxcar separation per width (SURVEY.md sec. 8(f2)): BOXDIT:<L_max>, "
                     "DIT or IGRID:<layers>; the width set is then evaluated on the paper's decimated grid")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config legs (the other BASELINE "
+                    "configs and the IG(1) width set, measured in the same run at N = 1)")
+    ap.add_argument("--per-config-steps", type=int, default=5)
+    ap.add_argument("--width-u8", action="store_true", help="uint8 width index (SPD_FLAG_WIDTH_U8): 9 B per sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -292,11 +296,170 @@ def measured_peak():
 # ----------------------------------------------------------------------------------------
 # the B200 arm
 # ----------------------------------------------------------------------------------------
+KERNEL_NAMES = {"tree_ws": "spd_tree_ws_kernel", "tree_block": "spd_tree_kernel", "tree_ig": "spd_tree_ig_kernel",
+                "grid_ws": "spd_tree_ws_kernel (grid)", "grid_tile": "grid_tile_kernel", "generic": "generic_tile_kernel"}
+
+
+def kernel_key(spd, info):
+    if info["path"] == spd.SPD_PATH_DYADIC_TREE:
+        return "tree_ws" if info["tree_kernel"] == 2 else "tree_block"
+    if info["path"] == spd.SPD_PATH_IGRID_TREE:
+        return "tree_ig"
+    if info["path"] == spd.SPD_PATH_GRID:
+        return "grid_ws" if info["tree_kernel"] == 2 else "grid_tile"
+    return "generic"
+
+
+class Workbench:
+    """One workload resident on the device: plane, statistics, outputs, plan; step() runs the hot path once."""
+
+    def __init__(self, spd, torch, w, dev, grid="", width_u8=False):
+        from workloads import make_plane_torch
+        self.spd, self.torch, self.w, self.dev = spd, torch, w, dev
+        self.widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
+        self.n = w.n_samples
+        self.plane, self.pulses = make_plane_torch(w, dev)
+        self.mean = torch.zeros(w.n_dm, dtype=torch.float32, device=dev)
+        self.sigma = torch.ones(w.n_dm, dtype=torch.float32, device=dev)
+        self.thr = w.candidate_threshold if w.candidate_threshold is not None else 6.0
+        self.cap = 1 << 22
+        seps = None
+        if grid:
+            gkind, _, gparam = grid.partition(":")
+            seps = spd.spd_separation_generate(gkind, int(gparam or 0), self.widths)
+        flags = spd.SPD_FLAG_WIDTH_U8 if width_u8 else 0
+        self.plan = spd.Plan(w.n_dm, w.n_t, self.widths, w.max_width, flags=flags, separations=seps)
+        self.info = self.plan.info
+        self.bytes_per_sample = 8 + self.info["width_bytes"]
+        self.out_snr = torch.empty((w.n_dm, w.n_t), dtype=torch.float32, device=dev)
+        self.out_width = torch.empty((w.n_dm, w.n_t), dtype=torch.uint8 if width_u8 else torch.int32, device=dev)
+        # Per-DM mu, sigma: supplied (0, 1) by the config, or measured (reading A6) by spd_row_stats.
+        if w.stats == "measured":
+            self.plan.row_stats(self.plane, 0.0, 0, self.mean, self.sigma)
+        self.activity = torch.empty(self.info["activity_bytes"], dtype=torch.uint8, device=dev)
+        self.cand_list = torch.empty(self.cap * 16, dtype=torch.uint8, device=dev)
+        self.cand_count = torch.zeros(1, dtype=torch.int64, device=dev)
+        # planes smaller than L2 would be re-read from cache: flush between steps
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if 3 * self.n * 4 <= (512 << 20) else None
+        self.stream = torch.cuda.current_stream()
+
+    def step(self, ev=None):
+        if self.flush is not None:
+            self.flush.fill_(1)
+        if ev is not None:
+            ev[0].record(self.stream)
+        self.plan.run_flagged(self.plane, self.mean, self.sigma, self.thr, self.out_snr, self.out_width, self.activity)
+        if ev is not None:
+            ev[1].record(self.stream)
+        lst, n_found = self.plan.find_candidates_flagged(self.out_snr, self.out_width, self.activity, self.thr,
+                                                         self.cap, lst=self.cand_list, n_found=self.cand_count)
+        if ev is not None:
+            ev[2].record(self.stream)
+        return lst, n_found
+
+    def timed(self, fn, reps=1):
+        """Device time of fn() in ms (CUDA events on the launching stream, one untimed call first)."""
+        torch = self.torch
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.stream)
+        for _ in range(reps):
+            fn()
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    def run_steps(self, steps, warmup, barrier=None, sampler=None):
+        """W warm-up steps, then exactly `steps` timed ones between barriers; returns the step record."""
+        torch = self.torch
+        barrier = barrier or torch.cuda.synchronize
+        for _ in range(max(warmup, 0)):
+            self.step()
+        barrier()
+        if sampler is not None:
+            sampler.start()
+            time.sleep(0.15)
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t0 = time.perf_counter()
+        e_beg.record(self.stream)
+        n_found = None
+        for i in range(steps):
+            _, n_found = self.step(evs[i])
+        e_end.record(self.stream)
+        barrier()
+        t1 = time.perf_counter()
+        clocks = sampler.stop(t0, t1) if sampler is not None else None
+        total_ms = e_beg.elapsed_time(e_end)
+        run_ms = [e[0].elapsed_time(e[1]) for e in evs]
+        cand_ms = [e[1].elapsed_time(e[2]) for e in evs]
+        flush_ms = 0.0
+        if self.flush is not None:  # the flush is not part of the path: take it out of the step time
+            flush_ms = (total_ms - sum(run_ms) - sum(cand_ms)) / steps
+            total_ms = sum(run_ms) + sum(cand_ms)
+        return {"total_ms": total_ms, "run_ms": run_ms, "cand_ms": cand_ms, "flush_ms": flush_ms, "clocks": clocks,
+                "n_cand": int(n_found.item())}
+
+    def roofline(self, rec, peak, peak_src):
+        k_ms = sum(rec["run_ms"]) / len(rec["run_ms"])
+        achieved = self.bytes_per_sample * self.n / (k_ms * 1e-3) / 1e9
+        key = kernel_key(self.spd, self.info)
+        traffic, traffic_src = ncu_traffic_bytes(key, self.w, self.info["width_bytes"])
+        return {
+            "bound": "hbm", "kernel": KERNEL_NAMES[key], "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
+            "algorithmic_bytes_per_launch": self.bytes_per_sample * self.n, "bytes_per_sample": self.bytes_per_sample,
+            "kernel_ms": k_ms, "kernel_ms_min": min(rec["run_ms"]),
+            "candidates_ms": sum(rec["cand_ms"]) / len(rec["cand_ms"]),
+            "kernel_share_of_step": sum(rec["run_ms"]) / (sum(rec["run_ms"]) + sum(rec["cand_ms"])),
+        }
+
+    def close(self):
+        self.plan.close()
+        for name in ("plane", "out_snr", "out_width", "activity", "cand_list", "flush"):
+            setattr(self, name, None)
+        self.torch.cuda.empty_cache()
+
+
+def per_config_legs(args, spd, torch, dev, peak, peak_src, uuid, local_rank):
+    """The other BASELINE configs and the paper's IG(1) width set, measured in this same run (N = 1):
+    the same step, fewer repetitions, each with its own clock record."""
+    from dataclasses import replace
+    from workloads import get_workload
+    legs = [(f"configs[{c - 1}]", get_workload(c), "") for c in (1, 2, 3, 4, 5) if c != args.workload]
+    ig = replace(get_workload(3), width_kind="IGRID", width_param=1)
+    legs.append(("configs[2] with the IG(1) width set (26 widths 2^k and 3*2^m, PAPER.md:364-387)", ig, ""))
+    legs.append(("configs[2] on the DIT grid (Alg. 3, PAPER.md:311)", get_workload(3), "DIT"))
+    legs.append(("configs[2], IG(1) widths on 4 layers (PAPER.md:356)", ig, "IGRID:4"))
+    legs.append(("configs[2], BoxDIT L_max = 8 (Alg. 1, eq. 14)",
+                 replace(get_workload(3), width_kind="BOXDIT", width_param=8), "BOXDIT:8"))
+    out = []
+    for name, w, grid in legs:
+        free, _ = torch.cuda.mem_get_info(dev)
+        if free < 13 * w.n_samples + (4 << 30):
+            out.append({"workload": name, "skipped": f"needs {(13 * w.n_samples) >> 30} GiB of device memory"})
+            continue
+        wb = Workbench(spd, torch, w, dev, grid=grid)
+        rec = wb.run_steps(args.per_config_steps, 3, sampler=ClockSampler(uuid if uuid else local_rank))
+        rf = wb.roofline(rec, peak, peak_src)
+        ms = rec["total_ms"] / args.per_config_steps
+        out.append({"workload": name, "n_dm": w.n_dm, "n_t": w.n_t, "n_widths": len(wb.widths),
+                    "width_set": f"{w.width_kind}<= {w.max_width}", "grid": grid or "every sample",
+                    "steps": args.per_config_steps, "ms_per_step": ms, "value": wb.n / (ms * 1e-3), "unit": UNIT,
+                    "kernel": rf["kernel"], "kernel_ms": rf["kernel_ms"], "kernel_ms_min": rf["kernel_ms_min"],
+                    "frac": rf["frac"], "achieved_gbs": rf["achieved"], "candidates_ms": rf["candidates_ms"],
+                    "candidates_found": rec["n_cand"], "clocks": rec["clocks"],
+                    **({"l2_flush_ms_per_step_excluded": rec["flush_ms"]} if wb.flush is not None else {})})
+        wb.close()
+        del wb
+    return out
+
+
 def run_b200(args):
-    import numpy as np
     import torch
     import paper_1910_08324_b200 as spd
-    from workloads import get_workload, make_plane_torch
+    from workloads import get_workload
 
     rank, local_rank, world = dist_env()
     if not torch.cuda.is_available():
@@ -314,133 +477,58 @@ def run_b200(args):
     if args.n_dm:
         w = w.scaled(args.n_dm, w.n_t)
     # weak scaling: every rank holds its own n_dm DM trials (different seed per rank)
-    w_rank = rank_workload(w, rank)
-    widths = spd.spd_width_set_generate(w.width_kind, w.width_param, w.max_width)
-    n = w.n_samples
+    wb = Workbench(spd, torch, rank_workload(w, rank), dev, grid=args.grid, width_u8=args.width_u8)
+    plan, info, widths, n = wb.plan, wb.info, wb.widths, wb.n
 
-    plane, pulses = make_plane_torch(w_rank, dev)
-    mean = torch.zeros(w.n_dm, dtype=torch.float32, device=dev)
-    sigma = torch.ones(w.n_dm, dtype=torch.float32, device=dev)
-    out_snr = torch.empty((w.n_dm, w.n_t), dtype=torch.float32, device=dev)
-    out_width = torch.empty((w.n_dm, w.n_t), dtype=torch.int32, device=dev)
-    thr = w.candidate_threshold if w.candidate_threshold is not None else 6.0
-    cap = 1 << 22
-    seps = None
-    if args.grid:
-        gkind, _, gparam = args.grid.partition(":")
-        seps = spd.spd_separation_generate(gkind, int(gparam or 0), widths)
-    plan = spd.Plan(w.n_dm, w.n_t, widths, w.max_width, separations=seps)
-    info = plan.info
-    # Per-DM mu, sigma: supplied (0, 1) by the config, or measured (reading A6) by spd_row_stats.
     # The step before the hot path: timed on its own, outside the step.
-    stats_ms = None
-    if w.stats == "measured":
-        plan.row_stats(plane, 0.0, 0, mean, sigma)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    s_mean, s_sigma = torch.empty_like(mean), torch.empty_like(sigma)
-    plan.row_stats(plane, 2.0, 2, s_mean, s_sigma)
-    e0.record(torch.cuda.current_stream())
-    plan.row_stats(plane, 2.0, 2, s_mean, s_sigma)
-    e1.record(torch.cuda.current_stream())
-    torch.cuda.synchronize()
-    stats_ms = e0.elapsed_time(e1)
+    s_mean, s_sigma = torch.empty_like(wb.mean), torch.empty_like(wb.sigma)
+    stats_ms = wb.timed(lambda: plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma))
+    n_pass = torch.empty(w.n_dm, dtype=torch.int32, device=dev)
+    conv_ms = wb.timed(lambda: plan.row_stats_converge(wb.plane, 2.0, 32, 1e-4, s_mean, s_sigma, n_pass))
+    conv_passes = float(n_pass.float().mean().item())
+    plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma)
     # sigma per width from power-of-two decimations (row f1): one more read of the plane
-    sw = plan.width_sigma(plane, s_mean)
-    e0.record(torch.cuda.current_stream())
-    plan.width_sigma(plane, s_mean, sw)
-    e1.record(torch.cuda.current_stream())
-    torch.cuda.synchronize()
-    wsig_ms = e0.elapsed_time(e1)
+    sw = plan.width_sigma(wb.plane, s_mean)
+    wsig_ms = wb.timed(lambda: plan.width_sigma(wb.plane, s_mean, sw))
     # the same pass with the measured sigma per width in place of eq. (5) (where the plan's kernels take it)
-    run_sw_ms = None
-    if info["tree_kernel"] == 2 or info["path"] in (spd.SPD_PATH_GENERIC, spd.SPD_PATH_GRID):
-        try:
-            plan.run_sigma_w(plane, s_mean, sw, out_snr, out_width)
-            e0.record(torch.cuda.current_stream())
-            plan.run_sigma_w(plane, s_mean, sw, out_snr, out_width)
-            e1.record(torch.cuda.current_stream())
-            torch.cuda.synchronize()
-            run_sw_ms = e0.elapsed_time(e1)
-        except spd.SpdError:
-            run_sw_ms = None
+    try:
+        run_sw_ms = wb.timed(lambda: plan.run_sigma_w(wb.plane, s_mean, sw, wb.out_snr, wb.out_width))
+    except spd.SpdError:
+        run_sw_ms = None
     del sw
-    activity = torch.empty(info["activity_bytes"], dtype=torch.uint8, device=dev)
-    cand_list = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
-    cand_count = torch.zeros(1, dtype=torch.int64, device=dev)
-    # planes smaller than L2 would be re-read from cache: flush between steps
-    need_flush = 3 * n * 4 <= (512 << 20)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if need_flush else None
-    stream = torch.cuda.current_stream()
-
-    def step(ev=None):
-        if flush is not None:
-            flush.fill_(1)
-        if ev is not None:
-            ev[0].record(stream)
-        plan.run_flagged(plane, mean, sigma, thr, out_snr, out_width, activity)
-        if ev is not None:
-            ev[1].record(stream)
-        lst, n_found = plan.find_candidates_flagged(out_snr, out_width, activity, thr, cap,
-                                                    lst=cand_list, n_found=cand_count)
-        if ev is not None:
-            ev[2].record(stream)
-        return lst, n_found
 
     def barrier():
         if distributed:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 0)):
-        step()
-    barrier()
-
     uuid = None
     try:
         uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
     except Exception:
         pass
-    sampler = ClockSampler(uuid if uuid else local_rank)
-    sampler.start()
-    time.sleep(0.15)
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-    e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0 = time.perf_counter()
-    e_beg.record(stream)
-    for i in range(args.steps):
-        lst, n_found = step(evs[i])
-    e_end.record(stream)
-    barrier()
-    t1 = time.perf_counter()
-    clocks = sampler.stop(t0, t1)
-    total_ms = e_beg.elapsed_time(e_end)
-    run_ms = [e[0].elapsed_time(e[1]) for e in evs]
-    cand_ms = [e[1].elapsed_time(e[2]) for e in evs]
-    flush_ms = 0.0
-    if flush is not None:  # the flush is not part of the path: take it out of the step time
-        flush_ms = total_ms - sum(run_ms) - sum(cand_ms)
-        total_ms = sum(run_ms) + sum(cand_ms)
-    total_ms = max_over_ranks(total_ms, dev)
+    rec = wb.run_steps(args.steps, args.warmup, barrier=barrier, sampler=ClockSampler(uuid if uuid else local_rank))
+    total_ms = max_over_ranks(rec["total_ms"], dev)
     ms_per_step = total_ms / args.steps
     value = whole_job_value(world, n, ms_per_step)
-    n_cand = int(n_found.item())
 
     # ---- roofline of the dominant kernel (the spd_run kernel) ---------------------------
     peak, peak_src = measured_peak()
-    k_ms = sum(run_ms) / len(run_ms)
-    achieved = BYTES_PER_SAMPLE * n / (k_ms * 1e-3) / 1e9
-    roofline = {
-        "bound": "hbm", "kernel": {spd.SPD_PATH_DYADIC_TREE: "spd_tree_ws_kernel" if info["tree_kernel"] == 2 else "spd_tree_kernel",
-                   spd.SPD_PATH_IGRID_TREE: "spd_tree_ig_kernel",
-                   spd.SPD_PATH_GRID: "spd_tree_ws_kernel (grid)" if info["tree_kernel"] == 2 else "grid_tile_kernel"}.get(
-                       info["path"], "generic_tile_kernel"),
-        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "peak_source": peak_src, "traffic": ncu_traffic_bytes(w),
-        "algorithmic_bytes_per_launch": BYTES_PER_SAMPLE * n, "bytes_per_sample": BYTES_PER_SAMPLE,
-        "kernel_ms": k_ms, "kernel_ms_min": min(run_ms), "candidates_ms": sum(cand_ms) / len(cand_ms),
-        "kernel_share_of_step": sum(run_ms) / (sum(run_ms) + sum(cand_ms)),
-    }
+    roofline = wb.roofline(rec, peak, peak_src)
+
+    # ---- row f4: the 2-D (DM x time) peak stage over the step's 1-D list (reading A18) -----
+    cluster = None
+    try:
+        lst2 = torch.empty(wb.cap * 16, dtype=torch.uint8, device=dev)
+        n2 = torch.zeros(1, dtype=torch.int64, device=dev)
+        c_ms = wb.timed(lambda: plan.cluster_candidates(wb.out_snr, wb.cand_list, wb.cand_count, wb.cap, 1, wb.cap,
+                                                        lst_out=lst2, n_out=n2))
+        cluster = {"what": "spd_cluster_candidates, dm_radius 1, over the step's 1-D list; not part of the step",
+                   "ms": c_ms, "candidates_in": min(rec["n_cand"], wb.cap), "kept": int(n2.item()),
+                   "injected_pulses": len(wb.pulses)}
+        del lst2
+    except spd.SpdError as e:
+        cluster = {"error": str(e)}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -450,35 +538,45 @@ def run_b200(args):
             **({"grid": args.grid + " (a boxcar separation per width: widths of later iterations only at "
                                     "every 2^i-th sample; one merged plane)"} if args.grid else {}),
             "parallelism": f"dm-rows x{world} (independent DM trials per GPU, no collective)",
-            "path": {spd.SPD_PATH_DYADIC_TREE: "dyadic_tree", spd.SPD_PATH_IGRID_TREE: "igrid_tree"}.get(
-                info["path"], "generic"),
+            "path": {spd.SPD_PATH_DYADIC_TREE: "dyadic_tree", spd.SPD_PATH_IGRID_TREE: "igrid_tree",
+                     spd.SPD_PATH_GRID: "grid"}.get(info["path"], "generic"),
+            "width_index_bytes": info["width_bytes"],
             "blocks": info["blocks"], "threads_per_block": info["threads_per_block"],
             "segments_per_row": info["segments_per_row"], "piece_chunks": info["piece_chunks"], "chunk": info["chunk"], "smem_bytes": info["smem_bytes"],
-            "candidate_threshold": thr, "candidates_found": n_cand}),
+            "candidate_threshold": wb.thr, "candidates_found": rec["n_cand"]}),
         "roofline": roofline,
-        "clocks": clocks,
+        "clocks": rec["clocks"],
         "gpu_launches": args.steps * (info["launches_per_run"] + 1),
         "real_time_factor_plane": (w.n_t * w.sampling_time_s) / (ms_per_step * 1e-3),
         "real_time_factor_ska_like": value / PAPER_SKA_SAMPLES_PER_S,
         "n_dm_real_time": value * w.sampling_time_s,
         "row_stats": {"what": "spd_row_stats, 3 passes (plain + 2 rejection passes at 2 sigma), not part of the step",
-                      "ms": stats_ms, "gbs": 3 * 4 * n / (stats_ms * 1e-3) / 1e9, "bytes_per_sample_per_pass": 4},
+                      "ms": stats_ms, "gbs": 3 * 4 * n / (stats_ms * 1e-3) / 1e9, "bytes_per_sample_per_pass": 4,
+                      "until_convergence": {"what": "spd_row_stats_converge, clip 2 sigma, rel_tol 1e-4, limit 32 passes "
+                                                    "(converged rows are skipped by later passes)",
+                                            "ms": conv_ms, "mean_rejection_passes": conv_passes}},
         "width_sigma": {"what": "spd_width_sigma: sigma per width from power-of-two decimations, interpolated; "
                                 "one pass, not part of the step",
                         "ms": wsig_ms, "gbs": 4 * n / (wsig_ms * 1e-3) / 1e9, "bytes_per_sample": 4,
                         "run_sigma_w_ms": run_sw_ms},
+        "cluster_stage": cluster,
     }
-    if flush is not None:
-        line["config"]["l2_flush_ms_per_step_excluded"] = flush_ms / args.steps
+    if wb.flush is not None:
+        line["config"]["l2_flush_ms_per_step_excluded"] = rec["flush_ms"]
 
-    # ---- end to end through the C ABI with HOST buffers (spd_run_host) -----------------
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------
     if not args.no_e2e:
-        line["e2e"] = run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev)
+        line["e2e"] = run_e2e(args, spd, w, widths, wb.plane, wb.mean, wb.sigma, world, distributed, dev, wb.thr)
     else:
         line["e2e"] = None
 
-    del plane, out_snr, out_width
-    plan.close()
+    wb.close()
+    del wb
+
+    # ---- the other configs, in the same run (rank 0, N = 1 only) --------------------------
+    if rank == 0 and world == 1 and not args.no_per_config and not args.n_dm and not args.grid and \
+            not args.width_set and not args.width_u8:
+        line["per_config"] = per_config_legs(args, spd, torch, dev, peak, peak_src, uuid, local_rank)
 
     # ---- CPU oracle on the same box (rank 0, N=1 only) ----------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -495,16 +593,45 @@ def run_b200(args):
     return 0
 
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per sample of the dominant kernel from
-# the committed `ncu --set full` capture (taken on 1024 of the workload's DM trials: the kernel
-# streams rows independently, so traffic scales with the sample count); None where not captured.
-# profiles/r01d_tree_ws_kernel_full.md: 4.335046 + 8.536421 GB for 2^30 samples of the config-3 recipe.
-NCU_DRAM_BYTES_PER_SAMPLE = {3: (4.335046e9 + 8.536421e9) / float(1 << 30)}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel come from the committed
+# `ncu --set full` captures listed in profiles/dram_traffic.csv (one row per kernel and workload: samples of the
+# captured launch, bytes read and written, the capture's summary file and commit, and the sha256 of the kernel's
+# source files at capture time).  The kernels stream rows independently, so the per-sample figure of the
+# captured launch scales to this launch.  If the kernel's sources have changed since the capture the figure is
+# stale: traffic is null and traffic_source says which capture is outdated.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+KERNEL_SOURCES = {
+    "tree_ws": ["spd_tree_ws.cu", "spd_tree_common.cuh"],
+    "tree_block": ["spd_tree.cu", "spd_tree_common.cuh"],
+    "tree_ig": ["spd_tree_ig.cu", "spd_tree_common.cuh"],
+}
 
 
-def ncu_traffic_bytes(w):
-    per_sample = NCU_DRAM_BYTES_PER_SAMPLE.get(w.index) if w.width_kind == "POW2" else None
-    return None if per_sample is None else per_sample * w.n_samples
+def kernel_source_hash(key):
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES.get(key, []):
+        with open(os.path.join(ROOT, "paper_1910_08324_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic_bytes(key, w, width_bytes):
+    import csv
+    if key not in KERNEL_SOURCES or not os.path.exists(TRAFFIC_CSV):
+        return None, None
+    with open(TRAFFIC_CSV) as f:
+        rows = [r for r in csv.DictReader(f) if r["kernel"] == key and int(r["workload"]) == w.index and
+                r["width_set"] == f"{w.width_kind}:{w.width_param}" and int(r["width_bytes"]) == width_bytes]
+    if not rows:
+        return None, None
+    r = rows[-1]
+    src = {"measured_in_run": False, "capture": r["capture"], "commit": r["commit"]}
+    if r["source_sha256_16"] != kernel_source_hash(key):
+        src["stale"] = "the kernel's sources have changed since this capture"
+        return None, src
+    per_sample = (float(r["dram_bytes_read"]) + float(r["dram_bytes_write"])) / float(r["samples"])
+    return per_sample * w.n_samples, src
 
 
 def host_mem_available_bytes():
@@ -518,9 +645,11 @@ def host_mem_available_bytes():
     return 8 << 30
 
 
-def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
-    """Same metric through spd_run_host: pinned HOST plane in, HOST SNR / width planes out,
-    every copy inside the timed region (wall clock around the blocking call, max over ranks)."""
+def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev, thr):
+    """Same metric end to end through the C ABI on HOST buffers, every copy inside the timed region (wall clock
+    around the blocking call, max over ranks).  The headline call is spd_run_host_candidates: pinned HOST plane
+    in, rows a1-a8 per row block and the 2-D peak stage (row f4) on the device, the candidate list out - what a
+    pipeline consumes.  `planes` adds spd_run_host, which also ships Y and W back (12 B per sample over the link)."""
     import torch
     # rows: the whole plane when host memory allows 12 B/sample of pinned buffers per rank
     budget = host_mem_available_bytes() // (3 * max(1, world))
@@ -530,32 +659,47 @@ def run_e2e(args, spd, w, widths, plane, mean, sigma, world, distributed, dev):
     h_plane.copy_(plane[:rows])
     h_mean = mean[:rows].cpu()
     h_sigma = sigma[:rows].cpu()
-    h_snr = torch.empty((rows, w.n_t), dtype=torch.float32, pin_memory=True)
-    h_width = torch.empty((rows, w.n_t), dtype=torch.int32, pin_memory=True)
+    cap = 1 << 20
+    h_list = torch.empty(cap * 16, dtype=torch.uint8, pin_memory=True)
     torch.cuda.synchronize()
-    times = []
     seps = None
     if args.grid:
         gkind, _, gparam = args.grid.partition(":")
         seps = spd.spd_separation_generate(gkind, int(gparam or 0), widths)
-    with spd.Plan(rows, w.n_t, widths, w.max_width, separations=seps) as plan:
+
+    def timed_calls(fn):
+        times = []
         for i in range(1 + max(1, args.e2e_steps)):
             if distributed:
                 torch.distributed.barrier()
             torch.cuda.synchronize()
             t = time.perf_counter()
-            plan.run_host(h_plane, h_mean, h_sigma, h_snr, h_width)
+            out = fn()
             dt = time.perf_counter() - t
             if i > 0:
                 times.append(dt)
-    dt = sum(times) / len(times)
-    dt = max_over_ranks(dt, dev)
-    checksum = float(h_snr[0, :1024].double().sum().item())
-    return {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": 4 * n + 8 * rows,
-            "d2h_bytes_per_step": 8 * n, "ms_per_step": 1e3 * dt, "steps": len(times), "rows": rows,
-            "api": "spd_run_host (pinned host buffers; H2D, kernels and D2H of Y and W inside the call)",
-            "note": "whole plane" if rows == w.n_dm else f"first {rows} of {w.n_dm} DM trials (host memory bound)",
-            "checksum": checksum}
+        return max_over_ranks(sum(times) / len(times), dev), len(times), out
+
+    note = "whole plane" if rows == w.n_dm else f"first {rows} of {w.n_dm} DM trials (host memory bound)"
+    with spd.Plan(rows, w.n_t, widths, w.max_width, separations=seps) as plan:
+        dt, k, (n_found, n_1d, cands) = timed_calls(
+            lambda: plan.run_host_candidates(h_plane, h_mean, h_sigma, thr, 1, cap, out_list=h_list))
+        res = {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": 4 * n + 8 * rows,
+               "d2h_bytes_per_step": 16 + 16 * min(n_found, cap), "ms_per_step": 1e3 * dt, "steps": k, "rows": rows,
+               "api": "spd_run_host_candidates (pinned host plane in; H2D, rows a1-a8 and the 2-D peak stage on the "
+                      "device; D2H of the candidate list)",
+               "note": note, "candidates_1d": n_1d, "candidates_2d": n_found,
+               "checksum": float(cands["snr"].astype("float64").sum()) if len(cands) else 0.0}
+    del h_list
+    h_snr = torch.empty((rows, w.n_t), dtype=torch.float32, pin_memory=True)
+    h_width = torch.empty((rows, w.n_t), dtype=torch.int32, pin_memory=True)
+    with spd.Plan(rows, w.n_t, widths, w.max_width, separations=seps) as plan:
+        dt, k, _ = timed_calls(lambda: plan.run_host(h_plane, h_mean, h_sigma, h_snr, h_width))
+        res["planes"] = {"value": world * n / dt, "unit": UNIT, "h2d_bytes_per_step": 4 * n + 8 * rows,
+                         "d2h_bytes_per_step": 8 * n, "ms_per_step": 1e3 * dt, "steps": k,
+                         "api": "spd_run_host (Y and W planes back to pinned host buffers)",
+                         "checksum": float(h_snr[0, :1024].double().sum().item())}
+    return res
 
 
 def apply_overrides(w, args):

@@ -1,10 +1,13 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
 (spd_run_flagged + spd_find_candidates_flagged through the C ABI).
 
-The planes (up to 16 GiB) never leave the device; the oracle is run on sampled windows it can
-compute one by one - around injected pulses, at row starts and row tails, across the kernel's
-chunk and segment boundaries, and at random places - by direct summation (oracle A) and, on
-longer windows, by the double-precision running sum (oracle B).  A window is a piece of one row
+EVERY sample of configs 2-5 is compared with oracle B (the double-precision running sum, SURVEY.md
+sec. 8(c) "Oracle B (accelerated, full planes)"), block-wise: <= 64 Mi samples of rows go to the
+host at a time, the oracle runs on them, and its three outputs go back to the device where the
+comparison rule of parity.py is evaluated with float64 tensor ops (the near-ties it leaves are settled
+on the host by direct summation of the chosen width).  Oracle B itself is pinned at this size by
+oracle A (direct summation) on sampled windows - around injected pulses, at row starts and row
+tails, across the kernel's chunk, segment and piece boundaries, and at random places.  A window is a piece of one row
 copied to the host together with the max_width - 1 samples that follow it, so every boxcar of
 every compared sample lies inside the piece (windows that reach the end of the row exercise the
 valid-windows-only rule instead).  Properties that hold at any size are checked on the whole
@@ -86,6 +89,92 @@ def _check_window(oracle, plane, snr, idx, mean_h, sigma_h, widths, M, row, t0, 
         ref_snr, ref_idx, ref_sec = ref_snr[:, :span], ref_idx[:, :span], ref_sec[:, :span]
     return parity.assert_parity(oracle, seg, mu, sg, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
                                 what=f"{what} row {row} t0 {t0}")
+
+
+def _prefix_oracle_block(oracle, x, mu, sg, widths):
+    """oracle.spd_prefix on a block of whole rows.  The oracle runs one row per thread; a block of fewer rows
+    than threads (config 5: one row of 2^26 samples) is cut into time segments that each carry the
+    max_width - 1 samples that follow them, so that every window of a compared sample lies inside its segment;
+    the last segment of a row keeps the row's real end (valid-windows-only rule)."""
+    r, n_t = x.shape
+    M = int(max(widths))
+    n_seg = max(1, min(oracle.num_threads() * 2 // r, n_t // (8 * M)))
+    if n_seg <= 1:
+        return oracle.spd_prefix(x, mu, sg, widths)
+    span = -(-n_t // n_seg)
+    outs = [np.empty((r, n_t), dtype=np.float64), np.empty((r, n_t), dtype=np.int32),
+            np.empty((r, n_t), dtype=np.float64)]
+    n_full = (n_t - (M - 1)) // span               # segments that have their whole look-ahead inside the row
+    n_full = min(n_full, n_seg - 1)
+    if n_full > 0:
+        seg = np.stack([x[d, s * span: s * span + span + M - 1] for d in range(r) for s in range(n_full)])
+        res = oracle.spd_prefix(seg, np.repeat(mu, n_full), np.repeat(sg, n_full), widths)
+        for o, a in zip(outs, res):
+            o[:, : n_full * span] = a[:, :span].reshape(r, n_full * span)
+    t0 = n_full * span
+    res = oracle.spd_prefix(np.ascontiguousarray(x[:, t0:]), mu, sg, widths)
+    for o, a in zip(outs, res):
+        o[:, t0:] = a
+    return tuple(outs)
+
+
+def _full_plane_parity(oracle, plane, snr, idx, mean_h, sigma_h, widths, what):
+    """parity.assert_parity's rule on every sample of the plane against oracle.spd_prefix, in row blocks."""
+    n_dm, n_t = plane.shape
+    dev = plane.device
+    rows = max(1, min(n_dm, (1 << 26) // n_t))
+    wl = np.asarray(sorted(set(int(v) for v in widths)), dtype=np.int64)
+    worst, n_diff, n_cmp = 0.0, 0, 0
+    ninf = float("-inf")
+    for r0 in range(0, n_dm, rows):
+        r1 = min(n_dm, r0 + rows)
+        x = plane[r0:r1].cpu().numpy()
+        ref_snr, ref_idx, ref_sec = _prefix_oracle_block(oracle, x, mean_h[r0:r1], sigma_h[r0:r1], widths)
+        with np.errstate(invalid="ignore"):
+            gap_h = (ref_snr - ref_sec).astype(np.float32)          # inf where there is no runner-up
+        rs = torch.from_numpy(ref_snr).to(dev)
+        ri = torch.from_numpy(ref_idx).to(dev)
+        gap = torch.from_numpy(gap_h).to(dev)
+        y = snr[r0:r1].double()
+        k = idx[r0:r1].to(torch.int32)
+        nofit = ri < 0
+        if bool(nofit.any()):
+            assert bool((y[nofit] == ninf).all()) and bool((k[nofit] == -1).all()), f"{what}: no-fit samples"
+        ok = ~nofit
+        assert bool(torch.isfinite(y[ok]).all()), f"{what}: non-finite SNR"
+        tol = parity.SNR_RTOL * torch.clamp(torch.where(ok, rs, torch.zeros_like(rs)).abs(), min=1.0)
+        ratio = torch.where(ok, (y - rs).abs() / tol, torch.zeros_like(rs))
+        w_blk = float(ratio.max())
+        if w_blk > 1.0:
+            i = int(torch.argmax(ratio))
+            raise AssertionError(f"{what}: SNR mismatch at row {r0 + i // n_t} sample {i % n_t}: cuda "
+                                 f"{float(y.flatten()[i])!r} oracle {float(rs.flatten()[i])!r} (err/tol {w_blk:.3g})")
+        worst = max(worst, w_blk)
+        assert bool(((k >= 0) & (k < len(wl)))[ok].all()), f"{what}: width index out of range"
+        diff = ok & (k != ri)
+        decisive = diff & (gap.double() > tol)
+        if bool(decisive.any()):
+            i = int(torch.nonzero(decisive.flatten())[0])
+            raise AssertionError(f"{what}: width index mismatch at row {r0 + i // n_t} sample {i % n_t} where the "
+                                 f"oracle's top two differ by more than the tolerance ({int(decisive.sum())} such)")
+        rr, cc = torch.nonzero(diff, as_tuple=True)
+        if rr.numel():
+            rr_h, cc_h = rr.cpu().numpy(), cc.cpu().numpy()
+            kk_h = k[rr, cc].cpu().numpy()
+            tol_h = tol[rr, cc].cpu().numpy()
+            for row in np.unique(rr_h):
+                sel = rr_h == row
+                for kw in np.unique(kk_h[sel]):
+                    m = sel & (kk_h == kw)
+                    s_w = oracle.snr_of_width(x[row], float(mean_h[r0 + row]), float(sigma_h[r0 + row]),
+                                              int(wl[kw]), cc_h[m].astype(np.int64))
+                    bad = ~(np.abs(s_w - ref_snr[row, cc_h[m]]) <= tol_h[m])
+                    assert not bad.any(), (f"{what}: near-tie width {wl[kw]} at row {r0 + row} sample "
+                                           f"{cc_h[m][bad][0]} is not within tolerance of the best")
+            n_diff += int(rr.numel())
+        n_cmp += (r1 - r0) * n_t
+        del rs, ri, gap, y, k, tol, ratio, diff, decisive
+    return worst, n_diff, n_cmp
 
 
 def _whole_plane_properties(plane, mean, sigma, snr, idx, n_widths, rows_per_block=64):
@@ -172,6 +261,13 @@ def test_full_size_config(spd, oracle_lib, cfg, width_kind):
                        direct=False, what=f"config {cfg} long-tail")
     worst, n_cmp = max(worst, st.max_err_over_tol), n_cmp + st.n
     assert worst <= 1.0 and n_cmp > 1 << 19
+
+    # ---- every sample against oracle B --------------------------------------------------------
+    worst_all, n_near, n_all = _full_plane_parity(oracle_lib, plane, snr, idx, mean_h, sigma_h, widths,
+                                                  f"config {cfg} full plane")
+    assert n_all == w.n_dm * w.n_t and worst_all <= 1.0
+    print(f"config {cfg}{' IG(1)' if width_kind else ''}: {n_all} samples compared, max |dSNR|/tol = {worst_all:.3g}, "
+          f"{n_near} near-tie width differences (all valid)")
 
     # ---- properties of the whole plane ------------------------------------------------------
     _whole_plane_properties(plane, mean, sigma, snr, idx, len(widths))
