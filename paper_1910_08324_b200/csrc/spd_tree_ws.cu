@@ -107,22 +107,45 @@ __device__ __forceinline__ float4 grid_mask(float4 q, uint32_t nb, const ChunkCt
     if (m > 1u) q.z = ninf;
     return q;
 }
-template <int j, int K, bool FAST, bool SW, bool GR>
+// One level of a grid plan folded into best.  A level whose separation is 4 or more has at most the FIRST
+// sample of a float4 on its grid: only that key is formed - one multiply, one tag, one select, one max instead
+// of the eight instructions of a full float4 - which is where the paper's grids save their work (PAPER.md:201,
+// 311: "wider pulses ... at every D^(i) point").  Separations do not decrease with the width, so these are the
+// levels k >= KX for some KX, a template parameter of the kernel (the host picks the smallest instantiated
+// value that is not below the plan's); the levels below take the full float4 with the off-grid elements masked,
+// which is right for any separation.
+constexpr int kWsNoGrid = 99;
+template <int k, int KX, bool FAST, bool SW>
+__device__ __forceinline__ void grid_level(float4& best, float4 p, int lim, uint32_t nb, const ChunkCtx& cx) {
+    const uint32_t m = cx.gmask[k];
+    if constexpr (k >= KX) {
+        float v = SW ? p.x * cx.ls[k] : p.x * level_scale<k>();
+        v = pack1<k>(v, cx.tm);
+        const float ninf = __int_as_float(0xff800000);
+        bool off = (nb & m) != 0u;
+        if constexpr (!FAST) off = off || (1 << k) > lim;
+        best.x = fmaxf(best.x, off ? ninf : v);
+    } else {
+        best = max4(best, grid_mask<k>(key_sw<k, FAST, SW>(p, lim, cx), nb, cx));
+    }
+}
+
+template <int j, int K, bool FAST, bool SW, int KX>
 __device__ __forceinline__ void fold_sw(float4& best, float4 before, float4 now, int lim, uint32_t nb,
                                         const ChunkCtx& cx) {
+    constexpr bool GR = KX != kWsNoGrid;
     if constexpr (j >= 3) {
-        if constexpr ((j & 1) == 0) {
-            float4 a = key_sw<j - 1, FAST, SW>(before, lim, cx);
-            float4 b = key_sw<j, FAST, SW>(now, lim, cx);
-            if constexpr (GR) {
-                a = grid_mask<j - 1>(a, nb, cx);
-                b = grid_mask<j>(b, nb, cx);
+        if constexpr (GR) {
+            if constexpr ((j & 1) == 0) {
+                grid_level<j - 1, KX, FAST, SW>(best, before, lim, nb, cx);
+                grid_level<j, KX, FAST, SW>(best, now, lim, nb, cx);
+            } else if constexpr (j == K - 1) {
+                grid_level<j, KX, FAST, SW>(best, now, lim, nb, cx);
             }
-            best = max4(best, a, b);
+        } else if constexpr ((j & 1) == 0) {
+            best = max4(best, key_sw<j - 1, FAST, SW>(before, lim, cx), key_sw<j, FAST, SW>(now, lim, cx));
         } else if constexpr (j == K - 1) {
-            float4 b = key_sw<j, FAST, SW>(now, lim, cx);
-            if constexpr (GR) b = grid_mask<j>(b, nb, cx);
-            best = max4(best, b);
+            best = max4(best, key_sw<j, FAST, SW>(now, lim, cx));
         }
     }
 }
@@ -140,7 +163,7 @@ __device__ __forceinline__ bool wants_out(const ChunkCtx& cx) {
     }
 }
 
-template <int K, int MODE, bool SW, bool GR, int k>
+template <int K, int MODE, bool SW, int KX, int k>
 __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows], float4 (&hs)[4],
                                             float4* __restrict__ xb,
@@ -160,16 +183,16 @@ __device__ __forceinline__ void lane_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], partner[r]);
-            if (wants_out<MODE>(cx)) fold_sw<k + 1, K, (MODE != 0), SW, GR>(best[r], P[r], now, lim[r], nb[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<k + 1, K, (MODE != 0), SW, KX>(best[r], P[r], now, lim[r], nb[r], cx);
             P[r] = now;
         }
-        lane_levels<K, MODE, SW, GR, k + 1>(P, best, lim, nb, hs, xb, lane, cx);
+        lane_levels<K, MODE, SW, KX, k + 1>(P, best, lim, nb, hs, xb, lane, cx);
     }
 }
 
 // Row levels j < JN: partner 2^j rows later, in this step or among the first rows of the
 // previous step (nr[2^j - 1 .. 2^(j+1) - 2]).
-template <int K, int MODE, bool SW, bool GR, int j>
+template <int K, int MODE, bool SW, int KX, int j>
 __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows],
                                             float4 (&nr)[WsGeo<K>::NEAR + 1], const ChunkCtx& cx) {
@@ -185,15 +208,15 @@ __device__ __forceinline__ void near_levels(float4 (&P)[kWsRows], float4 (&best)
         for (int i = 0; i < D; ++i) nr[off + i] = P[i];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, GR>(best[r], P[r], now[r], lim[r], nb[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, KX>(best[r], P[r], now[r], lim[r], nb[r], cx);
             P[r] = now[r];
         }
-        near_levels<K, MODE, SW, GR, j + 1>(P, best, lim, nb, nr, cx);
+        near_levels<K, MODE, SW, KX, j + 1>(P, best, lim, nb, nr, cx);
     }
 }
 
 // FIFO levels i < JF: partner 2^i steps back, same lane, same row: tensor memory.
-template <int K, int MODE, bool SW, bool GR, int i>
+template <int K, int MODE, bool SW, int KX, int i>
 __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)[kWsRows],
                                             const int (&lim)[kWsRows], const uint32_t (&nb)[kWsRows], uint32_t tbase,
                                             int it, const ChunkCtx& cx) {
@@ -209,21 +232,21 @@ __device__ __forceinline__ void fifo_levels(float4 (&P)[kWsRows], float4 (&best)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 now = add4(P[r], old[r]);
-            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, GR>(best[r], P[r], now, lim[r], nb[r], cx);
+            if (wants_out<MODE>(cx)) fold_sw<lvl, K, (MODE != 0), SW, KX>(best[r], P[r], now, lim[r], nb[r], cx);
             P[r] = now;
         }
-        fifo_levels<K, MODE, SW, GR, i + 1>(P, best, lim, nb, tbase, it, cx);
+        fifo_levels<K, MODE, SW, KX, i + 1>(P, best, lim, nb, tbase, it, cx);
     }
 }
 
 // One step of one warp: the kWsStage floats at st4 -> Y, W of its kWsStep samples.
-template <int K, int MODE, bool SW, bool GR, bool U8>
+template <int K, int MODE, bool SW, int KX, bool U8>
 __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 (&hs)[4],
                                          float4 (&nr)[WsGeo<K>::NEAR + 1], float4* __restrict__ xb, uint32_t tbase,
                                          int it, int lane, const ChunkCtx& cx) {
     constexpr int R = kWsRows;
+    constexpr bool GR = KX != kWsNoGrid;
     const float mu = cx.mu;
-    const uint32_t tm = cx.tm;
     float4 P[R], best[R];
     int lim[R];
     uint32_t nb[R];  // index of each float4's first sample (low 32 bits; grid plans only)
@@ -255,21 +278,21 @@ __device__ __forceinline__ float ws_step(const float4* __restrict__ st4, float4 
         const float4 p3 = make_float4(p3lo.x, p3lo.y, p3hi.x, p3hi.y);
         if (wants_out<MODE>(cx)) {
             constexpr bool F = MODE != 0;
-            float4 k0 = key_sw<0, F, SW>(a, lim[r], cx), k1 = key_sw<1, F, SW>(p1, lim[r], cx),
-                   k2 = key_sw<2, F, SW>(p2, lim[r], cx);
             if constexpr (GR) {
-                k0 = grid_mask<0>(k0, nb[r], cx);
-                k1 = grid_mask<1>(k1, nb[r], cx);
-                k2 = grid_mask<2>(k2, nb[r], cx);
+                best[r] = grid_mask<0>(key_sw<0, F, SW>(a, lim[r], cx), nb[r], cx);
+                grid_level<1, KX, F, SW>(best[r], p1, lim[r], nb[r], cx);
+                grid_level<2, KX, F, SW>(best[r], p2, lim[r], nb[r], cx);
+            } else {
+                best[r] = max4(key_sw<0, F, SW>(a, lim[r], cx), key_sw<1, F, SW>(p1, lim[r], cx),
+                               key_sw<2, F, SW>(p2, lim[r], cx));
             }
-            best[r] = max4(k0, k1, k2);
-            fold_sw<3, K, F, SW, GR>(best[r], p2, p3, lim[r], nb[r], cx);
+            fold_sw<3, K, F, SW, KX>(best[r], p2, p3, lim[r], nb[r], cx);
         }
         P[r] = p3;
     }
-    lane_levels<K, MODE, SW, GR, 3>(P, best, lim, nb, hs, xb, lane, cx);
-    near_levels<K, MODE, SW, GR, 0>(P, best, lim, nb, nr, cx);
-    fifo_levels<K, MODE, SW, GR, 0>(P, best, lim, nb, tbase, it, cx);
+    lane_levels<K, MODE, SW, KX, 3>(P, best, lim, nb, hs, xb, lane, cx);
+    near_levels<K, MODE, SW, KX, 0>(P, best, lim, nb, nr, cx);
+    fifo_levels<K, MODE, SW, KX, 0>(P, best, lim, nb, tbase, it, cx);
     if constexpr (WsGeo<K>::JF > 0) tmem_wait_st();
 
     float top = __int_as_float(0xff800000);
@@ -315,9 +338,10 @@ constexpr size_t kWsStagesBytes = static_cast<size_t>(kWsWarps) * kWsStages * kW
 constexpr size_t kWsXBytes = static_cast<size_t>(kWsWarps) * 2 * kWsXBuf * 16;
 constexpr size_t ws_smem_bytes() { return kWsStagesBytes + kWsXBytes + kWsWarps * kWsStages * 8 + 16; }
 
-template <int K, bool SW, bool GR, bool U8>
+template <int K, bool SW, int KX, bool U8>
 __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const TreeParams p, const int n_pieces) {
     using G = WsGeo<K>;
+    constexpr bool GR = KX != kWsNoGrid;
     constexpr int S = kWsStep;
     constexpr int M = 1 << (K - 1);
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -440,7 +464,7 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
             __syncwarp();
             cx.n0 = n0;
             cx.do_out = c < c_hi;
-            const float top = ws_step<K, 0, SW, GR, U8>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
+            const float top = ws_step<K, 0, SW, KX, U8>(reinterpret_cast<const float4*>(gbuf), hs, nr, xb, tbase, it, lane, cx);
             if (act && cx.do_out && top >= thr_key) act[c / kWsActSteps] = 1;
             __syncwarp();
         }
@@ -487,19 +511,19 @@ __global__ void __launch_bounds__(32 * kWsWarps, 1) spd_tree_ws_kernel(const Tre
         for (; f < n_warm; ++f, ++it) {
             ring_next(f);
             cx.n0 = static_cast<long long>(ring_top - 1 - f) * S;
-            ws_step<K, 2, SW, GR, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
+            ws_step<K, 2, SW, KX, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb, tbase, it, lane, cx);
             ring_done();
         }
         // Two steps per loop trip: the values kept from one step to the next (hs, nr: 11 float4)
         // alternate between two register sets instead of being moved, and the first levels of a
         // step overlap the last levels of the one before (10.70 -> 10.26 ms on config 3; x3: see DESIGN).
-        constexpr int kTrip = GR ? 1 : kWsUnroll;  // the grid body is larger: one step per trip
+        constexpr int kTrip = (GR && KX > 6) ? 1 : kWsUnroll;  // the all-masked grid body is larger: one step per trip
 #pragma unroll kTrip
         for (; f < n_ring; ++f, ++it) {
             ring_next(f);
             const int c = ring_top - 1 - f;
             cx.n0 = static_cast<long long>(c) * S;
-            const float top = ws_step<K, 1, SW, GR, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
+            const float top = ws_step<K, 1, SW, KX, U8>(reinterpret_cast<const float4*>(stages + stage * kWsStage), hs, nr, xb,
                                             tbase, it, lane, cx);
             if (act && top >= thr_key) act[c / kWsActSteps] = 1;
             ring_done();
@@ -524,16 +548,21 @@ bool ws_applicable(int K, uint32_t flags) {
     return K >= kWsMinK && K <= kWsMaxK && !(flags & SPD_FLAG_BLOCK_TREE);
 }
 
+// Instantiated values of KX for grid plans: the first level whose keys are formed for the first sample of a
+// float4 only (separation >= 4).  2: Alg. 3's DIT (width 2^k every 2^k-th sample); 4, 6: widths on four and
+// sixteen layers; kWsNoGrid - 1: every level masked (any separations).
+constexpr int kWsGridKx[4] = {2, 4, 6, kWsNoGrid - 1};
+
 template <int K>
 static cudaError_t ws_prepare(int smem) {
-    cudaError_t e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, false, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    cudaError_t e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsNoGrid, false>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, true, kWsNoGrid, false>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsNoGrid, true>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsGridKx[0], false>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsGridKx[1], false>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsGridKx[2], false>, attr, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(spd_tree_ws_kernel<K, false, kWsGridKx[3], false>, attr, smem);
     return e;
 }
 
@@ -650,17 +679,30 @@ int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     }
     const int np = static_cast<int>(n_pieces);
     const size_t sm = cfg.smem_bytes;
-#define SPD_LAUNCH(KK)                                                                              \
-    if (cfg.K == KK) {                                                                              \
-        if (sigma_w)                                                                                \
-            spd_tree_ws_kernel<KK, true, false, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
-        else if (!plan->separations.empty())                                                        \
-            spd_tree_ws_kernel<KK, false, true, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
-        else if (u8)                                                                                \
-            spd_tree_ws_kernel<KK, false, false, true><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
-        else                                                                                        \
-            spd_tree_ws_kernel<KK, false, false, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np); \
-        e = cudaGetLastError();                                                                     \
+    // grid plans: the first level with a separation of 4 or more, rounded up to an instantiated value
+    int kx_sel = 2;
+    if (!plan->separations.empty()) {
+        int kx = cfg.K;
+        for (int k = cfg.K - 1; k >= 0 && plan->separations[k] >= 4; --k) kx = k;
+        kx_sel = kx <= kWsGridKx[0] ? 0 : (kx <= kWsGridKx[1] ? 1 : (kx <= kWsGridKx[2] ? 2 : 3));
+    }
+#define SPD_LAUNCH(KK)                                                                                          \
+    if (cfg.K == KK) {                                                                                          \
+        if (sigma_w)                                                                                            \
+            spd_tree_ws_kernel<KK, true, kWsNoGrid, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);       \
+        else if (!plan->separations.empty() && kx_sel == 0)                                                     \
+            spd_tree_ws_kernel<KK, false, kWsGridKx[0], false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);   \
+        else if (!plan->separations.empty() && kx_sel == 1)                                                     \
+            spd_tree_ws_kernel<KK, false, kWsGridKx[1], false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);   \
+        else if (!plan->separations.empty() && kx_sel == 2)                                                     \
+            spd_tree_ws_kernel<KK, false, kWsGridKx[2], false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);   \
+        else if (!plan->separations.empty())                                                                    \
+            spd_tree_ws_kernel<KK, false, kWsGridKx[3], false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);   \
+        else if (u8)                                                                                            \
+            spd_tree_ws_kernel<KK, false, kWsNoGrid, true><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);       \
+        else                                                                                                    \
+            spd_tree_ws_kernel<KK, false, kWsNoGrid, false><<<grid, 32 * kWsWarps, sm, stream>>>(prm, np);      \
+        e = cudaGetLastError();                                                                                 \
     }
     SPD_WS_CASES(SPD_LAUNCH)
 #undef SPD_LAUNCH
