@@ -297,6 +297,7 @@ def measured_peak():
 # the B200 arm
 # ----------------------------------------------------------------------------------------
 KERNEL_NAMES = {"tree_ws": "spd_tree_ws_kernel", "tree_block": "spd_tree_kernel", "tree_ig": "spd_tree_ig_kernel",
+                "tree_ws_ig": "spd_tree_ws_kernel (IGRID depth-1 widths)",
                 "grid_ws": "spd_tree_ws_kernel (grid)", "grid_tile": "grid_tile_kernel", "generic": "generic_tile_kernel"}
 
 
@@ -304,7 +305,7 @@ def kernel_key(spd, info):
     if info["path"] == spd.SPD_PATH_DYADIC_TREE:
         return "tree_ws" if info["tree_kernel"] == 2 else "tree_block"
     if info["path"] == spd.SPD_PATH_IGRID_TREE:
-        return "tree_ig"
+        return "tree_ws_ig" if info["tree_kernel"] == 2 else "tree_ig"
     if info["path"] == spd.SPD_PATH_GRID:
         return "grid_ws" if info["tree_kernel"] == 2 else "grid_tile"
     return "generic"
@@ -601,7 +602,8 @@ def run_b200(args):
 # stale: traffic is null and traffic_source says which capture is outdated.
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
 KERNEL_SOURCES = {
-    "tree_ws": ["spd_tree_ws.cu", "spd_tree_common.cuh"],
+    "tree_ws": ["spd_tree_ws.cuh", "spd_tree_common.cuh"],
+    "tree_ws_ig": ["spd_tree_ws.cuh", "spd_tree_common.cuh"],
     "tree_block": ["spd_tree.cu", "spd_tree_common.cuh"],
     "tree_ig": ["spd_tree_ig.cu", "spd_tree_common.cuh"],
 }

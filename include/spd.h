@@ -128,8 +128,8 @@ typedef struct spd_plan_info {
     int64_t activity_bytes;     /* size of the activity map of spd_run_flagged (multiple of 128) */
     int32_t activity_block;     /* time samples of one row covered by one byte of that map */
     int32_t activity_per_row;   /* bytes of that map per DM row */
-    int32_t tree_kernel;        /* dyadic tree: 1 = one block per stream, 2 = one warp per stream (tensor-memory
-                                   delay lines, widths 2^k with 8 <= K <= 14); else 0 */
+    int32_t tree_kernel;        /* streaming trees: 1 = one block per stream, 2 = one warp per stream (tensor-memory
+                                   delay lines; max_width 256 .. 8192); grid plans that run on the latter: 2; else 0 */
     int32_t piece_chunks;       /* warp-per-stream kernel: steps per piece when the plane's steps are cut, in
                                    row-major order, into one piece per resident warp (pieces may span rows;
                                    segments_per_row is then 0); else 0 */
@@ -188,8 +188,10 @@ int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, 
  * plane: out_snr[d,n] = max over the widths whose grid contains n (and whose window fits,
  * reading A3), out_width the index of that width; -inf / -1 where no width's grid contains n
  * (only if separations[0] > 1).  Limits: max_width <= 45057, n_widths <= 1024.  A set {1, 2, 4, ..., 2^(K-1)}
- * with 9 <= K <= 14 runs on the warp-per-stream tree kernel (spd_plan_info.tree_kernel == 2), other sets on a
- * shared-memory tile kernel.
+ * with 9 <= K <= 14, and the IGRID depth-1 set {2^k} U {3 * 2^m} over the same range when the two widths of an
+ * octave share a separation (SPD_GRID_IGRID), run on the warp-per-stream tree kernel
+ * (spd_plan_info.tree_kernel == 2), where the keys of a level are formed on its grid points only; other sets
+ * run on a shared-memory tile kernel.
  * spd_plan_info.path is SPD_PATH_GRID.  Errors as spd_plan_create plus the conditions above.
  */
 int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t,
@@ -310,7 +312,9 @@ int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean,
  * spd_run_sigma_w - spd_run with SNR_L = (X_L - L mean) / sigma_w[d][L's index] (eq. 4, PAPER.md:69,
  * with the measured sigma(X_L) of spd_width_sigma in place of eq. 5's sqrt(L) sigma).
  * For every plan except SPD_PATH_GENERIC plans on the device-workspace kernels (max_width above about 45 000, or
- * SPD_FLAG_GENERIC_WORKSPACE) and SPD_FLAG_WIDTH_U8 plans, which return SPD_ERR_INVALID_ARG.  Other arguments
+ * SPD_FLAG_GENERIC_WORKSPACE), SPD_PATH_IGRID_TREE plans on the block-per-stream kernel (max_width below 256 or
+ * above 8192: create those with SPD_FLAG_FORCE_GENERIC) and SPD_FLAG_WIDTH_U8 plans, which return
+ * SPD_ERR_INVALID_ARG.  Other arguments
  * (alignment included) as spd_run.
  */
 int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,

@@ -179,6 +179,8 @@ int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const flo
              float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream) {
     if (plan->path == SPD_PATH_DYADIC_TREE)
         return tree_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (plan->path == SPD_PATH_IGRID_TREE && plan->tree.kind == 1)
+        return ws_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
     if (plan->path == SPD_PATH_IGRID_TREE)
         return ig_run(plan, n_rows, plane, mean, sigma, out_snr, static_cast<int32_t*>(out_width), threshold, activity,
                       stream);
@@ -398,9 +400,20 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
         rc = generic_configure(plan);
         // widths {2^k} on a grid: the warp-per-stream tree kernel with the keys of a level counted only on
         // that level's grid (the any-width-set grid kernel stays configured for spd_run_sigma_w)
+        int igl = 0;
         if (rc == SPD_OK && tree_applicable(w, n_t) && ws_applicable(static_cast<int>(w.size()), 0u)) {
             plan->tree.K = static_cast<int>(w.size());
             rc = ws_configure(plan);
+        } else if (rc == SPD_OK && (igl = ig_applicable(w, n_t)) > 0 && ws_applicable(igl, 0u)) {
+            // the IGRID depth-1 widths on a grid whose octaves share a separation (the widths of
+            // step 2^i on P layers): width 3 * 2^m goes with width 2^(m+1)
+            bool shared = true;
+            for (int m = 0; m + 2 < igl; ++m) shared = shared && seps[2 * m + 2] == seps[2 * (m + 1) - 1];
+            if (shared) {
+                plan->tree.K = igl;
+                plan->tree.ig = true;
+                rc = ws_configure(plan);
+            }
         }
     } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t)) {
         plan->path = SPD_PATH_DYADIC_TREE;
@@ -408,7 +421,12 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     } else if (!(flags & SPD_FLAG_FORCE_GENERIC) && (ig_levels = ig_applicable(w, n_t)) > 0) {
         plan->path = SPD_PATH_IGRID_TREE;
         plan->tree.K = ig_levels;
-        rc = ig_configure(plan);
+        if (ws_applicable(ig_levels, flags)) {
+            plan->tree.ig = true;
+            rc = ws_configure(plan);
+        } else {
+            rc = ig_configure(plan);
+        }
     } else {
         plan->path = SPD_PATH_GENERIC;
         rc = generic_configure(plan);
@@ -503,7 +521,7 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         info->chunk = plan->tree.chunk;
         info->segments_per_row = plan->tree.segs_per_row;
         info->smem_bytes = static_cast<int64_t>(plan->tree.smem_bytes);
-        if (plan->path == SPD_PATH_DYADIC_TREE) info->tree_kernel = plan->tree.kind == 1 ? 2 : 1;
+        if (is_tree_path(plan)) info->tree_kernel = plan->tree.kind == 1 ? 2 : 1;
         if (plan->tree.kind == 1 && plan->tree.segs_per_row == 0) info->piece_chunks = ws_piece_chunks(plan);
     } else {
         if (plan->generic_tile > 0) {
@@ -565,6 +583,8 @@ int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean,
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (plan->path == SPD_PATH_DYADIC_TREE)  // run-time scale 1 / sigma_{d, 2^k} per level
         return tree_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width, 0.0f, nullptr, stream, sigma_w);
+    if (plan->path == SPD_PATH_IGRID_TREE && plan->tree.kind == 1)
+        return ws_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, out_width, 0.0f, nullptr, stream, sigma_w);
     if (plan->path == SPD_PATH_IGRID_TREE)
         return ig_run(plan, plan->n_dm, plane, mean, nullptr, out_snr, static_cast<int32_t*>(out_width), 0.0f, nullptr,
                       stream, sigma_w);

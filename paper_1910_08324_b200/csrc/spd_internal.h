@@ -19,7 +19,8 @@ constexpr int kStages = 3;          // bulk-copy ring depth
 
 struct TreeConfig {
     int K = 0;            // number of widths: 2^0 .. 2^(K-1)
-    int kind = 0;         // 0: block per stream (spd_tree.cu), 1: warp per stream (spd_tree_ws.cu)
+    int kind = 0;         // 0: block per stream (spd_tree.cu), 1: warp per stream (spd_tree_ws.cuh)
+    bool ig = false;      // warp per stream: the IGRID depth-1 width set (2^k and 3 * 2^m) over the K levels
     int T = 0;            // threads per block
     int chunk = 0;        // 4 * T * R samples
     int act_block = 0;    // samples per activity-map byte (0: = chunk)
@@ -126,6 +127,12 @@ int ws_piece_chunks(const spd_plan* plan);
 int ws_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
            float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
            const float* sigma_w = nullptr);
+
+// spd_tree_ws_ig.cu: the warp-per-stream kernel for widths 2^k and 3 * 2^m (IGRID depth 1); plan->tree.K, .ig set
+int ws_ig_configure(spd_plan* plan);
+int ws_ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+              float* out_snr, void* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
+              const float* sigma_w);
 
 // spd_tree_ig.cu: widths 2^k and 3 * 2^m (IGRID depth 1)
 int ig_applicable(const std::vector<int32_t>& widths, int64_t n_t);  // K (pow-2 levels) or 0

@@ -297,7 +297,7 @@ __device__ __forceinline__ float4 keyx_rt(float4 p, int lim, uint32_t tm, float 
 }
 template <int j, int K, bool FAST>
 __device__ __forceinline__ void fold_rt(float4& best, float4 before, float4 now, int lim, uint32_t tm,
-                                        const float (&ls)[16]) {
+                                        const float (&ls)[32]) {
     if constexpr (j >= 3) {
         if constexpr ((j & 1) == 0) {
             best = max4(best, keyx_rt<j - 1, FAST>(before, lim, tm, ls[j - 1]), keyx_rt<j, FAST>(now, lim, tm, ls[j]));
@@ -355,7 +355,7 @@ struct ChunkCtx {
     bool do_out;
     int tid;
     uint32_t gmask[16];  // boxcar separation per level minus one (kernels instantiated for a grid plan)
-    float ls[16];    // run-time scale per level (kernels instantiated for a sigma per width)
+    float ls[32];    // run-time scale per width index (kernels instantiated for a sigma per width)
     uint32_t tbase;  // tensor-memory base of this thread's delay FIFOs (kernels that keep them there)
     int it;          // steps done on this stream (FIFO slot = it mod depth)
 };

@@ -847,6 +847,91 @@ def test_warp_stream_kernel_pieces_span_rows(spd, oracle_lib, K):
                          ref_sec, what=f"warp-stream K={K}")
 
 
+@pytest.mark.parametrize("K", [9, 12, 14])
+def test_igrid_block_and_warp_kernels_agree_and_take_a_sigma_table(spd, oracle_lib, K):
+    """The IGRID depth-1 widths run on the warp-per-stream kernel for 9 <= K <= 14 levels (tree_kernel 2) and on
+    the block-per-stream kernel with SPD_FLAG_BLOCK_TREE (tree_kernel 1): both pass parity on the same plane.
+    spd_run_sigma_w on the former (PAPER.md:728 for the paper's IG(1) set) against direct summation with the
+    same table on every sample; the table sqrt(L) sigma reproduces spd_run."""
+    M = 1 << (K - 1)
+    rng = np.random.default_rng(300 + K)
+    n_dm, n_t = 3, max(512 * 17 + 12, 2 * M + 600)
+    x = rng.standard_normal((n_dm, n_t))
+    x[1] = np.convolve(x[1], np.ones(5) / 2.0, mode="same")
+    S = max(1, 3 * M // 8)
+    x[2, n_t // 3: n_t // 3 + S] += 11.0 / np.sqrt(S)
+    x = (x + np.array([0.0, 2.0, -1.0])[:, None]).astype(np.float32)
+    widths = spd.spd_width_set_generate("IGRID", 1, M)
+    a_snr, a_idx, a_info = run_gpu(spd, x, 0.0, 1.0, widths)
+    b_snr, b_idx, b_info = run_gpu(spd, x, 0.0, 1.0, widths, flags=spd.SPD_FLAG_BLOCK_TREE)
+    assert a_info["path"] == b_info["path"] == spd.SPD_PATH_IGRID_TREE
+    assert a_info["tree_kernel"] == 2 and b_info["tree_kernel"] == 1
+    ref = oracle_lib.spd_prefix(x, 0.0, 1.0, widths)
+    for snr, idx, name in ((a_snr, a_idx, "warp"), (b_snr, b_idx, "block")):
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, snr, idx, *ref, what=f"igrid {name} K={K}")
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, M) as plan:
+        mean, sigma = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        white = (sigma[:, None] * torch.sqrt(torch.tensor(widths, dtype=torch.float32, device=dev))[None, :]).contiguous()
+        snr_w, idx_w = plan.run_sigma_w(plane, mean, white)
+        snr_0, idx_0 = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    if K <= 12:   # direct summation of every sample: seconds
+        ref_sw = oracle_lib.spd_direct_sw(x, mu64, sw64, widths)
+        parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, None, snr.cpu().numpy(), idx.cpu().numpy(),
+                                   *ref_sw, what=f"igrid sigma_w K={K}")
+    else:
+        for t0, t1 in [(n_t // 3 - 400, n_t // 3 + 400), (n_t - 600, n_t), (0, 400)]:
+            r = oracle_lib.spd_direct_sw(x, mu64, sw64, widths, t0, t1)
+            tol = parity.snr_tolerance(r[0])
+            fit = r[1] >= 0
+            assert np.all(np.abs(snr.cpu().numpy()[:, t0:t1] - r[0])[fit] <= tol[fit])
+            dec = fit & ((r[0] - r[2]) > tol)
+            assert np.array_equal(idx.cpu().numpy()[:, t0:t1][dec], r[1][dec])
+    a, b = snr_w.cpu().numpy(), snr_0.cpu().numpy()
+    assert np.all(np.abs(a - b) <= 1e-5 * np.maximum(1.0, np.abs(b)))
+    assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
+
+
+@pytest.mark.parametrize("K,layers", [(9, 4), (12, 4), (14, 4), (13, 16), (11, 1)])
+def test_igrid_widths_on_layer_grids_run_on_the_tree_kernel(spd, oracle_lib, K, layers):
+    """The paper's IG(1) grids (widths 2^k and 3 * 2^m with the widths of step 2^i on P layers):
+    the warp-per-stream kernel forms a level's keys on its grid points only; every sample against
+    oracle_spd_grid (direct summation on the grid), pieces stopping inside rows, a ragged tail."""
+    M = 1 << (K - 1)
+    widths = spd.spd_width_set_generate("IGRID", 1, M)
+    seps = spd.spd_separation_generate("IGRID", layers, widths)
+    rng = np.random.default_rng(700 + K)
+    n_dm, n_t = 3, max(512 * 9 + 20, 2 * M + 1100)
+    x = rng.standard_normal((n_dm, n_t)).astype(np.float32)
+    S = max(1, 3 * M // 8)
+    x[1, (n_t // 3) // 64 * 64: (n_t // 3) // 64 * 64 + S] += np.float32(12.0 / np.sqrt(S))
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(n_dm, device=dev), torch.ones(n_dm, device=dev)
+    with spd.Plan(n_dm, n_t, widths, M, separations=seps) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GRID and plan.info["tree_kernel"] == 2
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, 6.0)
+        lst, n_f = plan.find_candidates_flagged(snr, idx, act, 6.0, 1 << 16)
+        count, got = spd.candidates_to_numpy(lst, n_f, 1 << 16)
+        got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+    if K <= 12:
+        ref = oracle_lib.spd_grid(x, 0.0, 1.0, widths, seps)
+        parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, got_snr, got_idx, *ref, what=f"igrid grid K={K} P={layers}")
+    else:
+        for t0, t1 in [(n_t // 3 - 600, n_t // 3 + 600), (n_t - 700, n_t), (0, 500), (n_t // 2, n_t // 2 + 512)]:
+            ref = oracle_lib.spd_grid(x, 0.0, 1.0, widths, seps, t0, t1)
+            parity.assert_parity(oracle_lib, x, 0.0, 1.0, widths, got_snr[:, t0:t1], got_idx[:, t0:t1], *ref, t0=t0,
+                                 what=f"igrid grid K={K} P={layers} [{t0}, {t1})")
+    ref_count, c_dm, c_t, _, _ = oracle_lib.find_candidates(got_snr, got_idx, 6.0)
+    assert count == ref_count and count > 0 and np.array_equal(got["dm"], c_dm) and np.array_equal(got["t"], c_t)
+
+
 @pytest.mark.parametrize("K", [9, 14])
 def test_block_and_warp_kernels_agree(spd, oracle_lib, K):
     """SPD_FLAG_BLOCK_TREE keeps the block-per-stream kernel: both kernels pass parity on the same plane, and
