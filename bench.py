@@ -52,6 +52,8 @@ def parse_args():
                     "configs and the IG(1) width set, measured in the same run at N = 1)")
     ap.add_argument("--per-config-steps", type=int, default=5)
     ap.add_argument("--width-u8", action="store_true", help="uint8 width index (SPD_FLAG_WIDTH_U8): 9 B per sample")
+    ap.add_argument("--no-aux", action="store_true", help="skip the timings outside the step (row statistics, sigma "
+                    "per width, 2-D peak stage): a short launch list for profiling")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -284,6 +286,14 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def measured_sm_mhz():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["sm_max_mhz"])
+    except (OSError, KeyError, ValueError):
+        return 1965.0
+
+
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -406,7 +416,20 @@ class Workbench:
         k_ms = sum(rec["run_ms"]) / len(rec["run_ms"])
         achieved = self.bytes_per_sample * self.n / (k_ms * 1e-3) / 1e9
         key = kernel_key(self.spd, self.info)
-        traffic, traffic_src = ncu_traffic_bytes(key, self.w, self.info["width_bytes"])
+        traffic, traffic_src, lane_ops = ncu_traffic_bytes(key, self.w, self.info["width_bytes"])
+        alu = None
+        if lane_ops:
+            # FP32 and integer lanes are one pool of 128 lane-operations per clock and SM on B200 (measured:
+            # profiles/r02_lane_rates.md); lane-operations per sample from the committed ncu source page
+            sms = self.torch.cuda.get_device_properties(self.dev).multi_processor_count
+            clk_mhz = (rec.get("clocks") or {}).get("sm_mhz") or measured_sm_mhz()
+            peak_ops = sms * 128 * clk_mhz * 1e6
+            ach_ops = lane_ops * self.n / (k_ms * 1e-3)
+            alu = {"bound": "alu", "what": "FP32 + integer lane-operations (packed FADD2 / FMUL2 count two)",
+                   "lane_ops_per_sample": lane_ops, "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12,
+                   "unit": "T lane-op/s", "frac": ach_ops / peak_ops,
+                   "peak_source": f"{sms} SMs x 128 lanes x {clk_mhz:.0f} MHz (profiles/r02_lane_rates.md)",
+                   "source": traffic_src}
         return {
             "bound": "hbm", "kernel": KERNEL_NAMES[key], "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
@@ -414,6 +437,7 @@ class Workbench:
             "kernel_ms": k_ms, "kernel_ms_min": min(rec["run_ms"]),
             "candidates_ms": sum(rec["cand_ms"]) / len(rec["cand_ms"]),
             "kernel_share_of_step": sum(rec["run_ms"]) / (sum(rec["run_ms"]) + sum(rec["cand_ms"])),
+            "co_bound": alu,
         }
 
     def close(self):
@@ -482,21 +506,24 @@ def run_b200(args):
     plan, info, widths, n = wb.plan, wb.info, wb.widths, wb.n
 
     # The step before the hot path: timed on its own, outside the step.
-    s_mean, s_sigma = torch.empty_like(wb.mean), torch.empty_like(wb.sigma)
-    stats_ms = wb.timed(lambda: plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma))
-    n_pass = torch.empty(w.n_dm, dtype=torch.int32, device=dev)
-    conv_ms = wb.timed(lambda: plan.row_stats_converge(wb.plane, 2.0, 32, 1e-4, s_mean, s_sigma, n_pass))
-    conv_passes = float(n_pass.float().mean().item())
-    plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma)
-    # sigma per width from power-of-two decimations (row f1): one more read of the plane
-    sw = plan.width_sigma(wb.plane, s_mean)
-    wsig_ms = wb.timed(lambda: plan.width_sigma(wb.plane, s_mean, sw))
-    # the same pass with the measured sigma per width in place of eq. (5) (where the plan's kernels take it)
-    try:
-        run_sw_ms = wb.timed(lambda: plan.run_sigma_w(wb.plane, s_mean, sw, wb.out_snr, wb.out_width))
-    except spd.SpdError:
-        run_sw_ms = None
-    del sw
+    stats_ms = conv_ms = conv_passes = wsig_ms = run_sw_ms = None
+    if not args.no_aux:
+        s_mean, s_sigma = torch.empty_like(wb.mean), torch.empty_like(wb.sigma)
+        stats_ms = wb.timed(lambda: plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma))
+        n_pass = torch.empty(w.n_dm, dtype=torch.int32, device=dev)
+        conv_ms = wb.timed(lambda: plan.row_stats_converge(wb.plane, 2.0, 32, 1e-4, s_mean, s_sigma, n_pass))
+        conv_passes = float(n_pass.float().mean().item())
+        plan.row_stats(wb.plane, 2.0, 2, s_mean, s_sigma)
+        # sigma per width from power-of-two decimations (row f1): one more read of the plane
+        sw = plan.width_sigma(wb.plane, s_mean)
+        wsig_ms = wb.timed(lambda: plan.width_sigma(wb.plane, s_mean, sw))
+        # the same pass with the measured sigma per width in place of eq. (5) (where the plan's kernels take it)
+        if not args.width_u8:
+            try:
+                run_sw_ms = wb.timed(lambda: plan.run_sigma_w(wb.plane, s_mean, sw, wb.out_snr, wb.out_width))
+            except spd.SpdError:
+                run_sw_ms = None
+        del sw
 
     def barrier():
         if distributed:
@@ -520,6 +547,8 @@ def run_b200(args):
     # ---- row f4: the 2-D (DM x time) peak stage over the step's 1-D list (reading A18) -----
     cluster = None
     try:
+        if args.no_aux:
+            raise spd.SpdError(0, "skipped (--no-aux)")
         lst2 = torch.empty(wb.cap * 16, dtype=torch.uint8, device=dev)
         n2 = torch.zeros(1, dtype=torch.int64, device=dev)
         c_ms = wb.timed(lambda: plan.cluster_candidates(wb.out_snr, wb.cand_list, wb.cand_count, wb.cap, 1, wb.cap,
@@ -551,12 +580,14 @@ def run_b200(args):
         "real_time_factor_plane": (w.n_t * w.sampling_time_s) / (ms_per_step * 1e-3),
         "real_time_factor_ska_like": value / PAPER_SKA_SAMPLES_PER_S,
         "n_dm_real_time": value * w.sampling_time_s,
-        "row_stats": {"what": "spd_row_stats, 3 passes (plain + 2 rejection passes at 2 sigma), not part of the step",
+        "row_stats": None if stats_ms is None else {
+                      "what": "spd_row_stats, 3 passes (plain + 2 rejection passes at 2 sigma), not part of the step",
                       "ms": stats_ms, "gbs": 3 * 4 * n / (stats_ms * 1e-3) / 1e9, "bytes_per_sample_per_pass": 4,
                       "until_convergence": {"what": "spd_row_stats_converge, clip 2 sigma, rel_tol 1e-4, limit 32 passes "
                                                     "(converged rows are skipped by later passes)",
                                             "ms": conv_ms, "mean_rejection_passes": conv_passes}},
-        "width_sigma": {"what": "spd_width_sigma: sigma per width from power-of-two decimations, interpolated; "
+        "width_sigma": None if wsig_ms is None else {
+                        "what": "spd_width_sigma: sigma per width from power-of-two decimations, interpolated; "
                                 "one pass, not part of the step",
                         "ms": wsig_ms, "gbs": 4 * n / (wsig_ms * 1e-3) / 1e9, "bytes_per_sample": 4,
                         "run_sigma_w_ms": run_sw_ms},
@@ -605,6 +636,7 @@ KERNEL_SOURCES = {
     "tree_ws": ["spd_tree_ws.cuh", "spd_tree_common.cuh"],
     "tree_ws_ig": ["spd_tree_ws.cuh", "spd_tree_common.cuh"],
     "tree_block": ["spd_tree.cu", "spd_tree_common.cuh"],
+    "grid_ws": ["spd_tree_ws.cuh", "spd_tree_common.cuh"],
     "tree_ig": ["spd_tree_ig.cu", "spd_tree_common.cuh"],
 }
 
@@ -621,19 +653,20 @@ def kernel_source_hash(key):
 def ncu_traffic_bytes(key, w, width_bytes):
     import csv
     if key not in KERNEL_SOURCES or not os.path.exists(TRAFFIC_CSV):
-        return None, None
+        return None, None, None
     with open(TRAFFIC_CSV) as f:
         rows = [r for r in csv.DictReader(f) if r["kernel"] == key and int(r["workload"]) == w.index and
                 r["width_set"] == f"{w.width_kind}:{w.width_param}" and int(r["width_bytes"]) == width_bytes]
     if not rows:
-        return None, None
+        return None, None, None
     r = rows[-1]
     src = {"measured_in_run": False, "capture": r["capture"], "commit": r["commit"]}
     if r["source_sha256_16"] != kernel_source_hash(key):
         src["stale"] = "the kernel's sources have changed since this capture"
-        return None, src
+        return None, src, None
     per_sample = (float(r["dram_bytes_read"]) + float(r["dram_bytes_write"])) / float(r["samples"])
-    return per_sample * w.n_samples, src
+    lane_ops = float(r["lane_ops_per_sample"]) if r.get("lane_ops_per_sample") else None
+    return per_sample * w.n_samples, src, lane_ops
 
 
 def host_mem_available_bytes():
