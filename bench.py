@@ -416,20 +416,17 @@ class Workbench:
         k_ms = sum(rec["run_ms"]) / len(rec["run_ms"])
         achieved = self.bytes_per_sample * self.n / (k_ms * 1e-3) / 1e9
         key = kernel_key(self.spd, self.info)
-        traffic, traffic_src, lane_ops = ncu_traffic_bytes(key, self.w, self.info["width_bytes"])
+        traffic, traffic_src, cap = ncu_traffic_bytes(key, self.w, self.info["width_bytes"])
         alu = None
-        if lane_ops:
-            # FP32 and integer lanes are one pool of 128 lane-operations per clock and SM on B200 (measured:
-            # profiles/r02_lane_rates.md); lane-operations per sample from the committed ncu source page
-            sms = self.torch.cuda.get_device_properties(self.dev).multi_processor_count
-            clk_mhz = (rec.get("clocks") or {}).get("sm_mhz") or measured_sm_mhz()
-            peak_ops = sms * 128 * clk_mhz * 1e6
-            ach_ops = lane_ops * self.n / (k_ms * 1e-3)
-            alu = {"bound": "alu", "what": "FP32 + integer lane-operations (packed FADD2 / FMUL2 count two)",
-                   "lane_ops_per_sample": lane_ops, "achieved": ach_ops / 1e12, "peak": peak_ops / 1e12,
-                   "unit": "T lane-op/s", "frac": ach_ops / peak_ops,
-                   "peak_source": f"{sms} SMs x 128 lanes x {clk_mhz:.0f} MHz (profiles/r02_lane_rates.md)",
-                   "source": traffic_src}
+        if cap:
+            # The tree kernels are bound by their half-rate ALU-pipe instructions (width tags, 3-input maxima):
+            # busy time of that pipe per sample from the committed capture, scaled to this launch; `ceiling` is
+            # what the kernels' instruction mix reaches in a register-only microbenchmark
+            # (profiles/r02_lane_rates.md: 12 of 15.7 clocks).
+            busy_ms = cap["alu_pipe_pct"] / 100.0 * cap["kernel_ms"] * self.n / cap["samples"]
+            alu = {"bound": "alu", "what": "half-rate ALU pipe (LOP3 width tags, FMNMX3 running maxima)",
+                   "alu_pipe_busy_ms_per_launch": busy_ms, "frac": busy_ms / k_ms, "ceiling": 0.76,
+                   "fma_pipe_busy_frac_in_capture": cap["fma_pipe_pct"] / 100.0, "source": traffic_src}
         return {
             "bound": "hbm", "kernel": KERNEL_NAMES[key], "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
@@ -665,8 +662,9 @@ def ncu_traffic_bytes(key, w, width_bytes):
         src["stale"] = "the kernel's sources have changed since this capture"
         return None, src, None
     per_sample = (float(r["dram_bytes_read"]) + float(r["dram_bytes_write"])) / float(r["samples"])
-    lane_ops = float(r["lane_ops_per_sample"]) if r.get("lane_ops_per_sample") else None
-    return per_sample * w.n_samples, src, lane_ops
+    cap = {"samples": float(r["samples"]), "kernel_ms": float(r["kernel_ms"]),
+           "alu_pipe_pct": float(r["alu_pipe_pct"]), "fma_pipe_pct": float(r["fma_pipe_pct"])}
+    return per_sample * w.n_samples, src, cap
 
 
 def host_mem_available_bytes():

@@ -1,4 +1,4 @@
-// lane_rates.cu - register-only microbenchmarks behind the "ALU roofline" of DESIGN.md sec. 7b.
+// lane_rates.cu - register-only microbenchmarks behind the "ALU-pipe roofline" of DESIGN.md sec. 7b.
 //
 // Not part of libspd_b200.so (the build compiles csrc/*.cu only).  Build and run on a B200:
 //
@@ -8,9 +8,10 @@
 // the tree kernels are made of, 16 independent chains per thread, 16 warps per SM.
 // Part 2: the per-level instruction mix of the kernels - per float4 and level: 2 FADD2 (the partial sum),
 // 2 FMUL2 (the sqrt(width) scale), 4 LOP3 (the width tag), 2 FMNMX3 (the running maximum over two levels) -
-// and variants of it, in clocks per float4-level per sub-partition.  FP32 and integer lanes are one pool of
-// 32 lane-operations per clock and sub-partition (a packed FADD2 / FMUL2 counts two per thread): the mix needs
-// 14 clocks per float4-level at best and measures 15.9, whatever the number of resident warps.
+// and variants of it, in clocks per float4-level per sub-partition.  LOP3 and FMNMX3 share the half-rate ALU
+// pipe (two clocks each: 12 clocks for the mix), the packed FP32 instructions the FMA pipe (two clocks each:
+// 8.2 clocks); the two pipes overlap only in part: the mix measures 15.9 clocks whatever the number of resident
+// warps, 15.5 without the multiplies (the ALU pipe binds) and 10.2-10.8 without the tags.
 #include <cstdint>
 #include <cstdio>
 #include <cuda_runtime.h>
@@ -102,8 +103,8 @@ __device__ __forceinline__ float4 mul4(float4 p, float c) {
 __device__ __forceinline__ float tag(float v, uint32_t tm, uint32_t code) {
     return __uint_as_float((__float_as_uint(v) & tm) | code);
 }
-// PK: packed adds and multiplies; TAG: width tags; the running maximum is always the 3-input one.
-template <bool PK, bool TAG>
+// PK: packed adds and multiplies; TAG: width tags; MUL: the scale multiply; the running maximum is always the 3-input one.
+template <bool PK, bool TAG, bool MUL>
 __global__ void __launch_bounds__(256) mix_kernel(float* out, uint32_t tm, int iters) {
     float4 P[4], Q[4], best[4];
     for (int r = 0; r < 4; ++r) {
@@ -118,7 +119,11 @@ __global__ void __launch_bounds__(256) mix_kernel(float* out, uint32_t tm, int i
             for (int r = 0; r < 4; ++r) {
                 const float4 n1 = add4<PK>(P[r], Q[r]);
                 const float4 n2 = add4<PK>(n1, Q[(r + 1) & 3]);
-                float4 a = mul4<PK>(n1, 0.70710678f), b = mul4<PK>(n2, 0.5f);
+                float4 a = n1, b = n2;
+                if (MUL) {
+                    a = mul4<PK>(n1, 0.70710678f);
+                    b = mul4<PK>(n2, 0.5f);
+                }
                 if (TAG) {
                     a = make_float4(tag(a.x, tm, 31u - lv), tag(a.y, tm, 31u - lv), tag(a.z, tm, 31u - lv), tag(a.w, tm, 31u - lv));
                     b = make_float4(tag(b.x, tm, 30u - lv), tag(b.y, tm, 30u - lv), tag(b.z, tm, 30u - lv), tag(b.w, tm, 30u - lv));
@@ -134,7 +139,7 @@ __global__ void __launch_bounds__(256) mix_kernel(float* out, uint32_t tm, int i
     for (int r = 0; r < 4; ++r) s += best[r].x + best[r].y + best[r].z + best[r].w + P[r].x;
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
-template <bool PK, bool TAG>
+template <bool PK, bool TAG, bool MUL>
 static void mix(const char* name) {
     float* out;
     cudaMalloc(&out, 148 * 3 * 256 * 4);
@@ -143,9 +148,9 @@ static void mix(const char* name) {
     cudaEventCreate(&e1);
     const int iters = 20000;
     for (int bps = 1; bps <= 3; ++bps) {
-        mix_kernel<PK, TAG><<<148 * bps, 256>>>(out, 0xffffffe0u, 10);
+        mix_kernel<PK, TAG, MUL><<<148 * bps, 256>>>(out, 0xffffffe0u, 10);
         cudaEventRecord(e0);
-        mix_kernel<PK, TAG><<<148 * bps, 256>>>(out, 0xffffffe0u, iters);
+        mix_kernel<PK, TAG, MUL><<<148 * bps, 256>>>(out, 0xffffffe0u, iters);
         cudaEventRecord(e1);
         cudaEventSynchronize(e1);
         float ms;
@@ -169,8 +174,9 @@ int main() {
     rate<8>("IMAD", 16);
     rate<9>("FADD2 (packed pair)", 8);
     rate<10>("FMUL2 by an immediate (packed pair)", 8);
-    mix<true, true>("FADD2 FMUL2 LOP3 FMNMX3 (the kernels' mix)");
-    mix<true, false>("FADD2 FMUL2      FMNMX3 (no tags)");
-    mix<false, true>("FADD  FMUL  LOP3 FMNMX3 (scalar FP32)");
+    mix<true, true, true>("FADD2 FMUL2 LOP3 FMNMX3 (the kernels' mix)");
+    mix<true, false, true>("FADD2 FMUL2      FMNMX3 (no tags)");
+    mix<true, true, false>("FADD2       LOP3 FMNMX3 (no multiplies)");
+    mix<false, true, true>("FADD  FMUL  LOP3 FMNMX3 (scalar FP32)");
     return 0;
 }

@@ -124,10 +124,13 @@ __device__ __forceinline__ void register_levels(float4 (&P)[R], float4 (&best)[R
                 // 252 registers per thread): slot = step mod depth as a run-time column offset,
                 // one tcgen05.ld + tcgen05.st of R float4 per level.  Slots of the shallower FIFOs
                 // come first: Q - 1 of them.
-                static_assert(R == 4 || R == 2, "tensor-memory FIFOs move 2 or 4 float4 per level");
+                static_assert(R == 8 || R == 4 || R == 2, "tensor-memory FIFOs move 2, 4 or 8 float4 per level");
                 const uint32_t taddr = cx.tbase + 4u * R * static_cast<uint32_t>((Q - 1) + (cx.it & (Q - 1)));
                 float4 old[R];
-                if constexpr (R == 4) {
+                if constexpr (R == 8) {
+                    tmem_ld32(taddr, reinterpret_cast<float4(&)[8]>(old));
+                    tmem_st32(taddr, reinterpret_cast<const float4(&)[8]>(P));
+                } else if constexpr (R == 4) {
                     tmem_ld16(taddr, reinterpret_cast<float4(&)[4]>(old));
                     tmem_st16(taddr, reinterpret_cast<const float4(&)[4]>(P));
                 } else {
@@ -278,29 +281,12 @@ __device__ __forceinline__ float tree_chunk(const float4* __restrict__ st4, floa
 // sweeps in DESIGN.md "Tuning log").  K <= 14: T = 128, R = 4, 3 blocks (165 registers, no
 // spills): 11.5 ms on config 3.  T = 64 (one exchange level fewer) ties at 11.7 ms once its
 // chunk loop is not unrolled past the instruction cache, T = 256 (one more) is at 13.4 ms.
-// Above max_width 8192 the delay registers double: K = 15 runs 2 blocks of 128 threads
-// (247 registers), K = 16 one block of 512 threads with R = 2.
-#ifndef SPD_TREE_T
-#define SPD_TREE_T 128  // K <= 14
-#endif
-#ifndef SPD_TREE_ROWS
-#define SPD_TREE_ROWS 4
-#endif
-#ifndef SPD_TREE_BPS
-#define SPD_TREE_BPS 3
-#endif
-#ifndef SPD_TREE_T16
-#define SPD_TREE_T16 128
-#endif
-#ifndef SPD_TREE_R16
-#define SPD_TREE_R16 4
-#endif
-constexpr int tree_threads_for(int K) { return K <= 14 ? SPD_TREE_T : (K == 15 ? 128 : SPD_TREE_T16); }
-constexpr int tree_rows_for(int K) { return K <= 14 ? SPD_TREE_ROWS : (K == 15 ? 4 : SPD_TREE_R16); }
-#ifndef SPD_TREE_BPS15
-#define SPD_TREE_BPS15 4
-#endif
-constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? SPD_TREE_BPS : (K == 15 ? SPD_TREE_BPS15 : 2); }
+// K = 15, 16 keep their delay FIFOs in tensor memory: 4 and 2 blocks of 128 threads per SM.
+constexpr int tree_threads_for(int) { return 128; }
+// K = 16: eight rows per chunk (4096 samples, 255 registers, two blocks per SM) - half the barriers per sample of
+// four rows: config 4 in 7.23 ms against 7.35 ms
+constexpr int tree_rows_for(int K) { return K == 16 ? 8 : 4; }
+constexpr int tree_blocks_per_sm(int K) { return K <= 14 ? 3 : (K == 15 ? 4 : 2); }
 // Tensor-memory columns a block allocates for its FIFOs (K >= 15): 4 R columns per FIFO slot,
 // 2^JF - 1 slots, rounded up to a power of two.
 template <int T, int R, int K>
@@ -438,7 +424,7 @@ __global__ void __launch_bounds__(T, tree_blocks_per_sm(K)) spd_tree_kernel(cons
     int it = 0;
     while (it < n_fast) {
         // tensor-memory FIFOs take their slot at run time: two steps per trip only to overlap them
-        static_phases<0, (tree_tmem(K) ? 2 : G::U)>([&](auto ph) {
+        static_phases<0, (tree_tmem(K) ? (R >= 8 ? 1 : 2) : G::U)>([&](auto ph) {
             if (it < n_fast) {
                 if (tid == 0) {
                     const int nx = it + kStages - 1;

@@ -321,12 +321,10 @@ __device__ __forceinline__ void st_shared4(float4* dst, float4 v) {
 // the unroll gets a compile-time slot (no register moves), a deeper one is rotated by moves.
 // Code size grows with the factor; past the instruction cache the kernel stalls on fetch
 // (T = 64, R = 4 unrolled x4: smsp stall_no_instruction 2.6 per issue).
-#ifndef SPD_TREE_MAX_UNROLL
-#define SPD_TREE_MAX_UNROLL 2
-#endif
+constexpr int kTreeMaxUnroll = 2;
 // Block-per-stream dyadic kernel (spd_tree.cu): delay FIFOs in tensor memory from this depth on.
 constexpr bool tree_tmem(int K) { return K >= 15; }
-constexpr int tree_max_unroll(int K) { return K == 16 ? 4 : SPD_TREE_MAX_UNROLL; }
+constexpr int tree_max_unroll(int K) { return K == 16 ? 4 : kTreeMaxUnroll; }
 
 constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v / 2); }
 constexpr int imax(int a, int b) { return a > b ? a : b; }

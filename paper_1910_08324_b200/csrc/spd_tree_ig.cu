@@ -287,10 +287,8 @@ __device__ __forceinline__ float ig_chunk(const float4* __restrict__ st4, float4
 
 constexpr int ig_threads_for(int K) { return K <= 15 ? 128 : 256; }
 constexpr int ig_rows_for(int) { return 4; }
-#ifndef SPD_IG_BPS
-#define SPD_IG_BPS 3  // 168 registers, no spills: 18.1 ms vs 19.2 ms at 2 blocks (config-3 plane)
-#endif
-constexpr int ig_blocks_per_sm(int K) { return K <= 14 ? SPD_IG_BPS : (K == 15 ? 2 : 1); }
+// K <= 14: 3 blocks per SM (168 registers, no spills): 18.1 ms against 19.2 ms at 2 blocks (config-3 plane)
+constexpr int ig_blocks_per_sm(int K) { return K <= 14 ? 3 : (K == 15 ? 2 : 1); }
 
 template <int T, int R>
 constexpr size_t ig_smem_bytes() {
