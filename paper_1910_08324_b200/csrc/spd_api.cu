@@ -524,7 +524,12 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         if (is_tree_path(plan)) info->tree_kernel = plan->tree.kind == 1 ? 2 : 1;
         if (plan->tree.kind == 1 && plan->tree.segs_per_row == 0) info->piece_chunks = ws_piece_chunks(plan);
     } else {
-        if (plan->generic_tile > 0) {
+        if (plan->path == SPD_PATH_GENERIC && dense_applicable(plan)) {
+            info->launches_per_run = 1;
+            info->threads_per_block = 256;
+            info->blocks = dense_blocks(plan);
+            info->chunk = 1024;
+        } else if (plan->generic_tile > 0) {
             info->launches_per_run = 1;
             info->threads_per_block = 1024;
             info->blocks = static_cast<int32_t>(plan->n_dm * plan->generic_tiles_per_row);

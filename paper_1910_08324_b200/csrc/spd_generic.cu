@@ -485,6 +485,8 @@ void generic_release(spd_plan* plan) {
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                 float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w) {
     const long long n_t = plan->n_t;
+    if (dense_applicable(plan))  // max_width <= 64: running sums in registers (spd_dense.cu)
+        return dense_run(plan, n_dm, plane, mean, sigma, out_snr, out_width, stream, sigma_w);
     if (sigma_w && (plan->generic_tile <= 0 || static_cast<int>(plan->widths.size()) > kTileWidthsMax)) {
         set_error("a standard deviation per width needs the shared-memory tile kernel (max_width <= %d, at most %d "
                   "widths)", kTileSpanMax - 4095, kTileWidthsMax);

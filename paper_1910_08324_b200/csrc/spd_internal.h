@@ -159,6 +159,12 @@ int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const fl
                 const float* sigma, float* out_snr, int32_t* out_width, cudaStream_t stream,
                 const float* sigma_w = nullptr);
 
+// spd_dense.cu: any width set with max_width <= 64 (running sums in registers)
+bool dense_applicable(const spd_plan* plan);
+int dense_blocks(const spd_plan* plan);
+int dense_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+              float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w);
+
 // spd_stats.cu
 int stats_configure(spd_plan* plan);
 void stats_release(spd_plan* plan);

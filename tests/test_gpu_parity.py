@@ -217,6 +217,53 @@ def test_generic_width_sets(spd, oracle_lib, kind, param, max_width):
           expect_path=spd.SPD_PATH_GENERIC, direct_windows=[(4900, 5200), (10007 - 300, 10007)])
 
 
+DENSE_SETS = {"all64": list(range(1, 65)), "all37": list(range(1, 38)), "one": [1], "only64": [64],
+              "fib": [1, 2, 3, 5, 8, 13, 21, 34, 55], "odd": list(range(3, 64, 2)), "boxdit4": None}
+
+
+@pytest.mark.parametrize("n_t", [4, 60, 1024, 1028, 2048 + 64, 10008])
+@pytest.mark.parametrize("name", list(DENSE_SETS))
+def test_dense_kernel_small_width_sets(spd, oracle_lib, name, n_t):
+    """Width sets with max_width <= 64 (config 1's family) run on spd_dense_kernel (running sums in registers,
+    one 1024-sample tile per block): direct-summation oracle on every sample, row lengths inside one tile, on a
+    tile boundary, just past it (a one-float4 last tile) and with a look-ahead that ends inside the halo; sets
+    without width 1 leave -inf / -1 at the row's end (reading A3)."""
+    widths = [L for L in DENSE_SETS[name] or spd.spd_width_set_generate("BOXDIT", 4, 64) if L <= n_t]
+    if not widths:
+        pytest.skip("no width of the set fits the row")
+    rng = np.random.default_rng(n_t + len(widths))
+    x = (rng.standard_normal((3, n_t)) * 2.0 + 7.0).astype(np.float32)
+    if n_t > 200:
+        x[1, 100:140] += np.float32(3.0)
+        x[2, n_t - 30:] += np.float32(2.0)
+    mu, sg = oracle_lib.row_stats(x)
+    force = spd.SPD_FLAG_FORCE_GENERIC   # [1] is also a {2^k} set
+    with spd.Plan(3, n_t, widths, flags=force) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GENERIC and plan.info["threads_per_block"] == 256
+        assert plan.info["launches_per_run"] == 1 and plan.info["blocks"] == 3 * ((n_t + 1023) // 1024)
+    check(spd, oracle_lib, x, mu, sg, widths, f"dense {name} n_t={n_t}", direct=True, flags=force,
+          expect_path=spd.SPD_PATH_GENERIC)
+
+
+def test_dense_kernel_with_measured_sigma_per_width(spd, oracle_lib):
+    """spd_run_sigma_w on the dense kernel: all 64 widths (more than the tile kernel's table holds)."""
+    n_dm, n_t = 3, 20000
+    x = _plane_for_sigma_w(n_dm, n_t, 41)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    widths = list(range(1, 65))
+    with spd.Plan(n_dm, n_t, widths) as plan:
+        mean, _ = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    ref = oracle_lib.spd_direct_sw(x, mu64, sw64, widths)
+    parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, None, snr.cpu().numpy(), idx.cpu().numpy(), *ref,
+                               what="sigma_w dense")
+
+
 def test_generic_tile_kernel_wide_sets_and_tile_boundaries(spd, oracle_lib):
     """Any-width-set tile kernel: max_width in the thousands (several tiles per row, ragged last tile,
     look-ahead longer than the tile's remainder), on drifting data with a large offset."""
