@@ -190,13 +190,23 @@ int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, 
  * (only if separations[0] > 1).  Limits: max_width <= 45057, n_widths <= 1024.  A set {1, 2, 4, ..., 2^(K-1)}
  * with 9 <= K <= 14, and the IGRID depth-1 set {2^k} U {3 * 2^m} over the same range when the two widths of an
  * octave share a separation (SPD_GRID_IGRID), run on the warp-per-stream tree kernel
- * (spd_plan_info.tree_kernel == 2), where the keys of a level are formed on its grid points only; other sets
- * run on a shared-memory tile kernel.
+ * (spd_plan_info.tree_kernel == 2), where the keys of a level are formed on its grid points only.  The BoxDIT
+ * algorithm itself (Alg. 1) - the widths of SPD_WIDTHS_BOXDIT with L_max = 4, 8, 16 or 32 (the
+ * last iteration may be cut by max_width) on the separations of SPD_GRID_BOXDIT with the same L_max, at most 11
+ * iterations and 256 widths, n_t % 4 == 0 - runs on a streaming kernel of its own (spd_boxdit.cu: all iterations
+ * of a chunk in one block, decimated series and longest boxcars in shared memory; spd_plan_info.threads_per_block
+ * == 256, chunk == 4096).  Other sets run on a shared-memory tile kernel (threads_per_block == 1024).
  * spd_plan_info.path is SPD_PATH_GRID.  Errors as spd_plan_create plus the conditions above.
+ *
+ * spd_plan_create_grid_ex: the same with creation flags; SPD_FLAG_FORCE_GENERIC keeps the plan on the tile kernel
+ * (no tree, no BoxDIT kernel); the other flags are refused.
  */
 int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t,
                          const int32_t* width_set, const int32_t* separations, int32_t n_widths,
                          int32_t max_width);
+int spd_plan_create_grid_ex(spd_plan** out, int64_t n_dm, int64_t n_t,
+                            const int32_t* width_set, const int32_t* separations, int32_t n_widths,
+                            int32_t max_width, uint32_t flags);
 
 /* Frees the plan and everything it owns.  NULL is allowed. */
 void spd_plan_destroy(spd_plan* plan);

@@ -42,7 +42,7 @@ EXPORTS = (
     "spd_run_host", "spd_last_error_string", "spd_version",
     "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
     "spd_destroy", "spd_plan_set_option", "spd_row_stats_converge", "spd_cluster_candidates",
-    "spd_run_host_candidates",
+    "spd_run_host_candidates", "spd_plan_create_grid_ex",
 )
 
 
@@ -104,6 +104,8 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_plan_create_ex.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _i32, _i32, ctypes.c_uint32]
     lib.spd_plan_create_grid.restype = ctypes.c_int
     lib.spd_plan_create_grid.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _i32, _i32]
+    lib.spd_plan_create_grid_ex.restype = ctypes.c_int
+    lib.spd_plan_create_grid_ex.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _vp, _vp, _i32, _i32, ctypes.c_uint32]
     lib.spd_separation_generate.restype = ctypes.c_int
     lib.spd_separation_generate.argtypes = [_i32, _i32, _vp, _i32, _vp]
     lib.spd_width_sigma.restype = ctypes.c_int
@@ -193,16 +195,20 @@ def spd_separation_generate(kind, param: int, widths: Sequence[int]) -> np.ndarr
 
 
 def spd_plan_create_grid(n_dm: int, n_t: int, width_set: Sequence[int], separations: Sequence[int],
-                         max_width: int) -> int:
-    """Plan with a boxcar separation per width; returns the opaque handle."""
+                         max_width: int, flags: int = 0) -> int:
+    """Plan with a boxcar separation per width; returns the opaque handle (flags: spd_plan_create_grid_ex)."""
     lib = load()
     w = np.ascontiguousarray(np.asarray(width_set, dtype=np.int32).reshape(-1))
     sp = np.ascontiguousarray(np.asarray(separations, dtype=np.int32).reshape(-1))
     if w.size != sp.size:
         raise ValueError("width_set and separations differ in length")
     handle = _vp(0)
-    _check(lib.spd_plan_create_grid(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, sp.ctypes.data,
-                                    int(w.size), int(max_width)))
+    if flags:
+        _check(lib.spd_plan_create_grid_ex(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, sp.ctypes.data,
+                                           int(w.size), int(max_width), int(flags)))
+    else:
+        _check(lib.spd_plan_create_grid(ctypes.byref(handle), int(n_dm), int(n_t), w.ctypes.data, sp.ctypes.data,
+                                        int(w.size), int(max_width)))
     return int(handle.value)
 
 
@@ -484,7 +490,7 @@ class Plan:
         if separations is None:
             self.handle = spd_plan_create(n_dm, n_t, w, mw, flags)
         else:
-            self.handle = spd_plan_create_grid(n_dm, n_t, w, separations, mw)
+            self.handle = spd_plan_create_grid(n_dm, n_t, w, separations, mw, flags)
         self.info = spd_plan_get_info(self.handle)
         self.widths = spd_plan_get_widths(self.handle)
         self.n_dm, self.n_t = int(n_dm), int(n_t)

@@ -248,14 +248,24 @@ int spd_plan_create_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
     return plan_create(out, n_dm, n_t, width_set, nullptr, n_widths, max_width, flags);
 }
 
-int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
-                         const int32_t* separations, int32_t n_widths, int32_t max_width) {
+int spd_plan_create_grid_ex(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
+                            const int32_t* separations, int32_t n_widths, int32_t max_width, uint32_t flags) {
     if (!separations) {
         set_error("spd_plan_create_grid: separations is NULL");
         if (out) *out = nullptr;
         return SPD_ERR_INVALID_ARG;
     }
-    return plan_create(out, n_dm, n_t, width_set, separations, n_widths, max_width, 0u);
+    if (flags & ~SPD_FLAG_FORCE_GENERIC) {
+        set_error("spd_plan_create_grid_ex: only SPD_FLAG_FORCE_GENERIC applies to a grid plan (got 0x%x)", flags);
+        if (out) *out = nullptr;
+        return SPD_ERR_INVALID_ARG;
+    }
+    return plan_create(out, n_dm, n_t, width_set, separations, n_widths, max_width, flags);
+}
+
+int spd_plan_create_grid(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t* width_set,
+                         const int32_t* separations, int32_t n_widths, int32_t max_width) {
+    return spd_plan_create_grid_ex(out, n_dm, n_t, width_set, separations, n_widths, max_width, 0u);
 }
 
 int spd_separation_generate(int32_t kind, int32_t param, const int32_t* widths, int32_t n_widths, int32_t* out) {
@@ -401,10 +411,14 @@ static int plan_create(spd_plan** out, int64_t n_dm, int64_t n_t, const int32_t*
         // widths {2^k} on a grid: the warp-per-stream tree kernel with the keys of a level counted only on
         // that level's grid (the any-width-set grid kernel stays configured for spd_run_sigma_w)
         int igl = 0;
-        if (rc == SPD_OK && tree_applicable(w, n_t) && ws_applicable(static_cast<int>(w.size()), 0u)) {
+        if (rc == SPD_OK && !(flags & SPD_FLAG_FORCE_GENERIC) && boxdit_configure(plan)) {
+            // Alg. 1's widths on Alg. 1's grids: the BoxDIT streaming kernel (spd_boxdit.cu)
+        } else if (rc == SPD_OK && !(flags & SPD_FLAG_FORCE_GENERIC) && tree_applicable(w, n_t) &&
+                   ws_applicable(static_cast<int>(w.size()), 0u)) {
             plan->tree.K = static_cast<int>(w.size());
             rc = ws_configure(plan);
-        } else if (rc == SPD_OK && (igl = ig_applicable(w, n_t)) > 0 && ws_applicable(igl, 0u)) {
+        } else if (rc == SPD_OK && !(flags & SPD_FLAG_FORCE_GENERIC) && (igl = ig_applicable(w, n_t)) > 0 &&
+                   ws_applicable(igl, 0u)) {
             // the IGRID depth-1 widths on a grid whose octaves share a separation (the widths of
             // step 2^i on P layers): width 3 * 2^m goes with width 2^(m+1)
             bool shared = true;
@@ -462,6 +476,11 @@ int spd_plan_set_option(spd_plan* plan, int32_t option, int64_t value) {
     }
     switch (option) {
         case SPD_OPT_SEGMENTS_PER_ROW: {
+            if (plan->boxdit.B > 0 && value >= 0 && value <= 0x7fffffffll) {
+                plan->segs_option = static_cast<int>(value);
+                boxdit_configure(plan);
+                return SPD_OK;
+            }
             if (!runs_tree_kernel(plan) || value < 0 || value > 0x7fffffffll) {
                 set_error("SPD_OPT_SEGMENTS_PER_ROW needs a streaming-tree plan and a value >= 0 (got %lld)",
                           static_cast<long long>(value));
@@ -524,7 +543,14 @@ int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
         if (is_tree_path(plan)) info->tree_kernel = plan->tree.kind == 1 ? 2 : 1;
         if (plan->tree.kind == 1 && plan->tree.segs_per_row == 0) info->piece_chunks = ws_piece_chunks(plan);
     } else {
-        if (plan->path == SPD_PATH_GENERIC && dense_applicable(plan)) {
+        if (plan->boxdit.B > 0) {
+            info->launches_per_run = 1;
+            info->threads_per_block = 256;
+            info->blocks = static_cast<int32_t>(plan->n_dm * plan->boxdit.segs_per_row);
+            info->chunk = 4096;
+            info->segments_per_row = plan->boxdit.segs_per_row;
+            info->smem_bytes = plan->boxdit.smem_bytes;
+        } else if (plan->path == SPD_PATH_GENERIC && dense_applicable(plan)) {
             info->launches_per_run = 1;
             info->threads_per_block = 256;
             info->blocks = dense_blocks(plan);

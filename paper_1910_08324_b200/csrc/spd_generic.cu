@@ -492,6 +492,8 @@ int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const fl
                   "widths)", kTileSpanMax - 4095, kTileWidthsMax);
         return SPD_ERR_INVALID_ARG;
     }
+    if (plan->boxdit.B > 0)  // Alg. 1's widths on Alg. 1's grids (spd_boxdit.cu)
+        return boxdit_run(plan, n_dm, plane, mean, sigma, out_snr, out_width, stream, sigma_w);
     if (!plan->separations.empty()) {
         grid_tile_kernel<<<static_cast<unsigned>(n_dm * plan->generic_tiles_per_row), kTileThreads, plan->generic_smem,
                            stream>>>(plane, mean, sigma, plan->d_widths, plan->d_wscale,

@@ -32,6 +32,15 @@ struct TreeConfig {
     size_t smem_bytes = 0;
 };
 
+// Alg. 1's own widths on Alg. 1's own grids (spd_boxdit.cu); B = 0: not such a plan.
+struct BoxditConfig {
+    int B = 0;             // L_max per iteration (4, 8, 16 or 32; D = 2)
+    int levels = 0;        // iterations
+    int last_count = 0;    // widths of the last iteration (max_width may cut it)
+    int chunks_per_row = 0, segs_per_row = 1, seg_chunks = 0, warm_chunks = 0;
+    int smem_bytes = 0;
+};
+
 // Per-width boxcar separation (spd_plan_create_grid): consecutive widths of equal separation.
 constexpr int kGridGroupsMax = 32;
 struct GridGroups {
@@ -75,6 +84,7 @@ struct spd_plan {
     int sm_count = 0;
     // dyadic tree
     spd::TreeConfig tree;
+    spd::BoxditConfig boxdit;
     // generic path
     int32_t* d_widths = nullptr;   // [n_widths]
     float* d_wscale = nullptr;     // [n_widths] 1/sqrt(L)
@@ -164,6 +174,11 @@ bool dense_applicable(const spd_plan* plan);
 int dense_blocks(const spd_plan* plan);
 int dense_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w);
+
+// spd_boxdit.cu: the BoxDIT algorithm (widths of eq. 14 on their own grids) as one streaming kernel
+bool boxdit_configure(spd_plan* plan);
+int boxdit_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w);
 
 // spd_stats.cu
 int stats_configure(spd_plan* plan);

@@ -806,6 +806,74 @@ def test_grid_plans_match_oracle(spd, oracle_lib, wkind, wparam, gkind, gparam):
     assert np.all((n % np.asarray(seps)[np.where(on, got_idx, 0)] == 0) | ~on)
 
 
+@pytest.mark.parametrize("segs", [0, 3])
+@pytest.mark.parametrize("B,M,n_t", [(4, 200, 8192 + 4 * 33), (8, 8192, 40000), (8, 300, 4096), (8, 8, 1000),
+                                     (16, 5000, 3 * 4096 + 4), (16, 700, 20004), (32, 8192, 30000), (32, 1000, 9000),
+                                     (4, 8188, 25000)])
+def test_boxdit_kernel_matches_oracle(spd, oracle_lib, B, M, n_t, segs):
+    """Alg. 1's widths (eq. 14) on Alg. 1's grids run on spd_boxdit_kernel: every sample against
+    oracle_spd_grid (direct summation on each width's own grid) - 1 to 11 iterations, width sets cut by max_width
+    inside the last iteration, rows of one partial chunk up to several chunks with a ragged end, the default work
+    split and three segments per row (the warm-up replay), a drifting baseline with an offset, pulses between the
+    grid widths and one that runs off the row's end; the same plan with SPD_FLAG_FORCE_GENERIC stays on
+    grid_tile_kernel."""
+    widths = spd.spd_width_set_generate("BOXDIT", B, M)
+    seps = spd.spd_separation_generate("BOXDIT", B, widths)
+    rng = np.random.default_rng(B * 1000 + M + n_t)
+    x = (rng.standard_normal((3, n_t)) + 0.3 * np.sin(np.arange(n_t) / 3000.0) + 11.0).astype(np.float32)
+    for d, (t0, S) in enumerate([(n_t // 3, 23), (n_t // 2 + 1, 150), (n_t - 200, 400)]):
+        x[d, t0:t0 + S] += np.float32(14.0 / np.sqrt(S))
+    mu, sg = oracle_lib.row_stats(x)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean = torch.from_numpy(mu.astype(np.float32)).to(dev)
+    sigma = torch.from_numpy(sg.astype(np.float32)).to(dev)
+    with spd.Plan(3, n_t, widths, int(widths[-1]), separations=seps) as plan:
+        info = plan.info
+        assert info["path"] == spd.SPD_PATH_GRID and info["threads_per_block"] == 256 and info["chunk"] == 4096
+        if segs:
+            plan.set_option(spd.SPD_OPT_SEGMENTS_PER_ROW, segs)
+            chunks = (n_t + 4095) // 4096
+            assert plan.info["segments_per_row"] == -(-chunks // -(-chunks // segs))
+        snr, idx = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    with spd.Plan(3, n_t, widths, int(widths[-1]), separations=seps, flags=spd.SPD_FLAG_FORCE_GENERIC) as plan:
+        assert plan.info["threads_per_block"] == 1024
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sg64 = sigma.cpu().numpy().astype(np.float64)
+    ref_snr, ref_idx, ref_sec = oracle_lib.spd_grid(x, mu64, sg64, widths, seps)
+    got_snr, got_idx = snr.cpu().numpy(), idx.cpu().numpy()
+    st = parity.assert_parity(oracle_lib, x, mu64, sg64, widths, got_snr, got_idx, ref_snr, ref_idx, ref_sec,
+                              what=f"boxdit B={B} M={M} n_t={n_t} segs={segs}")
+    assert st.n == 3 * n_t
+    n = np.arange(n_t)[None, :]
+    assert np.all(n % np.asarray(seps)[got_idx] == 0)   # width 1 always fits: every sample has a width
+
+
+@pytest.mark.parametrize("B,M", [(8, 2000), (16, 8192)])
+def test_boxdit_kernel_with_measured_sigma_per_width(spd, oracle_lib, B, M):
+    """spd_run_sigma_w on the BoxDIT kernel, every sample against oracle_spd_grid_sw with the
+    table the device measured."""
+    n_dm, n_t = 3, 24000
+    x = _plane_for_sigma_w(n_dm, n_t, 5 + B)
+    widths = spd.spd_width_set_generate("BOXDIT", B, M)
+    seps = spd.spd_separation_generate("BOXDIT", B, widths)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    with spd.Plan(n_dm, n_t, widths, int(widths[-1]), separations=seps) as plan:
+        assert plan.info["threads_per_block"] == 256
+        mean, _ = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    ref = oracle_lib.spd_grid_sw(x, mu64, sw64, widths, seps)
+    st = parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, seps, snr.cpu().numpy(), idx.cpu().numpy(),
+                                    *ref, what=f"sigma_w boxdit B={B}")
+    assert st.n == n_dm * n_t
+
+
 @pytest.mark.parametrize("wkind,wparam,gkind,gparam", [("BOXDIT", 8, "BOXDIT", 8), ("IGRID", 1, "IGRID", 4),
                                                        ("POW2", 0, "DIT", 0)])
 def test_grid_sliding_pulses_recover_the_paper_bounds(spd, wkind, wparam, gkind, gparam):
