@@ -309,7 +309,8 @@ def measured_peak():
 KERNEL_NAMES = {"tree_ws": "spd_tree_ws_kernel", "tree_block": "spd_tree_kernel", "tree_ig": "spd_tree_ig_kernel",
                 "tree_ws_ig": "spd_tree_ws_kernel (IGRID depth-1 widths)",
                 "grid_ws": "spd_tree_ws_kernel (grid)", "grid_tile": "grid_tile_kernel", "generic": "generic_tile_kernel",
-                "dense": "spd_dense_kernel (max_width <= 64)"}
+                "dense": "spd_dense_kernel (max_width <= 64)",
+                "boxdit": "spd_boxdit_kernel (Alg. 1, all iterations in one block)"}
 
 
 def kernel_key(spd, info):
@@ -318,7 +319,9 @@ def kernel_key(spd, info):
     if info["path"] == spd.SPD_PATH_IGRID_TREE:
         return "tree_ws_ig" if info["tree_kernel"] == 2 else "tree_ig"
     if info["path"] == spd.SPD_PATH_GRID:
-        return "grid_ws" if info["tree_kernel"] == 2 else "grid_tile"
+        if info["tree_kernel"] == 2:
+            return "grid_ws"
+        return "boxdit" if info["threads_per_block"] == 256 else "grid_tile"   # the tile kernel runs 1024 threads
     return "dense" if info["threads_per_block"] == 256 else "generic"   # the tile kernel runs 1024 threads
 
 

@@ -322,9 +322,7 @@ int spd_width_sigma(const spd_plan* plan, const float* plane, const float* mean,
  * spd_run_sigma_w - spd_run with SNR_L = (X_L - L mean) / sigma_w[d][L's index] (eq. 4, PAPER.md:69,
  * with the measured sigma(X_L) of spd_width_sigma in place of eq. 5's sqrt(L) sigma).
  * For every plan except SPD_PATH_GENERIC plans on the device-workspace kernels (max_width above about 45 000, or
- * SPD_FLAG_GENERIC_WORKSPACE), SPD_PATH_IGRID_TREE plans on the block-per-stream kernel (max_width below 256 or
- * above 8192: create those with SPD_FLAG_FORCE_GENERIC) and SPD_FLAG_WIDTH_U8 plans, which return
- * SPD_ERR_INVALID_ARG.  Other arguments
+ * SPD_FLAG_GENERIC_WORKSPACE) and SPD_FLAG_WIDTH_U8 plans, which return SPD_ERR_INVALID_ARG.  Other arguments
  * (alignment included) as spd_run.
  */
 int spd_run_sigma_w(const spd_plan* plan, const float* plane, const float* mean, const float* sigma_w,

@@ -90,7 +90,8 @@ __device__ __forceinline__ void bd_task(const float* __restrict__ A, const float
         w[4 * v + 2] = q.z;
         w[4 * v + 3] = q.w;
     }
-    float t[4] = {xin.x, xin.y, xin.z, xin.w};
+    // the four running sums as two packed pairs (FADD2 / FMUL2: one issue slot for two points)
+    float2 t01 = make_float2(xin.x, xin.y), t23 = make_float2(xin.z, xin.w);
     const float ninf = __int_as_float(0xff800000);
     float pend[4];
 #pragma unroll
@@ -98,18 +99,24 @@ __device__ __forceinline__ void bd_task(const float* __restrict__ A, const float
 #pragma unroll
     for (int m = 0; m < B; ++m) {
         const float s = sc[m];
+        const float2 ss = make_float2(s, s);
         const uint32_t code = code0 - m;
+        // eq. (15): the boxcar of m + 1 elements of x^level on top of X^{level-1}
+        t01 = __fadd2_rn(t01, make_float2(w[m], w[m + 1]));
+        t23 = __fadd2_rn(t23, make_float2(w[m + 2], w[m + 3]));
+        const float2 k01 = __fmul2_rn(t01, ss), k23 = __fmul2_rn(t23, ss);
+        float key[4] = {k01.x, k01.y, k23.x, k23.y};
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            t[j] += w[j + m];  // eq. (15): the boxcar of m + 1 elements of x^level on top of X^{level-1}
-            float key = __uint_as_float((__float_as_uint(t[j] * s) & tag_mask) | code);
-            if (MASKED && m >= mlim[j]) key = ninf;  // does not fit the row (reading A3) or is not in the plan
+            key[j] = __uint_as_float((__float_as_uint(key[j]) & tag_mask) | code);
+            if (MASKED && m >= mlim[j]) key[j] = ninf;  // does not fit the row (reading A3) or is not in the plan
             if (m & 1)
-                best[j] = fmax3(best[j], pend[j], key);
+                best[j] = fmax3(best[j], pend[j], key[j]);
             else
-                pend[j] = key;
+                pend[j] = key[j];
         }
     }
+    const float t[4] = {t01.x, t01.y, t23.x, t23.y};
     if (!last) {
         // eq. (13): x^{level+1}[q'] = x^level[2q' + B] + x^level[2q' + B + 1]; and X^level at the even points
         *reinterpret_cast<float2*>(A_next + 2 * a) = make_float2(w[B] + w[B + 1], w[B + 2] + w[B + 3]);
@@ -232,7 +239,19 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
                 } else {
                     bd_task<B, false, false>(A, xin, a, mu, scale + i * B, code0, p.tag_mask, last, An, Xn, mlim, best);
                 }
-                *reinterpret_cast<float4*>(XB + 4 * a) = make_float4(best[0], best[1], best[2], best[3]);
+                if (i <= 2) {
+                    *reinterpret_cast<float4*>(XB + 4 * a) = make_float4(best[0], best[1], best[2], best[3]);
+                } else {
+                    // point q of level i is sample q * 2^i = entry q * 2^(i-2) of level 2's array: the best keys of the
+                    // levels above 2 are folded into it here, so that the gather below reads three values per task
+                    // instead of walking the levels (levels run one after the other: no two writers per entry)
+                    float* const fin = xb + bd_off_b(2) + ((4 * a) << (i - 2));
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        float* const q = fin + (j << (i - 2));
+                        *q = fmaxf(*q, best[j]);
+                    }
+                }
             }
             __syncthreads();
         }
@@ -247,9 +266,7 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
                 key[0] = fmaxf(key[0], b1.x);
                 key[2] = fmaxf(key[2], b1.y);
             }
-            if (I > 2) key[0] = fmaxf(key[0], xb[bd_off_b(2) + a]);
-            for (int i = 3; i < I && (a & ((1 << (i - 2)) - 1)) == 0; ++i)
-                key[0] = fmaxf(key[0], xb[bd_off_b(i) + (a >> (i - 2))]);
+            if (I > 2) key[0] = fmaxf(key[0], xb[bd_off_b(2) + a]);  // level 2 and, folded into it, the levels above
             const int n = t0 + 4 * a;
             if (store && n < n_t) {
                 float4 y;

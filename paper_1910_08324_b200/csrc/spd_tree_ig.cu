@@ -48,13 +48,15 @@ __device__ __forceinline__ float4 gkey(float4 p, float scale, int lim, uint32_t 
     return q;
 }
 // SNR key of width 2^k (eq. 5: scale 2^(-k/2)) and of width 3 * 2^m (scale 2^(-m/2) / sqrt 3).
-template <int k, bool FAST>
-__device__ __forceinline__ float4 kp(float4 p, int lim, uint32_t tm) {
-    return gkey<idx_pow2(k), (1 << k), FAST>(p, level_scale<k>(), lim, tm);
+// SW: a measured sigma per width instead: cx.ls[width index] = 1 / sigma_{d, L}.
+template <int k, bool FAST, bool SW>
+__device__ __forceinline__ float4 kp(float4 p, int lim, const ChunkCtx& cx) {
+    return gkey<idx_pow2(k), (1 << k), FAST>(p, SW ? cx.ls[idx_pow2(k)] : level_scale<k>(), lim, cx.tm);
 }
-template <int m, bool FAST>
-__device__ __forceinline__ float4 kg(float4 p, int lim, uint32_t tm) {
-    return gkey<idx_ig(m), 3 * (1 << m), FAST>(p, level_scale<m>() * 0.57735026918962576451f, lim, tm);
+template <int m, bool FAST, bool SW>
+__device__ __forceinline__ float4 kg(float4 p, int lim, const ChunkCtx& cx) {
+    return gkey<idx_ig(m), 3 * (1 << m), FAST>(p, SW ? cx.ls[idx_ig(m)] : level_scale<m>() * 0.57735026918962576451f, lim,
+                                               cx.tm);
 }
 
 // Halo slots per parity: the exchange levels use d4 slots each (sum T - 2), the extra
@@ -66,7 +68,7 @@ constexpr int ig_halo_slots() {
 
 // Exchange levels k = 3 .. LT+1.  The buffer holds P_k: partner d4 slots later gives P_{k+1},
 // partner d4 / 2 slots later gives width 3 * 2^(k-1) = P_{k-1}[n] + P_k[n + 2^(k-1)].
-template <int T, int R, int K, bool FAST, int k, int hoff>
+template <int T, int R, int K, bool FAST, bool SW, int k, int hoff>
 __device__ __forceinline__ void ig_exchange_levels(float4 (&P)[R], float4 (&Pprev)[R], float4 (&best)[R],
                                                    const int (&lim)[R], float4* __restrict__ pp,
                                                    float4* __restrict__ hr, float4* __restrict__ hw, int& xsel,
@@ -91,11 +93,11 @@ __device__ __forceinline__ void ig_exchange_levels(float4 (&P)[R], float4 (&Ppre
             const float4 now = add4(P[r], *s1);
             const float4 g = add4(Pprev[r], *s2);
             if (FAST || cx.do_out)
-                best[r] = max4(best[r], kp<k + 1, FAST>(now, lim[r], cx.tm), kg<k - 1, FAST>(g, lim[r], cx.tm));
+                best[r] = max4(best[r], kp<k + 1, FAST, SW>(now, lim[r], cx), kg<k - 1, FAST, SW>(g, lim[r], cx));
             Pprev[r] = P[r];
             P[r] = now;
         }
-        ig_exchange_levels<T, R, K, FAST, k + 1, hoff + d4>(P, Pprev, best, lim, pp, hr, hw, xsel, cx);
+        ig_exchange_levels<T, R, K, FAST, SW, k + 1, hoff + d4>(P, Pprev, best, lim, pp, hr, hw, xsel, cx);
     } else if constexpr (G::J >= 1) {
         // extra exchange: P = P_{LT+2}, Pprev = P_{LT+1}; width 3 * 2^(LT+1) needs P_{LT+2} half a row later
         constexpr int h4 = T / 2;
@@ -112,7 +114,7 @@ __device__ __forceinline__ void ig_exchange_levels(float4 (&P)[R], float4 (&Ppre
             const float4* s2 = buf + (tid + T * r + h4);
             if (r == R - 1 && tid + h4 >= T) s2 = hr + (hoff + tid + h4 - T);
             const float4 g = add4(Pprev[r], *s2);
-            if (FAST || cx.do_out) best[r] = max4(best[r], kg<G::LT + 1, FAST>(g, lim[r], cx.tm));
+            if (FAST || cx.do_out) best[r] = max4(best[r], kg<G::LT + 1, FAST, SW>(g, lim[r], cx));
         }
     }
 }
@@ -139,7 +141,7 @@ __device__ __forceinline__ float4 ig_delayed(const float4 (&dl)[Geo<T, R, K>::ND
 }
 
 // In-register levels j = 0 .. J-1 (own level k = LT + 2 + j, partner D = 2^j rows later).
-template <int T, int R, int K, bool FAST, int PH, int j>
+template <int T, int R, int K, bool FAST, bool SW, int PH, int j>
 __device__ __forceinline__ void ig_register_levels(float4 (&P)[R], float4 (&best)[R], const int (&lim)[R],
                                                    float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
     using G = Geo<T, R, K>;
@@ -170,12 +172,12 @@ __device__ __forceinline__ void ig_register_levels(float4 (&P)[R], float4 (&best
                 }
                 const float4 g = add4(P[r], nxt);
                 if (FAST || cx.do_out)
-                    best[r] = max4(best[r], kp<k + 1, FAST>(now[r], lim[r], cx.tm), kg<k, FAST>(g, lim[r], cx.tm));
+                    best[r] = max4(best[r], kp<k + 1, FAST, SW>(now[r], lim[r], cx), kg<k, FAST, SW>(g, lim[r], cx));
             }
         } else {
 #pragma unroll
             for (int r = 0; r < R; ++r)
-                if (FAST || cx.do_out) best[r] = max4(best[r], kp<k + 1, FAST>(now[r], lim[r], cx.tm));
+                if (FAST || cx.do_out) best[r] = max4(best[r], kp<k + 1, FAST, SW>(now[r], lim[r], cx));
         }
         // delay registers of this level take this chunk's inputs
         if constexpr (D < R) {
@@ -200,12 +202,12 @@ __device__ __forceinline__ void ig_register_levels(float4 (&P)[R], float4 (&best
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) P[r] = now[r];
-        ig_register_levels<T, R, K, FAST, PH, j + 1>(P, best, lim, dl, cx);
+        ig_register_levels<T, R, K, FAST, SW, PH, j + 1>(P, best, lim, dl, cx);
     }
 }
 
 // One streaming step (see tree_chunk in spd_tree.cu); needs K >= 5.
-template <int T, int R, int K, bool FAST, int PH>
+template <int T, int R, int K, bool FAST, int PH, bool SW>
 __device__ __forceinline__ float ig_chunk(const float4* __restrict__ st4, float4* __restrict__ pp,
                                           float4* __restrict__ halo, int& xsel, int& hsel,
                                           float4 (&dl)[Geo<T, R, K>::ND + 1], const ChunkCtx& cx) {
@@ -241,9 +243,9 @@ __device__ __forceinline__ float ig_chunk(const float4* __restrict__ st4, float4
         const float4 x3 = make_float4(a.x + s12, a.y + s23, a.z + s34, a.w + s45);
         const float4 x6 = make_float4(s01 + p2.z, s12 + p2.w, s23 + q4567, s34 + q5678);
         if (FAST || cx.do_out) {
-            float4 bb = max4(kp<0, FAST>(a, lim[r], tm), kp<1, FAST>(p1, lim[r], tm), kp<2, FAST>(p2, lim[r], tm));
-            bb = max4(bb, kp<3, FAST>(p3, lim[r], tm), kg<0, FAST>(x3, lim[r], tm));
-            best[r] = max4(bb, kg<1, FAST>(x6, lim[r], tm));
+            float4 bb = max4(kp<0, FAST, SW>(a, lim[r], cx), kp<1, FAST, SW>(p1, lim[r], cx), kp<2, FAST, SW>(p2, lim[r], cx));
+            bb = max4(bb, kp<3, FAST, SW>(p3, lim[r], cx), kg<0, FAST, SW>(x3, lim[r], cx));
+            best[r] = max4(bb, kg<1, FAST, SW>(x6, lim[r], cx));
         }
         Pprev[r] = p2;
         P[r] = p3;
@@ -254,10 +256,10 @@ __device__ __forceinline__ float ig_chunk(const float4* __restrict__ st4, float4
     float4* const hr = halo + hsel * HS;
     float4* const hw = halo + (hsel ^ 1) * HS;
     hsel ^= 1;
-    ig_exchange_levels<T, R, K, FAST, 3, 0>(P, Pprev, best, lim, pp, hr, hw, xsel, cx);
+    ig_exchange_levels<T, R, K, FAST, SW, 3, 0>(P, Pprev, best, lim, pp, hr, hw, xsel, cx);
 
     // ---- in-register levels ---------------------------------------------------------------
-    ig_register_levels<T, R, K, FAST, PH, 0>(P, best, lim, dl, cx);
+    ig_register_levels<T, R, K, FAST, SW, PH, 0>(P, best, lim, dl, cx);
 
     // ---- unpack and store -------------------------------------------------------------------
     float top = __int_as_float(0xff800000);
@@ -289,6 +291,8 @@ constexpr int ig_threads_for(int K) { return K <= 15 ? 128 : 256; }
 constexpr int ig_rows_for(int) { return 4; }
 // K <= 14: 3 blocks per SM (168 registers, no spills): 18.1 ms against 19.2 ms at 2 blocks (config-3 plane)
 constexpr int ig_blocks_per_sm(int K) { return K <= 14 ? 3 : (K == 15 ? 2 : 1); }
+// with a run-time scale per width (2K - 2 more registers) two blocks per SM up to K = 14
+constexpr int ig_blocks_per_sm(int K, bool SW) { return (SW && K <= 14) ? 2 : ig_blocks_per_sm(K); }
 
 template <int T, int R>
 constexpr size_t ig_smem_bytes() {
@@ -297,8 +301,8 @@ constexpr size_t ig_smem_bytes() {
 }
 
 // Same streaming driver as spd_tree_kernel (segments, guarded steps, bulk-copy ring).
-template <int T, int R, int K>
-__global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(const TreeParams p) {
+template <int T, int R, int K, bool SW>
+__global__ void __launch_bounds__(T, ig_blocks_per_sm(K, SW)) spd_tree_ig_kernel(const TreeParams p) {
     using G = Geo<T, R, K>;
     constexpr int C = G::C;
     constexpr int M = 1 << (K - 1);
@@ -324,8 +328,14 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(con
     const float* __restrict__ row = p.plane + static_cast<long long>(d) * n_t;
     ChunkCtx cx;
     cx.mu = p.mean[d];
-    const float sg = p.sigma[d];
+    const float sg = SW ? 1.0f : p.sigma[d];
     cx.inv = 1.0f / sg;
+    if constexpr (SW) {
+        // keys are SNRs already: 1 / sigma_{d, L} per width index, nothing left for the store
+        const float* __restrict__ swr = p.sigma_w + static_cast<long long>(d) * (2 * K - 2);
+#pragma unroll
+        for (int k = 0; k < 2 * K - 2; ++k) cx.ls[k] = 1.0f / __ldg(swr + k);
+    }
     cx.tm = p.tag_mask;
     cx.out_snr = p.out_snr + static_cast<long long>(d) * n_t;
     cx.out_width = p.out_width + static_cast<long long>(d) * n_t;
@@ -359,7 +369,7 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(con
         __syncthreads();
         cx.n0 = n0;
         cx.do_out = c < c_hi;
-        const float top = ig_chunk<T, R, K, false, 0>(reinterpret_cast<const float4*>(stages), pp, halo, xsel, hsel,
+        const float top = ig_chunk<T, R, K, false, 0, SW>(reinterpret_cast<const float4*>(stages), pp, halo, xsel, hsel,
                                                       dl, cx);
         if (act && cx.do_out && top >= thr_key) act[c] = 1;
         __syncthreads();
@@ -399,7 +409,7 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(con
                 mbar_wait(&bars[stage], phase);
                 const int c = first_fast - 1 - it;
                 cx.n0 = static_cast<long long>(c) * C;
-                const float top = ig_chunk<T, R, K, true, decltype(ph)::value>(
+                const float top = ig_chunk<T, R, K, true, decltype(ph)::value, SW>(
                     reinterpret_cast<const float4*>(stages + stage * (C + 8)), pp, halo, xsel, hsel, dl, cx);
                 if (act && top >= thr_key) act[c] = 1;
                 if (++stage == kStages) {
@@ -415,11 +425,14 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K)) spd_tree_ig_kernel(con
 template <int T, int R, int K>
 cudaError_t ig_prepare(TreeConfig& cfg) {
     cfg.smem_bytes = ig_smem_bytes<T, R>();
-    cudaError_t e = cudaFuncSetAttribute(spd_tree_ig_kernel<T, R, K>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(spd_tree_ig_kernel<T, R, K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(cfg.smem_bytes));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(spd_tree_ig_kernel<T, R, K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 static_cast<int>(cfg.smem_bytes));
     if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_ig_kernel<T, R, K>, T, cfg.smem_bytes);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, spd_tree_ig_kernel<T, R, K, false>, T, cfg.smem_bytes);
     if (e != cudaSuccess) return e;
     cfg.blocks_per_sm = nb;
     return cudaSuccess;
@@ -465,15 +478,11 @@ int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
            float* out_snr, int32_t* out_width, float threshold, uint8_t* activity, cudaStream_t stream,
            const float* sigma_w) {
     const TreeConfig& cfg = plan->tree;
-    if (sigma_w) {
-        set_error("the IGRID-tree kernel scales by sqrt(width) at compile time");
-        return SPD_ERR_INVALID_ARG;
-    }
     TreeParams prm;
     prm.plane = plane;
     prm.mean = mean;
     prm.sigma = sigma;
-    prm.sigma_w = nullptr;
+    prm.sigma_w = sigma_w;  // [n_dm][2K - 2] or nullptr
     for (int k = 0; k < 16; ++k) prm.gmask[k] = 0u;
     prm.out_snr = out_snr;
     prm.out_width = out_width;
@@ -496,7 +505,12 @@ int ig_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* 
     const dim3 grid(static_cast<unsigned>(n_dm * cfg.segs_per_row));
 #define SPD_LAUNCH(KK)                                                                                            \
     if (cfg.K == KK) {                                                                                            \
-        spd_tree_ig_kernel<ig_threads_for(KK), ig_rows_for(KK), KK><<<grid, ig_threads_for(KK), cfg.smem_bytes, stream>>>(prm); \
+        if (sigma_w)                                                                                              \
+            spd_tree_ig_kernel<ig_threads_for(KK), ig_rows_for(KK), KK, true>                                     \
+                <<<grid, ig_threads_for(KK), cfg.smem_bytes, stream>>>(prm);                                      \
+        else                                                                                                      \
+            spd_tree_ig_kernel<ig_threads_for(KK), ig_rows_for(KK), KK, false>                                    \
+                <<<grid, ig_threads_for(KK), cfg.smem_bytes, stream>>>(prm);                                      \
         e = cudaGetLastError();                                                                                   \
     }
     SPD_IG_CASES(SPD_LAUNCH)

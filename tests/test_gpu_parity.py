@@ -1013,6 +1013,53 @@ def test_igrid_block_and_warp_kernels_agree_and_take_a_sigma_table(spd, oracle_l
     assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
 
 
+@pytest.mark.parametrize("K,flags", [(6, 0), (8, 0), (11, "block"), (15, 0), (16, 0)])
+def test_igrid_block_kernel_with_measured_sigma_per_width(spd, oracle_lib, K, flags):
+    """spd_run_sigma_w on the block-per-stream IGRID kernel (max_width < 256 or > 8192, or SPD_FLAG_BLOCK_TREE):
+    PAPER.md:728 applies the interpolated sigma to every width of the IG(1) set.  Every sample against direct
+    summation with the same table where that takes seconds, windows otherwise; the table sqrt(L) sigma
+    reproduces spd_run."""
+    M = 1 << (K - 1)
+    rng = np.random.default_rng(900 + K)
+    n_dm = 3
+    n_t = 4 * ((max(2048 * 5 + 12, 2 * M + 600) + 3) // 4)
+    x = rng.standard_normal((n_dm, n_t))
+    x[1] = np.convolve(x[1], np.ones(5) / 2.0, mode="same")   # coloured row: sigma_L != sqrt(L) sigma
+    S = max(1, 3 * M // 8)
+    x[2, n_t // 3: n_t // 3 + S] += 11.0 / np.sqrt(S)
+    x = (x + np.array([0.0, 2.0, -1.0])[:, None]).astype(np.float32)
+    widths = spd.spd_width_set_generate("IGRID", 1, M)
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    fl = spd.SPD_FLAG_BLOCK_TREE if flags == "block" else 0
+    with spd.Plan(n_dm, n_t, widths, M, flags=fl) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_IGRID_TREE and plan.info["tree_kernel"] == 1
+        mean, sigma = plan.row_stats(plane)
+        sw = plan.width_sigma(plane, mean)
+        snr, idx = plan.run_sigma_w(plane, mean, sw)
+        white = (sigma[:, None] * torch.sqrt(torch.tensor(widths, dtype=torch.float32, device=dev))[None, :]).contiguous()
+        snr_w, idx_w = plan.run_sigma_w(plane, mean, white)
+        snr_0, idx_0 = plan.run(plane, mean, sigma)
+        torch.cuda.synchronize()
+    mu64 = mean.cpu().numpy().astype(np.float64)
+    sw64 = sw.cpu().numpy().astype(np.float64)
+    if K <= 11:   # direct summation of every sample: seconds
+        ref_sw = oracle_lib.spd_direct_sw(x, mu64, sw64, widths)
+        parity.assert_parity_table(oracle_lib, x, mu64, sw64, widths, None, snr.cpu().numpy(), idx.cpu().numpy(),
+                                   *ref_sw, what=f"igrid block sigma_w K={K}")
+    else:
+        for t0, t1 in [(n_t // 3 - 300, n_t // 3 + 300), (n_t - 500, n_t), (0, 300), (n_t - M - 150, n_t - M + 150)]:
+            r = oracle_lib.spd_direct_sw(x, mu64, sw64, widths, t0, t1)
+            tol = parity.snr_tolerance(r[0])
+            fit = r[1] >= 0
+            assert np.all(np.abs(snr.cpu().numpy()[:, t0:t1] - r[0])[fit] <= tol[fit])
+            dec = fit & ((r[0] - r[2]) > tol)
+            assert np.array_equal(idx.cpu().numpy()[:, t0:t1][dec], r[1][dec])
+    a, b = snr_w.cpu().numpy(), snr_0.cpu().numpy()
+    assert np.all(np.abs(a - b) <= 1e-5 * np.maximum(1.0, np.abs(b)))
+    assert np.mean(idx_w.cpu().numpy() == idx_0.cpu().numpy()) > 0.999
+
+
 @pytest.mark.parametrize("K,layers", [(9, 4), (12, 4), (14, 4), (13, 16), (11, 1)])
 def test_igrid_widths_on_layer_grids_run_on_the_tree_kernel(spd, oracle_lib, K, layers):
     """The paper's IG(1) grids (widths 2^k and 3 * 2^m with the widths of step 2^i on P layers):
