@@ -343,6 +343,30 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
                  float* out_snr, void* out_width);
 
 /*
+ * spd_row_stats_static - spd_row_stats for callers that may not allocate (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): no plan, and the call enqueues kernels and one memset on
+ * cuda_stream and nothing else - no cudaMalloc, cudaFree or allocating library routine, on the first call
+ * or later.  Same kernels, same arithmetic and the same work split rule as spd_row_stats (PAPER.md:720-726,
+ * reading A14): results agree with it to rounding, and exactly when both cut a row into the same parts.
+ *   plane            : DEVICE float32 [n_dm][n_t], row-major (16-byte aligned with n_t % 4 == 0 takes the
+ *                      vectorised loads; any alignment is accepted).
+ *   mean, sigma      : DEVICE float32 [n_dm], written (also read between the rejection passes).
+ *   clip_sigma, n_reject_passes : as spd_row_stats (0 <= n_reject_passes <= 64; 0 = all samples, reading A6).
+ * The scratch (partial moments per row part, per-row state) is a fixed array in the library's device image,
+ * SPD_STATIC_SCRATCH_BYTES (1.7 MiB), which every GPU that loads the library holds until exit.  Limits:
+ * n_dm <= SPD_STATIC_MAX_ROWS, else SPD_ERR_INVALID_ARG with a message naming the limit (n_t is unlimited:
+ * rows are cut into at most SPD_STATIC_MAX_PARTIALS / n_dm parts).  All calls on a device share that one
+ * array: it keeps the last call's contents (what must start at zero is cleared by the call itself), and two
+ * calls that overlap on the GPU - different streams without an ordering between them - race on it; serialise
+ * them (one stream, or events).  Asynchronous; SPD_ERR_UNSUPPORTED_DEVICE without an sm_100 device.
+ */
+#define SPD_STATIC_MAX_ROWS 8192
+#define SPD_STATIC_MAX_PARTIALS 65536
+#define SPD_STATIC_SCRATCH_BYTES (24 * SPD_STATIC_MAX_PARTIALS + 24 * SPD_STATIC_MAX_ROWS)
+int spd_row_stats_static(const float* plane, int64_t n_dm, int64_t n_t, float clip_sigma,
+                         int32_t n_reject_passes, float* mean, float* sigma, void* cuda_stream);
+
+/*
  * spd_row_stats_converge - spd_row_stats "repeated until convergence": rejection
  * passes go on, per DM row, until one changes neither the mean nor sigma by more than
  * rel_tol * sigma(previous pass), or max_reject_passes are done (1 <= max_reject_passes <= 64,

@@ -14,7 +14,8 @@ from .binding import (  # noqa: F401
     spd_separation_generate, spd_plan_create_grid, spd_width_sigma, spd_run_sigma_w,
     candidates_to_numpy, load, spd_destroy, spd_find_candidates, spd_last_error_string,
     spd_plan_create, spd_plan_destroy, spd_plan_get_info, spd_plan_get_widths, spd_run,
-    spd_run_flagged, spd_find_candidates_flagged, spd_row_stats,
+    spd_run_flagged, spd_find_candidates_flagged, spd_row_stats, spd_row_stats_static,
+    SPD_STATIC_MAX_ROWS, SPD_STATIC_MAX_PARTIALS,
     spd_run_host, spd_version, spd_width_set_generate,
 )
 
@@ -26,6 +27,7 @@ __all__ = [
     "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
     "spd_width_set_generate", "spd_plan_create", "spd_plan_destroy", "spd_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
-    "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats",
+    "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats", "spd_row_stats_static",
+    "SPD_STATIC_MAX_ROWS", "SPD_STATIC_MAX_PARTIALS",
     "spd_run_host", "spd_last_error_string", "spd_version", "candidates_to_numpy",
 ]

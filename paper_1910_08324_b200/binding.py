@@ -42,7 +42,7 @@ EXPORTS = (
     "spd_run_host", "spd_last_error_string", "spd_version",
     "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
     "spd_destroy", "spd_plan_set_option", "spd_row_stats_converge", "spd_cluster_candidates",
-    "spd_run_host_candidates", "spd_plan_create_grid_ex",
+    "spd_run_host_candidates", "spd_plan_create_grid_ex", "spd_row_stats_static",
 )
 
 
@@ -134,6 +134,8 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_destroy.argtypes = [_vp]
     lib.spd_plan_set_option.restype = ctypes.c_int
     lib.spd_plan_set_option.argtypes = [_vp, _i32, _i64]
+    lib.spd_row_stats_static.restype = ctypes.c_int
+    lib.spd_row_stats_static.argtypes = [_vp, _i64, _i64, ctypes.c_float, _i32, _vp, _vp, _vp]
     lib.spd_row_stats_converge.restype = ctypes.c_int
     lib.spd_row_stats_converge.argtypes = [_vp, _vp, ctypes.c_float, _i32, ctypes.c_float, _vp, _vp, _vp, _vp]
     lib.spd_cluster_candidates.restype = ctypes.c_int
@@ -349,6 +351,23 @@ def spd_row_stats(plan: int, plane, clip_sigma: float = 0.0, n_reject_passes: in
         _vp(plan), _dev_ptr(plane, torch.float32, n, "plane"), ctypes.c_float(clip_sigma), int(n_reject_passes),
         _dev_ptr(mean, torch.float32, info["n_dm"], "mean"), _dev_ptr(sigma, torch.float32, info["n_dm"], "sigma"),
         _vp(_stream_handle(stream))))
+    return mean, sigma
+
+
+SPD_STATIC_MAX_ROWS = 8192
+SPD_STATIC_MAX_PARTIALS = 65536
+
+
+def spd_row_stats_static(plane, mean, sigma, clip_sigma: float = 0.0, n_reject_passes: int = 0, stream=None):
+    """spd_row_stats without a plan and without any allocation (static device scratch, n_dm <= 8192): the
+    caller passes every buffer - ``plane`` [n_dm][n_t], ``mean`` and ``sigma`` [n_dm], float32 device tensors.
+    Calls that overlap on the GPU race on the shared scratch (include/spd.h)."""
+    import torch
+    n_dm, n_t = int(plane.shape[0]), int(plane.shape[1])
+    _check(load().spd_row_stats_static(
+        _dev_ptr(plane, torch.float32, n_dm * n_t, "plane"), n_dm, n_t, ctypes.c_float(clip_sigma),
+        int(n_reject_passes), _dev_ptr(mean, torch.float32, n_dm, "mean"),
+        _dev_ptr(sigma, torch.float32, n_dm, "sigma"), _vp(_stream_handle(stream))))
     return mean, sigma
 
 

@@ -25,6 +25,7 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "spd_internal.h"
 
@@ -236,4 +237,140 @@ int stats_run(const spd_plan* plan, const float* plane, float clip, int n_iter, 
     return SPD_OK;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// spd_row_stats_static: the same two kernels with their scratch (partial moments per (row, part), per-row state)
+// in a file-scope device array instead of a plan workspace, for callers that may not allocate (CUDA graph
+// capture, serving loops).  No plan, no cudaMalloc / cudaFree, nothing but kernel launches and one memset on
+// the caller's stream.
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr long long kStaticMaxRows = SPD_STATIC_MAX_ROWS;          // RowState entries
+constexpr long long kStaticMaxPartials = SPD_STATIC_MAX_PARTIALS;  // Moments entries (rows x parts)
+constexpr size_t kStaticStateOff = sizeof(Moments) * static_cast<size_t>(kStaticMaxPartials);
+constexpr size_t kStaticBytes = kStaticStateOff + sizeof(RowState) * static_cast<size_t>(kStaticMaxRows);
+static_assert(kStaticBytes == SPD_STATIC_SCRATCH_BYTES, "spd.h states the size of the scratch");
+static_assert(kStaticStateOff % 256 == 0, "the per-row state starts on a 256-byte boundary");
+static_assert(kStaticBytes <= (2u << 20), "the static scratch is meant to stay modest (2 MiB)");
+
+// Held by every device that loads the library, until exit.  In host code this NAME is a host-side stand-in,
+// not a device address: host code takes the address with cudaGetSymbolAddress (static_scratch below).
+static __device__ __align__(256) unsigned char g_stats_scratch[kStaticBytes];
+
+constexpr int kMaxDevices = 64;
+struct StaticSlot {
+    bool ready = false;
+    unsigned char* base = nullptr;  // device address of g_stats_scratch on this device
+    int sm_count = 0;
+};
+StaticSlot g_static_slot[kMaxDevices];
+std::mutex g_static_mutex;
+
+// Set-up, once per device, with that device current: device check (sm_100 only, as every other entry point),
+// SM count, device address of the scratch array.
+int static_scratch(StaticSlot* out) {
+    int device = -1;
+    cudaError_t e = cudaGetDevice(&device);
+    if (e != cudaSuccess) {
+        set_error("no usable CUDA device: %s (this library has no CPU fallback)", cudaGetErrorString(e));
+        cudaGetLastError();
+        return SPD_ERR_UNSUPPORTED_DEVICE;
+    }
+    if (device < 0 || device >= kMaxDevices) {
+        set_error("spd_row_stats_static: device ordinal %d outside 0 .. %d", device, kMaxDevices - 1);
+        return SPD_ERR_UNSUPPORTED_DEVICE;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticSlot& slot = g_static_slot[device];
+    if (!slot.ready) {
+        int major = 0, sms = 0;
+        if ((e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device)) != cudaSuccess ||
+            (e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) {
+            set_error("cannot query the CUDA device: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+            return SPD_ERR_UNSUPPORTED_DEVICE;
+        }
+        if (major != 10) {
+            set_error("device compute capability %d.x is not supported: this library is built for sm_100a only", major);
+            return SPD_ERR_UNSUPPORTED_DEVICE;
+        }
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_stats_scratch);
+        if (e != cudaSuccess || !ptr) {
+            set_error("spd_row_stats_static: cudaGetSymbolAddress of the scratch array failed: %s",
+                      cudaGetErrorString(e));
+            cudaGetLastError();
+            return SPD_ERR_CUDA;
+        }
+        slot.base = static_cast<unsigned char*>(ptr);
+        slot.sm_count = sms;
+        slot.ready = true;
+    }
+    *out = slot;
+    return SPD_OK;
+}
+
+}  // namespace
 }  // namespace spd
+
+extern "C" int spd_row_stats_static(const float* plane, int64_t n_dm, int64_t n_t, float clip_sigma,
+                                    int32_t n_reject_passes, float* mean, float* sigma, void* cuda_stream) {
+    using namespace spd;
+    if (!plane || !mean || !sigma) {
+        set_error("spd_row_stats_static: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (n_dm < 1 || n_t < 1) {
+        set_error("spd_row_stats_static: need n_dm >= 1 and n_t >= 1 (got %lld, %lld)", static_cast<long long>(n_dm),
+                  static_cast<long long>(n_t));
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (n_reject_passes < 0 || n_reject_passes > 64 || (n_reject_passes > 0 && !(clip_sigma > 0.0f))) {
+        set_error("spd_row_stats_static: need 0 <= n_reject_passes <= 64 and clip_sigma > 0 when rejecting (got %d, %g)",
+                  n_reject_passes, static_cast<double>(clip_sigma));
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (n_dm > kStaticMaxRows) {
+        set_error("spd_row_stats_static: n_dm = %lld exceeds the static scratch (SPD_STATIC_MAX_ROWS = %lld rows); "
+                  "use spd_row_stats with a plan",
+                  static_cast<long long>(n_dm), kStaticMaxRows);
+        return SPD_ERR_INVALID_ARG;
+    }
+    StaticSlot slot;
+    const int rc = static_scratch(&slot);
+    if (rc != SPD_OK) return rc;
+
+    // the work split of stats_configure (enough blocks to fill the machine, parts a multiple of 1024 samples),
+    // with the parts per row also bounded by the scratch
+    const long long want = 16ll * slot.sm_count;
+    long long parts = std::max<long long>(1, std::min<long long>(256, (want + n_dm - 1) / n_dm));
+    parts = std::max<long long>(1, std::min<long long>(parts, kStaticMaxPartials / n_dm));
+    long long part = (n_t + parts - 1) / parts;
+    part = (part + 1023) / 1024 * 1024;
+    parts = (n_t + part - 1) / part;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Moments* const ws = reinterpret_cast<Moments*>(slot.base);
+    RowState* const state = reinterpret_cast<RowState*>(slot.base + kStaticStateOff);
+    // the array keeps the last call's contents: the per-row state starts at zero (not converged, no pass done);
+    // the partial moments are all written by pass 0 before they are read
+    cudaError_t e = cudaMemsetAsync(state, 0, sizeof(RowState) * static_cast<size_t>(n_dm), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "clearing the static statistics state");
+    const unsigned grid = static_cast<unsigned>(n_dm * parts);  // <= kStaticMaxPartials
+    const bool vec = n_t % 4 == 0 && (reinterpret_cast<uintptr_t>(plane) & 15u) == 0;
+    const unsigned fin_grid = static_cast<unsigned>((n_dm + 127) / 128);
+    for (int pass = 0; pass <= n_reject_passes; ++pass) {
+        const int clip_on = pass > 0;
+        if (vec)
+            row_moments_kernel<true><<<grid, kStatThreads, 0, stream>>>(plane, n_t, part, static_cast<int>(parts), clip_on,
+                                                                        clip_sigma, mean, sigma, state, ws);
+        else
+            row_moments_kernel<false><<<grid, kStatThreads, 0, stream>>>(plane, n_t, part, static_cast<int>(parts),
+                                                                         clip_on, clip_sigma, mean, sigma, state, ws);
+        row_moments_finish_kernel<<<fin_grid, 128, 0, stream>>>(ws, static_cast<int>(parts), n_dm, pass, -1.0f, state,
+                                                                mean, sigma, nullptr);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "launching the statistics kernels (static scratch)");
+    return SPD_OK;
+}
