@@ -18,6 +18,8 @@ from .core import (  # noqa: F401
     spd_direct_sw,
     width_sigma,
     spd_grid,
+    spd_grid_iter,
+    grid_iterations,
     spd_grid_sw,
     spd_prefix,
 )

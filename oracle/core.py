@@ -41,6 +41,8 @@ def _load() -> ctypes.CDLL:
         lib.oracle_num_threads.restype = ctypes.c_int
         lib.oracle_spd_direct.restype = None
         lib.oracle_spd_direct.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
+        lib.oracle_spd_grid_iter.restype = None
+        lib.oracle_spd_grid_iter.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _vp, _i32, _i32, _vp, _vp, _vp]
         lib.oracle_spd_grid.restype = None
         lib.oracle_spd_grid.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _vp, _vp, _vp]
         lib.oracle_width_sigma.restype = None
@@ -127,6 +129,40 @@ def spd_grid(x, mean, sigma, widths, seps, t0: int = 0, t1: Optional[int] = None
     _load().oracle_spd_grid(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
                             w.ctypes.data, sp.ctypes.data, int(w.size), t0, t1,
                             snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
+    return snr, idx, sec
+
+
+def grid_iterations(seps):
+    """The iterations of a grid: runs [kb, ke) of consecutive widths that share a separation."""
+    sp = [int(v) for v in seps]
+    out, kb = [], 0
+    for k in range(1, len(sp) + 1):
+        if k == len(sp) or sp[k] != sp[kb]:
+            out.append((kb, k))
+            kb = k
+    return out
+
+
+def spd_grid_iter(x, mean, sigma, widths, seps, kb: int, ke: int
+                  ) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """The output of one iteration (eq. 12, PAPER.md:183): widths[kb:ke] share the separation s = seps[kb];
+    point m is sample s * m.  Returns (snr, width_idx, second), each [n_dm, ceil(n_t / s)]; width_idx is the
+    index in ``widths``."""
+    x = _plane(x)
+    n_dm, n_t = x.shape
+    w = np.ascontiguousarray([int(v) for v in widths], dtype=np.int32)
+    sp = np.ascontiguousarray([int(v) for v in seps], dtype=np.int32)
+    kb, ke = int(kb), int(ke)
+    assert w.size == sp.size and 0 <= kb < ke <= w.size and np.all(np.diff(w) > 0) and np.all(sp[kb:ke] == sp[kb])
+    s = int(sp[kb])
+    n_pts = (n_t + s - 1) // s
+    mu, sg = _stats(mean, n_dm), _stats(sigma, n_dm)
+    snr = np.empty((n_dm, n_pts), dtype=np.float64)
+    idx = np.empty((n_dm, n_pts), dtype=np.int32)
+    sec = np.empty((n_dm, n_pts), dtype=np.float64)
+    _load().oracle_spd_grid_iter(x.ctypes.data, n_dm, n_t, mu.ctypes.data, sg.ctypes.data,
+                                 w.ctypes.data, sp.ctypes.data, kb, ke,
+                                 snr.ctypes.data, idx.ctypes.data, sec.ctypes.data)
     return snr, idx, sec
 
 

@@ -29,6 +29,8 @@
  *                        oracle_spd_direct in tests (<= 1e-9).
  *   oracle_spd_grid    : oracle_spd_direct with a boxcar separation per width (the
  *                        paper's decimated grids, merged into one plane; reading A16).
+ *   oracle_spd_grid_iter: the output separated by iteration (eq. 12): one decimated plane per
+ *                        run of widths that share a separation, direct summation.
  *   oracle_width_sigma : standard deviation per width from power-of-two decimations,
  *                        interpolated (reading A17); oracle_spd_direct_sw uses it.
  *   oracle_snr_of_width: SNR_L[n] for one width at listed samples (near-tie checks).
@@ -146,6 +148,55 @@ void oracle_spd_grid(const float* x, int64_t n_dm, int64_t n_t,
                 }
             }
             const int64_t o = d * span + (n - t0);
+            out_snr[o] = best;
+            out_width[o] = idx;
+            if (out_second) out_second[o] = second;
+        }
+    }
+}
+
+/* Output separated by iteration, eq. (12): "the output for ith iteration is
+ * Y^i[n] = max_{L in B^i} SNR(X^i_L[n])", with "the width of the boxcar which produced the highest SNR
+ * value W^i"; Y^i has N / D^(i) samples.  An iteration here is a run of consecutive
+ * widths [kb, ke) of a grid plan that share one separation s = seps[kb] (BoxDIT iteration i: s = D^(i),
+ * widths of eq. 14; DIT: one width per iteration; IGRID: the widths of one step).  Point m of the
+ * iteration's plane is sample n = s m of the row, m < ceil(n_t / s):
+ *     Y^i[m] = max over k in [kb, ke) with n + L_k <= n_t of (X_{L_k}[n] - L_k mu) / (sqrt(L_k) sigma),
+ * X by direct summation (eq. 2), W^i[m] = that k (index in the plan's width set; -1 and -inf where no
+ * width of the iteration fits the row, reading A3), strict '>' in ascending order (A4).
+ * out_* are [n_dm][n_pts], n_pts = ceil(n_t / s).
+ * Pins (tests/test_oracle_pins.py): a literal transcription of Alg. 1 with eq. (13)'s shifted decimation
+ * and eq. (15) (x^{i+1}, X^i carried from iteration to iteration) gives the same planes; the maximum over
+ * the iterations at a sample is oracle_spd_grid's merged plane (reading A16); the constant-offset closed
+ * form on the example of PAPER.md:201 (widths 1..4 at every point, 6, 8, 10, 12 at every second). */
+void oracle_spd_grid_iter(const float* x, int64_t n_dm, int64_t n_t,
+                          const double* mean, const double* sigma,
+                          const int32_t* widths, const int32_t* seps, int32_t kb, int32_t ke,
+                          double* out_snr, int32_t* out_width, double* out_second) {
+    const int64_t s = seps[kb];
+    const int64_t n_pts = (n_t + s - 1) / s;
+#pragma omp parallel for collapse(2) schedule(dynamic, 256)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        for (int64_t m = 0; m < n_pts; ++m) {
+            const float* row = x + d * n_t;
+            const int64_t n = s * m;
+            double best = -INFINITY, second = -INFINITY;
+            int32_t idx = -1;
+            for (int32_t k = kb; k < ke; ++k) {
+                const int64_t L = widths[k];
+                if (n + L > n_t) break;                       /* valid windows only (A3) */
+                double X = 0.0;
+                for (int64_t j = 0; j < L; ++j) X += (double)row[n + j];      /* eq. (2) */
+                const double snr = (X - (double)L * mean[d]) / (sqrt((double)L) * sigma[d]); /* eq. (4),(5) */
+                if (snr > best) {                              /* strict '>' (A4) */
+                    second = best;
+                    best = snr;
+                    idx = k;
+                } else if (snr > second) {
+                    second = snr;
+                }
+            }
+            const int64_t o = d * n_pts + m;
             out_snr[o] = best;
             out_width[o] = idx;
             if (out_second) out_second[o] = second;

@@ -710,3 +710,127 @@ def test_cluster_random_planes_match_window_scan(oracle_lib):
         cnt, c_dm, c_t, c_snr, c_w = oracle_lib.find_candidates(snr.astype(np.float32), wid, 2.0)
         keep = oracle_lib.cluster_candidates(snr.astype(np.float32), widths, c_dm, c_t, c_w, R)
         assert cnt > 50 and np.array_equal(keep, _cluster_brute(snr, widths, c_dm, c_t, c_w, R))
+
+
+# --- output separated by iteration (eq. 12; Alg. 1, eq. 13-15) -----------------
+
+def _boxdit_literal(x, mu, sg, l_max, n_iter):
+    """Alg. 1 as printed, D = 2, in double: iteration i works on the decimated series x^i
+    and on X^{i-1}, the longest boxcar of the iteration before;
+        eq. (15)  X_L[n] = X^{i-1}[n] + sum_{j < m} x^i[n_s + j],  n_s = n / D^(i),  L = L_MAX^{i-1} + D^(i) m (eq. 14)
+        eq. (13)  x^{i+1}[n - L_max / D] = x^i[D n] + x^i[D n + 1]
+    Positions are kept in the iteration's own index q (sample n = 2^i q of the row).  Returns, per iteration,
+    (Y^i, m^i) over the points whose windows fit the row, with m the winning 1-based position in the
+    iteration's width list, plus the number of points."""
+    xi = np.asarray(x, dtype=np.float64) - mu          # x^0, mean removed (eq. 4's numerator, per sample)
+    n_t = xi.size
+    X_prev = np.zeros(n_t)                             # X^{-1} = 0 at the points of iteration 0
+    L_MAX_prev = 0
+    out = []
+    for i in range(n_iter):
+        step = 1 << i
+        n_pts = (n_t + step - 1) // step
+        Y = np.full(n_pts, -np.inf)
+        M = np.full(n_pts, -1, dtype=np.int64)
+        X_long = np.zeros(n_pts)
+        for q in range(n_pts):
+            n = q * step
+            acc = X_prev[q]
+            for m in range(1, l_max + 1):
+                L = L_MAX_prev + step * m                               # eq. (14)
+                if n + L > n_t:
+                    break
+                acc = acc + xi[q + m - 1]                                # eq. (15): one more element of x^i
+                snr = acc / (math.sqrt(L) * sg)                          # eq. (4) with eq. (5)
+                if snr > Y[q]:
+                    Y[q], M[q] = snr, m
+                if m == l_max:
+                    X_long[q] = acc
+        out.append((Y, M, n_pts))
+        # eq. (13): x^{i+1}[q'] = x^i[2 q' + l_max] + x^i[2 q' + l_max + 1]; X^i is handed on at every second point
+        n_next = (n_t + 2 * step - 1) // (2 * step)
+        nxt = np.zeros(n_next + l_max + 2)
+        for qn in range(nxt.size):
+            a, b = 2 * qn + l_max, 2 * qn + l_max + 1
+            nxt[qn] = (xi[a] if a < xi.size else 0.0) + (xi[b] if b < xi.size else 0.0)
+        xi = nxt
+        X_prev = X_long[::2].copy()
+        L_MAX_prev += step * l_max
+    return out
+
+
+@pytest.mark.parametrize("l_max,n_iter,n_t", [(4, 4, 203), (8, 3, 260), (4, 3, 64), (2, 5, 117)])
+def test_grid_iter_equals_the_literal_boxdit_algorithm(oracle_lib, l_max, n_iter, n_t):
+    """oracle_spd_grid_iter (direct summation of every window of an iteration) against Alg. 1 run step by step
+    with eq. (13)'s shifted decimation and eq. (15): the same Y^i, W^i at every point of every iteration."""
+    rng = np.random.default_rng(1000 + l_max + n_t)
+    x = (rng.standard_normal(n_t) * 1.7 + 0.4).astype(np.float32)
+    x[n_t // 3: n_t // 3 + 3 * l_max] += np.float32(2.0)
+    mu, sg = 0.4, 1.7
+    widths = [((1 << i) - 1) * l_max + (m << i) for i in range(n_iter) for m in range(1, l_max + 1)]
+    seps = [1 << i for i in range(n_iter) for _ in range(l_max)]
+    assert widths == F.widths_boxdit(l_max, widths[-1])
+    its = oracle_lib.grid_iterations(seps)
+    assert its == [(i * l_max, (i + 1) * l_max) for i in range(n_iter)]
+    lit = _boxdit_literal(x, mu, sg, l_max, n_iter)
+    for i, (kb, ke) in enumerate(its):
+        snr, idx, _ = oracle_lib.spd_grid_iter(x, mu, sg, widths, seps, kb, ke)
+        Y, M, n_pts = lit[i]
+        assert snr.shape == (1, n_pts)
+        fit = M >= 0
+        assert np.array_equal(idx[0] >= 0, fit)
+        assert np.array_equal(idx[0][fit], kb + M[fit] - 1)
+        assert np.allclose(snr[0][fit], Y[fit], rtol=1e-12, atol=1e-12)
+        assert np.all(np.isneginf(snr[0][~fit]))
+
+
+def test_grid_iter_planes_merge_into_the_grid_plane(oracle_lib):
+    """Reading A16: the merged plane of oracle_spd_grid is, at every sample, the maximum over the iterations
+    whose grid holds the sample (ties: the earlier iteration, i.e. the smaller width) - for the BoxDIT, DIT and
+    IGRID-layer grids."""
+    rng = np.random.default_rng(77)
+    x = rng.standard_normal((2, 333)).astype(np.float32)
+    cases = [
+        (F.widths_boxdit(8, 56), F.boxdit_separation(8)),
+        ([1 << k for k in range(7)], lambda L: L),
+        (F.widths_igrid(1, 64), F.igrid_separation(4)),
+    ]
+    for widths, sepf in cases:
+        seps = [sepf(L) for L in widths]
+        ref_snr, ref_idx, _ = oracle_lib.spd_grid(x, 0.2, 1.1, widths, seps)
+        snr = np.full(x.shape, -np.inf)
+        idx = np.full(x.shape, -1, dtype=np.int32)
+        for kb, ke in oracle_lib.grid_iterations(seps):
+            s = seps[kb]
+            y, w, _ = oracle_lib.spd_grid_iter(x, 0.2, 1.1, widths, seps, kb, ke)
+            assert y.shape[1] == (x.shape[1] + s - 1) // s
+            better = y > snr[:, ::s]
+            snr[:, ::s] = np.where(better, y, snr[:, ::s])
+            idx[:, ::s] = np.where(better, w, idx[:, ::s])
+        assert np.array_equal(snr, ref_snr) and np.array_equal(idx, ref_idx)
+
+
+def test_grid_iter_paper_example_closed_form(oracle_lib):
+    """PAPER.md:201 ("boxcar filters of width L = 1, 2, 3, 4 are calculated at every point; after decimation,
+    boxcar filters of width L = 6, 8, 10, 12 are calculated at every second point and so on") on a constant
+    offset a: SNR_L = a sqrt(L) / sigma, so every iteration's winner is its largest width that fits the row."""
+    n_t, mu, sg, a = 131, 0.5, 2.0, 1.5
+    widths = F.widths_boxdit(4, 28)
+    seps = [F.boxdit_separation(4)(L) for L in widths]
+    x = np.full(n_t, mu + a, dtype=np.float32)
+    for i, (kb, ke) in enumerate(oracle_lib.grid_iterations(seps)):
+        s = 1 << i
+        snr, idx, sec = oracle_lib.spd_grid_iter(x, mu, sg, widths, seps, kb, ke)
+        assert snr.shape == (1, (n_t + s - 1) // s)
+        for m in range(snr.shape[1]):
+            ok = [k for k in range(kb, ke) if s * m + widths[k] <= n_t]
+            if not ok:
+                assert idx[0][m] == -1 and np.isneginf(snr[0][m])
+                continue
+            assert idx[0][m] == ok[-1]
+            assert snr[0][m] == pytest.approx(a * math.sqrt(widths[ok[-1]]) / sg, rel=1e-12)
+            if len(ok) > 1:
+                assert sec[0][m] == pytest.approx(a * math.sqrt(widths[ok[-2]]) / sg, rel=1e-12)
+    # iteration 1 holds 6, 8, 10, 12 at samples 0, 2, 4, ...; its point 3 is sample 6
+    y1, w1, _ = oracle_lib.spd_grid_iter(x, mu, sg, widths, seps, 4, 8)
+    assert w1[0][3] == 7 and y1.shape[1] == 66
