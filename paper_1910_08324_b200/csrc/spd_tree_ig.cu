@@ -362,9 +362,23 @@ __global__ void __launch_bounds__(T, ig_blocks_per_sm(K, SW)) spd_tree_ig_kernel
 
     for (int c = c_top - 1; c >= first_fast; --c) {
         const long long n0 = static_cast<long long>(c) * C;
-        for (int i = tid; i < C + 8; i += T) {
-            const long long n = n0 + i;
-            stages[i] = n < n_t ? __ldg(row + n) : cx.mu;
+        {
+            // n0 and n_t are multiples of 4: a float4 lies entirely inside or outside the row.  All of a thread's
+            // 128-bit loads are issued before the first store (one memory latency per step, not one per element).
+            constexpr int NV = (C + 8) / 4, NJ = (NV + T - 1) / T;
+            const float4* const row4 = reinterpret_cast<const float4*>(row + n0);
+            const float4 fill = make_float4(cx.mu, cx.mu, cx.mu, cx.mu);
+            float4 v[NJ];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const int i = tid + T * j;
+                v[j] = (i < NV && n0 + 4ll * i < n_t) ? __ldg(row4 + i) : fill;
+            }
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const int i = tid + T * j;
+                if (i < NV) reinterpret_cast<float4*>(stages)[i] = v[j];
+            }
         }
         __syncthreads();
         cx.n0 = n0;
