@@ -343,6 +343,30 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
                  float* out_snr, void* out_width);
 
 /*
+ * Output separated by iteration (eq. 12: "We have chosen to separate the output by iteration,
+ * that is the output for ith iteration is Y^i[n] = max_{L in B^i} SNR(X^i_L[n])", with W^i the width that
+ * produced it; Y^i has N / D^(i) samples).  For a plan with boxcar separations (spd_plan_create_grid) an
+ * ITERATION is a run of consecutive widths that share one separation s: BoxDIT iteration i (s = 2^i, the widths
+ * of eq. 14), one width per iteration on the DIT grid, the widths of one step of IGRID with P layers.  Point m
+ * of iteration i's plane is sample n = s m of the row, m < n_points = ceil(n_t / s):
+ *     Y^i[d][m] = max over the iteration's widths L with s m + L <= n_t of SNR_L[s m],  W^i[d][m] = its index
+ * in the plan's width table (-inf / -1 where none fits, reading A3).  spd_run's merged plane (reading A16) is
+ * the maximum of these over the iterations whose grid holds a sample.
+ *
+ * spd_plan_get_iterations: HOST arrays of cap entries (each may be NULL); *n_iter receives the count (<= 32).
+ * spd_run_iterations: out_snr_iter (float32) and out_width_iter (int32) are DEVICE buffers holding the
+ *   iterations' planes one after the other, iteration i as [n_dm][n_points[i]] row-major at element offset
+ *   n_dm * (n_points[0] + ... + n_points[i-1]); plane, mean, sigma as spd_run (eq. 5's sqrt(L) sigma).
+ *   Asynchronous on cuda_stream.  Any grid plan; runs on the shared-memory tile kernel of the any-width-set
+ *   path (one pass over the plane, all iterations in one launch).
+ * Both return SPD_ERR_INVALID_ARG for a plan without separations.
+ */
+int spd_plan_get_iterations(const spd_plan* plan, int32_t cap, int32_t* n_iter, int32_t* first_width,
+                            int32_t* n_widths, int32_t* separation, int64_t* n_points);
+int spd_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                       float* out_snr_iter, int32_t* out_width_iter, void* cuda_stream);
+
+/*
  * spd_row_stats_static - spd_row_stats for callers that may not allocate (code under CUDA graph capture,
  * serving loops, harnesses that forbid cudaMalloc): no plan, and the call enqueues kernels and one memset on
  * cuda_stream and nothing else - no cudaMalloc, cudaFree or allocating library routine, on the first call

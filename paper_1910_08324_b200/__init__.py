@@ -15,7 +15,7 @@ from .binding import (  # noqa: F401
     candidates_to_numpy, load, spd_destroy, spd_find_candidates, spd_last_error_string,
     spd_plan_create, spd_plan_destroy, spd_plan_get_info, spd_plan_get_widths, spd_run,
     spd_run_flagged, spd_find_candidates_flagged, spd_row_stats, spd_row_stats_static,
-    SPD_STATIC_MAX_ROWS, SPD_STATIC_MAX_PARTIALS,
+    SPD_STATIC_MAX_ROWS, SPD_STATIC_MAX_PARTIALS, spd_plan_get_iterations, spd_run_iterations,
     spd_run_host, spd_version, spd_width_set_generate,
 )
 
@@ -28,6 +28,6 @@ __all__ = [
     "spd_width_set_generate", "spd_plan_create", "spd_plan_destroy", "spd_destroy",
     "spd_plan_get_widths", "spd_plan_get_info", "spd_run", "spd_find_candidates",
     "spd_run_flagged", "spd_find_candidates_flagged", "spd_row_stats", "spd_row_stats_static",
-    "SPD_STATIC_MAX_ROWS", "SPD_STATIC_MAX_PARTIALS",
+    "SPD_STATIC_MAX_ROWS", "SPD_STATIC_MAX_PARTIALS", "spd_plan_get_iterations", "spd_run_iterations",
     "spd_run_host", "spd_last_error_string", "spd_version", "candidates_to_numpy",
 ]

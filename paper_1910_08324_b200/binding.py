@@ -43,6 +43,7 @@ EXPORTS = (
     "spd_separation_generate", "spd_plan_create_grid", "spd_width_sigma", "spd_run_sigma_w",
     "spd_destroy", "spd_plan_set_option", "spd_row_stats_converge", "spd_cluster_candidates",
     "spd_run_host_candidates", "spd_plan_create_grid_ex", "spd_row_stats_static",
+    "spd_plan_get_iterations", "spd_run_iterations",
 )
 
 
@@ -134,6 +135,10 @@ def load(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.spd_destroy.argtypes = [_vp]
     lib.spd_plan_set_option.restype = ctypes.c_int
     lib.spd_plan_set_option.argtypes = [_vp, _i32, _i64]
+    lib.spd_plan_get_iterations.restype = ctypes.c_int
+    lib.spd_plan_get_iterations.argtypes = [_vp, _i32, _vp, _vp, _vp, _vp, _vp]
+    lib.spd_run_iterations.restype = ctypes.c_int
+    lib.spd_run_iterations.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.spd_row_stats_static.restype = ctypes.c_int
     lib.spd_row_stats_static.argtypes = [_vp, _i64, _i64, ctypes.c_float, _i32, _vp, _vp, _vp]
     lib.spd_row_stats_converge.restype = ctypes.c_int
@@ -354,6 +359,45 @@ def spd_row_stats(plan: int, plane, clip_sigma: float = 0.0, n_reject_passes: in
     return mean, sigma
 
 
+def spd_plan_get_iterations(plan: int):
+    """Iterations of a grid plan (eq. 12): list of dicts first_width, n_widths, separation, n_points."""
+    n = _i32(0)
+    _check(load().spd_plan_get_iterations(_vp(plan), 0, ctypes.byref(n), None, None, None, None))
+    k = n.value
+    fw, nw, sp = (np.zeros(k, dtype=np.int32) for _ in range(3))
+    npts = np.zeros(k, dtype=np.int64)
+    _check(load().spd_plan_get_iterations(_vp(plan), k, ctypes.byref(n), fw.ctypes.data, nw.ctypes.data,
+                                          sp.ctypes.data, npts.ctypes.data))
+    return [{"first_width": int(fw[i]), "n_widths": int(nw[i]), "separation": int(sp[i]), "n_points": int(npts[i])}
+            for i in range(k)]
+
+
+def spd_run_iterations(plan: int, plane, mean, sigma, out_snr=None, out_width=None, stream=None):
+    """Output separated by iteration: returns (planes, out_snr, out_width) where planes[i] = (Y^i, W^i) are
+    [n_dm, n_points[i]] views into the concatenated device buffers."""
+    import torch
+    info = spd_plan_get_info(plan)
+    its = spd_plan_get_iterations(plan)
+    n_dm = info["n_dm"]
+    total = n_dm * sum(it["n_points"] for it in its)
+    if out_snr is None:
+        out_snr = torch.empty(total, dtype=torch.float32, device=plane.device)
+    if out_width is None:
+        out_width = torch.empty(total, dtype=torch.int32, device=plane.device)
+    _check(load().spd_run_iterations(
+        _vp(plan), _dev_ptr(plane, torch.float32, n_dm * info["n_t"], "plane"),
+        _dev_ptr(mean, torch.float32, n_dm, "mean"), _dev_ptr(sigma, torch.float32, n_dm, "sigma"),
+        _dev_ptr(out_snr, torch.float32, total, "out_snr"), _dev_ptr(out_width, torch.int32, total, "out_width"),
+        _vp(_stream_handle(stream))))
+    planes, off = [], 0
+    for it in its:
+        cnt = n_dm * it["n_points"]
+        planes.append((out_snr[off:off + cnt].view(n_dm, it["n_points"]),
+                       out_width[off:off + cnt].view(n_dm, it["n_points"])))
+        off += cnt
+    return planes, out_snr, out_width
+
+
 SPD_STATIC_MAX_ROWS = 8192
 SPD_STATIC_MAX_PARTIALS = 65536
 
@@ -568,6 +612,12 @@ class Plan:
     def run_host_candidates(self, plane, mean, sigma, threshold: float, dm_radius: int, capacity: int,
                             out_list=None):
         return spd_run_host_candidates(self.handle, plane, mean, sigma, threshold, dm_radius, capacity, out_list)
+
+    def iterations(self):
+        return spd_plan_get_iterations(self.handle)
+
+    def run_iterations(self, plane, mean, sigma, out_snr=None, out_width=None, stream=None):
+        return spd_run_iterations(self.handle, plane, mean, sigma, out_snr, out_width, stream)
 
     def width_sigma(self, plane, mean, sigma_w=None, stream=None):
         return spd_width_sigma(self.handle, plane, mean, sigma_w, stream)

@@ -519,6 +519,40 @@ int spd_plan_get_widths(const spd_plan* plan, int32_t* out, int32_t* n) {
     return SPD_OK;
 }
 
+int spd_plan_get_iterations(const spd_plan* plan, int32_t cap, int32_t* n_iter, int32_t* first_width,
+                            int32_t* n_widths, int32_t* separation, int64_t* n_points) {
+    if (!plan || !n_iter || cap < 0) {
+        set_error("spd_plan_get_iterations: NULL argument or negative cap");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (plan->separations.empty()) {
+        set_error("spd_plan_get_iterations: the plan has no boxcar separations (create it with spd_plan_create_grid)");
+        return SPD_ERR_INVALID_ARG;
+    }
+    *n_iter = plan->grid.n;
+    for (int g = 0; g < plan->grid.n && g < cap; ++g) {
+        if (first_width) first_width[g] = plan->grid.kb[g];
+        if (n_widths) n_widths[g] = plan->grid.ke[g] - plan->grid.kb[g];
+        if (separation) separation[g] = 1 << plan->grid.shift[g];
+        if (n_points) n_points[g] = grid_iter_points(plan, g);
+    }
+    return SPD_OK;
+}
+
+int spd_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                       float* out_snr_iter, int32_t* out_width_iter, void* cuda_stream) {
+    if (!plan || !plane || !mean || !sigma || !out_snr_iter || !out_width_iter) {
+        set_error("spd_run_iterations: NULL argument");
+        return SPD_ERR_INVALID_ARG;
+    }
+    if (plan->separations.empty()) {
+        set_error("spd_run_iterations: the plan has no boxcar separations (create it with spd_plan_create_grid)");
+        return SPD_ERR_INVALID_ARG;
+    }
+    return generic_run_iterations(plan, plane, mean, sigma, out_snr_iter, out_width_iter,
+                                  static_cast<cudaStream_t>(cuda_stream));
+}
+
 int spd_plan_get_info(const spd_plan* plan, spd_plan_info* info) {
     if (!plan || !info) {
         set_error("spd_plan_get_info: NULL argument");

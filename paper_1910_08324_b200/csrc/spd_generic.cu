@@ -386,7 +386,104 @@ __global__ void __launch_bounds__(kTileThreads) grid_tile_kernel(
     }
 }
 
+// ---- output separated by iteration (eq. 12) ----------------------------------------------
+// The same tile and running sum as grid_tile_kernel, but the groups of equal separation (the paper's iterations)
+// are not merged: group g writes its own decimated plane Y^g[d][m], W^g[d][m], point m = sample m * 2^shift,
+// at out + off[g] + d * npts[g] + m.  One thread per grid point and group; a point where no width of the group
+// fits the row gets -inf / -1 (reading A3).
+struct GridIterLayout {
+    long long off[kGridGroupsMax];   // element offset of group g's plane in the concatenated outputs
+    long long npts[kGridGroupsMax];  // points per row: ceil(n_t / 2^shift)
+};
+
+__global__ void __launch_bounds__(kTileThreads) grid_iter_kernel(
+    const float* __restrict__ plane, const float* __restrict__ mean, const float* __restrict__ sigma,
+    const int32_t* __restrict__ widths, const float* __restrict__ wscale, int n_w, const GridGroups groups,
+    const GridIterLayout lay, long long n_t, int tile, int span, long long tiles_per_row,
+    float* __restrict__ out_snr, int32_t* __restrict__ out_width) {
+    extern __shared__ __align__(16) unsigned char gsm[];
+    const int n_sub = span / kSub;
+    double* const B = reinterpret_cast<double*>(gsm);
+    float* const c = reinterpret_cast<float*>(gsm + (n_sub + 2) / 2 * 16);
+    int32_t* const sw = reinterpret_cast<int32_t*>(c + (span + 4) / 4 * 4);
+    float* const ss = reinterpret_cast<float*>(sw + kTileWidthsMax);
+    const long long d = blockIdx.x / tiles_per_row;
+    const long long t0 = (blockIdx.x - d * tiles_per_row) * tile;
+    const float* __restrict__ row = plane + d * n_t;
+    const float mu = mean[d];
+    const float inv = 1.0f / sigma[d];
+    const long long avail = n_t - t0;
+    for (int k = threadIdx.x; k < n_w; k += kTileThreads) {  // n_w <= kTileWidthsMax (checked at plan creation)
+        sw[k] = __ldg(widths + k);
+        ss[k] = __ldg(wscale + k) * inv;
+    }
+    build_running_sum(row, t0, avail, mu, n_sub, span, B, c);
+    const int n_out = static_cast<int>(min(static_cast<long long>(tile), avail));
+    for (int g = 0; g < groups.n; ++g) {
+        const int sh = groups.shift[g];
+        const int kb = groups.kb[g], ke = groups.ke[g];
+        const long long step = 1ll << sh;
+        const int i0 = static_cast<int>((step - (t0 & (step - 1))) & (step - 1));  // first grid point of the tile
+        const int count = i0 < n_out ? static_cast<int>((n_out - i0 + step - 1) >> sh) : 0;
+        float* const ys = out_snr + lay.off[g] + d * lay.npts[g];
+        int32_t* const yw = out_width + lay.off[g] + d * lay.npts[g];
+        for (int item = threadIdx.x; item < count; item += kTileThreads) {
+            const int i = i0 + (item << sh);
+            const long long room = avail - i;
+            const float c0 = c[i];
+            const double b0 = B[i / kSub];
+            float best = __int_as_float(0xff800000);
+            int idx = -1;
+            for (int k = kb; k < ke; ++k) {
+                const int L = sw[k];
+                if (L > room) break;  // valid windows only (reading A3); widths ascend
+                const int e = i + L;
+                const float x = static_cast<float>(B[e / kSub] - b0) + (c[e] - c0);
+                const float snr = x * ss[k];  // eq. (4) with eq. (5)
+                if (snr > best) {             // strict '>' in ascending width order
+                    best = snr;
+                    idx = k;
+                }
+            }
+            const long long m = (t0 + i) >> sh;
+            ys[m] = best;
+            yw[m] = idx;
+        }
+    }
+}
+
 }  // namespace
+
+// Iterations of a grid plan = its groups of equal separation; points per row of group g.
+int64_t grid_iter_points(const spd_plan* plan, int g) {
+    const int64_t step = int64_t(1) << plan->grid.shift[g];
+    return (plan->n_t + step - 1) / step;
+}
+
+int generic_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                           float* out_snr, int32_t* out_width, cudaStream_t stream) {
+    static bool configured = false;  // per process; the attribute is sticky
+    if (!configured) {
+        const cudaError_t e = cudaFuncSetAttribute(grid_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   227 * 1024);  // the most a block can have
+        if (e != cudaSuccess) return cuda_fail(e, "configuring the per-iteration kernel");
+        configured = true;
+    }
+    GridIterLayout lay = {};
+    long long off = 0;
+    for (int g = 0; g < plan->grid.n; ++g) {
+        lay.off[g] = off;
+        lay.npts[g] = grid_iter_points(plan, g);
+        off += plan->n_dm * lay.npts[g];
+    }
+    grid_iter_kernel<<<static_cast<unsigned>(plan->n_dm * plan->generic_tiles_per_row), kTileThreads, plan->generic_smem,
+                       stream>>>(plane, mean, sigma, plan->d_widths, plan->d_wscale,
+                                 static_cast<int>(plan->widths.size()), plan->grid, lay, plan->n_t, plan->generic_tile,
+                                 plan->generic_span, plan->generic_tiles_per_row, out_snr, out_width);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "launching the per-iteration kernel");
+    return SPD_OK;
+}
 
 int generic_configure(spd_plan* plan) {
     const int n_w = static_cast<int>(plan->widths.size());

@@ -163,6 +163,10 @@ inline bool runs_tree_kernel(const spd_plan* plan) {
 // spd_generic.cu
 int generic_configure(spd_plan* plan);
 void generic_release(spd_plan* plan);
+// output separated by iteration (grid plans): planes of the groups of equal separation, concatenated
+int64_t grid_iter_points(const spd_plan* plan, int g);
+int generic_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                           float* out_snr, int32_t* out_width, cudaStream_t stream);
 // sigma_w: nullptr (eq. 5: sqrt(L) sigma[d]) or [n_dm][n_widths] measured standard deviations
 // (tile kernels only); then `sigma` is not read.
 int generic_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean,

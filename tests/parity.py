@@ -31,9 +31,10 @@ def snr_tolerance(ref: np.ndarray) -> np.ndarray:
 
 def assert_parity(oracle, plane_rows: np.ndarray, mu, sg, widths, got_snr: np.ndarray, got_idx: np.ndarray,
                   ref_snr: np.ndarray, ref_idx: np.ndarray, ref_second: np.ndarray, t0: int = 0,
-                  what: str = "") -> ParityStats:
+                  what: str = "", stride: int = 1) -> ParityStats:
     """plane_rows [r, n_t] float32 are the rows the outputs belong to; outputs cover samples
-    [t0, t0 + span) of those rows.  mu, sg: per-row float64 arrays (or scalars)."""
+    [t0, t0 + span) of those rows - or, for the decimated plane of one iteration (eq. 12), column c is
+    sample (t0 + c) * stride.  mu, sg: per-row float64 arrays (or scalars)."""
     got_snr = np.asarray(got_snr)
     got_idx = np.asarray(got_idx)
     assert got_snr.shape == ref_snr.shape == got_idx.shape == ref_idx.shape, what
@@ -82,7 +83,7 @@ def assert_parity(oracle, plane_rows: np.ndarray, mu, sg, widths, got_snr: np.nd
             for L in np.unique(chosen):
                 m = chosen == L
                 s = oracle.snr_of_width(plane_rows[row], float(mu[row]), float(sg[row]), int(L),
-                                        (c[m] + t0).astype(np.int64))
+                                        ((c[m] + t0) * stride).astype(np.int64))
                 bad = ~(np.abs(s - ref_snr[row, c[m]]) <= tol[row, c[m]])
                 assert not bad.any(), (
                     f"{what}: near-tie width {L} at row {row} sample {t0 + c[m][bad][0]} has oracle SNR "
