@@ -357,8 +357,9 @@ int spd_run_host(spd_plan* plan, const float* plane, const float* mean, const fl
  * spd_run_iterations: out_snr_iter (float32) and out_width_iter (int32) are DEVICE buffers holding the
  *   iterations' planes one after the other, iteration i as [n_dm][n_points[i]] row-major at element offset
  *   n_dm * (n_points[0] + ... + n_points[i-1]); plane, mean, sigma as spd_run (eq. 5's sqrt(L) sigma).
- *   Asynchronous on cuda_stream.  Any grid plan; runs on the shared-memory tile kernel of the any-width-set
- *   path (one pass over the plane, all iterations in one launch).
+ *   Asynchronous on cuda_stream.  Any grid plan, one pass over the plane and one launch for all iterations: BoxDIT
+ *   plans (Alg. 1's widths on Alg. 1's grids) on the BoxDIT streaming kernel, whose levels are the iterations;
+ *   every other grid on the shared-memory tile kernel of the any-width-set path.
  * Both return SPD_ERR_INVALID_ARG for a plan without separations.
  */
 int spd_plan_get_iterations(const spd_plan* plan, int32_t cap, int32_t* n_iter, int32_t* first_width,

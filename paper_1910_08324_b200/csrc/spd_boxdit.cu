@@ -56,6 +56,12 @@ struct BdParams {
     int last_count;    // widths of the last level (1 .. B; a width set cut by max_width)
     int l_max_total;   // the largest width
     uint32_t tag_mask;  // ~127 or ~255
+    // output separated by iteration (eq. 12; spd_run_iterations): level i's plane Y^i, W^i [n_dm][it_npts[i]] at
+    // element offset it_off[i] of it_snr / it_width; out_snr / out_width are not written then
+    float* it_snr;
+    int32_t* it_width;
+    long long it_off[kBdMaxLevels];
+    long long it_npts[kBdMaxLevels];
 };
 
 template <int B>
@@ -124,7 +130,39 @@ __device__ __forceinline__ void bd_task(const float* __restrict__ A, const float
     }
 }
 
-template <int B>
+// ITER: the best key of the four points of a task goes to its iteration's own plane (tag split off), scalar stores
+// (a decimated row starts at any alignment); point q of level `level` is sample q << level of the row.
+__device__ __forceinline__ void bd_store_iteration(const BdParams& p, const long long d, const int level,
+                                                   const long long q0, const float (&key)[4]) {
+    const uint32_t code_top = ~p.tag_mask;
+    const long long npts = p.it_npts[level];
+    const long long base = p.it_off[level] + d * npts;
+    float* const ys = p.it_snr + base;
+    int32_t* const yw = p.it_width + base;
+    float y[4];
+    int w[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t b = __float_as_uint(key[j]);
+        const bool none = key[j] == __int_as_float(0xff800000);
+        y[j] = none ? key[j] : __uint_as_float(b & p.tag_mask);
+        w[j] = none ? -1 : static_cast<int>(code_top - (b & code_top));
+    }
+    if (((base + q0) & 3) == 0 && q0 + 3 < npts) {  // the usual case (row lengths that are multiples of 2^(level+2))
+        *reinterpret_cast<float4*>(ys + q0) = make_float4(y[0], y[1], y[2], y[3]);
+        *reinterpret_cast<int4*>(yw + q0) = make_int4(w[0], w[1], w[2], w[3]);
+        return;
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (q0 + j < npts) {
+            ys[q0 + j] = y[j];
+            yw[q0 + j] = w[j];
+        }
+    }
+}
+
+template <int B, bool ITER>
 __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p) {
     constexpr int T = kBdChunk, NT = kBdThreads, TASKS0 = T / 4 / NT;
     extern __shared__ __align__(128) float sm[];
@@ -180,6 +218,7 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
         float* const A0 = x0 + buf * (T + B);
         mbar_wait(&full[buf], (step >> 1) & 1);
         const int t0 = c * T;
+        const bool store = c < c_hi;  // chunks walked ahead of the segment only fill the carries
         // a window of this chunk may cross the end of the row: per-key test of fit
         const bool masked = static_cast<long long>(t0) + T + p.l_max_total > p.n_t;
         // ---- level 0 --------------------------------------------------------------------
@@ -204,6 +243,9 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
                 } else {
                     bd_task<B, true, false>(A0, make_float4(0.f, 0.f, 0.f, 0.f), a, mu, scale, code_top, p.tag_mask,
                                             last, A1, X1, mlim, best0[k]);
+                }
+                if constexpr (ITER) {
+                    if (store) bd_store_iteration(p, d, 0, static_cast<long long>(t0) + 4 * a, best0[k]);
                 }
             }
         }
@@ -239,7 +281,9 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
                 } else {
                     bd_task<B, false, false>(A, xin, a, mu, scale + i * B, code0, p.tag_mask, last, An, Xn, mlim, best);
                 }
-                if (i <= 2) {
+                if constexpr (ITER) {
+                    if (store) bd_store_iteration(p, d, i, (static_cast<long long>(t0) >> i) + 4 * a, best);
+                } else if (i <= 2) {
                     *reinterpret_cast<float4*>(XB + 4 * a) = make_float4(best[0], best[1], best[2], best[3]);
                 } else {
                     // point q of level i is sample q * 2^i = entry q * 2^(i-2) of level 2's array: the best keys of the
@@ -256,9 +300,8 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
             __syncthreads();
         }
         // ---- gather the levels per sample, store; carry x^i, i >= 1 -------------------------------
-        const bool store = c < c_hi;
 #pragma unroll
-        for (int k = 0; k < TASKS0; ++k) {
+        for (int k = 0; k < (ITER ? 0 : TASKS0); ++k) {
             const int a = tid + k * NT;
             float* const key = best0[k];
             if (I > 1) {
@@ -299,12 +342,17 @@ int bd_launch(const BdParams& prm, unsigned blocks, cudaStream_t stream) {
     static bool configured = false;  // per process and instantiation; the attribute is sticky
     const size_t smem = static_cast<size_t>(bd_smem_floats<B>()) * sizeof(float);
     if (!configured) {
-        const cudaError_t e =
-            cudaFuncSetAttribute(spd_boxdit_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        cudaError_t e =
+            cudaFuncSetAttribute(spd_boxdit_kernel<B, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(spd_boxdit_kernel<B, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
         if (e != cudaSuccess) return cuda_fail(e, "configuring the BoxDIT kernel");
         configured = true;
     }
-    spd_boxdit_kernel<B><<<blocks, kBdThreads, smem, stream>>>(prm);
+    if (prm.it_snr)
+        spd_boxdit_kernel<B, true><<<blocks, kBdThreads, smem, stream>>>(prm);
+    else
+        spd_boxdit_kernel<B, false><<<blocks, kBdThreads, smem, stream>>>(prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "launching the BoxDIT kernel");
     return SPD_OK;
@@ -355,10 +403,37 @@ bool boxdit_configure(spd_plan* plan) {
     return true;
 }
 
+static int boxdit_run_any(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+                          float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w,
+                          float* it_snr, int32_t* it_width);
+
 int boxdit_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w) {
+    return boxdit_run_any(plan, n_dm, plane, mean, sigma, out_snr, out_width, stream, sigma_w, nullptr, nullptr);
+}
+
+// Output separated by iteration (eq. 12): the levels' best keys go to their own decimated planes, concatenated
+// in it_snr / it_width (layout of spd_run_iterations); whole planes only (n_dm = plan->n_dm).
+int boxdit_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                          float* it_snr, int32_t* it_width, cudaStream_t stream) {
+    return boxdit_run_any(plan, plan->n_dm, plane, mean, sigma, nullptr, nullptr, stream, nullptr, it_snr, it_width);
+}
+
+static int boxdit_run_any(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
+                          float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w,
+                          float* it_snr, int32_t* it_width) {
     const BoxditConfig& c = plan->boxdit;
     BdParams prm = {};
+    prm.it_snr = it_snr;
+    prm.it_width = it_width;
+    if (it_snr) {
+        long long off = 0;
+        for (int i = 0; i < c.levels; ++i) {
+            prm.it_off[i] = off;
+            prm.it_npts[i] = (plan->n_t + (1ll << i) - 1) >> i;
+            off += n_dm * prm.it_npts[i];
+        }
+    }
     prm.plane = plane;
     prm.mean = mean;
     prm.sigma = sigma;

@@ -462,6 +462,8 @@ int64_t grid_iter_points(const spd_plan* plan, int g) {
 
 int generic_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
                            float* out_snr, int32_t* out_width, cudaStream_t stream) {
+    if (plan->boxdit.B > 0)  // Alg. 1's widths on Alg. 1's grids: the BoxDIT streaming kernel keeps its levels apart
+        return boxdit_run_iterations(plan, plane, mean, sigma, out_snr, out_width, stream);
     static bool configured = false;  // per process; the attribute is sticky
     if (!configured) {
         const cudaError_t e = cudaFuncSetAttribute(grid_iter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,

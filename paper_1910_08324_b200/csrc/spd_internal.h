@@ -181,6 +181,8 @@ int dense_run(const spd_plan* plan, int64_t n_dm, const float* plane, const floa
 
 // spd_boxdit.cu: the BoxDIT algorithm (widths of eq. 14 on their own grids) as one streaming kernel
 bool boxdit_configure(spd_plan* plan);
+int boxdit_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
+                          float* it_snr, int32_t* it_width, cudaStream_t stream);
 int boxdit_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w);
 
