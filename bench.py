@@ -436,6 +436,7 @@ class Workbench:
             "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
             "algorithmic_bytes_per_launch": self.bytes_per_sample * self.n, "bytes_per_sample": self.bytes_per_sample,
             "kernel_ms": k_ms, "kernel_ms_min": min(rec["run_ms"]),
+            "kernel_ms_each": [round(v, 3) for v in rec["run_ms"]],
             "candidates_ms": sum(rec["cand_ms"]) / len(rec["cand_ms"]),
             "kernel_share_of_step": sum(rec["run_ms"]) / (sum(rec["run_ms"]) + sum(rec["cand_ms"])),
             "co_bound": alu,

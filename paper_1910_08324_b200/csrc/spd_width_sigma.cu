@@ -26,6 +26,7 @@
 #include <algorithm>
 
 #include "spd_internal.h"
+#include "spd_tree_common.cuh"  // mbarrier + 1-D bulk copy helpers
 
 namespace spd {
 namespace {
@@ -72,11 +73,21 @@ __device__ __forceinline__ void level_add(const float (&v)[N], int j, long long 
     s2 += static_cast<double>(b);
 }
 
+// TMA variant (rows 16-byte aligned): the full super-blocks of a block's part arrive by 1-D bulk copies through
+// a ring of kWsgStages stages of 32 KB, so that two to three super-blocks per block are in flight whatever the
+// threads are doing (with plain loads a thread's 128 B were requested, awaited and consumed in turn: 3.2 TB/s).
+// A thread reads its 8 float4 in the order q ^ (t & 7): consecutive threads are 128 B apart, the rotation spreads
+// a quarter-warp over all banks; XOR by a constant maps aligned blocks of 2^k float4 onto aligned blocks, so every
+// level still sums the same groups - only the order of a thread's additions changes.
+constexpr int kWsgStages = 3;
+constexpr size_t kWsgRingBytes = static_cast<size_t>(kWsgStages) * kWsgBlock * sizeof(float);
+
 // One block walks super-blocks of 8192 samples.  Thread t owns the 32 consecutive samples
 // 32 t .. 32 t + 31: levels 0..5 in its registers; the 256 level-5 sums go through shared memory to
 // warp 0, whose lane l owns 8 of them: levels 5..8 in registers, levels 8..13 across lanes by
 // shuffles.  One block barrier per super-block (two buffers).  Sums of a few values are formed in
 // float32 (they ARE the decimated series), the running S1 / S2 of each level in double.
+template <bool TMA>
 __global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float* __restrict__ plane,
                                                                       const float* __restrict__ mean, long long n_t,
                                                                       int sb_per_row, int sb_per_part, int parts,
@@ -84,9 +95,11 @@ __global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float*
                                                                       double* __restrict__ totals) {
     __shared__ float v5[2][kWsgThreads];
     __shared__ double scratch[kWsgThreads / 32];
+    __shared__ __align__(8) uint64_t full[kWsgStages];
+    extern __shared__ __align__(128) float ring[];  // TMA: kWsgStages stages of kWsgBlock floats
     const int d = blockIdx.x / parts;
     const int part = blockIdx.x - d * parts;
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const float* __restrict__ row = plane + static_cast<long long>(d) * n_t;
     const float mu = mean[d];
     double s1[kWsgLevels], s2[kWsgLevels];
@@ -94,13 +107,44 @@ __global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float*
     for (int j = 0; j < kWsgLevels; ++j) s1[j] = s2[j] = 0.0;
     const int sb_lo = part * sb_per_part;
     const int sb_hi = min(sb_lo + sb_per_part, sb_per_row);
+    // super-blocks [sb_lo, sb_full) are complete (only a row's last one can be ragged): they go through the ring
+    const int sb_full = TMA ? min(sb_hi, static_cast<int>(n_t / kWsgBlock)) : sb_lo;
+    if constexpr (TMA) {
+        if (tid == 0) {
+#pragma unroll
+            for (int i = 0; i < kWsgStages; ++i) mbar_init(&full[i], 1);
+            fence_mbar_init();
+            fence_proxy_async();
+#pragma unroll
+            for (int i = 0; i < kWsgStages; ++i) {
+                if (sb_lo + i < sb_full) {
+                    mbar_arrive_expect_tx(&full[i], kWsgBlock * 4);
+                    bulk_g2s(ring + i * kWsgBlock, row + static_cast<long long>(sb_lo + i) * kWsgBlock, kWsgBlock * 4,
+                             &full[i]);
+                }
+            }
+        }
+        __syncthreads();
+    }
     int buf = 0;
     for (int sb = sb_lo; sb < sb_hi; ++sb, buf ^= 1) {
         const long long base = static_cast<long long>(sb) * kWsgBlock;
         const long long avail = n_t - base;  // samples of the row from here on (> 0)
         const long long mine = 32ll * tid;
+        const int k = sb - sb_lo, stage = k % kWsgStages;
         float x[32];
-        if (mine + 32 <= avail && ((reinterpret_cast<uintptr_t>(row + base) & 15u) == 0)) {
+        if (TMA && sb < sb_full) {
+            mbar_wait(&full[stage], (k / kWsgStages) & 1);
+            const float4* s4 = reinterpret_cast<const float4*>(ring + stage * kWsgBlock) + 8 * tid;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float4 f = s4[q ^ (tid & 7)];
+                x[4 * q] = f.x;
+                x[4 * q + 1] = f.y;
+                x[4 * q + 2] = f.z;
+                x[4 * q + 3] = f.w;
+            }
+        } else if (mine + 32 <= avail && ((reinterpret_cast<uintptr_t>(row + base) & 15u) == 0)) {
             const float4* p4 = reinterpret_cast<const float4*>(row + base + mine);
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
@@ -132,7 +176,17 @@ __global__ void __launch_bounds__(kWsgThreads) width_moments_kernel(const float*
         y1[0] = y2[0] + y2[1];
         v5[buf][tid] = y1[0];
         __syncthreads();  // the other buffer is free again: its readers passed this barrier one trip ago
-        if (tid < 32) {
+        if constexpr (TMA) {
+            // every thread has read this stage: refill it with the super-block kWsgStages ahead
+            if (tid == 0 && sb < sb_full && sb + kWsgStages < sb_full) {
+                mbar_arrive_expect_tx(&full[stage], kWsgBlock * 4);
+                bulk_g2s(ring + stage * kWsgBlock, row + static_cast<long long>(sb + kWsgStages) * kWsgBlock,
+                         kWsgBlock * 4, &full[stage]);
+            }
+        }
+        // the upper levels of a super-block are one warp's work: the warps take turns (every thread's sums are
+        // block-reduced at the end, so it does not matter whose registers hold them)
+        if (warp == (TMA ? (k & (kWsgThreads / 32 - 1)) : 0)) {
             // lane l: level-5 sums 8 l .. 8 l + 7 of the super-block (first sample 256 l)
             const long long first = 256ll * lane;
             float z8[8], z4[4], z2[2], z1[1];
@@ -242,7 +296,7 @@ __global__ void __launch_bounds__(64) width_sigma_finish_kernel(const LevelSums*
 int wsig_configure(spd_plan* plan) {
     const int64_t sb_per_row = (plan->n_t + kWsgBlock - 1) / kWsgBlock;
     // parts: enough blocks to fill the machine
-    const int64_t want = std::max<int64_t>(1, (8 * int64_t(plan->sm_count) + plan->n_dm - 1) / plan->n_dm);
+    const int64_t want = std::max<int64_t>(1, (16 * int64_t(plan->sm_count) + plan->n_dm - 1) / plan->n_dm);
     const int64_t parts = std::max<int64_t>(1, std::min<int64_t>(sb_per_row, want));
     plan->wsig_sb_per_part = static_cast<int>((sb_per_row + parts - 1) / parts);
     plan->wsig_parts = static_cast<int>((sb_per_row + plan->wsig_sb_per_part - 1) / plan->wsig_sb_per_part);
@@ -283,8 +337,22 @@ void wsig_release(spd_plan* plan) {
 int wsig_run(const spd_plan* plan, const float* plane, const float* mean, float* sigma_w, cudaStream_t stream) {
     LevelSums* partial = static_cast<LevelSums*>(plan->d_wsig_partial);
     double* totals = static_cast<double*>(plan->d_wsig_totals);
-    width_moments_kernel<<<static_cast<unsigned>(plan->n_dm * plan->wsig_parts), kWsgThreads, 0, stream>>>(
-        plane, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_sb_per_part, plan->wsig_parts, partial, totals);
+    const unsigned grid = static_cast<unsigned>(plan->n_dm * plan->wsig_parts);
+    if (plan->n_t % 4 == 0 && (reinterpret_cast<uintptr_t>(plane) & 15u) == 0) {  // rows 16-byte aligned: bulk copies
+        static bool configured = false;  // per process; the attribute is sticky
+        if (!configured) {
+            const cudaError_t ea = cudaFuncSetAttribute(width_moments_kernel<true>,
+                                                        cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                        static_cast<int>(kWsgRingBytes));
+            if (ea != cudaSuccess) return cuda_fail(ea, "configuring the width-sigma kernel");
+            configured = true;
+        }
+        width_moments_kernel<true><<<grid, kWsgThreads, kWsgRingBytes, stream>>>(
+            plane, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_sb_per_part, plan->wsig_parts, partial, totals);
+    } else {
+        width_moments_kernel<false><<<grid, kWsgThreads, 0, stream>>>(
+            plane, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_sb_per_part, plan->wsig_parts, partial, totals);
+    }
     width_sigma_finish_kernel<<<static_cast<unsigned>(plan->n_dm), 64, 0, stream>>>(
         partial, totals, mean, plan->n_t, plan->wsig_sb_per_row, plan->wsig_parts, plan->wsig_levels,
         static_cast<const int32_t*>(plan->d_wsig_widths), static_cast<int>(plan->widths.size()), sigma_w);
