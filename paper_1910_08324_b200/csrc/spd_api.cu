@@ -186,6 +186,9 @@ int run_rows(const spd_plan* plan, int64_t n_rows, const float* plane, const flo
                       stream);
     if (plan->path == SPD_PATH_GRID && plan->tree.kind == 1)
         return ws_run(plan, n_rows, plane, mean, sigma, out_snr, out_width, threshold, activity, stream);
+    if (plan->boxdit.B > 0 && plan->width_bytes == 4)  // the BoxDIT streaming kernel fuses the threshold test as well
+        return boxdit_run(plan, n_rows, plane, mean, sigma, out_snr, static_cast<int32_t*>(out_width), stream, nullptr,
+                          threshold, activity);
     if (activity) {
         // any-width-set path: no fused test, every block stays active (padding included: the
         // candidate kernel bounds the flag index itself)

@@ -58,6 +58,9 @@ struct BdParams {
     uint32_t tag_mask;  // ~127 or ~255
     // output separated by iteration (eq. 12; spd_run_iterations): level i's plane Y^i, W^i [n_dm][it_npts[i]] at
     // element offset it_off[i] of it_snr / it_width; out_snr / out_width are not written then
+    // threshold test of row a8 fused (spd_run_flagged): a chunk with a key >= thr_key sets activity[d][c]
+    uint8_t* activity;  // [n_dm][chunks_per_row] or nullptr (cleared by the host)
+    float thr_key;      // threshold in SNR units, lowered by the tag's perturbation so that rounding only adds chunks
     float* it_snr;
     int32_t* it_width;
     long long it_off[kBdMaxLevels];
@@ -310,6 +313,8 @@ __global__ void __launch_bounds__(kBdThreads) spd_boxdit_kernel(const BdParams p
                 key[2] = fmaxf(key[2], b1.y);
             }
             if (I > 2) key[0] = fmaxf(key[0], xb[bd_off_b(2) + a]);  // level 2 and, folded into it, the levels above
+            if (p.activity && store && fmax3(fmaxf(key[0], key[1]), key[2], key[3]) >= p.thr_key)
+                p.activity[d * p.chunks_per_row + c] = 1;  // any thread of the block may set it
             const int n = t0 + 4 * a;
             if (store && n < n_t) {
                 float4 y;
@@ -405,11 +410,13 @@ bool boxdit_configure(spd_plan* plan) {
 
 static int boxdit_run_any(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                           float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w,
-                          float* it_snr, int32_t* it_width);
+                          float* it_snr, int32_t* it_width, float threshold = 0.f, uint8_t* activity = nullptr);
 
 int boxdit_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w) {
-    return boxdit_run_any(plan, n_dm, plane, mean, sigma, out_snr, out_width, stream, sigma_w, nullptr, nullptr);
+               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w, float threshold,
+               uint8_t* activity) {
+    return boxdit_run_any(plan, n_dm, plane, mean, sigma, out_snr, out_width, stream, sigma_w, nullptr, nullptr,
+                          threshold, activity);
 }
 
 // Output separated by iteration (eq. 12): the levels' best keys go to their own decimated planes, concatenated
@@ -421,9 +428,17 @@ int boxdit_run_iterations(const spd_plan* plan, const float* plane, const float*
 
 static int boxdit_run_any(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
                           float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w,
-                          float* it_snr, int32_t* it_width) {
+                          float* it_snr, int32_t* it_width, float threshold, uint8_t* activity) {
     const BoxditConfig& c = plan->boxdit;
     BdParams prm = {};
+    prm.activity = activity;
+    // the tag replaces up to 8 low mantissa bits of a key (2^-15 relative): lower the threshold by more than that
+    prm.thr_key = threshold - fabsf(threshold) * 4e-5f;
+    if (activity) {
+        const size_t bytes = (static_cast<size_t>(n_dm) * static_cast<size_t>(c.chunks_per_row) + 127) / 128 * 128;
+        const cudaError_t em = cudaMemsetAsync(activity, 0, bytes, stream);
+        if (em != cudaSuccess) return cuda_fail(em, "clearing the activity map");
+    }
     prm.it_snr = it_snr;
     prm.it_width = it_width;
     if (it_snr) {

@@ -252,8 +252,8 @@ int candidates_run(const spd_plan* plan, int64_t n_rows, int64_t dm_offset, cons
     if (clear && (e = cudaMemsetAsync(n_found, 0, sizeof(int64_t), stream)) != cudaSuccess)
         return cuda_fail(e, "clearing the candidate counter");
     // the any-width-set path marks everything: visiting every sample with the dense kernel is
-    // the same work with more parallelism
-    if (activity && runs_tree_kernel(plan)) {
+    // the same work with more parallelism (BoxDIT plans: the streaming kernel fills the map, 4096 samples per flag)
+    if (activity && (runs_tree_kernel(plan) || plan->boxdit.B > 0)) {
         const long long per_row = activity_per_row(plan);
         const long long n_flags = n_rows * per_row;
         const long long steps = (n_flags + 31) / 32;

@@ -183,8 +183,11 @@ int dense_run(const spd_plan* plan, int64_t n_dm, const float* plane, const floa
 bool boxdit_configure(spd_plan* plan);
 int boxdit_run_iterations(const spd_plan* plan, const float* plane, const float* mean, const float* sigma,
                           float* it_snr, int32_t* it_width, cudaStream_t stream);
+// activity: nullptr, or [n_dm][ceil(n_t / 4096)] bytes, cleared here and set for every 4096-sample chunk with a key
+// that reaches `threshold` (row a8's threshold test fused, as the tree kernels do)
 int boxdit_run(const spd_plan* plan, int64_t n_dm, const float* plane, const float* mean, const float* sigma,
-               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w);
+               float* out_snr, int32_t* out_width, cudaStream_t stream, const float* sigma_w, float threshold = 0.f,
+               uint8_t* activity = nullptr);
 
 // spd_stats.cu
 int stats_configure(spd_plan* plan);

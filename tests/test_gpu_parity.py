@@ -1328,3 +1328,45 @@ def test_grid_tree_plan_flagged_candidates(spd, oracle_lib):
     assert count == ref_count and count > 0
     assert np.array_equal(cands["dm"], c_dm) and np.array_equal(cands["t"], c_t)
     assert 0 < int(act.sum().item()) < act.numel()
+
+
+@pytest.mark.parametrize("B,M,thr", [(8, 1016, 5.0), (16, 2000, 6.0), (4, 124, -1.0)])
+def test_boxdit_plan_flagged_candidates(spd, oracle_lib, B, M, thr):
+    """The BoxDIT streaming kernel fuses the threshold test of row a8 like the tree kernels (one flag per
+    4096-sample chunk): the flagged run writes the same planes, the flagged candidate kernel returns exactly
+    the rule's candidates on them (also through the row-block path of spd_run_host_candidates), and only
+    some chunks are marked."""
+    rng = np.random.default_rng(300 + B)
+    n_dm, n_t = 5, 4096 * 9 + 4 * 33
+    widths = spd.spd_width_set_generate("BOXDIT", B, M)
+    seps = spd.spd_separation_generate("BOXDIT", B, widths)
+    x = rng.standard_normal((n_dm, n_t)).astype(np.float32)
+    x[1, 4096 * 3 - 40: 4096 * 3 - 40 + M // 2] += np.float32(9.0 / np.sqrt(M // 2))   # across a chunk boundary
+    x[4, n_t - 300:] += np.float32(0.8)                                                 # at the row's end
+    dev = torch.device("cuda:0")
+    plane = torch.from_numpy(x).to(dev)
+    mean, sigma = torch.zeros(n_dm, device=dev), torch.full((n_dm,), 1.1, device=dev)
+    with spd.Plan(n_dm, n_t, widths, M, separations=seps) as plan:
+        assert plan.info["path"] == spd.SPD_PATH_GRID and plan.info["threads_per_block"] == 256
+        assert plan.info["activity_block"] == 4096
+        snr0, idx0 = plan.run(plane, mean, sigma)
+        snr, idx, act = plan.run_flagged(plane, mean, sigma, thr)
+        lst, n_found = plan.find_candidates_flagged(snr, idx, act, thr, 1 << 18)
+        lst_all, n_all = plan.find_candidates(snr, idx, thr, 1 << 18)
+        torch.cuda.synchronize()
+        count, cands = spd.candidates_to_numpy(lst, n_found, 1 << 18)
+        count_all, cands_all = spd.candidates_to_numpy(lst_all, n_all, 1 << 18)
+        plan.set_option(spd.SPD_OPT_HOST_ROWS_PER_BLOCK, 2)
+        host_found, host_1d, host_arr = plan.run_host_candidates(
+            torch.from_numpy(x).pin_memory(), mean.cpu().pin_memory(), sigma.cpu().pin_memory(), thr, 0, 1 << 18)
+    assert torch.equal(snr, snr0) and torch.equal(idx, idx0)
+    ref_count, c_dm, c_t, _, _ = oracle_lib.find_candidates(snr.cpu().numpy(), idx.cpu().numpy(), thr)
+    assert count == ref_count == count_all and count > 0
+    order = np.lexsort((cands["t"], cands["dm"]))
+    assert np.array_equal(cands["dm"][order], c_dm) and np.array_equal(cands["t"][order], c_t)
+    assert host_1d == ref_count
+    marked = int(act[: n_dm * ((n_t + 4095) // 4096)].sum().item())
+    if thr > 0:
+        assert 0 < marked < n_dm * ((n_t + 4095) // 4096)
+    else:
+        assert marked == n_dm * ((n_t + 4095) // 4096)     # a negative threshold marks every chunk
