@@ -28,6 +28,9 @@ CASES = [
     ("POW2", 0, 1024, "DIT", 0, 3, 9000),                  # one width per iteration
     ("IGRID", 1, 512, "IGRID", 4, 2, 8192 + 12),           # the widths of a step on four layers
     ("IGRID", 1, 256, "EVERY_SAMPLE", 0, 2, 3000),         # a single iteration = the every-sample plane
+    ("BOXDIT", 4, 28, "BOXDIT", 4, 1, 28),                 # a row no longer than the widest boxcar, one DM trial
+    ("BOXDIT", 8, 56, "BOXDIT", 8, 3, 4096),               # exactly one chunk of the streaming kernel
+    ("POW2", 0, 8, "DIT", 0, 2, 9),                        # nine samples
 ]
 
 
@@ -37,7 +40,7 @@ def test_run_iterations_matches_the_oracle(spd, oracle_lib, wkind, wparam, M, gk
     x = (rng.standard_normal((n_dm, n_t)) * 1.3 + 0.25).astype(np.float32)
     S = max(1, M // 3)
     t_p = (n_t // 3) // 64 * 64
-    x[1, t_p: t_p + S] += np.float32(12.0 * 1.3 / np.sqrt(S))
+    x[n_dm - 1, t_p: t_p + S] += np.float32(12.0 * 1.3 / np.sqrt(S))
     x[0, n_t - M // 2:] += np.float32(0.7)                 # a step near the row's end: windows that do not fit
     mu = np.array([0.25, 0.2, 0.3][:n_dm])
     sg = np.array([1.3, 1.25, 1.35][:n_dm])
